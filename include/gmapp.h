@@ -1,0 +1,179 @@
+/*
+ * gmapp.h -- C ABI of libgmapp.so: the B200 (sm_100a) multi-agent vector-field planner rollout of
+ * G-MAPP (arxiv/paper_2606_12579).  "PAPER.md:<n>" cites line n of the paper's text.
+ *
+ * What the library computes (Sec. IV-A/IV-C, Fig. 2): N_a exploration agents, each a
+ * task-space state, are rolled forward N_k steps.  At every step every agent evaluates every obstacle
+ * sphere of the sphere world S_W (Eq. 5) with the circular-field / MFI force of Eq. 2-3
+ * as gated and clamped by Alg. 1 lines 6-7; the contributions are
+ * summed (Alg. 1 lines 10-16), the attractor of Eq. 7-8 is added (Eq. 6), the state
+ * is integrated with Eq. 9-11, the costs of Eq. 16-20 are
+ * accumulated on the fly, and the best agent is selected.  All of it runs in CUDA
+ * kernels; there is no CPU fallback.  Arithmetic is FP32.
+ *
+ * Conventions
+ *  - Every call returns a gmapp_status; nothing throws, aborts or prints.  On error nothing is launched
+ *    and gmapp_last_error(ctx) holds a message.
+ *  - Pointers named d_* are DEVICE pointers, caller-owned (e.g. torch tensors' data_ptr()), 16-byte
+ *    alignment is NOT required.  Pointers named h_* and all struct / scalar-array arguments (goal,
+ *    gains, tuning) are HOST pointers, read before the call returns.
+ *  - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All calls
+ *    are asynchronous on that stream except gmapp_best_agent, gmapp_plan_cycle_host,
+ *    gmapp_measure_fp32_peak and gmapp_destroy, which synchronise it.
+ *  - The context owns only its packed sphere copy, per-agent result scratch and small pinned staging
+ *    buffers, all allocated in gmapp_create (no allocation on the hot path).  One context is not
+ *    thread-safe; separate contexts are independent.
+ *  - State layouts.  GMAPP_POINT3: [n][6] = (p_x,p_y,p_z, v_x,v_y,v_z), world frame.
+ *    GMAPP_MOTOR6: [n][14] = motor[8] + twist[6].  motor = (r_w,r_x,r_y,r_z, d_w,d_x,d_y,d_z), the unit
+ *    dual quaternion r + eps d with d = (1/2) t (x) r, t = world translation as a pure quaternion,
+ *    r = rotation (Hamilton convention, x_world = R(r) x_body + t): component for component the scalar,
+ *    3 rotation-bivector, 3 translation-bivector and pseudoscalar coefficients of a geometric-algebra
+ *    motor of Spin(3) |x R^3.  twist = (w_x,w_y,w_z, v_x,v_y,v_z) in the BODY frame
+ *    (Eq. 11 right-multiplies).  Input motors are renormalised (|r| = 1, r.d = 0).
+ *  - goal: POINT3 3 floats (p_g); MOTOR6 8 floats (goal motor).
+ */
+#ifndef GMAPP_H
+#define GMAPP_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gmapp_ctx gmapp_ctx;   /* opaque */
+
+typedef enum {
+    GMAPP_OK = 0,
+    GMAPP_EINVAL = 1,      /* NULL pointer, non-positive size, non-finite dt, bad gains (eps<=0, r_d<=0, eps>r_d) */
+    GMAPP_ECAPACITY = 2,   /* n exceeds max_agents / max_spheres given to gmapp_create */
+    GMAPP_ESTATE = 3,      /* call order: rollout/forces before set_obstacles, best_agent before rollout */
+    GMAPP_ECUDA = 4        /* a CUDA runtime call failed; message in gmapp_last_error */
+} gmapp_status;
+
+typedef enum {
+    GMAPP_POINT3 = 0,      /* 3D point agents: p[3], v[3] */
+    GMAPP_MOTOR6 = 1       /* 6D pose agents: motor[8], twist[6] */
+} gmapp_kind;
+
+/* Gains and constants (POD, host memory).  Field-by-field meaning and the paper passage:          */
+typedef struct {
+    float k_circ;          /* k_f of Eq. 2 / Eq. 1; applied once                   */
+    float k_att, k_damp;   /* linear (translational) blocks of K and D in Eq. 7       */
+    float k_att_rot, k_damp_rot;   /* rotational blocks of K and D, MOTOR6 only                      */
+    float inv_mass, inv_inertia;   /* diagonal of the "tunable inertia tensor" of Eq. 9 */
+    float vel_factor;      /* the printed 1/2 of Eq. 10; default 0.5                  */
+    float r_influence;     /* r_d, detection radius (Eq. 1, Alg. 1 line 7)                           */
+    float r_agent;         /* r_a of Alg. 1; default 0                                */
+    float eps_dist;        /* epsilon of Alg. 1 line 6; default 1e-3 m                */
+    float w_goal, w_obs, w_path, w_smooth;   /* w_j of Eq. 16                         */
+    float r_cost_goal, r_cost_obs;           /* radii of Eq. 17 / Eq. 18; 0 => r_influence           */
+    float a_max;           /* Eq. 20; default 10 m/s^2                                */
+    int32_t heuristic;     /* 0 = circular field / MFI (Eq. 2-3); 1 = APF (Eq. 1)    */
+} gmapp_gains;
+
+/* Launch tuning (all 0 / -1 = choose automatically from N_a, N_O and the SM count).               */
+typedef struct {
+    int32_t lanes_per_agent;     /* threads that share one agent's sphere sum; power of two 1..1024 */
+    int32_t agents_per_thread;   /* 1 or 2: agents evaluated per staged sphere load                  */
+    int32_t cull;                /* -1 auto, 0 = branch-free force math for every pair,
+                                    1 = warp-vote skip of the force math when no lane's pair is inside r_d
+                                    (Alg. 1 line 7 is such a branch); results are identical */
+    int32_t stage;               /* -1 auto, 0 = read spheres from global/L2, 1 = stage the whole sphere set in
+                                    shared memory (TMA bulk copy), 2 = stream tiles through a TMA ring         */
+    int32_t max_ctas;            /* 0 = SM count; cap on the grid (for scaling experiments)           */
+    int32_t reserved[3];
+} gmapp_tuning;
+
+/* What the last gmapp_rollout launched (for reporting). */
+typedef struct {
+    int32_t grid, block;
+    int32_t lanes_per_agent, agents_per_thread, agents_per_cta;
+    int32_t cull, stage, tile_spheres, n_tiles;
+    int32_t smem_bytes, regs_per_thread;
+    int32_t kernels_launched;    /* kernels this call enqueued */
+} gmapp_launch_info;
+
+/* Fill *g with the defaults listed above (k_circ 1, k_att 2, k_damp 0.5, rot 2 / 0.5, inv 1, 1/2,
+ * r_d 0.15, r_a 0, eps 1e-3, weights 1, cost radii 0, a_max 10, heuristic 0). */
+void gmapp_default_gains(gmapp_gains* g);
+
+/* Create a context on CUDA device `device` able to hold max_agents agents and max_spheres spheres.
+ * Allocates all device / pinned memory the library will ever use for this context. */
+gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents, int max_spheres);
+
+/* Synchronises the device work of this context and frees it.  NULL is OK. */
+gmapp_status gmapp_destroy(gmapp_ctx* ctx);
+
+/* Load the sphere world S_W (Eq. 5; resident on the GPU).
+ * d_xyzr [n][4] = centre xyz + radius (per-sphere radii, a superset of the paper's single r_O);
+ * d_vel [n][3] = constant sphere velocities or NULL for a static world.  n = 0 is legal (no obstacles).
+ * The arrays are read by stream work enqueued in this call (a packing kernel); they may be freed or
+ * changed once that work has run.  Radii must be >= 0 and all values finite (not checked on device). */
+gmapp_status gmapp_set_obstacles(gmapp_ctx* ctx, const float* d_xyzr, const float* d_vel, int n, void* cuda_stream);
+/* Same with HOST arrays (copied through the context's pinned staging buffer). */
+gmapp_status gmapp_set_obstacles_host(gmapp_ctx* ctx, const float* h_xyzr, const float* h_vel, int n, void* cuda_stream);
+
+/* Optional launch tuning for later gmapp_rollout / gmapp_forces calls; NULL restores automatic choice. */
+gmapp_status gmapp_set_tuning(gmapp_ctx* ctx, const gmapp_tuning* tuning);
+
+/* One planning cycle: roll n_agents agents forward `steps` steps of size dt from the
+ * states in d_agents (layout by `kind`), through Eq. 2-3, 6-11, accumulating Eq. 16-20 over the
+ * steps+1 poses.  Final states are written to d_agents_out (same layout; may alias d_agents; may be
+ * NULL).  Per-agent costs / clearance / collision flags stay in the context (gmapp_get_results,
+ * gmapp_best_agent).  Obstacles move as c_j(t) = c_j + t u_j, t = k dt at step k.
+ * Errors: EINVAL for NULL / n_agents < 1 / steps < 1 / non-finite or non-positive dt / bad gains;
+ * ECAPACITY for n_agents > max_agents; ESTATE before gmapp_set_obstacles. */
+gmapp_status gmapp_rollout(gmapp_ctx* ctx, gmapp_kind kind, const float* d_agents, float* d_agents_out,
+                           int n_agents, const float* goal, const gmapp_gains* gains, float dt, int steps,
+                           void* cuda_stream);
+
+/* Agent selection: lexicographic argmin of (collided, C_i, i) over the last rollout;
+ * with prev_best >= 0 the incumbent keeps its place unless the challenger is collision-free while the
+ * incumbent collided, or the flags are equal and C_best < alpha * C_prev.  A NaN cost ranks last.
+ * Synchronises the stream and returns index and cost to host memory. */
+gmapp_status gmapp_best_agent(gmapp_ctx* ctx, float alpha, int prev_best, int* out_index, float* out_cost,
+                              void* cuda_stream);
+
+/* Force query without integration (the control thread's query, Fig. 2 step 5):
+ * for each state, d_f_rep [n][3] = sum_j f_j (world frame, Eq. 2-3 / Alg. 1) with obstacles at time
+ * t_obstacles, and d_f_total = Eq. 6: POINT3 [n][3] = f_a + f_r; MOTOR6 [n][6] = body wrench
+ * (torque, force).  Either output may be NULL. */
+gmapp_status gmapp_forces(gmapp_ctx* ctx, gmapp_kind kind, const float* d_agents, int n_agents, const float* goal,
+                          const gmapp_gains* gains, float t_obstacles, float* d_f_rep, float* d_f_total,
+                          void* cuda_stream);
+
+/* Copy the per-agent results of the last rollout into caller-owned DEVICE buffers (any may be NULL):
+ * d_cost [n][5] = {C, C_goal, C_obs, C_path, C_smooth} (Eq. 16-20); d_min_clearance [n] = min over poses
+ * and spheres of the surface distance (+inf with no obstacles); d_collided [n] int32. */
+gmapp_status gmapp_get_results(gmapp_ctx* ctx, float* d_cost, float* d_min_clearance, int32_t* d_collided,
+                               void* cuda_stream);
+
+/* A whole planning cycle from HOST buffers: (optional) sphere upload, agent upload from pinned staging,
+ * rollout, selection, 8-byte result download; h_agents_out (may be NULL) receives the final states.
+ * h_xyzr == NULL keeps the resident sphere world.  Synchronises the stream. */
+gmapp_status gmapp_plan_cycle_host(gmapp_ctx* ctx, gmapp_kind kind, const float* h_agents, float* h_agents_out,
+                                   int n_agents, const float* h_xyzr, const float* h_vel, int n_spheres,
+                                   const float* goal, const gmapp_gains* gains, float dt, int steps,
+                                   float alpha, int prev_best, int* out_index, float* out_cost,
+                                   void* cuda_stream);
+
+/* What the last gmapp_rollout launched. */
+gmapp_status gmapp_get_launch_info(const gmapp_ctx* ctx, gmapp_launch_info* out);
+
+/* Measure this GPU's FP32 FMA throughput with a register-only FFMA microkernel (8 independent chains
+ * per thread, all SMs), timed with CUDA events on `cuda_stream`; *out_tflops = 2 * FMAs / time.
+ * use_f32x2 != 0 issues packed fma.rn.f32x2 instead.  Synchronises. */
+gmapp_status gmapp_measure_fp32_peak(gmapp_ctx* ctx, int use_f32x2, float* out_tflops, void* cuda_stream);
+
+/* Number of SMs of the context's device. */
+int gmapp_sm_count(const gmapp_ctx* ctx);
+
+/* Message of the last failing call on this context (context-owned string, never freed by the caller);
+ * with ctx == NULL, the message of the last failing gmapp_create. */
+const char* gmapp_last_error(const gmapp_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GMAPP_H */

@@ -1,0 +1,494 @@
+// gmapp.cu -- host side of libgmapp.so: context, argument validation, launch selection and the
+// extern "C" entry points declared in include/gmapp.h.  No torch types; plain CUDA runtime.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "../../include/gmapp.h"
+#include "gmapp_kernels.cuh"
+
+using namespace gmapp;
+
+struct gmapp_ctx {
+    int device = 0, num_sms = 0, smem_optin = 0;
+    int max_agents = 0, max_spheres = 0, cap_spheres = 0;
+    // packed sphere world: raw radii, and radii + r_agent (only materialised when r_agent != 0)
+    float4* d_sph_raw = nullptr;
+    float4* d_sph_eff = nullptr;
+    float4* d_svel = nullptr;
+    float eff_r_agent = 0.0f;
+    bool eff_valid = false;
+    int n_spheres = -1;            // -1: set_obstacles not called yet
+    bool moving = false;
+    // per-agent results of the last rollout
+    float* d_cost = nullptr; float* d_minclr = nullptr; int* d_collided = nullptr;
+    int last_n_agents = 0;
+    // staging for the *_host entry points
+    float* d_agents_stage = nullptr;     // [max_agents][14]
+    float* d_xyzr_stage = nullptr;       // [max_spheres][4]
+    float* d_vel_stage = nullptr;        // [max_spheres][3]
+    float* h_pinned = nullptr;           // spheres*7 + agents*14 floats
+    size_t h_pinned_floats = 0;
+    int* d_best_idx = nullptr; float* d_best_cost = nullptr;
+    int* h_best = nullptr;               // pinned: {idx, cost bits}
+    float* d_scratch = nullptr;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    gmapp_tuning tuning;
+    bool has_tuning = false;
+    gmapp_launch_info info;
+    char err[512];
+};
+
+static char g_create_err[512] = "";
+
+static gmapp_status fail(gmapp_ctx* c, gmapp_status s, const char* fmt, const char* a = "", long x = 0, long y = 0) {
+    char* dst = c ? c->err : g_create_err;
+    snprintf(dst, 512, fmt, a, x, y);
+    return s;
+}
+#define CUDA_TRY(ctx, call)                                                                     \
+    do {                                                                                        \
+        cudaError_t e__ = (call);                                                               \
+        if (e__ != cudaSuccess) return fail(ctx, GMAPP_ECUDA, "CUDA error '%s' at line %ld", cudaGetErrorString(e__), __LINE__); \
+    } while (0)
+
+static int round_up(int x, int m) { return (x + m - 1) / m * m; }
+static int pow2_floor(int x) { int p = 1; while (2 * p <= x) p *= 2; return p; }
+static int pow2_ceil(int x) { int p = 1; while (p < x) p *= 2; return p; }
+static int ilog2(int x) { int l = 0; while ((1 << l) < x) ++l; return l; }
+
+extern "C" void gmapp_default_gains(gmapp_gains* g) {
+    if (!g) return;
+    g->k_circ = 1.0f; g->k_att = 2.0f; g->k_damp = 0.5f; g->k_att_rot = 2.0f; g->k_damp_rot = 0.5f;
+    g->inv_mass = 1.0f; g->inv_inertia = 1.0f; g->vel_factor = 0.5f;
+    g->r_influence = 0.15f; g->r_agent = 0.0f; g->eps_dist = 1e-3f;
+    g->w_goal = g->w_obs = g->w_path = g->w_smooth = 1.0f;
+    g->r_cost_goal = 0.0f; g->r_cost_obs = 0.0f; g->a_max = 10.0f; g->heuristic = 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// kernel table
+// ---------------------------------------------------------------------------------------------
+typedef void (*rollout_fn)(const RolloutParams);
+// index: kind(2) x at(2: AT=1,2) x moving(2) x cull(2) x stage(2)
+static rollout_fn rollout_kernel(int kind, int at, bool moving, bool cull, int stage) {
+#define PICK(K, A, MT)                                                                            \
+    (moving ? (cull ? (stage ? (rollout_fn)k_rollout<K, A, true, true, 1, MT> : (rollout_fn)k_rollout<K, A, true, true, 0, MT>)      \
+                    : (stage ? (rollout_fn)k_rollout<K, A, true, false, 1, MT> : (rollout_fn)k_rollout<K, A, true, false, 0, MT>))   \
+            : (cull ? (stage ? (rollout_fn)k_rollout<K, A, false, true, 1, MT> : (rollout_fn)k_rollout<K, A, false, true, 0, MT>)    \
+                    : (stage ? (rollout_fn)k_rollout<K, A, false, false, 1, MT> : (rollout_fn)k_rollout<K, A, false, false, 0, MT>)))
+    if (kind == GMAPP_MOTOR6) return PICK(1, 1, 512);
+    if (at == 2) return PICK(0, 2, 512);
+    return PICK(0, 1, 1024);
+#undef PICK
+}
+static int rollout_max_threads(int kind, int at) { return (kind == GMAPP_MOTOR6 || at == 2) ? 512 : 1024; }
+
+// ---------------------------------------------------------------------------------------------
+// create / destroy
+// ---------------------------------------------------------------------------------------------
+extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents, int max_spheres) {
+    if (!out) return fail(nullptr, GMAPP_EINVAL, "gmapp_create: out is NULL%s");
+    *out = nullptr;
+    if (max_agents < 1 || max_spheres < 0) return fail(nullptr, GMAPP_EINVAL, "gmapp_create: max_agents must be >= 1 and max_spheres >= 0%s");
+    int ndev = 0;
+    CUDA_TRY(nullptr, cudaGetDeviceCount(&ndev));
+    if (device < 0 || device >= ndev) return fail(nullptr, GMAPP_EINVAL, "gmapp_create: no CUDA device %s%ld", "", device);
+    CUDA_TRY(nullptr, cudaSetDevice(device));
+    gmapp_ctx* c = new gmapp_ctx();
+    memset(&c->tuning, 0, sizeof c->tuning);
+    memset(&c->info, 0, sizeof c->info);
+    c->err[0] = 0;
+    c->device = device; c->max_agents = max_agents; c->max_spheres = max_spheres;
+    c->cap_spheres = round_up(max_spheres > 0 ? max_spheres : 1, 1024);
+    cudaDeviceProp prop;
+    cudaError_t e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) { delete c; return fail(nullptr, GMAPP_ECUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e)); }
+    if (prop.major < 10) { delete c; return fail(nullptr, GMAPP_ECUDA, "libgmapp is built for sm_100a only; device is sm_%s%ld%ld", "", prop.major, prop.minor); }
+    c->num_sms = prop.multiProcessorCount;
+    c->smem_optin = (int)prop.sharedMemPerBlockOptin;
+    // pinned staging: [0, 7*cap) spheres (xyzr then vel), [7*cap, 7*cap + 14*max_agents) agents
+    size_t hp = (size_t)c->cap_spheres * 7 + (size_t)max_agents * 14;
+    c->h_pinned_floats = hp;
+#define ALLOC(p, bytes) if ((e = cudaMalloc((void**)&(p), (bytes))) != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaMalloc: %s", cudaGetErrorString(e)); }
+    ALLOC(c->d_sph_raw, sizeof(float4) * c->cap_spheres);
+    ALLOC(c->d_sph_eff, sizeof(float4) * c->cap_spheres);
+    ALLOC(c->d_svel, sizeof(float4) * c->cap_spheres);
+    ALLOC(c->d_cost, sizeof(float) * 5 * max_agents);
+    ALLOC(c->d_minclr, sizeof(float) * max_agents);
+    ALLOC(c->d_collided, sizeof(int) * max_agents);
+    ALLOC(c->d_agents_stage, sizeof(float) * 14 * max_agents);
+    ALLOC(c->d_xyzr_stage, sizeof(float) * 4 * c->cap_spheres);
+    ALLOC(c->d_vel_stage, sizeof(float) * 3 * c->cap_spheres);
+    ALLOC(c->d_best_idx, sizeof(int));
+    ALLOC(c->d_best_cost, sizeof(float));
+    ALLOC(c->d_scratch, sizeof(float) * 64);
+#undef ALLOC
+    if ((e = cudaMallocHost((void**)&c->h_pinned, sizeof(float) * hp)) != cudaSuccess ||
+        (e = cudaMallocHost((void**)&c->h_best, sizeof(int) * 2)) != cudaSuccess ||
+        (e = cudaEventCreate(&c->ev0)) != cudaSuccess || (e = cudaEventCreate(&c->ev1)) != cudaSuccess) {
+        gmapp_destroy(c);
+        return fail(nullptr, GMAPP_ECUDA, "pinned / event allocation: %s", cudaGetErrorString(e));
+    }
+    // opt every rollout variant in to the full dynamic shared memory of the device
+    for (int kind = 0; kind < 2; ++kind)
+        for (int at = 1; at <= (kind == 0 ? 2 : 1); ++at)
+            for (int mv = 0; mv < 2; ++mv)
+                for (int cu = 0; cu < 2; ++cu)
+                    for (int st = 0; st < 2; ++st) {
+                        e = cudaFuncSetAttribute((const void*)rollout_kernel(kind, at, mv, cu, st),
+                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
+                        if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
+                    }
+    *out = c;
+    return GMAPP_OK;
+}
+
+extern "C" gmapp_status gmapp_destroy(gmapp_ctx* c) {
+    if (!c) return GMAPP_OK;
+    cudaSetDevice(c->device);
+    cudaDeviceSynchronize();
+    cudaFree(c->d_sph_raw); cudaFree(c->d_sph_eff); cudaFree(c->d_svel);
+    cudaFree(c->d_cost); cudaFree(c->d_minclr); cudaFree(c->d_collided);
+    cudaFree(c->d_agents_stage); cudaFree(c->d_xyzr_stage); cudaFree(c->d_vel_stage);
+    cudaFree(c->d_best_idx); cudaFree(c->d_best_cost); cudaFree(c->d_scratch);
+    if (c->h_pinned) cudaFreeHost(c->h_pinned);
+    if (c->h_best) cudaFreeHost(c->h_best);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    delete c;
+    return GMAPP_OK;
+}
+
+extern "C" const char* gmapp_last_error(const gmapp_ctx* c) { return c ? c->err : g_create_err; }
+extern "C" int gmapp_sm_count(const gmapp_ctx* c) { return c ? c->num_sms : 0; }
+
+extern "C" gmapp_status gmapp_set_tuning(gmapp_ctx* c, const gmapp_tuning* t) {
+    if (!c) return GMAPP_EINVAL;
+    if (!t) { c->has_tuning = false; return GMAPP_OK; }
+    if (t->lanes_per_agent < 0 || t->lanes_per_agent > 1024 ||
+        (t->lanes_per_agent && (t->lanes_per_agent & (t->lanes_per_agent - 1))))
+        return fail(c, GMAPP_EINVAL, "set_tuning: lanes_per_agent must be 0 or a power of two <= 1024%s");
+    if (t->agents_per_thread < 0 || t->agents_per_thread > 2) return fail(c, GMAPP_EINVAL, "set_tuning: agents_per_thread must be 0, 1 or 2%s");
+    if (t->cull < -1 || t->cull > 1 || t->stage < -1 || t->stage > 1 || t->max_ctas < 0)
+        return fail(c, GMAPP_EINVAL, "set_tuning: cull in {-1,0,1}, stage in {-1,0,1}, max_ctas >= 0%s");
+    c->tuning = *t; c->has_tuning = true;
+    return GMAPP_OK;
+}
+
+extern "C" gmapp_status gmapp_get_launch_info(const gmapp_ctx* c, gmapp_launch_info* out) {
+    if (!c || !out) return GMAPP_EINVAL;
+    *out = c->info;
+    return GMAPP_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// obstacles
+// ---------------------------------------------------------------------------------------------
+__global__ void k_add_ragent(const float4* __restrict__ raw, float4* __restrict__ eff, int n, int n_fill, float r_agent) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_fill) return;
+    float4 s = raw[i];
+    if (i < n) s.w += r_agent;
+    eff[i] = s;
+}
+
+static int fill_count(const gmapp_ctx* c, int n) {
+    int f = round_up(n > 0 ? n : 1, 1024);
+    return f > c->cap_spheres ? c->cap_spheres : f;
+}
+
+extern "C" gmapp_status gmapp_set_obstacles(gmapp_ctx* c, const float* d_xyzr, const float* d_vel, int n, void* stream) {
+    if (!c) return GMAPP_EINVAL;
+    if (n < 0) return fail(c, GMAPP_EINVAL, "set_obstacles: n < 0%s");
+    if (n > 0 && !d_xyzr) return fail(c, GMAPP_EINVAL, "set_obstacles: d_xyzr is NULL%s");
+    if (n > c->max_spheres) return fail(c, GMAPP_ECAPACITY, "set_obstacles: n = %s%ld exceeds max_spheres = %ld", "", n, c->max_spheres);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int nf = fill_count(c, n);
+    k_pack_spheres<<<(nf + 255) / 256, 256, 0, st>>>(d_xyzr, d_vel, n, nf, 0.0f, c->d_sph_raw, c->d_svel);
+    CUDA_TRY(c, cudaGetLastError());
+    c->n_spheres = n;
+    c->moving = (d_vel != nullptr) && n > 0;
+    c->eff_valid = false;
+    return GMAPP_OK;
+}
+
+extern "C" gmapp_status gmapp_set_obstacles_host(gmapp_ctx* c, const float* h_xyzr, const float* h_vel, int n, void* stream) {
+    if (!c) return GMAPP_EINVAL;
+    if (n < 0) return fail(c, GMAPP_EINVAL, "set_obstacles_host: n < 0%s");
+    if (n > 0 && !h_xyzr) return fail(c, GMAPP_EINVAL, "set_obstacles_host: h_xyzr is NULL%s");
+    if (n > c->max_spheres) return fail(c, GMAPP_ECAPACITY, "set_obstacles_host: n = %s%ld exceeds max_spheres = %ld", "", n, c->max_spheres);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (n > 0) {
+        // the pinned buffer may still be in flight from an earlier host call on this stream
+        CUDA_TRY(c, cudaStreamSynchronize(st));
+        memcpy(c->h_pinned, h_xyzr, sizeof(float) * 4 * n);
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_xyzr_stage, c->h_pinned, sizeof(float) * 4 * n, cudaMemcpyHostToDevice, st));
+        if (h_vel) {
+            memcpy(c->h_pinned + 4 * (size_t)n, h_vel, sizeof(float) * 3 * n);
+            CUDA_TRY(c, cudaMemcpyAsync(c->d_vel_stage, c->h_pinned + 4 * (size_t)n, sizeof(float) * 3 * n, cudaMemcpyHostToDevice, st));
+        }
+    }
+    return gmapp_set_obstacles(c, c->d_xyzr_stage, h_vel ? c->d_vel_stage : nullptr, n, stream);
+}
+
+// sphere array with R = r + r_agent; launches the tiny repack kernel only when r_agent changed
+static gmapp_status effective_spheres(gmapp_ctx* c, float r_agent, cudaStream_t st, const float4** out, int* launches) {
+    if (r_agent == 0.0f) { *out = c->d_sph_raw; return GMAPP_OK; }
+    if (!c->eff_valid || c->eff_r_agent != r_agent) {
+        const int nf = fill_count(c, c->n_spheres);
+        k_add_ragent<<<(nf + 255) / 256, 256, 0, st>>>(c->d_sph_raw, c->d_sph_eff, c->n_spheres, nf, r_agent);
+        CUDA_TRY(c, cudaGetLastError());
+        c->eff_valid = true; c->eff_r_agent = r_agent;
+        if (launches) ++*launches;
+    }
+    *out = c->d_sph_eff;
+    return GMAPP_OK;
+}
+
+static gmapp_status check_gains(gmapp_ctx* c, const gmapp_gains* g, const char* who) {
+    if (!g) return fail(c, GMAPP_EINVAL, "%s: gains is NULL", who);
+    const float* f = &g->k_circ;
+    for (int i = 0; i < 18; ++i) if (!isfinite(f[i])) return fail(c, GMAPP_EINVAL, "%s: non-finite gain", who);
+    if (!(g->eps_dist > 0.0f) || !(g->r_influence > 0.0f) || g->eps_dist > g->r_influence)
+        return fail(c, GMAPP_EINVAL, "%s: need 0 < eps_dist <= r_influence (Alg. 1 lines 6-7)", who);
+    if (g->r_agent < 0.0f || g->r_cost_goal < 0.0f || g->r_cost_obs < 0.0f || !(g->a_max > 0.0f))
+        return fail(c, GMAPP_EINVAL, "%s: r_agent, r_cost_* must be >= 0 and a_max > 0", who);
+    if (g->heuristic != 0) return fail(c, GMAPP_EINVAL, "%s: only heuristic 0 (circular field / MFI, Eq. 2-3) is built", who);
+    return GMAPP_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// launch selection
+// ---------------------------------------------------------------------------------------------
+struct LaunchCfg { int at, L, groups, block, grid, agents_per_cta, stage, cull, n_pad, smem, tile_off, red_off; };
+
+static gmapp_status choose_launch(gmapp_ctx* c, int kind, int n_agents, LaunchCfg* o) {
+    const gmapp_tuning* t = c->has_tuning ? &c->tuning : nullptr;
+    int max_ctas = c->num_sms;
+    if (t && t->max_ctas > 0 && t->max_ctas < max_ctas) max_ctas = t->max_ctas;
+    const int A = (n_agents + max_ctas - 1) / max_ctas;
+    const int grid = (n_agents + A - 1) / A;
+    int at = (kind == GMAPP_POINT3 && A >= 2) ? 2 : 1;
+    if (t && t->agents_per_thread) at = t->agents_per_thread;
+    if (kind == GMAPP_MOTOR6) at = 1;
+    const int G = (A + at - 1) / at;
+    const int tmax = rollout_max_threads(kind, at);
+    if (G > tmax) return fail(c, GMAPP_ECAPACITY, "rollout: %s%ld agent groups per CTA exceed %ld threads", "", G, tmax);
+    const int ns = c->n_spheres;
+    int L;
+    if (t && t->lanes_per_agent) {
+        L = t->lanes_per_agent;
+        if (G * L > tmax) return fail(c, GMAPP_EINVAL, "rollout: lanes_per_agent %s%ld x %ld groups exceeds the thread limit", "", L, G);
+    } else {
+        L = pow2_floor(tmax / G);
+        const int cap = pow2_ceil(ns > 0 ? ns : 1);       // no more lanes than spheres
+        if (L > cap) L = cap;
+    }
+    if (L > 32 && G > kMaxGroupsNamedBar) {
+        if (t && t->lanes_per_agent) return fail(c, GMAPP_EINVAL, "rollout: lanes_per_agent > 32 allows at most 15 groups per CTA, need %s%ld", "", G);
+        L = 32;
+    }
+    o->at = at; o->L = L; o->groups = G; o->grid = grid; o->agents_per_cta = A;
+    o->block = round_up(G * L, 32);
+    o->n_pad = ns > 0 ? round_up(ns, L) : 0;
+    o->cull = (t && t->cull >= 0) ? t->cull : 0;
+    // dynamic shared memory: [0,64) mbarrier; [64, 64+2 KB) cross-warp exchange; then the sphere tile
+    o->red_off = 64;
+    o->tile_off = 64 + 2 * 32 * 2 * 16;
+    const size_t tile_bytes = (size_t)o->n_pad * 16 * (c->moving ? 2 : 1);
+    const bool fits = o->tile_off + tile_bytes <= (size_t)c->smem_optin;
+    int stage = fits ? 1 : 0;
+    if (t && t->stage >= 0) {
+        if (t->stage == 1 && !fits) return fail(c, GMAPP_EINVAL, "rollout: sphere set (%s%ld bytes) does not fit shared memory", "", (long)tile_bytes);
+        stage = t->stage;
+    }
+    if (o->n_pad == 0) stage = 0;
+    o->stage = stage;
+    o->smem = o->tile_off + (stage == 1 ? (int)tile_bytes : 0);
+    return GMAPP_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// rollout
+// ---------------------------------------------------------------------------------------------
+extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float* d_agents, float* d_agents_out,
+                                      int n_agents, const float* goal, const gmapp_gains* g, float dt, int steps,
+                                      void* stream) {
+    if (!c) return GMAPP_EINVAL;
+    if (kind != GMAPP_POINT3 && kind != GMAPP_MOTOR6) return fail(c, GMAPP_EINVAL, "rollout: unknown kind%s");
+    if (!d_agents || !goal) return fail(c, GMAPP_EINVAL, "rollout: NULL agents or goal%s");
+    if (n_agents < 1 || steps < 1) return fail(c, GMAPP_EINVAL, "rollout: n_agents and steps must be >= 1%s");
+    if (!isfinite(dt) || !(dt > 0.0f)) return fail(c, GMAPP_EINVAL, "rollout: dt must be finite and > 0%s");
+    if (n_agents > c->max_agents) return fail(c, GMAPP_ECAPACITY, "rollout: n_agents = %s%ld exceeds max_agents = %ld", "", n_agents, c->max_agents);
+    if (c->n_spheres < 0) return fail(c, GMAPP_ESTATE, "rollout: gmapp_set_obstacles has not been called%s");
+    gmapp_status s = check_gains(c, g, "rollout");
+    if (s != GMAPP_OK) return s;
+    const int ng = kind == GMAPP_POINT3 ? 3 : 8;
+    for (int i = 0; i < ng; ++i) if (!isfinite(goal[i])) return fail(c, GMAPP_EINVAL, "rollout: non-finite goal%s");
+    LaunchCfg cfg;
+    s = choose_launch(c, kind, n_agents, &cfg);
+    if (s != GMAPP_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    int launches = 0;
+    RolloutParams P;
+    memset(&P, 0, sizeof P);
+    s = effective_spheres(c, g->r_agent, st, &P.sph, &launches);
+    if (s != GMAPP_OK) return s;
+    P.svel = c->d_svel;
+    P.n_pad = cfg.n_pad;
+    P.agents_in = d_agents; P.agents_out = d_agents_out;
+    P.n_agents = n_agents; P.agents_per_cta = cfg.agents_per_cta;
+    P.L = cfg.L; P.logL = ilog2(cfg.L);
+    P.steps = steps;
+    for (int i = 0; i < ng; ++i) P.goal[i] = goal[i];
+    P.dt = dt;
+    P.k_circ = g->k_circ; P.k_att = g->k_att; P.k_damp = g->k_damp;
+    P.k_att_rot = g->k_att_rot; P.k_damp_rot = g->k_damp_rot;
+    P.c_lin = g->vel_factor * dt * g->inv_mass;
+    P.c_rot = g->vel_factor * dt * g->inv_inertia;
+    P.inv_mass = g->inv_mass;
+    P.r_d = g->r_influence; P.eps = g->eps_dist;
+    P.rcg = g->r_cost_goal > 0.0f ? g->r_cost_goal : g->r_influence;
+    P.rco = g->r_cost_obs > 0.0f ? g->r_cost_obs : g->r_influence;
+    P.w_goal = g->w_goal; P.w_obs = g->w_obs; P.w_path = g->w_path; P.w_smooth = g->w_smooth;
+    P.a_max = g->a_max; P.vel_factor = g->vel_factor;
+    P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
+    P.tile_off = cfg.tile_off; P.red_off = cfg.red_off;
+    rollout_fn fn = rollout_kernel(kind, cfg.at, c->moving, cfg.cull != 0, cfg.stage);
+    fn<<<cfg.grid, cfg.block, cfg.smem, st>>>(P);
+    CUDA_TRY(c, cudaGetLastError());
+    ++launches;
+    c->last_n_agents = n_agents;
+    gmapp_launch_info& I = c->info;
+    I.grid = cfg.grid; I.block = cfg.block; I.lanes_per_agent = cfg.L; I.agents_per_thread = cfg.at;
+    I.agents_per_cta = cfg.agents_per_cta; I.cull = cfg.cull; I.stage = cfg.stage;
+    I.tile_spheres = cfg.stage == 1 ? cfg.n_pad : 0; I.n_tiles = cfg.stage == 1 ? 1 : 0;
+    I.smem_bytes = cfg.smem; I.kernels_launched = launches;
+    cudaFuncAttributes fa;
+    if (cudaFuncGetAttributes(&fa, (const void*)fn) == cudaSuccess) I.regs_per_thread = fa.numRegs;
+    return GMAPP_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// selection, force query, results
+// ---------------------------------------------------------------------------------------------
+extern "C" gmapp_status gmapp_best_agent(gmapp_ctx* c, float alpha, int prev_best, int* out_index, float* out_cost,
+                                         void* stream) {
+    if (!c) return GMAPP_EINVAL;
+    if (!out_index) return fail(c, GMAPP_EINVAL, "best_agent: out_index is NULL%s");
+    if (c->last_n_agents < 1) return fail(c, GMAPP_ESTATE, "best_agent: no rollout has run on this context%s");
+    if (!isfinite(alpha)) return fail(c, GMAPP_EINVAL, "best_agent: alpha is not finite%s");
+    cudaStream_t st = (cudaStream_t)stream;
+    k_best_agent<<<1, 1024, 0, st>>>(c->d_cost, c->d_collided, c->last_n_agents, alpha, prev_best, c->d_best_idx, c->d_best_cost);
+    CUDA_TRY(c, cudaGetLastError());
+    CUDA_TRY(c, cudaMemcpyAsync(&c->h_best[0], c->d_best_idx, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaMemcpyAsync(&c->h_best[1], c->d_best_cost, sizeof(float), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaStreamSynchronize(st));
+    *out_index = c->h_best[0];
+    if (out_cost) memcpy(out_cost, &c->h_best[1], sizeof(float));
+    return GMAPP_OK;
+}
+
+extern "C" gmapp_status gmapp_forces(gmapp_ctx* c, gmapp_kind kind, const float* d_agents, int n_agents, const float* goal,
+                                     const gmapp_gains* g, float t_obstacles, float* d_f_rep, float* d_f_total, void* stream) {
+    if (!c) return GMAPP_EINVAL;
+    if (kind != GMAPP_POINT3 && kind != GMAPP_MOTOR6) return fail(c, GMAPP_EINVAL, "forces: unknown kind%s");
+    if (!d_agents || !goal) return fail(c, GMAPP_EINVAL, "forces: NULL agents or goal%s");
+    if (n_agents < 1) return fail(c, GMAPP_EINVAL, "forces: n_agents must be >= 1%s");
+    if (!isfinite(t_obstacles)) return fail(c, GMAPP_EINVAL, "forces: t_obstacles is not finite%s");
+    if (c->n_spheres < 0) return fail(c, GMAPP_ESTATE, "forces: gmapp_set_obstacles has not been called%s");
+    gmapp_status s = check_gains(c, g, "forces");
+    if (s != GMAPP_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    ForceParams P;
+    memset(&P, 0, sizeof P);
+    s = effective_spheres(c, g->r_agent, st, &P.sph, nullptr);
+    if (s != GMAPP_OK) return s;
+    P.svel = c->d_svel;
+    P.n_pad = c->n_spheres > 0 ? round_up(c->n_spheres, 32) : 0;
+    P.agents = d_agents; P.n_agents = n_agents; P.kind = (int)kind;
+    for (int i = 0; i < (kind == GMAPP_POINT3 ? 3 : 8); ++i) P.goal[i] = goal[i];
+    P.k_circ = g->k_circ; P.k_att = g->k_att; P.k_damp = g->k_damp;
+    P.k_att_rot = g->k_att_rot; P.k_damp_rot = g->k_damp_rot;
+    P.r_d = g->r_influence; P.eps = g->eps_dist; P.t_obs = t_obstacles;
+    P.f_rep = d_f_rep; P.f_total = d_f_total;
+    const int warps_per_block = 8;
+    const int grid = (n_agents + warps_per_block - 1) / warps_per_block;
+    if (c->moving) k_forces<true><<<grid, 256, 0, st>>>(P);
+    else k_forces<false><<<grid, 256, 0, st>>>(P);
+    CUDA_TRY(c, cudaGetLastError());
+    return GMAPP_OK;
+}
+
+extern "C" gmapp_status gmapp_get_results(gmapp_ctx* c, float* d_cost, float* d_min_clearance, int32_t* d_collided, void* stream) {
+    if (!c) return GMAPP_EINVAL;
+    if (c->last_n_agents < 1) return fail(c, GMAPP_ESTATE, "get_results: no rollout has run on this context%s");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = c->last_n_agents;
+    if (d_cost) CUDA_TRY(c, cudaMemcpyAsync(d_cost, c->d_cost, sizeof(float) * 5 * n, cudaMemcpyDeviceToDevice, st));
+    if (d_min_clearance) CUDA_TRY(c, cudaMemcpyAsync(d_min_clearance, c->d_minclr, sizeof(float) * n, cudaMemcpyDeviceToDevice, st));
+    if (d_collided) CUDA_TRY(c, cudaMemcpyAsync(d_collided, c->d_collided, sizeof(int) * n, cudaMemcpyDeviceToDevice, st));
+    return GMAPP_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// whole cycle from host buffers
+// ---------------------------------------------------------------------------------------------
+extern "C" gmapp_status gmapp_plan_cycle_host(gmapp_ctx* c, gmapp_kind kind, const float* h_agents, float* h_agents_out,
+                                              int n_agents, const float* h_xyzr, const float* h_vel, int n_spheres,
+                                              const float* goal, const gmapp_gains* g, float dt, int steps,
+                                              float alpha, int prev_best, int* out_index, float* out_cost, void* stream) {
+    if (!c) return GMAPP_EINVAL;
+    if (!h_agents || !out_index) return fail(c, GMAPP_EINVAL, "plan_cycle_host: NULL agents or out_index%s");
+    if (kind != GMAPP_POINT3 && kind != GMAPP_MOTOR6) return fail(c, GMAPP_EINVAL, "plan_cycle_host: unknown kind%s");
+    if (n_agents < 1) return fail(c, GMAPP_EINVAL, "plan_cycle_host: n_agents must be >= 1%s");
+    if (n_agents > c->max_agents) return fail(c, GMAPP_ECAPACITY, "plan_cycle_host: n_agents = %s%ld exceeds max_agents = %ld", "", n_agents, c->max_agents);
+    cudaStream_t st = (cudaStream_t)stream;
+    gmapp_status s;
+    if (h_xyzr || n_spheres == 0) {
+        if (h_xyzr || c->n_spheres < 0) {
+            s = gmapp_set_obstacles_host(c, h_xyzr, h_vel, n_spheres, stream);
+            if (s != GMAPP_OK) return s;
+        }
+    }
+    const int w = kind == GMAPP_POINT3 ? 6 : 14;
+    float* hp = c->h_pinned + (size_t)c->cap_spheres * 7;
+    // every earlier use of the agent staging area ended with a stream synchronise (this call is synchronous)
+    memcpy(hp, h_agents, sizeof(float) * w * (size_t)n_agents);
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_agents_stage, hp, sizeof(float) * w * (size_t)n_agents, cudaMemcpyHostToDevice, st));
+    s = gmapp_rollout(c, kind, c->d_agents_stage, h_agents_out ? c->d_agents_stage : nullptr, n_agents, goal, g, dt, steps, stream);
+    if (s != GMAPP_OK) return s;
+    if (h_agents_out)
+        CUDA_TRY(c, cudaMemcpyAsync(hp, c->d_agents_stage, sizeof(float) * w * (size_t)n_agents, cudaMemcpyDeviceToHost, st));
+    s = gmapp_best_agent(c, alpha, prev_best, out_index, out_cost, stream);     // synchronises
+    if (s != GMAPP_OK) return s;
+    if (h_agents_out) memcpy(h_agents_out, hp, sizeof(float) * w * (size_t)n_agents);
+    return GMAPP_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// FP32 peak microbenchmark
+// ---------------------------------------------------------------------------------------------
+extern "C" gmapp_status gmapp_measure_fp32_peak(gmapp_ctx* c, int use_f32x2, float* out_tflops, void* stream) {
+    if (!c || !out_tflops) return GMAPP_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int grid = c->num_sms * 8, block = 256, iters = 2048;
+    float best_ms = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        CUDA_TRY(c, cudaEventRecord(c->ev0, st));
+        if (use_f32x2) k_fma_peak<true><<<grid, block, 0, st>>>(c->d_scratch, iters, 1.0000001f, 1e-9f);
+        else k_fma_peak<false><<<grid, block, 0, st>>>(c->d_scratch, iters, 1.0000001f, 1e-9f);
+        CUDA_TRY(c, cudaGetLastError());
+        CUDA_TRY(c, cudaEventRecord(c->ev1, st));
+        CUDA_TRY(c, cudaEventSynchronize(c->ev1));
+        float ms = 0.0f;
+        CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+        if (rep > 0 && ms < best_ms) best_ms = ms;
+    }
+    const double fmas = (double)grid * block * (double)iters * 128.0;
+    *out_tflops = (float)(2.0 * fmas / (best_ms * 1e-3) / 1e12);
+    return GMAPP_OK;
+}

@@ -1,0 +1,641 @@
+// gmapp_kernels.cuh -- the rollout / force / selection kernels (sm_100a, FP32).
+//
+// Thread mapping.  A "group" is L = lanes_per_agent consecutive threads (L a power of two).  A group
+// owns AT (1 or 2) agents and keeps their state in registers for the whole rollout; lane l of the group
+// evaluates spheres l, l+L, l+2L, ... at every step, so the sphere sum of an agent is split over the L
+// lanes and combined once per step by a fixed-order xor-shuffle tree (plus a shared-memory exchange and
+// one named barrier when the group spans several warps).  Every lane then integrates the group's
+// agents redundantly, so no state is ever broadcast back; the group's first warp alone accumulates the
+// costs.  Groups never wait for each other, so one group's reduce / integrate tail overlaps the other
+// groups' pair loops on the same SM.  Reductions use no atomics and a fixed order: results are
+// bit-reproducible run to run.
+//
+// Sphere staging.  STAGE 1: the whole packed sphere set (16 B per static sphere, +16 B velocity) is
+// copied once per rollout into shared memory by 1-D TMA bulk copies completing on an mbarrier, and
+// reused by every agent of the CTA for every step.  STAGE 0: spheres are read from global memory
+// through L1/L2 (sets that exceed shared memory; round-1 fallback for the tile ring).
+//
+// Pair math (static spheres), per agent-sphere pair, branch-free:
+//   d = c - p; q = |d|^2 (+1e-30 so q > 0); y = MUFU.RSQ(q); t = q y; dist = t + (y/2)(q - t^2)  (1 Newton step)
+//   ds = dist - R (R = r_j + r_a packed at set-up); dmin = min(dmin, ds); dO = max(ds, eps)
+//   s = d.v; w = s * MUFU.RCP(dO q); if (ds <= r_d) B += w d
+// and once per agent-step  f_r = k_f [ ((B.v)/|v|) v - |v| B ]   (BAC-CAB form of Eq. 2-3).
+// Moving spheres use the per-pair relative velocity and accumulate the force vector directly.
+#pragma once
+#include "gmapp_device.cuh"
+
+namespace gmapp {
+
+constexpr float kTiny = 1e-30f;          // bias that keeps squared norms > 0 (absorbed exactly otherwise)
+constexpr int kMaxGroupsNamedBar = 15;   // named barriers 1..15
+
+struct RolloutParams {
+    const float4* sph;        // [n_pad] (cx, cy, cz, r_j + r_a), sentinel-padded
+    const float4* svel;       // [n_pad] (ux, uy, uz, 0) or nullptr
+    int n_pad;                // multiple of L
+    const float* agents_in;   // [n][6] or [n][14]
+    float* agents_out;        // same layout or nullptr
+    int n_agents, agents_per_cta;
+    int L, logL;
+    int steps;
+    float goal[8];
+    float dt;
+    float k_circ, k_att, k_damp, k_att_rot, k_damp_rot;
+    float c_lin, c_rot;       // vel_factor * dt * inv_mass, vel_factor * dt * inv_inertia  (Eq. 9-10)
+    float inv_mass;
+    float r_d, eps;
+    float rcg, rco;           // Eq. 17 / 18 radii
+    float w_goal, w_obs, w_path, w_smooth, a_max, vel_factor;
+    float* cost;              // [n][5]
+    float* minclr;            // [n]
+    int* collided;            // [n]
+    int tile_off;             // byte offset of the sphere tile in dynamic shared memory
+    int red_off;              // byte offset of the cross-warp exchange scratch
+};
+
+// ---------------------------------------------------------------------------------------------
+// per-pair math
+// ---------------------------------------------------------------------------------------------
+template <int NA>
+struct StaticAcc {            // per-lane partial sums for NA agents, static spheres
+    float bx[NA], by[NA], bz[NA], dmin[NA];
+    __device__ __forceinline__ void clear() {
+#pragma unroll
+        for (int a = 0; a < NA; ++a) { bx[a] = by[a] = bz[a] = 0.0f; dmin[a] = __int_as_float(0x7f800000); }
+    }
+};
+
+// distance part shared by all variants: returns ds, leaves d, q
+__device__ __forceinline__ float pair_distance(float cx, float cy, float cz, float R,
+                                               float px, float py, float pz,
+                                               float& dx, float& dy, float& dz, float& q) {
+    dx = cx - px; dy = cy - py; dz = cz - pz;
+    q = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, kTiny)));
+    float y = rsqrt_approx(q);
+    float t = q * y;
+    float e = fmaf(-t, t, q);
+    return fmaf(0.5f * y, e, t - R);
+}
+
+template <int NA, bool FORCE, bool CULL>
+__device__ __forceinline__ void pair_static(const float4 s, const float (&p)[NA][3], const float (&v)[NA][3],
+                                            float r_d, float eps, unsigned mask, StaticAcc<NA>& acc) {
+    float dx[NA], dy[NA], dz[NA], q[NA], ds[NA];
+    bool any = false;
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        ds[a] = pair_distance(s.x, s.y, s.z, s.w, p[a][0], p[a][1], p[a][2], dx[a], dy[a], dz[a], q[a]);
+        acc.dmin[a] = fminf(acc.dmin[a], ds[a]);
+        any = any || (ds[a] <= r_d);
+    }
+    if (!FORCE) return;
+    if (CULL) { if (!__any_sync(mask, any)) return; }
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        float dO = fmaxf(ds[a], eps);
+        float sv = fmaf(dx[a], v[a][0], fmaf(dy[a], v[a][1], dz[a] * v[a][2]));
+        float w = sv * rcp_approx(dO * q[a]);
+        if (ds[a] <= r_d) {
+            acc.bx[a] = fmaf(w, dx[a], acc.bx[a]);
+            acc.by[a] = fmaf(w, dy[a], acc.by[a]);
+            acc.bz[a] = fmaf(w, dz[a], acc.bz[a]);
+        }
+    }
+}
+
+// moving spheres: centre advected to obstacle time tk, relative velocity per pair, force accumulated
+// directly:  f_j = w [ (s/|vr|) vr - |vr| d ],  w = s / (dO q),  s = d.vr   (k_f applied after the sum)
+template <int NA, bool FORCE, bool CULL>
+__device__ __forceinline__ void pair_moving(const float4 s, const float4 su, float tk,
+                                            const float (&p)[NA][3], const float (&v)[NA][3],
+                                            float r_d, float eps, unsigned mask, StaticAcc<NA>& acc) {
+    const float cx = fmaf(tk, su.x, s.x), cy = fmaf(tk, su.y, s.y), cz = fmaf(tk, su.z, s.z);
+    float dx[NA], dy[NA], dz[NA], q[NA], ds[NA];
+    bool any = false;
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        ds[a] = pair_distance(cx, cy, cz, s.w, p[a][0], p[a][1], p[a][2], dx[a], dy[a], dz[a], q[a]);
+        acc.dmin[a] = fminf(acc.dmin[a], ds[a]);
+        any = any || (ds[a] <= r_d);
+    }
+    if (!FORCE) return;
+    if (CULL) { if (!__any_sync(mask, any)) return; }
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        float vx = v[a][0] - su.x, vy = v[a][1] - su.y, vz = v[a][2] - su.z;
+        float n2 = fmaf(vx, vx, fmaf(vy, vy, fmaf(vz, vz, kTiny)));
+        float inv = rsqrt_approx(n2);
+        float nv = n2 * inv;
+        float dO = fmaxf(ds[a], eps);
+        float sv = fmaf(dx[a], vx, fmaf(dy[a], vy, dz[a] * vz));
+        float w = sv * rcp_approx(dO * q[a]);
+        float c1 = w * sv * inv, c2 = -w * nv;
+        if (ds[a] <= r_d) {
+            acc.bx[a] = fmaf(c1, vx, fmaf(c2, dx[a], acc.bx[a]));
+            acc.by[a] = fmaf(c1, vy, fmaf(c2, dy[a], acc.by[a]));
+            acc.bz[a] = fmaf(c1, vz, fmaf(c2, dz[a], acc.bz[a]));
+        }
+    }
+}
+
+// One lane's slice of the sphere sum for NA agents at obstacle time tk.
+template <int NA, bool MOVING, bool FORCE, bool CULL>
+__device__ __forceinline__ void sphere_sweep(const float4* __restrict__ sph, const float4* __restrict__ svel,
+                                             int n_pad, int lane, int L, float tk,
+                                             const float (&p)[NA][3], const float (&v)[NA][3],
+                                             float r_d, float eps, unsigned mask, StaticAcc<NA>& acc) {
+    constexpr int U = (NA == 1) ? 4 : 2;
+    int j = lane;
+    const int step = L * U;
+    for (; j + step - L < n_pad; j += step) {
+        float4 s[U], su[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) { s[u] = sph[j + u * L]; if (MOVING) su[u] = svel[j + u * L]; }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (MOVING) pair_moving<NA, FORCE, CULL>(s[u], su[u], tk, p, v, r_d, eps, mask, acc);
+            else        pair_static<NA, FORCE, CULL>(s[u], p, v, r_d, eps, mask, acc);
+        }
+    }
+    for (; j < n_pad; j += L) {
+        float4 s = sph[j];
+        if (MOVING) pair_moving<NA, FORCE, CULL>(s, svel[j], tk, p, v, r_d, eps, mask, acc);
+        else        pair_static<NA, FORCE, CULL>(s, p, v, r_d, eps, mask, acc);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// group all-reduce: sum of (bx,by,bz), min of dmin over the L lanes of a group; every lane gets the
+// result.  Fixed order -> deterministic; fp add is commutative so xor partners agree bitwise.
+// ---------------------------------------------------------------------------------------------
+template <int NA>
+__device__ __forceinline__ void group_allreduce(StaticAcc<NA>& acc, int L, int lane_in_group, int group_in_cta,
+                                                float* red, int parity, unsigned mask) {
+    const int wl = L < 32 ? L : 32;
+    for (int off = wl >> 1; off > 0; off >>= 1) {
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            acc.bx[a] += __shfl_xor_sync(mask, acc.bx[a], off);
+            acc.by[a] += __shfl_xor_sync(mask, acc.by[a], off);
+            acc.bz[a] += __shfl_xor_sync(mask, acc.bz[a], off);
+            acc.dmin[a] = fminf(acc.dmin[a], __shfl_xor_sync(mask, acc.dmin[a], off));
+        }
+    }
+    if (L > 32) {
+        // cross-warp exchange: red[parity][warp_in_cta][2 agents] float4; the group's warps are contiguous.
+        // Double-buffered by step parity so one named barrier per step is enough (a warp can run at most
+        // one barrier ahead of the slowest warp of its group).
+        const int W = L >> 5;
+        const int w0 = (group_in_cta * L) >> 5;
+        float4* base = reinterpret_cast<float4*>(red) + (parity * 32 + w0) * 2;
+        if ((lane_in_group & 31) == 0) {
+            const int wig = lane_in_group >> 5;
+#pragma unroll
+            for (int a = 0; a < NA; ++a)
+                base[wig * 2 + a] = make_float4(acc.bx[a], acc.by[a], acc.bz[a], acc.dmin[a]);
+        }
+        named_bar_sync(1 + group_in_cta, L);
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            float4 t = base[a];
+            for (int w = 1; w < W; ++w) {
+                float4 o = base[w * 2 + a];
+                t.x += o.x; t.y += o.y; t.z += o.z; t.w = fminf(t.w, o.w);
+            }
+            acc.bx[a] = t.x; acc.by[a] = t.y; acc.bz[a] = t.z; acc.dmin[a] = t.w;
+        }
+    }
+}
+
+// circular-field force from the reduced sums (static spheres): f_r = k_f [ ((B.v)/|v|) v - |v| B ]
+__device__ __forceinline__ void cf_force_static(float k_circ, float bx, float by, float bz,
+                                                float vx, float vy, float vz, float& fx, float& fy, float& fz) {
+    float n2 = fmaf(vx, vx, fmaf(vy, vy, fmaf(vz, vz, kTiny)));
+    float inv = rsqrt_approx(n2);
+    inv = inv * fmaf(-0.5f * n2 * inv, inv, 1.5f);        // Newton step: 1/|v| to ~1 ulp
+    float nv = n2 * inv;
+    float A = fmaf(bx, vx, fmaf(by, vy, bz * vz));
+    float c1 = k_circ * A * inv, c2 = -k_circ * nv;
+    fx = fmaf(c1, vx, c2 * bx); fy = fmaf(c1, vy, c2 * by); fz = fmaf(c1, vz, c2 * bz);
+}
+
+// ---------------------------------------------------------------------------------------------
+// cost accumulators (Eq. 16-20), kept by the first warp of a group
+// ---------------------------------------------------------------------------------------------
+struct CostAcc {
+    float sumG, sumO, sumV, sumJ, minclr, d1;
+    int collided;
+    __device__ __forceinline__ void init(float dg) {
+        sumG = sumO = sumV = sumJ = 0.0f; minclr = __int_as_float(0x7f800000); d1 = dg; collided = 0;
+    }
+    // one pose: Eq. 17 / 18 summands, clearance and collision record
+    __device__ __forceinline__ void pose(float dg, float dmin, float rcg, float rco) {
+        sumG += fminf(dg, rcg);
+        sumO += fminf(fmaxf(dmin, 0.0f), rco);
+        minclr = fminf(minclr, dmin);
+        collided |= (dmin < 0.0f) ? 1 : 0;
+    }
+    __device__ __forceinline__ void finish(const RolloutParams& P, float L_path, float J, float* out5) const {
+        const float Nk = float(P.steps) + 1.0f;
+        float Cg = sumG / (P.rcg * Nk);
+        float Co = 1.0f - sumO / (P.rco * Nk);
+        float Cp;
+        if (L_path == 0.0f && d1 == 0.0f) Cp = 0.0f;
+        else if (L_path >= d1) Cp = 1.0f - d1 / L_path;
+        else Cp = 1.0f - L_path / d1;
+        float dt2 = P.dt * P.dt;
+        float Cs = fminf(1.0f, J / (Nk * dt2 * dt2 * P.a_max * P.a_max));
+        out5[0] = P.w_goal * Cg + P.w_obs * Co + P.w_path * Cp + P.w_smooth * Cs;
+        out5[1] = Cg; out5[2] = Co; out5[3] = Cp; out5[4] = Cs;
+    }
+};
+
+__device__ __forceinline__ float norm3f(float x, float y, float z) {
+    float n2 = fmaf(x, x, fmaf(y, y, fmaf(z, z, kTiny)));
+    float inv;
+    float n = sqrt_refined(n2, inv);
+    return n2 <= kTiny ? 0.0f : n;
+}
+
+// ---------------------------------------------------------------------------------------------
+// 3D point agents
+// ---------------------------------------------------------------------------------------------
+template <int NA, bool MOVING, bool CULL>
+__device__ __forceinline__ void rollout_point3(const RolloutParams& P, const float4* sph, const float4* svel,
+                                               int first_agent, int lane_in_group, int group_in_cta, float* red) {
+    const unsigned mask = __activemask();      // lanes of this warp on this code path (sub-warp groups may differ)
+    float p[NA][3], v[NA][3];
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        const float* s = P.agents_in + 6 * size_t(first_agent + a);
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { p[a][i] = s[i]; v[a][i] = s[3 + i]; }
+    }
+    const bool cost_warp = lane_in_group < 32;
+    CostAcc ca[NA];
+    float ap[NA][3];                                      // previous acceleration (Eq. 20 via differences of a)
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        ca[a].init(norm3f(P.goal[0] - p[a][0], P.goal[1] - p[a][1], P.goal[2] - p[a][2]));
+        ap[a][0] = ap[a][1] = ap[a][2] = 0.0f;
+    }
+    StaticAcc<NA> acc;
+    for (int k = 0; k < P.steps; ++k) {
+        const float tk = float(k) * P.dt;
+        acc.clear();
+        sphere_sweep<NA, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, mask, acc);
+        group_allreduce<NA>(acc, P.L, lane_in_group, group_in_cta, red, k & 1, mask);
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            float ex = P.goal[0] - p[a][0], ey = P.goal[1] - p[a][1], ez = P.goal[2] - p[a][2];
+            float fx, fy, fz;
+            if (MOVING) { fx = P.k_circ * acc.bx[a]; fy = P.k_circ * acc.by[a]; fz = P.k_circ * acc.bz[a]; }
+            else cf_force_static(P.k_circ, acc.bx[a], acc.by[a], acc.bz[a], v[a][0], v[a][1], v[a][2], fx, fy, fz);
+            fx = fmaf(P.k_att, ex, fmaf(-P.k_damp, v[a][0], fx));      // Eq. 6-7
+            fy = fmaf(P.k_att, ey, fmaf(-P.k_damp, v[a][1], fy));
+            fz = fmaf(P.k_att, ez, fmaf(-P.k_damp, v[a][2], fz));
+            if (cost_warp) {
+                ca[a].pose(norm3f(ex, ey, ez), acc.dmin[a], P.rcg, P.rco);
+                if (k >= 2) {                                          // third difference = vf dt^2 (a_k - a_{k-1})
+                    float jx = fx - ap[a][0], jy = fy - ap[a][1], jz = fz - ap[a][2];
+                    ca[a].sumJ += fmaf(jx, jx, fmaf(jy, jy, jz * jz));
+                }
+                ap[a][0] = fx; ap[a][1] = fy; ap[a][2] = fz;
+            }
+            v[a][0] = fmaf(P.c_lin, fx, v[a][0]);                      // Eq. 9-10
+            v[a][1] = fmaf(P.c_lin, fy, v[a][1]);
+            v[a][2] = fmaf(P.c_lin, fz, v[a][2]);
+            p[a][0] = fmaf(P.dt, v[a][0], p[a][0]);                    // Eq. 11 (point mass)
+            p[a][1] = fmaf(P.dt, v[a][1], p[a][1]);
+            p[a][2] = fmaf(P.dt, v[a][2], p[a][2]);
+            if (cost_warp) ca[a].sumV += norm3f(v[a][0], v[a][1], v[a][2]);   // |p_new - p| = dt |v|
+        }
+    }
+    // final pose: distance-only pass
+    acc.clear();
+    sphere_sweep<NA, MOVING, false, false>(sph, svel, P.n_pad, lane_in_group, P.L, float(P.steps) * P.dt, p, v,
+                                           P.r_d, P.eps, mask, acc);
+    group_allreduce<NA>(acc, P.L, lane_in_group, group_in_cta, red, P.steps & 1, mask);
+    if (lane_in_group == 0) {
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            const int i = first_agent + a;
+            ca[a].pose(norm3f(P.goal[0] - p[a][0], P.goal[1] - p[a][1], P.goal[2] - p[a][2]), acc.dmin[a], P.rcg, P.rco);
+            // sumJ holds sum |f_k - f_{k-1}|^2; a = inv_mass f; third difference = vel_factor dt^2 (a_k - a_{k-1})
+            float cj = P.vel_factor * P.dt * P.dt * P.inv_mass;
+            ca[a].finish(P, P.dt * ca[a].sumV, cj * cj * ca[a].sumJ, P.cost + 5 * size_t(i));
+            P.minclr[i] = ca[a].minclr;
+            P.collided[i] = ca[a].collided;
+            if (P.agents_out) {
+                float* o = P.agents_out + 6 * size_t(i);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { o[c] = p[a][c]; o[3 + c] = v[a][c]; }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// 6D pose agents (8-float motor + 6-float body twist), one agent per group
+// ---------------------------------------------------------------------------------------------
+struct Pose6 { Quat r, d; Vec3 w, nu; };
+
+__device__ __forceinline__ Pose6 load_pose6(const float* s) {
+    Pose6 x;
+    x.r = Quat{s[0], s[1], s[2], s[3]}; x.d = Quat{s[4], s[5], s[6], s[7]};
+    x.w = v3(s[8], s[9], s[10]); x.nu = v3(s[11], s[12], s[13]);
+    motor_normalise(x.r, x.d);
+    return x;
+}
+
+// body wrench (Eq. 6-8): tau = k_ar e_w - k_dr w;  f = k_att e_v - k_damp nu + R^T f_r
+__device__ __forceinline__ void pose6_wrench(const RolloutParams& P, const Pose6& x, Vec3 pos, Quat rg, Vec3 pg,
+                                             Vec3 f_r_world, Vec3& tau, Vec3& f) {
+    Quat qrel = qmul(qconj(x.r), rg);
+    Vec3 trel = qrot_inv(x.r, pg - pos);
+    Vec3 ew, ev;
+    se3_log_from_quat(qrel, trel, ew, ev);
+    Vec3 fb = qrot_inv(x.r, f_r_world);
+    tau = fma3(P.k_att_rot, ew, (-P.k_damp_rot) * x.w);
+    f = fma3(P.k_att, ev, fma3(-P.k_damp, x.nu, fb));
+}
+
+template <bool MOVING, bool CULL>
+__device__ __forceinline__ void rollout_pose6(const RolloutParams& P, const float4* sph, const float4* svel,
+                                              int agent, int lane_in_group, int group_in_cta, float* red) {
+    const unsigned mask = __activemask();
+    Pose6 x = load_pose6(P.agents_in + 14 * size_t(agent));
+    Quat rg = Quat{P.goal[0], P.goal[1], P.goal[2], P.goal[3]}, dg = Quat{P.goal[4], P.goal[5], P.goal[6], P.goal[7]};
+    motor_normalise(rg, dg);
+    const Vec3 pg = motor_translation(rg, dg);
+    const bool cost_warp = lane_in_group < 32;
+    CostAcc ca;
+    Vec3 pos = motor_translation(x.r, x.d);
+    ca.init(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z));
+    Vec3 dp1 = v3(0, 0, 0), dp2 = v3(0, 0, 0);            // previous two world displacements (Eq. 20)
+    float sumL = 0.0f;
+    StaticAcc<1> acc;
+    float p[1][3], v[1][3];
+    for (int k = 0; k < P.steps; ++k) {
+        const float tk = float(k) * P.dt;
+        pos = motor_translation(x.r, x.d);
+        Vec3 pdot = qrot(x.r, x.nu);                      // world linear velocity of the body origin
+        p[0][0] = pos.x; p[0][1] = pos.y; p[0][2] = pos.z;
+        v[0][0] = pdot.x; v[0][1] = pdot.y; v[0][2] = pdot.z;
+        acc.clear();
+        sphere_sweep<1, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, mask, acc);
+        group_allreduce<1>(acc, P.L, lane_in_group, group_in_cta, red, k & 1, mask);
+        Vec3 fr;
+        if (MOVING) fr = P.k_circ * v3(acc.bx[0], acc.by[0], acc.bz[0]);
+        else cf_force_static(P.k_circ, acc.bx[0], acc.by[0], acc.bz[0], pdot.x, pdot.y, pdot.z, fr.x, fr.y, fr.z);
+        if (cost_warp) ca.pose(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z), acc.dmin[0], P.rcg, P.rco);
+        Vec3 tau, f;
+        pose6_wrench(P, x, pos, rg, pg, fr, tau, f);
+        x.w = fma3(P.c_rot, tau, x.w);                    // Eq. 9-10
+        x.nu = fma3(P.c_lin, f, x.nu);
+        Quat rd, dd; Vec3 td;
+        se3_exp_motor(P.dt * x.w, P.dt * x.nu, rd, dd, td);           // Eq. 11: M <- M exp(dt v)
+        if (cost_warp) {
+            Vec3 dp = qrot(x.r, td);                      // world displacement p_new - p
+            sumL += norm3f(td.x, td.y, td.z);
+            if (k >= 2) {
+                Vec3 t3 = dp - 2.0f * dp1 + dp2;          // p4 - 3 p3 + 3 p2 - p1 from displacements
+                ca.sumJ += dot(t3, t3);
+            }
+            dp2 = dp1; dp1 = dp;
+        }
+        Quat rn = qmul(x.r, rd);
+        Quat a1 = qmul(x.r, dd), a2 = qmul(x.d, rd);
+        x.r = rn;
+        x.d = Quat{a1.w + a2.w, a1.x + a2.x, a1.y + a2.y, a1.z + a2.z};
+        motor_normalise(x.r, x.d);
+    }
+    pos = motor_translation(x.r, x.d);
+    p[0][0] = pos.x; p[0][1] = pos.y; p[0][2] = pos.z;
+    v[0][0] = v[0][1] = v[0][2] = 0.0f;
+    acc.clear();
+    sphere_sweep<1, MOVING, false, false>(sph, svel, P.n_pad, lane_in_group, P.L, float(P.steps) * P.dt, p, v,
+                                          P.r_d, P.eps, mask, acc);
+    group_allreduce<1>(acc, P.L, lane_in_group, group_in_cta, red, P.steps & 1, mask);
+    if (lane_in_group == 0) {
+        ca.pose(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z), acc.dmin[0], P.rcg, P.rco);
+        ca.finish(P, sumL, ca.sumJ, P.cost + 5 * size_t(agent));
+        P.minclr[agent] = ca.minclr;
+        P.collided[agent] = ca.collided;
+        if (P.agents_out) {
+            float* o = P.agents_out + 14 * size_t(agent);
+            o[0] = x.r.w; o[1] = x.r.x; o[2] = x.r.y; o[3] = x.r.z;
+            o[4] = x.d.w; o[5] = x.d.x; o[6] = x.d.y; o[7] = x.d.z;
+            o[8] = x.w.x; o[9] = x.w.y; o[10] = x.w.z; o[11] = x.nu.x; o[12] = x.nu.y; o[13] = x.nu.z;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// the persistent rollout kernel: one launch per planning cycle
+// ---------------------------------------------------------------------------------------------
+template <int KIND, int AT, bool MOVING, bool CULL, int STAGE, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) k_rollout(const __grid_constant__ RolloutParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
+    float* red = reinterpret_cast<float*>(smem_raw + P.red_off);
+    const float4* sph = P.sph;
+    const float4* svel = P.svel;
+    const int tid = threadIdx.x;
+    if (STAGE == 1) {
+        float4* tile = reinterpret_cast<float4*>(smem_raw + P.tile_off);
+        if (tid == 0) { mbar_init(bar, 1); fence_mbar_init(); }
+        __syncthreads();
+        if (tid == 0) {
+            const uint32_t bytes = uint32_t(P.n_pad) * 16u;
+            mbar_arrive_expect_tx(bar, MOVING ? 2u * bytes : bytes);
+            const uint32_t chunk = 32768u;
+            for (uint32_t o = 0; o < bytes; o += chunk) {
+                uint32_t nb = bytes - o < chunk ? bytes - o : chunk;
+                tma_bulk_g2s(reinterpret_cast<unsigned char*>(tile) + o,
+                             reinterpret_cast<const unsigned char*>(P.sph) + o, nb, bar);
+                if (MOVING)
+                    tma_bulk_g2s(reinterpret_cast<unsigned char*>(tile) + bytes + o,
+                                 reinterpret_cast<const unsigned char*>(P.svel) + o, nb, bar);
+            }
+        }
+        sph = tile;
+        svel = tile + P.n_pad;
+    }
+    const int group_in_cta = tid >> P.logL;
+    const int lane_in_group = tid & (P.L - 1);
+    const int cta_first = blockIdx.x * P.agents_per_cta;
+    int cta_end = cta_first + P.agents_per_cta;
+    if (cta_end > P.n_agents) cta_end = P.n_agents;
+    const int first = cta_first + group_in_cta * AT;
+    int na = cta_end - first;
+    if (STAGE == 1) mbar_wait(bar, 0);
+    if (na <= 0) return;
+    if (KIND == 0) {
+        if (AT == 2 && na >= 2) rollout_point3<(AT == 2 ? 2 : 1), MOVING, CULL>(P, sph, svel, first, lane_in_group, group_in_cta, red);
+        else rollout_point3<1, MOVING, CULL>(P, sph, svel, first, lane_in_group, group_in_cta, red);
+    } else {
+        rollout_pose6<MOVING, CULL>(P, sph, svel, first, lane_in_group, group_in_cta, red);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// force query (no integration): warp per agent, spheres from global / L2
+// ---------------------------------------------------------------------------------------------
+struct ForceParams {
+    const float4* sph; const float4* svel; int n_pad;
+    const float* agents; int n_agents; int kind;
+    float goal[8];
+    float k_circ, k_att, k_damp, k_att_rot, k_damp_rot, r_d, eps, t_obs;
+    float* f_rep; float* f_total;
+};
+
+template <bool MOVING>
+__global__ void __launch_bounds__(256) k_forces(const __grid_constant__ ForceParams P) {
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (warp >= P.n_agents) return;
+    float p[1][3], v[1][3];
+    Pose6 x;
+    Vec3 pos;
+    if (P.kind == 0) {
+        const float* s = P.agents + 6 * size_t(warp);
+        for (int i = 0; i < 3; ++i) { p[0][i] = s[i]; v[0][i] = s[3 + i]; }
+    } else {
+        x = load_pose6(P.agents + 14 * size_t(warp));
+        pos = motor_translation(x.r, x.d);
+        Vec3 pdot = qrot(x.r, x.nu);
+        p[0][0] = pos.x; p[0][1] = pos.y; p[0][2] = pos.z;
+        v[0][0] = pdot.x; v[0][1] = pdot.y; v[0][2] = pdot.z;
+    }
+    StaticAcc<1> acc;
+    acc.clear();
+    sphere_sweep<1, MOVING, true, false>(P.sph, P.svel, P.n_pad, lane, 32, P.t_obs, p, v, P.r_d, P.eps, 0xffffffffu, acc);
+    group_allreduce<1>(acc, 32, lane, 0, nullptr, 0, 0xffffffffu);
+    Vec3 fr;
+    if (MOVING) fr = P.k_circ * v3(acc.bx[0], acc.by[0], acc.bz[0]);
+    else cf_force_static(P.k_circ, acc.bx[0], acc.by[0], acc.bz[0], v[0][0], v[0][1], v[0][2], fr.x, fr.y, fr.z);
+    if (lane != 0) return;
+    if (P.f_rep) { float* o = P.f_rep + 3 * size_t(warp); o[0] = fr.x; o[1] = fr.y; o[2] = fr.z; }
+    if (P.f_total) {
+        if (P.kind == 0) {
+            float* o = P.f_total + 3 * size_t(warp);
+            for (int i = 0; i < 3; ++i)
+                o[i] = fmaf(P.k_att, P.goal[i] - p[0][i], fmaf(-P.k_damp, v[0][i], i == 0 ? fr.x : (i == 1 ? fr.y : fr.z)));
+        } else {
+            Quat rg = Quat{P.goal[0], P.goal[1], P.goal[2], P.goal[3]}, dg = Quat{P.goal[4], P.goal[5], P.goal[6], P.goal[7]};
+            motor_normalise(rg, dg);
+            Vec3 pg = motor_translation(rg, dg);
+            RolloutParams R{};
+            R.k_att = P.k_att; R.k_damp = P.k_damp; R.k_att_rot = P.k_att_rot; R.k_damp_rot = P.k_damp_rot;
+            Vec3 tau, f;
+            pose6_wrench(R, x, pos, rg, pg, fr, tau, f);
+            float* o = P.f_total + 6 * size_t(warp);
+            o[0] = tau.x; o[1] = tau.y; o[2] = tau.z; o[3] = f.x; o[4] = f.y; o[5] = f.z;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// obstacle packing: (xyz, r) [+ vel] -> float4 arrays, R = r + r_a, sentinel padding to n_cap
+// ---------------------------------------------------------------------------------------------
+__global__ void k_pack_spheres(const float* __restrict__ xyzr, const float* __restrict__ vel, int n, int n_cap,
+                               float r_agent, float4* __restrict__ sph, float4* __restrict__ svel) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_cap) return;
+    if (i < n) {
+        sph[i] = make_float4(xyzr[4 * i], xyzr[4 * i + 1], xyzr[4 * i + 2], xyzr[4 * i + 3] + r_agent);
+        svel[i] = vel ? make_float4(vel[3 * i], vel[3 * i + 1], vel[3 * i + 2], 0.0f) : make_float4(0, 0, 0, 0);
+    } else {
+        // sentinel: far away (|d|^2 ~ 3e36 stays finite in FP32), never gated, never the minimum
+        sph[i] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f);
+        svel[i] = make_float4(0, 0, 0, 0);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// selection: lexicographic argmin of (collided, C, index) + hysteresis
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool key_less(int ca, float Ca, int ia, int cb, float Cb, int ib) {
+    if (ca != cb) return ca < cb;
+    if (Ca != Cb) return Ca < Cb;
+    return ia < ib;
+}
+
+__global__ void __launch_bounds__(1024) k_best_agent(const float* __restrict__ cost5, const int* __restrict__ collided,
+                                                     int n, float alpha, int prev_best, int* out_idx, float* out_cost) {
+    __shared__ int s_c[32]; __shared__ float s_C[32]; __shared__ int s_i[32];
+    int bc = 2, bi = 0x7fffffff; float bC = __int_as_float(0x7f800000);
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        float C = cost5[5 * size_t(i)]; int c = collided[i] ? 1 : 0;
+        if (C != C) { C = __int_as_float(0x7f800000); c = 1; }
+        if (key_less(c, C, i, bc, bC, bi)) { bc = c; bC = C; bi = i; }
+    }
+    for (int off = 16; off > 0; off >>= 1) {
+        int oc = __shfl_xor_sync(0xffffffffu, bc, off);
+        float oC = __shfl_xor_sync(0xffffffffu, bC, off);
+        int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+        if (key_less(oc, oC, oi, bc, bC, bi)) { bc = oc; bC = oC; bi = oi; }
+    }
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) { s_c[w] = bc; s_C[w] = bC; s_i[w] = bi; }
+    __syncthreads();
+    if (w == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        bc = l < nw ? s_c[l] : 2; bC = l < nw ? s_C[l] : __int_as_float(0x7f800000); bi = l < nw ? s_i[l] : 0x7fffffff;
+        for (int off = 16; off > 0; off >>= 1) {
+            int oc = __shfl_xor_sync(0xffffffffu, bc, off);
+            float oC = __shfl_xor_sync(0xffffffffu, bC, off);
+            int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+            if (key_less(oc, oC, oi, bc, bC, bi)) { bc = oc; bC = oC; bi = oi; }
+        }
+        if (l == 0) {
+            if (n > 0 && prev_best >= 0 && prev_best < n && prev_best != bi) {
+                float Cp = cost5[5 * size_t(prev_best)]; int cp = collided[prev_best] ? 1 : 0;
+                if (Cp != Cp) { Cp = __int_as_float(0x7f800000); cp = 1; }
+                bool improves = (bc < cp) || (bc == cp && bC < alpha * Cp);
+                if (!improves) { bi = prev_best; bC = Cp; }
+            }
+            *out_idx = n > 0 ? bi : -1;
+            *out_cost = n > 0 ? bC : __int_as_float(0x7fc00000);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// FP32 peak microkernel: 8 independent FMA chains per thread, register only
+// ---------------------------------------------------------------------------------------------
+template <bool X2>
+__global__ void __launch_bounds__(256) k_fma_peak(float* out, int iters, float a, float b) {
+    float x[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = float(threadIdx.x + i) * 1e-3f;
+    if (X2) {
+        unsigned long long X[8], A, Bv;
+        asm("mov.b64 %0, {%1, %2};" : "=l"(A) : "f"(a), "f"(a));
+        asm("mov.b64 %0, {%1, %2};" : "=l"(Bv) : "f"(b), "f"(b));
+#pragma unroll
+        for (int i = 0; i < 8; ++i) asm("mov.b64 %0, {%1, %2};" : "=l"(X[i]) : "f"(x[2 * i]), "f"(x[2 * i + 1]));
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int i = 0; i < 8; ++i) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(X[i]) : "l"(A), "l"(Bv));
+        }
+#pragma unroll
+        for (int i = 0; i < 8; ++i) asm("mov.b64 {%0, %1}, %2;" : "=f"(x[2 * i]), "=f"(x[2 * i + 1]) : "l"(X[i]));
+    } else {
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int i = 0; i < 16; ++i) x[i] = fmaf(x[i], a, b);
+        }
+    }
+    float s = 0.0f;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += x[i];
+    if (s == 123.456f) out[0] = s;      // never true in practice; keeps the chains alive
+}
+
+}  // namespace gmapp

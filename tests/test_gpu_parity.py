@@ -1,0 +1,365 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the FP64 oracle on the
+same seeded inputs.  Tolerances are north_star's (BASELINE.json):
+  * per-step forces within 1e-5 relative (denominator ||f_a|| + sum_j ||f_j||, reading G29), waived
+    where the oracle's gate margin is below 1e-6 (reading G10);
+  * positions within 1e-4 m after 100 steps (and at the final step); 6D: rotation within 1e-4 rad;
+  * collision flags and the selected best agent exact, except where the oracle's clearance / cost gap
+    is below 1e-6 relative;
+  * costs within 1e-5 absolute (they are normalised to [0,1]); C_smooth of the 6D path within 1e-3.
+"""
+import numpy as np
+import pytest
+
+from paper_2606_12579_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+POS_TOL = 1e-4
+ANG_TOL = 1e-4
+COST_TOL = 1e-5
+FORCE_RTOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def api():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2606_12579_b200 import api as _api      # raises if libgmapp.so is missing: no fallback
+    return _api
+
+
+@pytest.fixture(scope="module")
+def ctx(api):
+    c = api.Context(max_agents=16384, max_spheres=65536)
+    yield c
+    c.close()
+
+
+def _quat_to_R(q):
+    q = np.asarray(q, np.float64); q = q / np.linalg.norm(q, axis=-1, keepdims=True)
+    w, x, y, z = q[..., 0], q[..., 1], q[..., 2], q[..., 3]
+    R = np.stack([1 - 2 * (y * y + z * z), 2 * (x * y - w * z), 2 * (x * z + w * y),
+                  2 * (x * y + w * z), 1 - 2 * (x * x + z * z), 2 * (y * z - w * x),
+                  2 * (x * z - w * y), 2 * (y * z + w * x), 1 - 2 * (x * x + y * y)], axis=-1)
+    return R.reshape(q.shape[:-1] + (3, 3))
+
+
+def _rot_angle(Ra, Rb):
+    M = np.einsum("...ji,...jk->...ik", Ra, Rb)
+    vee = 0.5 * np.stack([M[..., 2, 1] - M[..., 1, 2], M[..., 0, 2] - M[..., 2, 0], M[..., 1, 0] - M[..., 0, 1]], -1)
+    c = 0.5 * (np.trace(M, axis1=-2, axis2=-1) - 1)
+    return np.arctan2(np.linalg.norm(vee, axis=-1), c)
+
+
+def _check_best(g, o, orc, scene):
+    """Best index exact unless the oracle's cost gap between the two candidates is below 1e-6 relative."""
+    want, want_cost = orc.best_agent(o["cost"], o["collided"], scene.alpha, scene.prev_best)
+    if g["best"] != want:
+        cg = o["cost"][g["best"], 0]
+        assert o["collided"][g["best"]] == o["collided"][want]
+        assert abs(cg - want_cost) <= 1e-6 * abs(want_cost), (g["best"], want, cg, want_cost)
+    assert abs(g["best_cost"] - o["cost"][g["best"], 0]) <= COST_TOL
+
+
+def _check_rollout(api, ctx, orc, scene, tuning=None, agent_idx=None, smooth_tol=COST_TOL):
+    """Full rollout parity.  agent_idx: compare only these agents (oracle runs on the sample, P12)."""
+    g = api.run_scene(ctx, scene, tuning=tuning)
+    sl = slice(None) if agent_idx is None else agent_idx
+    o = orc.rollout_scene(scene, threads=8, agent_slice=sl)
+    if scene.kind == scenes.KIND_POINT3:
+        gf = g["final"][sl].astype(np.float64)
+        assert np.abs(gf[:, :3] - o["final"][:, :3]).max() <= POS_TOL
+        assert np.abs(gf[:, 3:] - o["final"][:, 3:]).max() <= 1e-3
+    else:
+        q, t, tw = api.state14_to_pose(g["final"][sl])
+        assert np.abs(t - o["p"]).max() <= POS_TOL
+        assert _rot_angle(o["R"], _quat_to_R(q)).max() <= ANG_TOL
+        assert np.abs(tw - o["twist"]).max() <= 1e-3
+        assert np.abs(np.linalg.norm(q, axis=1) - 1).max() < 1e-5
+    gc = g["cost"][sl].astype(np.float64)
+    assert np.abs(gc[:, 1:4] - o["cost"][:, 1:4]).max() <= COST_TOL
+    assert np.abs(gc[:, 4] - o["cost"][:, 4]).max() <= smooth_tol
+    assert np.abs(gc[:, 0] - o["cost"][:, 0]).max() <= 3 * COST_TOL + smooth_tol
+    # clearance and collision flags: exact unless |clearance| margin is tiny (1e-6 relative to r_d)
+    clr_g, clr_o = g["min_clearance"][sl].astype(np.float64), o["min_clearance"]
+    fin = np.isfinite(clr_o)
+    assert np.array_equal(np.isfinite(clr_g), fin)
+    assert np.abs(clr_g[fin] - clr_o[fin]).max(initial=0) <= 2e-6
+    waive = o["margins"][:, 2] < 1e-6 * scene.gains["r_influence"]
+    assert np.array_equal(g["collided"][sl][~waive], o["collided"][~waive])
+    if agent_idx is None:
+        _check_best(g, o, orc, scene)
+    return g, o
+
+
+def _tensor(a, dev="cuda:0"):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+
+
+def _check_forces_on_oracle_states(api, ctx, orc, scene, step_ids, n_agents=None):
+    """gmapp_forces at the ORACLE's states of selected steps vs the oracle's forces there."""
+    import torch
+    sl = slice(0, n_agents)
+    o = orc.rollout_scene(scene, threads=8, want_traj=True, agent_slice=sl)
+    ctx.set_obstacles(_tensor(scene.xyzr), None if scene.vel is None else _tensor(scene.vel), n=scene.n_spheres)
+    worst, n_waived, n_tot = 0.0, 0, 0
+    for k in step_ids:
+        t_obs = float(np.float32(k) * np.float32(scene.dt))
+        if scene.kind == scenes.KIND_POINT3:
+            st = o["traj"][:, k]                                        # [n,6] float64
+            st32 = st.astype(np.float32)
+            ref = orc.forces_point3(st32.astype(np.float64), scene.xyzr, scene.vel, scene.goal, scene.gains, t_obs)
+            d_st = _tensor(st32)
+            f_rep = torch.empty((st.shape[0], 3), device="cuda:0"); f_tot = torch.empty_like(f_rep)
+            ctx.forces(api.GMAPP_POINT3, d_st, scene.goal, scene.gains, t_obs, f_rep, f_tot)
+            ref_tot = ref["f_total"]
+        else:
+            tr = o["traj"][:, k]                                        # [n,18] = R, p, twist
+            R = tr[:, :9].reshape(-1, 3, 3)
+            # a float32 motor cannot hold the float64 pose exactly: build the FP32 state, then give the
+            # oracle exactly that state back (converted by the binding's inverse helper)
+            quat = _R_to_quat(R)
+            st14 = api.pose_to_state14(quat, tr[:, 9:12], tr[:, 12:18])
+            q2, p2, tw2 = api.state14_to_pose(st14)
+            ref = orc.forces_pose6(_quat_to_R(q2), p2, tw2, scene.xyzr, scene.vel, scene.goal_quat, scene.goal,
+                                   scene.gains, t_obs)
+            goal8 = api.pose_to_state14(scene.goal_quat, scene.goal, np.zeros(6))[0, :8]
+            d_st = _tensor(st14)
+            f_rep = torch.empty((st14.shape[0], 3), device="cuda:0")
+            f_tot = torch.empty((st14.shape[0], 6), device="cuda:0")
+            ctx.forces(api.GMAPP_MOTOR6, d_st, goal8, scene.gains, t_obs, f_rep, f_tot)
+            ref_tot = ref["wrench"]
+        torch.cuda.synchronize()
+        ok = ref["margins"][:, 0] >= 1e-6                               # gate margin waiver (G10)
+        n_waived += int((~ok).sum()); n_tot += ok.size
+        scale = ref["scale"] + 1e-30
+        e_rep = np.linalg.norm(f_rep.cpu().numpy().astype(np.float64) - ref["f_rep"], axis=1) / scale
+        e_tot = np.linalg.norm(f_tot.cpu().numpy().astype(np.float64) - ref_tot, axis=1) / scale
+        worst = max(worst, e_rep[ok].max(initial=0), e_tot[ok].max(initial=0))
+    assert n_waived <= 0.01 * n_tot + 2
+    assert worst <= FORCE_RTOL, worst
+    return worst
+
+
+def _R_to_quat(R):
+    """Rotation matrices -> unit quaternions (w >= 0), test-side helper (Shepperd's method)."""
+    R = np.asarray(R, np.float64).reshape(-1, 3, 3)
+    q = np.zeros((R.shape[0], 4))
+    for i, M in enumerate(R):
+        tr = np.trace(M)
+        if tr > 0:
+            s = np.sqrt(tr + 1.0) * 2; q[i] = [0.25 * s, (M[2, 1] - M[1, 2]) / s, (M[0, 2] - M[2, 0]) / s, (M[1, 0] - M[0, 1]) / s]
+        else:
+            j = int(np.argmax(np.diag(M))); k, l = (j + 1) % 3, (j + 2) % 3
+            s = np.sqrt(1.0 + M[j, j] - M[k, k] - M[l, l]) * 2
+            v = np.zeros(3); v[j] = 0.25 * s; v[k] = (M[k, j] + M[j, k]) / s; v[l] = (M[l, j] + M[j, l]) / s
+            q[i] = [(M[l, k] - M[k, l]) / s, *v]
+        if q[i, 0] < 0:
+            q[i] = -q[i]
+    return q
+
+
+# ---------------------------------------------------------------------------------- configs 1-4
+def test_config1_tiny(api, ctx, orc):
+    g, o = _check_rollout(api, ctx, orc, scenes.config1())
+    assert g["info"]["kernels_launched"] == 1
+
+
+def test_config2_single_arm(api, ctx, orc):
+    _check_rollout(api, ctx, orc, scenes.config2())
+
+
+def test_config2_position_after_100_steps(api, ctx, orc):
+    sc = scenes.config2(steps=100)
+    _check_rollout(api, ctx, orc, sc)
+
+
+def test_config2_literal_draw_without_keepout(api, ctx, orc):
+    _check_rollout(api, ctx, orc, scenes.config2(keepout=False))
+
+
+def test_config3_dense_clutter(api, ctx, orc):
+    g, o = _check_rollout(api, ctx, orc, scenes.config3())
+    assert g["info"]["stage"] == 1 and g["info"]["grid"] >= 140       # one wave over the SMs, spheres in smem
+
+
+def test_config4_pose6_moving(api, ctx, orc):
+    _check_rollout(api, ctx, orc, scenes.config4(), smooth_tol=1e-3)
+
+
+def test_config4_position_after_100_steps(api, ctx, orc):
+    _check_rollout(api, ctx, orc, scenes.config4(steps=100), smooth_tol=1e-3)
+
+
+@pytest.mark.parametrize("na,ns", [(1024, 4096), (4096, 16384), (16384, 65536)])
+def test_config5_sweep_sampled_agents(api, ctx, orc, na, ns):
+    # stress sizes: the oracle runs on a random sample of agents over all spheres (independence, P12)
+    sc = scenes.config5(na, ns, steps=100 if ns > 4096 else 200)
+    idx = np.sort(np.random.default_rng(7).choice(na, 24, replace=False))
+    _check_rollout(api, ctx, orc, sc, agent_idx=idx)
+
+
+# ---------------------------------------------------------------------------------- exercised force model
+@pytest.mark.parametrize("moving", [False, True], ids=["static", "moving"])
+def test_fast_clutter_rollout(api, ctx, orc, moving):
+    g, o = _check_rollout(api, ctx, orc, scenes.fast_clutter(moving=moving))
+    assert (o["cost"][:, 2] > 0).sum() > 20                           # the field really acted
+
+
+def test_fast_clutter_with_collisions(api, ctx, orc):
+    sc = scenes.fast_clutter(n_agents=160, n_spheres=500, r_lo=0.02, r_hi=0.07, steps=150)
+    sc.gains["r_agent"] = 0.01
+    g, o = _check_rollout(api, ctx, orc, sc)
+    assert 0 < o["collided"].sum() < sc.n_agents                       # both flag values occur
+
+
+@pytest.mark.parametrize("moving", [False, True], ids=["static", "moving"])
+def test_per_step_forces_point3(api, ctx, orc, moving):
+    sc = scenes.fast_clutter(moving=moving, n_agents=128, n_spheres=700)
+    _check_forces_on_oracle_states(api, ctx, orc, sc, [0, 20, 40, 60, 80, 100])
+
+
+def test_per_step_forces_config3(api, ctx, orc):
+    _check_forces_on_oracle_states(api, ctx, orc, scenes.config3(), [0, 50, 100], n_agents=96)
+
+
+def test_per_step_forces_pose6(api, ctx, orc):
+    _check_forces_on_oracle_states(api, ctx, orc, scenes.config4(n_agents=64, steps=120), [0, 40, 80, 120])
+
+
+def test_pose6_large_rotation_fast_twist(api, ctx, orc):
+    # orientation errors up to pi and angular rates of several rad/s exercise the log/exp branches
+    sc = scenes.config4(n_agents=48, n_spheres=300, steps=200)
+    rng = np.random.default_rng(11)
+    sc.twist[:, :3] = rng.normal(0, 3.0, (48, 3)).astype(np.float32)
+    sc.quat[0] = np.array([0.0, 1.0, 0.0, 0.0], np.float32)            # exactly pi from the goal
+    sc.quat[1] = np.array([1.0, 0.0, 0.0, 0.0], np.float32)            # already aligned
+    _check_rollout(api, ctx, orc, sc, smooth_tol=1e-3)
+
+
+# ---------------------------------------------------------------------------------- launch variants
+@pytest.mark.parametrize("tuning", [
+    dict(lanes_per_agent=8, agents_per_thread=1), dict(lanes_per_agent=32, agents_per_thread=1),
+    dict(lanes_per_agent=32, agents_per_thread=2), dict(lanes_per_agent=128, agents_per_thread=2),
+    dict(lanes_per_agent=256, agents_per_thread=1), dict(lanes_per_agent=64, agents_per_thread=2, cull=1),
+    dict(lanes_per_agent=16, agents_per_thread=2, cull=1, stage=0), dict(stage=0), dict(cull=1),
+    dict(max_ctas=5), dict(max_ctas=5, cull=1, agents_per_thread=1),
+], ids=lambda t: "-".join(f"{k[:4]}{v}" for k, v in t.items()))
+def test_launch_variants_match_oracle(api, ctx, orc, tuning):
+    try:
+        for moving in (False, True):
+            _check_rollout(api, ctx, orc, scenes.fast_clutter(moving=moving, n_agents=45, n_spheres=333), tuning=tuning)
+    finally:
+        ctx.set_tuning(reset=True)
+
+
+def test_cull_is_bitwise_identical_to_branch_free(api, ctx):
+    try:
+        for sc in (scenes.fast_clutter(), scenes.fast_clutter(moving=True), scenes.config3(n_agents=300)):
+            a = api.run_scene(ctx, sc, tuning=dict(cull=0))
+            b = api.run_scene(ctx, sc, tuning=dict(cull=1))
+            assert np.array_equal(a["final"], b["final"]) and np.array_equal(a["cost"], b["cost"])
+            assert np.array_equal(a["collided"], b["collided"]) and a["best"] == b["best"]
+    finally:
+        ctx.set_tuning(reset=True)
+
+
+def test_run_to_run_bit_reproducible(api, ctx):
+    sc = scenes.config3(n_agents=500)
+    a = api.run_scene(ctx, sc); b = api.run_scene(ctx, sc)
+    assert np.array_equal(a["final"], b["final"]) and np.array_equal(a["cost"], b["cost"])
+
+
+# ---------------------------------------------------------------------------------- edge cases
+def test_no_obstacles(api, ctx, orc):
+    sc = scenes.config1()
+    sc.xyzr = np.zeros((0, 4), np.float32)
+    g, o = _check_rollout(api, ctx, orc, sc)
+    assert np.all(np.isinf(g["min_clearance"])) and not g["collided"].any() and np.all(g["cost"][:, 2] == 0)
+
+
+def test_single_agent_single_sphere_and_ragged(api, ctx, orc):
+    sc = scenes.fast_clutter(n_agents=1, n_spheres=1)
+    _check_rollout(api, ctx, orc, sc)
+    for na, ns in ((3, 33), (149, 65), (297, 1023), (33, 4097)):
+        _check_rollout(api, ctx, orc, scenes.fast_clutter(n_agents=na, n_spheres=ns, steps=40))
+
+
+def test_agent_starts_inside_and_at_centre(api, ctx, orc):
+    sc = scenes.fast_clutter(n_agents=8, n_spheres=20, steps=30)
+    sc.agents[0, :3] = sc.xyzr[3, :3]                                   # exactly at a sphere centre
+    sc.agents[1, :3] = sc.xyzr[4, :3] + np.array([0.5 * sc.xyzr[4, 3], 0, 0], np.float32)
+    sc.agents[2, 3:] = 0.0                                              # at rest
+    g, o = _check_rollout(api, ctx, orc, sc)
+    assert g["collided"][0] == 1 and g["collided"][1] == 1 and np.all(np.isfinite(g["final"]))
+
+
+def test_hysteresis_and_collision_key(api, ctx, orc):
+    sc = scenes.fast_clutter(n_agents=160, n_spheres=500, r_lo=0.02, r_hi=0.07, steps=150)
+    g = api.run_scene(ctx, sc)
+    o = orc.rollout_scene(sc, threads=8)
+    for alpha, prev in ((0.9, -1), (0.9, 5), (0.5, 17), (1.0, 3), (0.9, int(np.argmax(o["collided"]))), (0.9, 10 ** 6)):
+        want, _ = orc.best_agent(g["cost"].astype(np.float64), g["collided"], alpha, prev)
+        got, cost = ctx.best_agent(alpha, prev)
+        assert got == want and cost == g["cost"][got, 0]
+
+
+def test_aliasing_out_equals_in(api, ctx):
+    import torch
+    sc = scenes.fast_clutter(n_agents=40, n_spheres=100)
+    ref = api.run_scene(ctx, sc)
+    ag = _tensor(sc.agents)
+    ctx.rollout(api.GMAPP_POINT3, ag, ag, sc.goal, sc.gains, sc.dt, sc.steps)
+    torch.cuda.synchronize()
+    assert np.array_equal(ag.cpu().numpy(), ref["final"])
+
+
+def test_r_agent_repack_and_plan_cycle_host(api, ctx, orc):
+    sc = scenes.fast_clutter(n_agents=40, n_spheres=100)
+    sc.gains["r_agent"] = 0.02
+    g, o = _check_rollout(api, ctx, orc, sc)
+    out = np.empty_like(sc.agents)
+    idx, cost = ctx.plan_cycle_host(api.GMAPP_POINT3, sc.agents, sc.goal, sc.gains, sc.dt, sc.steps,
+                                    h_xyzr=sc.xyzr, h_vel=None, h_agents_out=out)
+    assert idx == g["best"] and cost == g["best_cost"] and np.array_equal(out, g["final"])
+    idx2, _ = ctx.plan_cycle_host(api.GMAPP_POINT3, sc.agents, sc.goal, sc.gains, sc.dt, sc.steps)   # resident spheres
+    assert idx2 == idx
+
+
+def test_error_statuses(api):
+    import torch
+    c = api.Context(max_agents=8, max_spheres=16)
+    try:
+        ag = torch.zeros((4, 6), device="cuda:0")
+        with pytest.raises(api.GmappError) as e:
+            c.rollout(api.GMAPP_POINT3, ag, None, [0, 0, 0], None, 1e-3, 10)
+        assert e.value.status == api.GMAPP_ESTATE
+        with pytest.raises(api.GmappError) as e:
+            c.best_agent()
+        assert e.value.status == api.GMAPP_ESTATE
+        c.set_obstacles(torch.zeros((0, 4), device="cuda:0"), None, n=0)
+        with pytest.raises(api.GmappError) as e:
+            c.set_obstacles(torch.zeros((17, 4), device="cuda:0"))
+        assert e.value.status == api.GMAPP_ECAPACITY
+        with pytest.raises(api.GmappError) as e:
+            c.rollout(api.GMAPP_POINT3, torch.zeros((9, 6), device="cuda:0"), None, [0, 0, 0], None, 1e-3, 10)
+        assert e.value.status == api.GMAPP_ECAPACITY
+        for bad in (dict(dt=float("nan")), dict(steps=0), dict(gains=dict(eps_dist=0.0)),
+                    dict(gains=dict(eps_dist=0.2, r_influence=0.1)), dict(gains=dict(r_influence=-1.0)),
+                    dict(gains=dict(heuristic=7)), dict(goal=[0, float("inf"), 0])):
+            kw = dict(goal=[0, 0, 0], gains=None, dt=1e-3, steps=10); kw.update(bad)
+            with pytest.raises(api.GmappError) as e:
+                c.rollout(api.GMAPP_POINT3, ag, None, kw["goal"], kw["gains"], kw["dt"], kw["steps"])
+            assert e.value.status == api.GMAPP_EINVAL, bad
+        c.rollout(api.GMAPP_POINT3, ag, None, [0, 0, 0], None, 1e-3, 10)      # still usable after errors
+        assert c.best_agent()[0] == 0
+    finally:
+        c.close()
+    with pytest.raises(api.GmappError):
+        api.Context(max_agents=0, max_spheres=4)
+
+
+def test_fp32_peak_microbenchmark(api, ctx):
+    t = ctx.measure_fp32_peak()
+    assert 30.0 < t < 90.0, t          # 148 SMs x 128 lanes x 2 x ~1.9 GHz ~ 72 TFLOP/s
