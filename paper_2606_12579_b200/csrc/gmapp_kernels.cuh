@@ -222,23 +222,34 @@ __device__ __forceinline__ void cf_force_static(float k_circ, float bx, float by
 // ---------------------------------------------------------------------------------------------
 // cost accumulators (Eq. 16-20), kept by the first warp of a group
 // ---------------------------------------------------------------------------------------------
+// Kahan-compensated add: the sums run over up to thousands of poses and must stay within 1e-5 absolute
+__device__ __forceinline__ void kahan_add(float& s, float& c, float x) {
+    float y = x - c;
+    float t = s + y;
+    c = (t - s) - y;
+    s = t;
+}
+
 struct CostAcc {
-    float sumG, sumO, sumV, sumJ, minclr, d1;
+    float sumG, cG, sumO, cO, sumV, cV, sumJ, cJ, minclr, d1;
     int collided;
     __device__ __forceinline__ void init(float dg) {
-        sumG = sumO = sumV = sumJ = 0.0f; minclr = __int_as_float(0x7f800000); d1 = dg; collided = 0;
+        sumG = cG = sumO = cO = sumV = cV = sumJ = cJ = 0.0f;
+        minclr = __int_as_float(0x7f800000); d1 = dg; collided = 0;
     }
-    // one pose: Eq. 17 / 18 summands, clearance and collision record
+    // one pose: Eq. 17 / 18 summands (exactly 1 / exactly 0 when saturated), clearance and collision record
     __device__ __forceinline__ void pose(float dg, float dmin, float rcg, float rco) {
-        sumG += fminf(dg, rcg);
-        sumO += fminf(fmaxf(dmin, 0.0f), rco);
+        kahan_add(sumG, cG, dg >= rcg ? 1.0f : dg / rcg);
+        kahan_add(sumO, cO, dmin >= rco ? 0.0f : 1.0f - fmaxf(dmin, 0.0f) / rco);
         minclr = fminf(minclr, dmin);
         collided |= (dmin < 0.0f) ? 1 : 0;
     }
+    __device__ __forceinline__ void add_len(float x) { kahan_add(sumV, cV, x); }
+    __device__ __forceinline__ void add_jerk(float x) { kahan_add(sumJ, cJ, x); }
     __device__ __forceinline__ void finish(const RolloutParams& P, float L_path, float J, float* out5) const {
         const float Nk = float(P.steps) + 1.0f;
-        float Cg = sumG / (P.rcg * Nk);
-        float Co = 1.0f - sumO / (P.rco * Nk);
+        float Cg = sumG / Nk;
+        float Co = sumO / Nk;
         float Cp;
         if (L_path == 0.0f && d1 == 0.0f) Cp = 0.0f;
         else if (L_path >= d1) Cp = 1.0f - d1 / L_path;
@@ -298,7 +309,7 @@ __device__ __forceinline__ void rollout_point3(const RolloutParams& P, const flo
                 ca[a].pose(norm3f(ex, ey, ez), acc.dmin[a], P.rcg, P.rco);
                 if (k >= 2) {                                          // third difference = vf dt^2 (a_k - a_{k-1})
                     float jx = fx - ap[a][0], jy = fy - ap[a][1], jz = fz - ap[a][2];
-                    ca[a].sumJ += fmaf(jx, jx, fmaf(jy, jy, jz * jz));
+                    ca[a].add_jerk(fmaf(jx, jx, fmaf(jy, jy, jz * jz)));
                 }
                 ap[a][0] = fx; ap[a][1] = fy; ap[a][2] = fz;
             }
@@ -308,7 +319,7 @@ __device__ __forceinline__ void rollout_point3(const RolloutParams& P, const flo
             p[a][0] = fmaf(P.dt, v[a][0], p[a][0]);                    // Eq. 11 (point mass)
             p[a][1] = fmaf(P.dt, v[a][1], p[a][1]);
             p[a][2] = fmaf(P.dt, v[a][2], p[a][2]);
-            if (cost_warp) ca[a].sumV += norm3f(v[a][0], v[a][1], v[a][2]);   // |p_new - p| = dt |v|
+            if (cost_warp) ca[a].add_len(norm3f(v[a][0], v[a][1], v[a][2]));   // |p_new - p| = dt |v|
         }
     }
     // final pose: distance-only pass
@@ -338,13 +349,19 @@ __device__ __forceinline__ void rollout_point3(const RolloutParams& P, const flo
 // ---------------------------------------------------------------------------------------------
 // 6D pose agents (8-float motor + 6-float body twist), one agent per group
 // ---------------------------------------------------------------------------------------------
-struct Pose6 { Quat r, d; Vec3 w, nu; };
+// The motor's translation is carried as the world vector p = 2 d r^* and its rotor r: the motor product
+// M <- M dM is then r <- r r_d, p <- p + R(r) t_d (identical group operation; the additive update keeps
+// the FP32 position error at the 3D path's level instead of compounding it through d (x) r_d products).
+// The dual part d = (1/2) p (x) r is rebuilt when the state is written out.
+struct Pose6 { Quat r; Vec3 p; Vec3 w, nu; };
 
 __device__ __forceinline__ Pose6 load_pose6(const float* s) {
     Pose6 x;
-    x.r = Quat{s[0], s[1], s[2], s[3]}; x.d = Quat{s[4], s[5], s[6], s[7]};
+    Quat d = Quat{s[4], s[5], s[6], s[7]};
+    x.r = Quat{s[0], s[1], s[2], s[3]};
     x.w = v3(s[8], s[9], s[10]); x.nu = v3(s[11], s[12], s[13]);
-    motor_normalise(x.r, x.d);
+    motor_normalise(x.r, d);
+    x.p = motor_translation(x.r, d);
     return x;
 }
 
@@ -370,15 +387,14 @@ __device__ __forceinline__ void rollout_pose6(const RolloutParams& P, const floa
     const Vec3 pg = motor_translation(rg, dg);
     const bool cost_warp = lane_in_group < 32;
     CostAcc ca;
-    Vec3 pos = motor_translation(x.r, x.d);
+    Vec3 pos = x.p;
     ca.init(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z));
     Vec3 dp1 = v3(0, 0, 0), dp2 = v3(0, 0, 0);            // previous two world displacements (Eq. 20)
-    float sumL = 0.0f;
     StaticAcc<1> acc;
     float p[1][3], v[1][3];
     for (int k = 0; k < P.steps; ++k) {
         const float tk = float(k) * P.dt;
-        pos = motor_translation(x.r, x.d);
+        pos = x.p;
         Vec3 pdot = qrot(x.r, x.nu);                      // world linear velocity of the body origin
         p[0][0] = pos.x; p[0][1] = pos.y; p[0][2] = pos.z;
         v[0][0] = pdot.x; v[0][1] = pdot.y; v[0][2] = pdot.z;
@@ -395,22 +411,21 @@ __device__ __forceinline__ void rollout_pose6(const RolloutParams& P, const floa
         x.nu = fma3(P.c_lin, f, x.nu);
         Quat rd, dd; Vec3 td;
         se3_exp_motor(P.dt * x.w, P.dt * x.nu, rd, dd, td);           // Eq. 11: M <- M exp(dt v)
+        Vec3 dp = qrot(x.r, td);                          // world displacement p_new - p
         if (cost_warp) {
-            Vec3 dp = qrot(x.r, td);                      // world displacement p_new - p
-            sumL += norm3f(td.x, td.y, td.z);
+            ca.add_len(norm3f(td.x, td.y, td.z));
             if (k >= 2) {
                 Vec3 t3 = dp - 2.0f * dp1 + dp2;          // p4 - 3 p3 + 3 p2 - p1 from displacements
-                ca.sumJ += dot(t3, t3);
+                ca.add_jerk(dot(t3, t3));
             }
             dp2 = dp1; dp1 = dp;
         }
-        Quat rn = qmul(x.r, rd);
-        Quat a1 = qmul(x.r, dd), a2 = qmul(x.d, rd);
-        x.r = rn;
-        x.d = Quat{a1.w + a2.w, a1.x + a2.x, a1.y + a2.y, a1.z + a2.z};
-        motor_normalise(x.r, x.d);
+        x.p = x.p + dp;
+        x.r = qmul(x.r, rd);
+        Quat dz = Quat{0, 0, 0, 0};
+        motor_normalise(x.r, dz);
     }
-    pos = motor_translation(x.r, x.d);
+    pos = x.p;
     p[0][0] = pos.x; p[0][1] = pos.y; p[0][2] = pos.z;
     v[0][0] = v[0][1] = v[0][2] = 0.0f;
     acc.clear();
@@ -419,13 +434,16 @@ __device__ __forceinline__ void rollout_pose6(const RolloutParams& P, const floa
     group_allreduce<1>(acc, P.L, lane_in_group, group_in_cta, red, P.steps & 1, mask);
     if (lane_in_group == 0) {
         ca.pose(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z), acc.dmin[0], P.rcg, P.rco);
-        ca.finish(P, sumL, ca.sumJ, P.cost + 5 * size_t(agent));
+        ca.finish(P, ca.sumV, ca.sumJ, P.cost + 5 * size_t(agent));
         P.minclr[agent] = ca.minclr;
         P.collided[agent] = ca.collided;
         if (P.agents_out) {
             float* o = P.agents_out + 14 * size_t(agent);
+            // dual part d = (1/2) (0, p) (x) r
+            Vec3 rv = v3(x.r.x, x.r.y, x.r.z);
+            Vec3 dv = 0.5f * (fma3(x.r.w, x.p, cross(x.p, rv)));
             o[0] = x.r.w; o[1] = x.r.x; o[2] = x.r.y; o[3] = x.r.z;
-            o[4] = x.d.w; o[5] = x.d.x; o[6] = x.d.y; o[7] = x.d.z;
+            o[4] = -0.5f * dot(x.p, rv); o[5] = dv.x; o[6] = dv.y; o[7] = dv.z;
             o[8] = x.w.x; o[9] = x.w.y; o[10] = x.w.z; o[11] = x.nu.x; o[12] = x.nu.y; o[13] = x.nu.z;
         }
     }
@@ -503,7 +521,7 @@ __global__ void __launch_bounds__(256) k_forces(const __grid_constant__ ForcePar
         for (int i = 0; i < 3; ++i) { p[0][i] = s[i]; v[0][i] = s[3 + i]; }
     } else {
         x = load_pose6(P.agents + 14 * size_t(warp));
-        pos = motor_translation(x.r, x.d);
+        pos = x.p;
         Vec3 pdot = qrot(x.r, x.nu);
         p[0][0] = pos.x; p[0][1] = pos.y; p[0][2] = pos.z;
         v[0][0] = pdot.x; v[0][1] = pdot.y; v[0][2] = pdot.z;
