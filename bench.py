@@ -1,0 +1,358 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the G-MAPP rollout on B200.
+
+A "step" is one planning cycle of the whole hot path: one persistent rollout
+launch over all agents x spheres x rollout steps, then the selection kernel and its 8-byte download.
+Workload at N=1: BASELINE.json configs[2], "dense depth-derived clutter" = 1024 agents x 4096 spheres x
+100 rollout steps, the configuration north_star's target is quoted on.  Synthetic, seeded inputs
+(paper_2606_12579_b200/scenes.py) stand in for the paper's scenes, whose geometry the paper does not give.
+
+    python bench.py --gpus 1 --steps 20 --warmup 5
+    python -m torch.distributed.run --nproc-per-node N ... bench.py --gpus N ...   (weak scaling by agents)
+    python bench.py --impl reference ...     (the FP64 oracle on the host cores, bounded sample)
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "agent-sphere force interactions/s"
+UNIT = "interactions/s"
+# Algorithmic FP32 work of one agent-sphere pair: distance + gate
+# 17 flop, circular-field force 18 flop, an FFMA counted as 2.  Newton-refinement instructions that this
+# implementation adds for accuracy are NOT counted.
+FLOP_PER_PAIR = 35.0
+# FP32 peak from the guide's unit counts and clock: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz
+NOMINAL_SMS, LANES_PER_SM, MAX_GHZ = 148, 128, 1.965
+PEAK_TFLOPS = NOMINAL_SMS * LANES_PER_SM * 2 * MAX_GHZ / 1e3
+# dram__bytes_read.sum + dram__bytes_write.sum of one rollout launch from the committed ncu capture
+# (profiles/); None until a capture exists
+TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="config3", help="config1|config2|config3|config4|sweep:<agents>x<spheres>")
+    ap.add_argument("--cull", type=int, default=-1, help="-1 library default, 0 branch-free, 1 warp-vote skip")
+    ap.add_argument("--lanes", type=int, default=0)
+    ap.add_argument("--agents-per-thread", type=int, default=0)
+    ap.add_argument("--stage", type=int, default=-1)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
+    return ap.parse_args()
+
+
+def make_scene(name: str, seed: int = 0):
+    from paper_2606_12579_b200 import scenes
+    if name.startswith("sweep:"):
+        a, s = name[6:].split("x")
+        return scenes.config5(int(a), int(s), seed=seed)
+    return getattr(scenes, name)(seed=seed)
+
+
+# ------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML during the timed region."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz, self._stop = [], set(), None, threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:          # NVML missing: report that, do not fail the bench
+            self.err = repr(e)
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            self._stop.wait(0.01)
+
+    def __enter__(self):
+        if self.ok:
+            self.t = threading.Thread(target=self._run, daemon=True)
+            self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        if self.ok:
+            self._stop.set()
+            self.t.join()
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "note": "NVML unavailable"}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------ oracle legs
+def oracle_rate(scene, target_seconds: float):
+    """Time the FP64 oracle, as it stands, on the host cores over a bounded sample of `scene`:
+    the first n agents, all spheres, all rollout steps.  Returns (interactions/s, cores, sample text, seconds)."""
+    from oracle import oracle
+    cores = oracle.max_threads()
+    n_all = scene.n_agents
+    probe = min(n_all, cores)
+    t0 = time.perf_counter()
+    oracle.rollout_scene(scene, threads=cores, agent_slice=slice(0, probe))
+    t_probe = max(time.perf_counter() - t0, 1e-4)
+    n = int(min(n_all, max(probe, (target_seconds / t_probe) * probe)))
+    n = max(cores, (n // cores) * cores) if n >= cores else n
+    t0 = time.perf_counter()
+    oracle.rollout_scene(scene, threads=cores, agent_slice=slice(0, n))
+    dt = time.perf_counter() - t0
+    pairs = float(n) * scene.n_spheres * scene.steps
+    sample = f"first {n} of {n_all} agents x {scene.n_spheres} spheres x {scene.steps} steps, OpenMP over agents"
+    return pairs / dt, cores, sample, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    scene = make_scene(args.config)
+    per_step = max(2.0, min(args.cpu_seconds, 150.0 / max(1, args.steps + args.warmup)))
+    rates, secs, info = [], [], None
+    for i in range(args.warmup + args.steps):
+        r, cores, sample, dt = oracle_rate(scene, per_step)
+        if i >= args.warmup:
+            rates.append(r); secs.append(dt)
+        info = (cores, sample)
+    value = float(np.mean(rates))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean(secs) * 1e3),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": scene.name, "n_agents": scene.n_agents, "n_spheres": scene.n_spheres,
+                   "rollout_steps": scene.steps, "note": "each step times a bounded sample of the workload"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": info[0], "kind": "oracle", "sample": info[1]},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------ our arm
+def scaled_scene(name: str, world: int):
+    """Weak scaling: the global problem has world x the config's agents; the sphere world is replicated."""
+    from paper_2606_12579_b200 import scenes
+    if world == 1:
+        return make_scene(name)
+    if name.startswith("sweep:"):
+        a, s = name[6:].split("x")
+        return scenes.config5(int(a) * world, int(s))
+    base = {"config1": 16, "config2": 64, "config3": 1024, "config4": 256}[name]
+    if name == "config1":
+        raise SystemExit("config1 is fully specified (16 agents) and is not a multi-GPU workload")
+    return getattr(scenes, name)(n_agents=base * world)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}: launch with torch.distributed.run --nproc-per-node {args.gpus}")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_2606_12579_b200 import api, scenes, sharding
+
+    scene = scaled_scene(args.config, world)
+    lo, hi = sharding.shard_range(scene.n_agents, rank, world)
+    kind = scene.kind
+    if kind == scenes.KIND_POINT3:
+        h_agents = np.ascontiguousarray(scene.agents[lo:hi]); goal = scene.goal
+    else:
+        h_agents = api.pose_to_state14(scene.quat[lo:hi], scene.pos[lo:hi], scene.twist[lo:hi])
+        goal = api.pose_to_state14(scene.goal_quat, scene.goal, np.zeros(6))[0, :8]
+    n_local = hi - lo
+    pairs_local = float(n_local) * scene.n_spheres * scene.steps
+    pairs_global = float(scene.n_agents) * scene.n_spheres * scene.steps
+    gains = api.make_gains(scene.gains)
+
+    ctx = api.Context(max_agents=n_local, max_spheres=max(scene.n_spheres, 1), device=local_rank)
+    tune = dict(lanes_per_agent=args.lanes, agents_per_thread=args.agents_per_thread, cull=args.cull, stage=args.stage)
+    ctx.set_tuning(**tune)
+    d_xyzr = torch.from_numpy(scene.xyzr).to(dev)
+    d_vel = None if scene.vel is None else torch.from_numpy(scene.vel).to(dev)
+    ctx.set_obstacles(d_xyzr, d_vel, n=scene.n_spheres)
+    d_agents = torch.from_numpy(h_agents).to(dev)
+    d_out = torch.empty_like(d_agents)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)      # > 126 MB L2
+
+    def cycle():
+        ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
+        idx, cost, col = ctx.best_agent_ex(scene.alpha, scene.prev_best)
+        if world > 1:
+            idx = sharding.all_gather_best(sharding.local_key(col, cost, idx, lo))[2]
+        return idx, cost
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    K, W = args.steps, max(args.warmup, 3)
+    for _ in range(W):
+        flush.zero_(); cycle()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+    host_ms = []
+    sampler = ClockSampler(local_rank)
+    barrier()
+    t_wall0 = time.perf_counter()
+    with sampler:
+        for i in range(K):
+            flush.zero_()                                    # L2 flush between timed iterations (untimed)
+            torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            ev[i][0].record()
+            ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
+            ev[i][1].record()
+            idx, cost, col = ctx.best_agent_ex(scene.alpha, scene.prev_best)    # synchronises, 12-byte D2H
+            if world > 1:
+                idx = sharding.all_gather_best(sharding.local_key(col, cost, idx, lo))[2]
+            ev[i][2].record()
+            host_ms.append((time.perf_counter() - t0) * 1e3)
+        barrier()
+    wall_ms = (time.perf_counter() - t_wall0) * 1e3
+    step_ms = np.array([e[0].elapsed_time(e[2]) for e in ev])
+    roll_ms = np.array([e[0].elapsed_time(e[1]) for e in ev])
+    total_ms = float(step_ms.sum())
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    info = ctx.launch_info()
+    launches = K * (info["kernels_launched"] + 1)
+
+    # ---- roofline of the dominant kernel (the rollout), branch-free variant: every pair does the full math
+    ctx.set_tuning(**{**tune, "cull": 0})
+    for _ in range(3):
+        ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
+    rev = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(K)]
+    torch.cuda.synchronize(dev)
+    for i in range(K):
+        flush.zero_()
+        rev[i][0].record()
+        ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
+        rev[i][1].record()
+    torch.cuda.synchronize(dev)
+    bf_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in rev]))
+    info_bf = ctx.launch_info()
+    achieved = pairs_local * FLOP_PER_PAIR / (bf_ms * 1e-3) / 1e12
+    ctx.set_tuning(**tune)
+    peak_meas = ctx.measure_fp32_peak(False)
+    peak_meas_x2 = ctx.measure_fp32_peak(True)
+
+    # ---- end to end through the C ABI with HOST buffers (sphere + agent upload, 8-byte result download)
+    for _ in range(3):
+        ctx.plan_cycle_host(kind, h_agents, goal, gains, scene.dt, scene.steps, h_xyzr=scene.xyzr, h_vel=scene.vel,
+                            alpha=scene.alpha, prev_best=scene.prev_best)
+    barrier()
+    e2e_s = 0.0
+    for i in range(K):
+        flush.zero_(); torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        idx_e, cost_e = ctx.plan_cycle_host(kind, h_agents, goal, gains, scene.dt, scene.steps, h_xyzr=scene.xyzr,
+                                            h_vel=scene.vel, alpha=scene.alpha, prev_best=scene.prev_best)
+        if world > 1:
+            col_e = ctx.best_agent_ex(scene.alpha, scene.prev_best)[2]
+            idx_e = sharding.all_gather_best(sharding.local_key(col_e, cost_e, idx_e, lo))[2]
+        e2e_s += time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = scene.xyzr.nbytes + (0 if scene.vel is None else scene.vel.nbytes) + h_agents.nbytes
+    d2h = 12
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": pairs_global * K / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": K, "warmup": W, "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": scene.name, "n_agents": scene.n_agents, "n_spheres": scene.n_spheres,
+                       "rollout_steps": scene.steps, "agents_per_gpu": n_local, "parallelism": f"agents x{world}",
+                       "l2": "flushed between timed iterations (256 MB write, untimed)",
+                       "step": "one planning cycle: rollout kernel + selection kernel + 8-byte download",
+                       "launch": info},
+            "planning_cycle_latency_ms": {"device_p50": float(np.percentile(step_ms, 50)),
+                                          "device_p99": float(np.percentile(step_ms, 99)),
+                                          "host_p50": float(np.percentile(host_ms, 50)),
+                                          "host_p99": float(np.percentile(host_ms, 99)),
+                                          "rollout_kernel_mean": float(roll_ms.mean())},
+            "wall_ms_per_step_incl_flush": wall_ms / K,
+            "e2e": {"value": pairs_global * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                    "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_s / K * 1e3,
+                    "call": "gmapp_plan_cycle_host (host spheres + agents in, best index out)"},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_TFLOPS, "unit": "TFLOP/s",
+                         "frac": achieved / PEAK_TFLOPS, "traffic": TRAFFIC_BYTES_PER_LAUNCH,
+                         "kernel": "k_rollout (branch-free variant, cull=0)", "kernel_ms": bf_ms,
+                         "flop_per_pair": FLOP_PER_PAIR, "pairs_per_launch": pairs_local,
+                         "peak_how": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (guide unit counts, max clock)",
+                         "peak_measured_ffma_tflops": peak_meas, "peak_measured_ffma2_tflops": peak_meas_x2,
+                         "frac_of_measured_ffma": achieved / peak_meas if peak_meas else None,
+                         "launch": info_bf},
+            "clocks": sampler.summary(),
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            r, cores, sample, dt = oracle_rate(scene, args.cpu_seconds)
+            line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                                    "seconds": dt}
+        print(json.dumps(line), flush=True)
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -135,6 +135,11 @@ gmapp_status gmapp_rollout(gmapp_ctx* ctx, gmapp_kind kind, const float* d_agent
 gmapp_status gmapp_best_agent(gmapp_ctx* ctx, float alpha, int prev_best, int* out_index, float* out_cost,
                               void* cuda_stream);
 
+/* Same, and also returns the winner's collision flag (needed to merge winners of several GPUs, each
+ * of which rolled its own block of agents). */
+gmapp_status gmapp_best_agent_ex(gmapp_ctx* ctx, float alpha, int prev_best, int* out_index, float* out_cost,
+                                 int* out_collided, void* cuda_stream);
+
 /* Force query without integration (the control thread's query, Fig. 2 step 5):
  * for each state, d_f_rep [n][3] = sum_j f_j (world frame, Eq. 2-3 / Alg. 1) with obstacles at time
  * t_obstacles, and d_f_total = Eq. 6: POINT3 [n][3] = f_a + f_r; MOTOR6 [n][6] = body wrench

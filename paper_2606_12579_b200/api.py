@@ -44,7 +44,8 @@ class gmapp_launch_info(C.Structure):
 
 
 EXPORTS = ["gmapp_default_gains", "gmapp_create", "gmapp_destroy", "gmapp_set_obstacles",
-           "gmapp_set_obstacles_host", "gmapp_set_tuning", "gmapp_rollout", "gmapp_best_agent", "gmapp_forces",
+           "gmapp_set_obstacles_host", "gmapp_set_tuning", "gmapp_rollout", "gmapp_best_agent", "gmapp_best_agent_ex",
+           "gmapp_forces",
            "gmapp_get_results", "gmapp_plan_cycle_host", "gmapp_get_launch_info", "gmapp_measure_fp32_peak",
            "gmapp_sm_count", "gmapp_last_error"]
 
@@ -77,6 +78,7 @@ def _load():
     lib.gmapp_set_tuning.argtypes = [vp, C.POINTER(gmapp_tuning)]
     lib.gmapp_rollout.argtypes = [vp, C.c_int, vp, vp, C.c_int, fp, C.POINTER(gmapp_gains), C.c_float, C.c_int, vp]
     lib.gmapp_best_agent.argtypes = [vp, C.c_float, C.c_int, ip, fp, vp]
+    lib.gmapp_best_agent_ex.argtypes = [vp, C.c_float, C.c_int, ip, fp, ip, vp]
     lib.gmapp_forces.argtypes = [vp, C.c_int, vp, C.c_int, fp, C.POINTER(gmapp_gains), C.c_float, vp, vp, vp]
     lib.gmapp_get_results.argtypes = [vp, vp, vp, vp, vp]
     lib.gmapp_plan_cycle_host.argtypes = [vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, fp, C.POINTER(gmapp_gains),
@@ -208,6 +210,12 @@ class Context:
         self._check(_lib.gmapp_best_agent(self._h, C.c_float(alpha), int(prev_best), C.byref(idx), C.byref(cost),
                                           _stream(stream)))
         return idx.value, cost.value
+
+    def best_agent_ex(self, alpha=0.9, prev_best=-1, stream=None):
+        idx, cost, col = C.c_int(), C.c_float(), C.c_int()
+        self._check(_lib.gmapp_best_agent_ex(self._h, C.c_float(alpha), int(prev_best), C.byref(idx), C.byref(cost),
+                                             C.byref(col), _stream(stream)))
+        return idx.value, cost.value, col.value
 
     def forces(self, kind, d_agents, goal, gains, t_obstacles, d_f_rep, d_f_total, n_agents=None, stream=None):
         n = int(d_agents.shape[0]) if n_agents is None else n_agents

@@ -122,12 +122,12 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
     ALLOC(c->d_agents_stage, sizeof(float) * 14 * max_agents);
     ALLOC(c->d_xyzr_stage, sizeof(float) * 4 * c->cap_spheres);
     ALLOC(c->d_vel_stage, sizeof(float) * 3 * c->cap_spheres);
-    ALLOC(c->d_best_idx, sizeof(int));
+    ALLOC(c->d_best_idx, sizeof(int) * 2);
     ALLOC(c->d_best_cost, sizeof(float));
     ALLOC(c->d_scratch, sizeof(float) * 64);
 #undef ALLOC
     if ((e = cudaMallocHost((void**)&c->h_pinned, sizeof(float) * hp)) != cudaSuccess ||
-        (e = cudaMallocHost((void**)&c->h_best, sizeof(int) * 2)) != cudaSuccess ||
+        (e = cudaMallocHost((void**)&c->h_best, sizeof(int) * 4)) != cudaSuccess ||
         (e = cudaEventCreate(&c->ev0)) != cudaSuccess || (e = cudaEventCreate(&c->ev1)) != cudaSuccess) {
         gmapp_destroy(c);
         return fail(nullptr, GMAPP_ECUDA, "pinned / event allocation: %s", cudaGetErrorString(e));
@@ -375,8 +375,8 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
 // ---------------------------------------------------------------------------------------------
 // selection, force query, results
 // ---------------------------------------------------------------------------------------------
-extern "C" gmapp_status gmapp_best_agent(gmapp_ctx* c, float alpha, int prev_best, int* out_index, float* out_cost,
-                                         void* stream) {
+extern "C" gmapp_status gmapp_best_agent_ex(gmapp_ctx* c, float alpha, int prev_best, int* out_index, float* out_cost,
+                                            int* out_collided, void* stream) {
     if (!c) return GMAPP_EINVAL;
     if (!out_index) return fail(c, GMAPP_EINVAL, "best_agent: out_index is NULL%s");
     if (c->last_n_agents < 1) return fail(c, GMAPP_ESTATE, "best_agent: no rollout has run on this context%s");
@@ -384,12 +384,18 @@ extern "C" gmapp_status gmapp_best_agent(gmapp_ctx* c, float alpha, int prev_bes
     cudaStream_t st = (cudaStream_t)stream;
     k_best_agent<<<1, 1024, 0, st>>>(c->d_cost, c->d_collided, c->last_n_agents, alpha, prev_best, c->d_best_idx, c->d_best_cost);
     CUDA_TRY(c, cudaGetLastError());
-    CUDA_TRY(c, cudaMemcpyAsync(&c->h_best[0], c->d_best_idx, sizeof(int), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(c, cudaMemcpyAsync(&c->h_best[1], c->d_best_cost, sizeof(float), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaMemcpyAsync(&c->h_best[0], c->d_best_idx, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(c, cudaMemcpyAsync(&c->h_best[2], c->d_best_cost, sizeof(float), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(c, cudaStreamSynchronize(st));
     *out_index = c->h_best[0];
-    if (out_cost) memcpy(out_cost, &c->h_best[1], sizeof(float));
+    if (out_collided) *out_collided = c->h_best[1];
+    if (out_cost) memcpy(out_cost, &c->h_best[2], sizeof(float));
     return GMAPP_OK;
+}
+
+extern "C" gmapp_status gmapp_best_agent(gmapp_ctx* c, float alpha, int prev_best, int* out_index, float* out_cost,
+                                         void* stream) {
+    return gmapp_best_agent_ex(c, alpha, prev_best, out_index, out_cost, nullptr, stream);
 }
 
 extern "C" gmapp_status gmapp_forces(gmapp_ctx* c, gmapp_kind kind, const float* d_agents, int n_agents, const float* goal,

@@ -582,6 +582,7 @@ __device__ __forceinline__ bool key_less(int ca, float Ca, int ia, int cb, float
 
 __global__ void __launch_bounds__(1024) k_best_agent(const float* __restrict__ cost5, const int* __restrict__ collided,
                                                      int n, float alpha, int prev_best, int* out_idx, float* out_cost) {
+    // out_idx[0] = winner, out_idx[1] = its collision flag
     __shared__ int s_c[32]; __shared__ float s_C[32]; __shared__ int s_i[32];
     int bc = 2, bi = 0x7fffffff; float bC = __int_as_float(0x7f800000);
     for (int i = threadIdx.x; i < n; i += blockDim.x) {
@@ -612,9 +613,10 @@ __global__ void __launch_bounds__(1024) k_best_agent(const float* __restrict__ c
                 float Cp = cost5[5 * size_t(prev_best)]; int cp = collided[prev_best] ? 1 : 0;
                 if (Cp != Cp) { Cp = __int_as_float(0x7f800000); cp = 1; }
                 bool improves = (bc < cp) || (bc == cp && bC < alpha * Cp);
-                if (!improves) { bi = prev_best; bC = Cp; }
+                if (!improves) { bi = prev_best; bC = Cp; bc = cp; }
             }
-            *out_idx = n > 0 ? bi : -1;
+            out_idx[0] = n > 0 ? bi : -1;
+            out_idx[1] = n > 0 ? bc : 0;
             *out_cost = n > 0 ? bC : __int_as_float(0x7fc00000);
         }
     }
