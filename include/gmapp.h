@@ -82,7 +82,9 @@ typedef struct {
     int32_t stage;               /* -1 auto, 0 = read spheres from global/L2, 1 = stage the whole sphere set in
                                     shared memory (TMA bulk copy), 2 = stream tiles through a TMA ring         */
     int32_t max_ctas;            /* 0 = SM count; cap on the grid (for scaling experiments)           */
-    int32_t reserved[3];
+    int32_t scalar_path;         /* 0 = packed f32x2 kernel where it applies (POINT3, static spheres);
+                                    1 = force the scalar FP32 kernel (A/B comparison)                     */
+    int32_t reserved[2];
 } gmapp_tuning;
 
 /* What the last gmapp_rollout launched (for reporting). */
@@ -92,6 +94,7 @@ typedef struct {
     int32_t cull, stage, tile_spheres, n_tiles;
     int32_t smem_bytes, regs_per_thread;
     int32_t kernels_launched;    /* kernels this call enqueued */
+    int32_t packed_x2;           /* 1 = the packed f32x2 kernel ran, 0 = the scalar kernel */
 } gmapp_launch_info;
 
 /* Fill *g with the defaults listed above (k_circ 1, k_att 2, k_damp 0.5, rot 2 / 0.5, inv 1, 1/2,

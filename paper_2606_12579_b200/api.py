@@ -31,13 +31,13 @@ class gmapp_gains(C.Structure):
 
 class gmapp_tuning(C.Structure):
     _fields_ = [("lanes_per_agent", C.c_int32), ("agents_per_thread", C.c_int32), ("cull", C.c_int32),
-                ("stage", C.c_int32), ("max_ctas", C.c_int32), ("reserved", C.c_int32 * 3)]
+                ("stage", C.c_int32), ("max_ctas", C.c_int32), ("scalar_path", C.c_int32), ("reserved", C.c_int32 * 2)]
 
 
 class gmapp_launch_info(C.Structure):
     _fields_ = [(k, C.c_int32) for k in
                 ("grid", "block", "lanes_per_agent", "agents_per_thread", "agents_per_cta", "cull", "stage",
-                 "tile_spheres", "n_tiles", "smem_bytes", "regs_per_thread", "kernels_launched")]
+                 "tile_spheres", "n_tiles", "smem_bytes", "regs_per_thread", "kernels_launched", "packed_x2")]
 
     def as_dict(self):
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
@@ -191,11 +191,12 @@ class Context:
                                                   None if v is None else v.ctypes.data_as(C.c_void_p),
                                                   int(x.shape[0]), _stream(stream)))
 
-    def set_tuning(self, lanes_per_agent=0, agents_per_thread=0, cull=-1, stage=-1, max_ctas=0, reset=False):
+    def set_tuning(self, lanes_per_agent=0, agents_per_thread=0, cull=-1, stage=-1, max_ctas=0, scalar_path=0,
+                   reset=False):
         if reset:
             self._check(_lib.gmapp_set_tuning(self._h, None))
             return
-        t = gmapp_tuning(lanes_per_agent, agents_per_thread, cull, stage, max_ctas)
+        t = gmapp_tuning(lanes_per_agent, agents_per_thread, cull, stage, max_ctas, scalar_path)
         self._check(_lib.gmapp_set_tuning(self._h, C.byref(t)))
 
     def rollout(self, kind, d_agents, d_agents_out, goal, gains, dt, steps, n_agents=None, stream=None):

@@ -8,6 +8,7 @@
 
 #include "../../include/gmapp.h"
 #include "gmapp_kernels.cuh"
+#include "gmapp_rollout_x2.cuh"
 
 using namespace gmapp;
 
@@ -18,6 +19,11 @@ struct gmapp_ctx {
     float4* d_sph_raw = nullptr;
     float4* d_sph_eff = nullptr;
     float4* d_svel = nullptr;
+    // sphere-pair layout of the packed f32x2 rollout kernel: (cx0,cx1,cy0,cy1), (cz0,cz1,-R0,-R1), R = r + r_agent
+    float4* d_pairA = nullptr;
+    float4* d_pairB = nullptr;
+    float pair_r_agent = 0.0f;
+    bool pair_valid = false;
     float eff_r_agent = 0.0f;
     bool eff_valid = false;
     int n_spheres = -1;            // -1: set_obstacles not called yet
@@ -84,6 +90,16 @@ static rollout_fn rollout_kernel(int kind, int at, bool moving, bool cull, int s
     return PICK(0, 1, 1024);
 #undef PICK
 }
+typedef void (*rollout_x2_fn)(const RolloutX2Params);
+static const int kX2MaxThreads = 512;
+static rollout_x2_fn rollout_x2_kernel(int at, bool wide, bool cull, int stage) {
+#define PICKX(A, W)                                                                                                  \
+    (cull ? (stage ? (rollout_x2_fn)k_rollout_x2<A, W, true, 1, 512> : (rollout_x2_fn)k_rollout_x2<A, W, true, 0, 512>)     \
+          : (stage ? (rollout_x2_fn)k_rollout_x2<A, W, false, 1, 512> : (rollout_x2_fn)k_rollout_x2<A, W, false, 0, 512>))
+    if (at == 2) return wide ? PICKX(2, true) : PICKX(2, false);
+    return wide ? PICKX(1, true) : PICKX(1, false);
+#undef PICKX
+}
 static int rollout_max_threads(int kind, int at) { return (kind == GMAPP_MOTOR6 || at == 2) ? 512 : 1024; }
 
 // ---------------------------------------------------------------------------------------------
@@ -102,7 +118,7 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
     memset(&c->info, 0, sizeof c->info);
     c->err[0] = 0;
     c->device = device; c->max_agents = max_agents; c->max_spheres = max_spheres;
-    c->cap_spheres = round_up(max_spheres > 0 ? max_spheres : 1, 1024);
+    c->cap_spheres = round_up(max_spheres > 0 ? max_spheres : 1, 2048);
     cudaDeviceProp prop;
     cudaError_t e = cudaGetDeviceProperties(&prop, device);
     if (e != cudaSuccess) { delete c; return fail(nullptr, GMAPP_ECUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e)); }
@@ -116,6 +132,8 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
     ALLOC(c->d_sph_raw, sizeof(float4) * c->cap_spheres);
     ALLOC(c->d_sph_eff, sizeof(float4) * c->cap_spheres);
     ALLOC(c->d_svel, sizeof(float4) * c->cap_spheres);
+    ALLOC(c->d_pairA, sizeof(float4) * (c->cap_spheres / 2));
+    ALLOC(c->d_pairB, sizeof(float4) * (c->cap_spheres / 2));
     ALLOC(c->d_cost, sizeof(float) * 5 * max_agents);
     ALLOC(c->d_minclr, sizeof(float) * max_agents);
     ALLOC(c->d_collided, sizeof(int) * max_agents);
@@ -142,6 +160,14 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
                                                  cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
                         if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
                     }
+    for (int at = 1; at <= 2; ++at)
+        for (int wd = 0; wd < 2; ++wd)
+            for (int cu = 0; cu < 2; ++cu)
+                for (int st = 0; st < 2; ++st) {
+                    e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, wd, cu, st),
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
+                    if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
+                }
     *out = c;
     return GMAPP_OK;
 }
@@ -150,7 +176,7 @@ extern "C" gmapp_status gmapp_destroy(gmapp_ctx* c) {
     if (!c) return GMAPP_OK;
     cudaSetDevice(c->device);
     cudaDeviceSynchronize();
-    cudaFree(c->d_sph_raw); cudaFree(c->d_sph_eff); cudaFree(c->d_svel);
+    cudaFree(c->d_sph_raw); cudaFree(c->d_sph_eff); cudaFree(c->d_svel); cudaFree(c->d_pairA); cudaFree(c->d_pairB);
     cudaFree(c->d_cost); cudaFree(c->d_minclr); cudaFree(c->d_collided);
     cudaFree(c->d_agents_stage); cudaFree(c->d_xyzr_stage); cudaFree(c->d_vel_stage);
     cudaFree(c->d_best_idx); cudaFree(c->d_best_cost); cudaFree(c->d_scratch);
@@ -172,8 +198,8 @@ extern "C" gmapp_status gmapp_set_tuning(gmapp_ctx* c, const gmapp_tuning* t) {
         (t->lanes_per_agent && (t->lanes_per_agent & (t->lanes_per_agent - 1))))
         return fail(c, GMAPP_EINVAL, "set_tuning: lanes_per_agent must be 0 or a power of two <= 1024%s");
     if (t->agents_per_thread < 0 || t->agents_per_thread > 2) return fail(c, GMAPP_EINVAL, "set_tuning: agents_per_thread must be 0, 1 or 2%s");
-    if (t->cull < -1 || t->cull > 1 || t->stage < -1 || t->stage > 1 || t->max_ctas < 0)
-        return fail(c, GMAPP_EINVAL, "set_tuning: cull in {-1,0,1}, stage in {-1,0,1}, max_ctas >= 0%s");
+    if (t->cull < -1 || t->cull > 1 || t->stage < -1 || t->stage > 1 || t->max_ctas < 0 || t->scalar_path < 0 || t->scalar_path > 1)
+        return fail(c, GMAPP_EINVAL, "set_tuning: cull in {-1,0,1}, stage in {-1,0,1}, max_ctas >= 0, scalar_path in {0,1}%s");
     c->tuning = *t; c->has_tuning = true;
     return GMAPP_OK;
 }
@@ -196,9 +222,11 @@ __global__ void k_add_ragent(const float4* __restrict__ raw, float4* __restrict_
 }
 
 static int fill_count(const gmapp_ctx* c, int n) {
-    int f = round_up(n > 0 ? n : 1, 1024);
+    int f = round_up(n > 0 ? n : 1, 2048);
     return f > c->cap_spheres ? c->cap_spheres : f;
 }
+
+static gmapp_status effective_pairs(gmapp_ctx* c, float r_agent, cudaStream_t st, int* launches);
 
 extern "C" gmapp_status gmapp_set_obstacles(gmapp_ctx* c, const float* d_xyzr, const float* d_vel, int n, void* stream) {
     if (!c) return GMAPP_EINVAL;
@@ -212,6 +240,12 @@ extern "C" gmapp_status gmapp_set_obstacles(gmapp_ctx* c, const float* d_xyzr, c
     c->n_spheres = n;
     c->moving = (d_vel != nullptr) && n > 0;
     c->eff_valid = false;
+    c->pair_valid = false;
+    if (!c->moving) {
+        // sphere-pair layout of the packed kernel, for r_agent = 0 (repacked lazily if a rollout asks for another r_agent)
+        gmapp_status s = effective_pairs(c, 0.0f, st, nullptr);
+        if (s != GMAPP_OK) return s;
+    }
     return GMAPP_OK;
 }
 
@@ -245,6 +279,17 @@ static gmapp_status effective_spheres(gmapp_ctx* c, float r_agent, cudaStream_t 
         if (launches) ++*launches;
     }
     *out = c->d_sph_eff;
+    return GMAPP_OK;
+}
+
+// sphere-pair arrays with R = r + r_agent; launches the tiny repack kernel only when spheres or r_agent changed
+static gmapp_status effective_pairs(gmapp_ctx* c, float r_agent, cudaStream_t st, int* launches) {
+    if (c->pair_valid && c->pair_r_agent == r_agent) return GMAPP_OK;
+    const int n2f = fill_count(c, c->n_spheres) / 2;
+    k_pack_pairs<<<(n2f + 255) / 256, 256, 0, st>>>(c->d_sph_raw, c->n_spheres, n2f, r_agent, c->d_pairA, c->d_pairB);
+    CUDA_TRY(c, cudaGetLastError());
+    c->pair_valid = true; c->pair_r_agent = r_agent;
+    if (launches) ++*launches;
     return GMAPP_OK;
 }
 
@@ -311,6 +356,86 @@ static gmapp_status choose_launch(gmapp_ctx* c, int kind, int n_agents, LaunchCf
     return GMAPP_OK;
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// packed f32x2 rollout (POINT3, static spheres): launch selection + launch
+// ---------------------------------------------------------------------------------------------
+static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float* d_agents_out, int n_agents,
+                                      const float* goal, const gmapp_gains* g, float dt, int steps, cudaStream_t st) {
+    const gmapp_tuning* t = c->has_tuning ? &c->tuning : nullptr;
+    int max_ctas = c->num_sms;
+    if (t && t->max_ctas > 0 && t->max_ctas < max_ctas) max_ctas = t->max_ctas;
+    const int A = (n_agents + max_ctas - 1) / max_ctas;           // agents per CTA: one wave of the SMs
+    const int grid = (n_agents + A - 1) / A;
+    int at = A >= 2 ? 2 : 1;
+    if (t && t->agents_per_thread) at = t->agents_per_thread;
+    const int G = (A + at - 1) / at;                              // groups per CTA
+    const int tmax = kX2MaxThreads;
+    if (G > tmax) return fail(c, GMAPP_ECAPACITY, "rollout: %s%ld agent groups per CTA exceed %ld threads", "", G, tmax);
+    const int ns = c->n_spheres;
+    const int n2 = (ns + 1) / 2;
+    int L;
+    if (t && t->lanes_per_agent) {
+        L = t->lanes_per_agent;
+        if (G * L > tmax) return fail(c, GMAPP_EINVAL, "rollout: lanes_per_agent %s%ld x %ld groups exceeds the thread limit", "", L, G);
+        if (L > 32 && G > 7) return fail(c, GMAPP_EINVAL, "rollout: lanes_per_agent > 32 allows at most 7 groups per CTA, need %s%ld", "", G);
+    } else {
+        L = pow2_floor(tmax / G);
+        const int cap = pow2_ceil(n2 > 0 ? n2 : 1);               // no more lanes than sphere pairs
+        if (L > cap) L = cap;
+        if (L > 32 && G > 7) L = 32;                              // two named barriers per multi-warp group
+    }
+    const bool wide = L >= 32;
+    const int n2p = n2 > 0 ? round_up(n2, L) : 0;
+    const int cull = (t && t->cull >= 0) ? t->cull : 0;
+    // dynamic shared memory: [0,64) mbarrier; [64, 64+4 KB) cross-warp exchange; sphere-pair tile at 4224
+    const int xch_off = 64, tile_off = 4224;
+    const size_t tile_bytes = (size_t)n2p * 32;
+    const bool fits = tile_off + tile_bytes <= (size_t)c->smem_optin;
+    int stage = fits ? 1 : 0;
+    if (t && t->stage >= 0) {
+        if (t->stage == 1 && !fits) return fail(c, GMAPP_EINVAL, "rollout: sphere set (%s%ld bytes) does not fit shared memory", "", (long)tile_bytes);
+        stage = t->stage;
+    }
+    if (n2p == 0) stage = 0;
+    int launches = 0;
+    gmapp_status s = effective_pairs(c, g->r_agent, st, &launches);
+    if (s != GMAPP_OK) return s;
+    RolloutX2Params P;
+    memset(&P, 0, sizeof P);
+    P.pairA = c->d_pairA; P.pairB = c->d_pairB; P.n2p = n2p;
+    P.agents_in = d_agents; P.agents_out = d_agents_out;
+    P.n_agents = n_agents; P.agents_per_cta = A;
+    P.L = L; P.logL = ilog2(L);
+    P.steps = steps;
+    for (int i = 0; i < 3; ++i) P.goal[i] = goal[i];
+    P.dt = dt;
+    P.k_circ = g->k_circ; P.k_att = g->k_att; P.k_damp = g->k_damp;
+    P.c_lin = g->vel_factor * dt * g->inv_mass;
+    P.inv_mass = g->inv_mass; P.vel_factor = g->vel_factor;
+    P.r_d = g->r_influence; P.eps = g->eps_dist;
+    P.rcg = g->r_cost_goal > 0.0f ? g->r_cost_goal : g->r_influence;
+    P.rco = g->r_cost_obs > 0.0f ? g->r_cost_obs : g->r_influence;
+    P.w_goal = g->w_goal; P.w_obs = g->w_obs; P.w_path = g->w_path; P.w_smooth = g->w_smooth; P.a_max = g->a_max;
+    P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
+    P.tile_off = tile_off; P.xch_off = xch_off;
+    const int block = round_up(G * L, 32);
+    const int smem = tile_off + (stage == 1 ? (int)tile_bytes : 0);
+    rollout_x2_fn fn = rollout_x2_kernel(at, wide, cull != 0, stage);
+    fn<<<grid, block, smem, st>>>(P);
+    CUDA_TRY(c, cudaGetLastError());
+    ++launches;
+    c->last_n_agents = n_agents;
+    gmapp_launch_info& I = c->info;
+    I.grid = grid; I.block = block; I.lanes_per_agent = L; I.agents_per_thread = at;
+    I.agents_per_cta = A; I.cull = cull; I.stage = stage;
+    I.tile_spheres = stage == 1 ? 2 * n2p : 0; I.n_tiles = stage == 1 ? 1 : 0;
+    I.smem_bytes = smem; I.kernels_launched = launches; I.packed_x2 = 1;
+    cudaFuncAttributes fa;
+    if (cudaFuncGetAttributes(&fa, (const void*)fn) == cudaSuccess) I.regs_per_thread = fa.numRegs;
+    return GMAPP_OK;
+}
+
 // ---------------------------------------------------------------------------------------------
 // rollout
 // ---------------------------------------------------------------------------------------------
@@ -328,6 +453,8 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
     if (s != GMAPP_OK) return s;
     const int ng = kind == GMAPP_POINT3 ? 3 : 8;
     for (int i = 0; i < ng; ++i) if (!isfinite(goal[i])) return fail(c, GMAPP_EINVAL, "rollout: non-finite goal%s");
+    if (kind == GMAPP_POINT3 && !c->moving && !(c->has_tuning && c->tuning.scalar_path))
+        return launch_rollout_x2(c, d_agents, d_agents_out, n_agents, goal, g, dt, steps, (cudaStream_t)stream);
     LaunchCfg cfg;
     s = choose_launch(c, kind, n_agents, &cfg);
     if (s != GMAPP_OK) return s;
@@ -366,7 +493,7 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
     I.grid = cfg.grid; I.block = cfg.block; I.lanes_per_agent = cfg.L; I.agents_per_thread = cfg.at;
     I.agents_per_cta = cfg.agents_per_cta; I.cull = cfg.cull; I.stage = cfg.stage;
     I.tile_spheres = cfg.stage == 1 ? cfg.n_pad : 0; I.n_tiles = cfg.stage == 1 ? 1 : 0;
-    I.smem_bytes = cfg.smem; I.kernels_launched = launches;
+    I.smem_bytes = cfg.smem; I.kernels_launched = launches; I.packed_x2 = 0;
     cudaFuncAttributes fa;
     if (cudaFuncGetAttributes(&fa, (const void*)fn) == cudaSuccess) I.regs_per_thread = fa.numRegs;
     return GMAPP_OK;

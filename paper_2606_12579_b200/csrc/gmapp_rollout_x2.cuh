@@ -1,0 +1,426 @@
+// gmapp_rollout_x2.cuh -- the fast rollout kernel for 3D point agents over static spheres (sm_100a).
+//
+// Same method as gmapp_kernels.cuh (Eq. 2-3, 6-11, 16-20 of the paper), different machine mapping:
+//
+//  * Packed FP32 math.  Spheres are stored as PAIRS, A[j] = (cx0,cx1, cy0,cy1), B[j] = (cz0,cz1, -R0,-R1)
+//    (R = r_j + r_a), so one LDS.128 pair feeds fma.rn.f32x2 / add.f32x2 / mul.f32x2 (SASS FFMA2 / FADD2 /
+//    FMUL2: one issue slot for two pairs).  The agent state is the broadcast operand.  MUFU.RSQ / MUFU.RCP,
+//    the clamp, the gate and q - t^2 (needs a negated operand) stay scalar.  The gate is a predicated
+//    MUFU.RCP into a zeroed register, so a pair outside r_d contributes exactly 0.
+//  * A group of L lanes owns NA (1 or 2) agents; lane l sweeps sphere pairs l, l+L, ...  The 3 NA partial
+//    sums are combined by a TRANSPOSED xor-butterfly (each step halves the number of live values: 8 SHFL
+//    for 6 values instead of 30), the clearance minimum by one REDUX.MIN on an order-preserving integer
+//    key.  Fixed order, no atomics: bit-reproducible.
+//  * When a group spans several warps (L > 32), warps 1.. post their partial sums to shared memory and
+//    warp 0 alone adds them, integrates BOTH agents at once (agent a on lanes 0-15, agent b on lanes
+//    16-31), accumulates the costs and publishes the new state; the other warps pick it up after a named
+//    barrier.  Split arrive / sync barriers and parity double-buffering: one round trip per step, and the
+//    cost arithmetic runs after the state has been published.
+//
+// Shares nothing with oracle/.
+#pragma once
+#include "gmapp_kernels.cuh"
+
+namespace gmapp {
+
+typedef unsigned long long u64;
+
+__device__ __forceinline__ u64 pk2(float lo, float hi) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void upk2(u64 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ u64 bc2(float x) { return pk2(x, x); }      // ptxas folds this into the .F32 broadcast operand form
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ float min3f(float a, float b, float c) { float y; asm("min.f32 %0, %1, %2, %3;" : "=f"(y) : "f"(a), "f"(b), "f"(c)); return y; }
+__device__ __forceinline__ void named_bar_arrive(int id, int count) {
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory");
+}
+// order-preserving float <-> int key (an involution): integer order of the keys = float order of the values
+__device__ __forceinline__ int fkey(float x) { int b = __float_as_int(x); return b ^ ((b >> 31) & 0x7fffffff); }
+__device__ __forceinline__ float fkey_inv(int k) { return __int_as_float(k ^ ((k >> 31) & 0x7fffffff)); }
+
+struct RolloutX2Params {
+    const float4* pairA;      // [n2p] (cx0,cx1,cy0,cy1)
+    const float4* pairB;      // [n2p] (cz0,cz1,-R0,-R1)
+    int n2p;                  // sphere pairs, padded to a multiple of L with sentinels
+    const float* agents_in;   // [n][6]
+    float* agents_out;        // [n][6] or nullptr
+    int n_agents, agents_per_cta;
+    int L, logL;
+    int steps;
+    float goal[3];
+    float dt;
+    float k_circ, k_att, k_damp;
+    float c_lin;              // vel_factor * dt * inv_mass   (Eq. 9-10)
+    float inv_mass, vel_factor;
+    float r_d, eps;
+    float rcg, rco;           // Eq. 17 / 18 radii
+    float w_goal, w_obs, w_path, w_smooth, a_max;
+    float* cost;              // [n][5]
+    float* minclr;            // [n]
+    int* collided;            // [n]
+    int tile_off;             // byte offset of the sphere tile in dynamic shared memory
+    int xch_off;              // byte offset of the cross-warp exchange area
+};
+
+// per-lane partial sums of NA agents over the lane's sphere pairs (both halves of a pair kept apart)
+template <int NA>
+struct X2Acc {
+    u64 bx[NA], by[NA], bz[NA];
+    float dmin[NA];
+    __device__ __forceinline__ void clear() {
+#pragma unroll
+        for (int a = 0; a < NA; ++a) { bx[a] = by[a] = bz[a] = 0ull; dmin[a] = __int_as_float(0x7f800000); }
+    }
+};
+
+// One lane's slice of the sphere sum: pairs lane, lane+L, ... ; FORCE=false is the distance-only final pass.
+template <int NA, bool FORCE, bool CULL>
+__device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const float4* __restrict__ tB, int n2p,
+                                         int lane, int L, const float (&p)[NA][3], const float (&v)[NA][3],
+                                         float r_d, float eps, unsigned mask, X2Acc<NA>& acc) {
+    const u64 tiny = bc2(kTiny), half = bc2(0.5f);
+#pragma unroll 2
+    for (int j = lane; j < n2p; j += L) {
+        const float4 s0 = tA[j], s1 = tB[j];
+        const u64 cx = pk2(s0.x, s0.y), cy = pk2(s0.z, s0.w), cz = pk2(s1.x, s1.y), nR = pk2(s1.z, s1.w);
+        u64 dx[NA], dy[NA], dz[NA], q[NA];
+        float d0[NA], d1[NA];
+        bool any = false;
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            dx[a] = sub2(cx, bc2(p[a][0])); dy[a] = sub2(cy, bc2(p[a][1])); dz[a] = sub2(cz, bc2(p[a][2]));
+            q[a] = fma2(dx[a], dx[a], fma2(dy[a], dy[a], fma2(dz[a], dz[a], tiny)));
+            float q0, q1; upk2(q[a], q0, q1);
+            const u64 y = pk2(rsqrt_approx(q0), rsqrt_approx(q1));
+            const u64 t = mul2(q[a], y);
+            const u64 hy = mul2(y, half);
+            float t0, t1; upk2(t, t0, t1);
+            const u64 e = pk2(fmaf(-t0, t0, q0), fmaf(-t1, t1, q1));     // Newton residual q - t^2 (exact in the FMA)
+            const u64 ds = fma2(hy, e, add2(t, nR));                     // dist - R, dist to ~1 ulp
+            upk2(ds, d0[a], d1[a]);
+            acc.dmin[a] = min3f(acc.dmin[a], d0[a], d1[a]);
+            if (CULL) any = any || (fminf(d0[a], d1[a]) <= r_d);
+        }
+        if (!FORCE) continue;
+        if (CULL) { if (!__any_sync(mask, any)) continue; }
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            const u64 den = mul2(pk2(fmaxf(d0[a], eps), fmaxf(d1[a], eps)), q[a]);     // d_O * |d|^2
+            float n0, n1; upk2(den, n0, n1);
+            float r0 = 0.0f, r1 = 0.0f;
+            if (d0[a] <= r_d) r0 = rcp_approx(n0);                       // Alg. 1 line 7: outside r_d contributes 0
+            if (d1[a] <= r_d) r1 = rcp_approx(n1);
+            const u64 s = fma2(dx[a], bc2(v[a][0]), fma2(dy[a], bc2(v[a][1]), mul2(dz[a], bc2(v[a][2]))));
+            const u64 w = mul2(s, pk2(r0, r1));
+            acc.bx[a] = fma2(w, dx[a], acc.bx[a]);
+            acc.by[a] = fma2(w, dy[a], acc.by[a]);
+            acc.bz[a] = fma2(w, dz[a], acc.bz[a]);
+        }
+    }
+}
+
+// Transposed butterfly over a full warp.  In: per-lane partial (x,y,z) of NA agents.  Out: every lane of
+// half h (lanes 16h..16h+15; NA == 1: both halves) holds the warp total (X,Y,Z) of agent h.
+template <int NA>
+__device__ __forceinline__ void warp_sum3(const float (&x)[NA], const float (&y)[NA], const float (&z)[NA],
+                                          int lane, float& X, float& Y, float& Z) {
+    const unsigned full = 0xffffffffu;
+    float u;
+    if (NA == 2) {
+        const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4;
+        // step 16: lower half keeps agent 0, upper half keeps agent 1
+        float kx = h16 ? x[NA - 1] : x[0], ky = h16 ? y[NA - 1] : y[0], kz = h16 ? z[NA - 1] : z[0];
+        float sx = h16 ? x[0] : x[NA - 1], sy = h16 ? y[0] : y[NA - 1], sz = h16 ? z[0] : z[NA - 1];
+        kx += __shfl_xor_sync(full, sx, 16); ky += __shfl_xor_sync(full, sy, 16); kz += __shfl_xor_sync(full, sz, 16);
+        // step 8: lanes with bit 3 clear keep (x, y), the others keep z
+        float r1 = __shfl_xor_sync(full, h8 ? kx : kz, 8);
+        float r2 = __shfl_xor_sync(full, ky, 8);
+        if (h8) kz += r1; else { kx += r1; ky += r2; }
+        // step 4: (x, y) lanes split into x and y; z lanes plain
+        float send = h8 ? kz : (h4 ? kx : ky);
+        float keep = h8 ? kz : (h4 ? ky : kx);
+        u = keep + __shfl_xor_sync(full, send, 4);
+        u += __shfl_xor_sync(full, u, 2);
+        u += __shfl_xor_sync(full, u, 1);
+        const int base = lane & 16;
+        X = __shfl_sync(full, u, base); Y = __shfl_sync(full, u, base | 4); Z = __shfl_sync(full, u, base | 8);
+    } else {
+        const bool h16 = lane & 16, h8 = lane & 8;
+        float kx = x[0], ky = y[0], kz = z[0];
+        float r1 = __shfl_xor_sync(full, h16 ? kx : kz, 16);
+        float r2 = __shfl_xor_sync(full, ky, 16);
+        if (h16) kz += r1; else { kx += r1; ky += r2; }
+        float send = h16 ? kz : (h8 ? kx : ky);
+        float keep = h16 ? kz : (h8 ? ky : kx);
+        u = keep + __shfl_xor_sync(full, send, 8);
+        u += __shfl_xor_sync(full, u, 4);
+        u += __shfl_xor_sync(full, u, 2);
+        u += __shfl_xor_sync(full, u, 1);
+        X = __shfl_sync(full, u, 0); Y = __shfl_sync(full, u, 8); Z = __shfl_sync(full, u, 16);
+    }
+}
+
+// Plain xor butterfly for sub-warp groups (L < 32): every lane of the group gets every agent's totals.
+template <int NA>
+__device__ __forceinline__ void subwarp_allreduce(float (&x)[NA], float (&y)[NA], float (&z)[NA], float (&m)[NA],
+                                                  int L, unsigned mask) {
+    for (int off = L >> 1; off > 0; off >>= 1) {
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            x[a] += __shfl_xor_sync(mask, x[a], off);
+            y[a] += __shfl_xor_sync(mask, y[a], off);
+            z[a] += __shfl_xor_sync(mask, z[a], off);
+            m[a] = fminf(m[a], __shfl_xor_sync(mask, m[a], off));
+        }
+    }
+}
+
+// One agent's per-step state update and cost accumulation (Eq. 6-11, 17-20), executed by the lane(s) that own it.
+struct AgentX2 {
+    float p[3], v[3], ap[3];
+    CostAcc ca;
+    __device__ __forceinline__ void init(const float* s, const float* goal) {
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { p[i] = s[i]; v[i] = s[3 + i]; ap[i] = 0.0f; }
+        ca.init(norm3f(goal[0] - p[0], goal[1] - p[1], goal[2] - p[2]));
+    }
+    // state update only (the critical path): returns the net force for the cost part
+    __device__ __forceinline__ void integrate(const RolloutX2Params& P, float bx, float by, float bz,
+                                              float& fx, float& fy, float& fz, float& ex, float& ey, float& ez) {
+        ex = P.goal[0] - p[0]; ey = P.goal[1] - p[1]; ez = P.goal[2] - p[2];
+        cf_force_static(P.k_circ, bx, by, bz, v[0], v[1], v[2], fx, fy, fz);
+        fx = fmaf(P.k_att, ex, fmaf(-P.k_damp, v[0], fx));             // Eq. 6-7
+        fy = fmaf(P.k_att, ey, fmaf(-P.k_damp, v[1], fy));
+        fz = fmaf(P.k_att, ez, fmaf(-P.k_damp, v[2], fz));
+        v[0] = fmaf(P.c_lin, fx, v[0]); v[1] = fmaf(P.c_lin, fy, v[1]); v[2] = fmaf(P.c_lin, fz, v[2]);   // Eq. 9-10
+        p[0] = fmaf(P.dt, v[0], p[0]); p[1] = fmaf(P.dt, v[1], p[1]); p[2] = fmaf(P.dt, v[2], p[2]);      // Eq. 11
+    }
+    // costs of the pose the step started from (uses e = goal - p_old and that pose's clearance) and of the move
+    __device__ __forceinline__ void costs(const RolloutX2Params& P, int k, float dmin, float fx, float fy, float fz,
+                                          float ex, float ey, float ez) {
+        ca.pose(norm3f(ex, ey, ez), dmin, P.rcg, P.rco);
+        if (k >= 2) {                                                   // third difference = vf dt^2 (a_k - a_{k-1})
+            float jx = fx - ap[0], jy = fy - ap[1], jz = fz - ap[2];
+            ca.add_jerk(fmaf(jx, jx, fmaf(jy, jy, jz * jz)));
+        }
+        ap[0] = fx; ap[1] = fy; ap[2] = fz;
+        ca.add_len(norm3f(v[0], v[1], v[2]));                           // |p_new - p| = dt |v_new|
+    }
+    __device__ __forceinline__ void finish(const RolloutX2Params& P, int i, float dmin_final) {
+        ca.pose(norm3f(P.goal[0] - p[0], P.goal[1] - p[1], P.goal[2] - p[2]), dmin_final, P.rcg, P.rco);
+        const float cj = P.vel_factor * P.dt * P.dt * P.inv_mass;
+        const float Nk = float(P.steps) + 1.0f;
+        const float Lp = P.dt * ca.sumV, J = cj * cj * ca.sumJ, d1 = ca.d1;
+        float Cg = ca.sumG / Nk, Co = ca.sumO / Nk, Cp;
+        if (Lp == 0.0f && d1 == 0.0f) Cp = 0.0f;
+        else if (Lp >= d1) Cp = 1.0f - d1 / Lp;
+        else Cp = 1.0f - Lp / d1;
+        const float dt2 = P.dt * P.dt;
+        const float Cs = fminf(1.0f, J / (Nk * dt2 * dt2 * P.a_max * P.a_max));
+        float* out5 = P.cost + 5 * size_t(i);
+        out5[0] = P.w_goal * Cg + P.w_obs * Co + P.w_path * Cp + P.w_smooth * Cs;
+        out5[1] = Cg; out5[2] = Co; out5[3] = Cp; out5[4] = Cs;
+        P.minclr[i] = ca.minclr;
+        P.collided[i] = ca.collided;
+        if (P.agents_out) {
+            float* o = P.agents_out + 6 * size_t(i);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { o[c] = p[c]; o[3 + c] = v[c]; }
+        }
+    }
+};
+
+// ---------------------------------------------------------------------------------------------
+// group body, L >= 32: warp 0 of the group is the epilogue warp
+// ---------------------------------------------------------------------------------------------
+// shared exchange area per group: part[2][W][NA] float4 (x, y, z, dmin), state[2][NA][2] float4 (p,0),(v,0)
+template <int NA, bool CULL>
+__device__ __forceinline__ void group_rollout_wide(const RolloutX2Params& P, const float4* tA, const float4* tB,
+                                                   int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
+    const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
+    const int half = (NA == 2) ? (lane >> 4) : 0;          // which of the group's agents this lane integrates
+    const unsigned full = 0xffffffffu;
+    float4* part = xch;                                    // [2][W][NA]
+    float4* state = xch + 2 * W * NA;                      // [2][NA][2]
+    const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta;
+    float p[NA][3], v[NA][3];
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        const float* s = P.agents_in + 6 * size_t(first_agent + a);
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { p[a][i] = s[i]; v[a][i] = s[3 + i]; }
+    }
+    AgentX2 me;                                            // warp 0 only: the agent of this lane's half
+    if (wig == 0) me.init(P.agents_in + 6 * size_t(first_agent + half), P.goal);
+    X2Acc<NA> acc;
+    for (int k = 0; k <= P.steps; ++k) {
+        const bool last = (k == P.steps);                  // pose S+1: distance-only pass
+        acc.clear();
+        if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
+        else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
+        float x[NA], y[NA], z[NA], dm[NA];
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            float lo, hi;
+            upk2(acc.bx[a], lo, hi); x[a] = lo + hi;
+            upk2(acc.by[a], lo, hi); y[a] = lo + hi;
+            upk2(acc.bz[a], lo, hi); z[a] = lo + hi;
+            dm[a] = fkey_inv(__reduce_min_sync(full, fkey(acc.dmin[a])));
+        }
+        float X, Y, Z;
+        warp_sum3<NA>(x, y, z, lane, X, Y, Z);
+        float D = (NA == 2 && half) ? dm[NA - 1] : dm[0];
+        const int par = k & 1;
+        if (W > 1) {
+            if (wig != 0) {
+                if ((lane & 15) == 0 && (NA == 2 || lane == 0)) part[(par * W + wig) * NA + half] = make_float4(X, Y, Z, D);
+                named_bar_arrive(bar_part, P.L);
+                if (last) return;
+                named_bar_sync(bar_state, P.L);
+#pragma unroll
+                for (int a = 0; a < NA; ++a) {
+                    const float4 sp = state[(par * NA + a) * 2], sv = state[(par * NA + a) * 2 + 1];
+                    p[a][0] = sp.x; p[a][1] = sp.y; p[a][2] = sp.z; v[a][0] = sv.x; v[a][1] = sv.y; v[a][2] = sv.z;
+                }
+                continue;
+            }
+            named_bar_sync(bar_part, P.L);
+            for (int w = 1; w < W; ++w) {
+                const float4 o = part[(par * W + w) * NA + half];
+                X += o.x; Y += o.y; Z += o.z; D = fminf(D, o.w);
+            }
+        }
+        // epilogue warp: lanes of half h own agent h
+        if (last) {
+            if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.finish(P, first_agent + half, D);
+            return;
+        }
+        float fx, fy, fz, ex, ey, ez;
+        me.integrate(P, X, Y, Z, fx, fy, fz, ex, ey, ez);
+        if (W > 1) {
+            if ((lane & 15) == 0 && (NA == 2 || lane == 0)) {
+                state[(par * NA + half) * 2] = make_float4(me.p[0], me.p[1], me.p[2], 0.0f);
+                state[(par * NA + half) * 2 + 1] = make_float4(me.v[0], me.v[1], me.v[2], 0.0f);
+            }
+            named_bar_arrive(bar_state, P.L);
+        }
+        me.costs(P, k, D, fx, fy, fz, ex, ey, ez);
+        // this warp's own copy of both agents' state
+        if (NA == 2) {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+                p[0][i] = __shfl_sync(full, me.p[i], 0);  v[0][i] = __shfl_sync(full, me.v[i], 0);
+                p[NA - 1][i] = __shfl_sync(full, me.p[i], 16); v[NA - 1][i] = __shfl_sync(full, me.v[i], 16);
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// group body, L < 32 (several groups per warp): plain butterfly, every lane integrates its group's agents
+// ---------------------------------------------------------------------------------------------
+template <int NA, bool CULL>
+__device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, const float4* tA, const float4* tB,
+                                                     int first_agent, int lane_in_group) {
+    const unsigned mask = __activemask();
+    AgentX2 ag[NA];
+    float p[NA][3], v[NA][3];
+#pragma unroll
+    for (int a = 0; a < NA; ++a) ag[a].init(P.agents_in + 6 * size_t(first_agent + a), P.goal);
+    X2Acc<NA> acc;
+    for (int k = 0; k <= P.steps; ++k) {
+        const bool last = (k == P.steps);
+#pragma unroll
+        for (int a = 0; a < NA; ++a)
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { p[a][i] = ag[a].p[i]; v[a][i] = ag[a].v[i]; }
+        acc.clear();
+        if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, mask, acc);
+        else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, mask, acc);
+        float x[NA], y[NA], z[NA], dm[NA];
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            float lo, hi;
+            upk2(acc.bx[a], lo, hi); x[a] = lo + hi;
+            upk2(acc.by[a], lo, hi); y[a] = lo + hi;
+            upk2(acc.bz[a], lo, hi); z[a] = lo + hi;
+            dm[a] = acc.dmin[a];
+        }
+        subwarp_allreduce<NA>(x, y, z, dm, P.L, mask);
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            if (last) { if (lane_in_group == 0) ag[a].finish(P, first_agent + a, dm[a]); continue; }
+            float fx, fy, fz, ex, ey, ez;
+            ag[a].integrate(P, x[a], y[a], z[a], fx, fy, fz, ex, ey, ez);
+            ag[a].costs(P, k, dm[a], fx, fy, fz, ex, ey, ez);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// the kernel: one launch per planning cycle
+// ---------------------------------------------------------------------------------------------
+// AT = agents per group (1 or 2); WIDE = (L >= 32); STAGE 1 = sphere pairs staged in shared memory by TMA
+template <int AT, bool WIDE, bool CULL, int STAGE, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ RolloutX2Params P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
+    const float4* tA = P.pairA;
+    const float4* tB = P.pairB;
+    const int tid = threadIdx.x;
+    if (STAGE == 1) {
+        float4* tile = reinterpret_cast<float4*>(smem_raw + P.tile_off);
+        if (tid == 0) { mbar_init(bar, 1); fence_mbar_init(); }
+        __syncthreads();
+        if (tid == 0) {
+            const uint32_t bytes = uint32_t(P.n2p) * 16u;
+            mbar_arrive_expect_tx(bar, 2u * bytes);
+            const uint32_t chunk = 32768u;
+            for (uint32_t o = 0; o < bytes; o += chunk) {
+                const uint32_t nb = bytes - o < chunk ? bytes - o : chunk;
+                tma_bulk_g2s(reinterpret_cast<unsigned char*>(tile) + o, reinterpret_cast<const unsigned char*>(P.pairA) + o, nb, bar);
+                tma_bulk_g2s(reinterpret_cast<unsigned char*>(tile) + bytes + o, reinterpret_cast<const unsigned char*>(P.pairB) + o, nb, bar);
+            }
+        }
+        tA = tile;
+        tB = tile + P.n2p;
+    }
+    const int group_in_cta = tid >> P.logL;
+    const int lane_in_group = tid & (P.L - 1);
+    const int cta_first = blockIdx.x * P.agents_per_cta;
+    int cta_end = cta_first + P.agents_per_cta;
+    if (cta_end > P.n_agents) cta_end = P.n_agents;
+    const int first = cta_first + group_in_cta * AT;
+    const int na = cta_end - first;
+    if (STAGE == 1) mbar_wait(bar, 0);
+    if (na <= 0) return;
+    if (WIDE) {
+        const int W = P.L >> 5;
+        float4* xch = reinterpret_cast<float4*>(smem_raw + P.xch_off) + group_in_cta * (2 * W * 2 + 2 * 2 * 2);
+        if (AT == 2 && na >= 2) group_rollout_wide<(AT == 2 ? 2 : 1), CULL>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
+        else group_rollout_wide<1, CULL>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
+    } else {
+        if (AT == 2 && na >= 2) group_rollout_narrow<(AT == 2 ? 2 : 1), CULL>(P, tA, tB, first, lane_in_group);
+        else group_rollout_narrow<1, CULL>(P, tA, tB, first, lane_in_group);
+    }
+}
+
+// pack (xyz, r) -> sphere-pair layout; R = r + r_agent stored negated; sentinel pairs up to n2_fill
+__global__ void k_pack_pairs(const float4* __restrict__ sph_raw, int n, int n2_fill, float r_agent,
+                             float4* __restrict__ pairA, float4* __restrict__ pairB) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n2_fill) return;
+    const float far = 1.0e18f;
+    float4 s0 = make_float4(far, far, far, 0.0f), s1 = s0;
+    if (2 * j < n) { s0 = sph_raw[2 * j]; s0.w += r_agent; }
+    if (2 * j + 1 < n) { s1 = sph_raw[2 * j + 1]; s1.w += r_agent; }
+    pairA[j] = make_float4(s0.x, s1.x, s0.y, s1.y);
+    pairB[j] = make_float4(s0.z, s1.z, -s0.w, -s1.w);
+}
+
+}  // namespace gmapp

@@ -289,6 +289,8 @@ def test_pose6_large_rotation_fast_twist(api, ctx, orc):
     dict(lanes_per_agent=256, agents_per_thread=1), dict(lanes_per_agent=64, agents_per_thread=2, cull=1),
     dict(lanes_per_agent=16, agents_per_thread=2, cull=1, stage=0), dict(stage=0), dict(cull=1),
     dict(max_ctas=5), dict(max_ctas=5, cull=1, agents_per_thread=1),
+    dict(scalar_path=1), dict(scalar_path=1, lanes_per_agent=128, agents_per_thread=2, cull=1),
+    dict(lanes_per_agent=512, agents_per_thread=1), dict(lanes_per_agent=1, agents_per_thread=2, max_ctas=3),
 ], ids=lambda t: "-".join(f"{k[:4]}{v}" for k, v in t.items()))
 def test_launch_variants_match_oracle(api, ctx, orc, tuning):
     try:
