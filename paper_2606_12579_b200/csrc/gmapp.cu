@@ -91,13 +91,13 @@ static rollout_fn rollout_kernel(int kind, int at, bool moving, bool cull, int s
 #undef PICK
 }
 typedef void (*rollout_x2_fn)(const RolloutX2Params);
-static const int kX2MaxThreads = 512;
-static rollout_x2_fn rollout_x2_kernel(int at, bool wide, bool cull, int stage) {
-#define PICKX(A, W)                                                                                                  \
-    (cull ? (stage ? (rollout_x2_fn)k_rollout_x2<A, W, true, 1, 512> : (rollout_x2_fn)k_rollout_x2<A, W, true, 0, 512>)     \
-          : (stage ? (rollout_x2_fn)k_rollout_x2<A, W, false, 1, 512> : (rollout_x2_fn)k_rollout_x2<A, W, false, 0, 512>))
-    if (at == 2) return wide ? PICKX(2, true) : PICKX(2, false);
-    return wide ? PICKX(1, true) : PICKX(1, false);
+static const int kX2SweepThreads = 512;       // sweep threads per CTA; mode 2 adds one epilogue warp per group (<= 672 in all)
+static rollout_x2_fn rollout_x2_kernel(int at, int mode, bool cull, int stage) {
+#define PICKX(A, M, MT)                                                                                              \
+    (cull ? (stage ? (rollout_x2_fn)k_rollout_x2<A, M, true, 1, MT> : (rollout_x2_fn)k_rollout_x2<A, M, true, 0, MT>)     \
+          : (stage ? (rollout_x2_fn)k_rollout_x2<A, M, false, 1, MT> : (rollout_x2_fn)k_rollout_x2<A, M, false, 0, MT>))
+    if (at == 2) return mode == 2 ? PICKX(2, 2, 672) : (mode == 1 ? PICKX(2, 1, 512) : PICKX(2, 0, 512));
+    return mode == 2 ? PICKX(1, 2, 672) : (mode == 1 ? PICKX(1, 1, 512) : PICKX(1, 0, 512));
 #undef PICKX
 }
 static int rollout_max_threads(int kind, int at) { return (kind == GMAPP_MOTOR6 || at == 2) ? 512 : 1024; }
@@ -161,10 +161,10 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
                         if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
                     }
     for (int at = 1; at <= 2; ++at)
-        for (int wd = 0; wd < 2; ++wd)
+        for (int md = 0; md < 3; ++md)
             for (int cu = 0; cu < 2; ++cu)
                 for (int st = 0; st < 2; ++st) {
-                    e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, wd, cu, st),
+                    e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, md, cu, st),
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
                     if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
                 }
@@ -370,7 +370,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     int at = A >= 2 ? 2 : 1;
     if (t && t->agents_per_thread) at = t->agents_per_thread;
     const int G = (A + at - 1) / at;                              // groups per CTA
-    const int tmax = kX2MaxThreads;
+    const int tmax = kX2SweepThreads;
     if (G > tmax) return fail(c, GMAPP_ECAPACITY, "rollout: %s%ld agent groups per CTA exceed %ld threads", "", G, tmax);
     const int ns = c->n_spheres;
     const int n2 = (ns + 1) / 2;
@@ -385,7 +385,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
         if (L > cap) L = cap;
         if (L > 32 && G > 7) L = 32;                              // two named barriers per multi-warp group
     }
-    const bool wide = L >= 32;
+    const int mode = L >= 64 ? 2 : (L == 32 ? 1 : 0);
     const int n2p = n2 > 0 ? round_up(n2, L) : 0;
     const int cull = (t && t->cull >= 0) ? t->cull : 0;
     // dynamic shared memory: [0,64) mbarrier; [64, 64+4 KB) cross-warp exchange; sphere-pair tile at 4224
@@ -419,9 +419,9 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     P.w_goal = g->w_goal; P.w_obs = g->w_obs; P.w_path = g->w_path; P.w_smooth = g->w_smooth; P.a_max = g->a_max;
     P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
     P.tile_off = tile_off; P.xch_off = xch_off;
-    const int block = round_up(G * L, 32);
+    const int block = mode == 2 ? G * L + 32 * G : round_up(G * L, 32);
     const int smem = tile_off + (stage == 1 ? (int)tile_bytes : 0);
-    rollout_x2_fn fn = rollout_x2_kernel(at, wide, cull != 0, stage);
+    rollout_x2_fn fn = rollout_x2_kernel(at, mode, cull != 0, stage);
     fn<<<grid, block, smem, st>>>(P);
     CUDA_TRY(c, cudaGetLastError());
     ++launches;

@@ -11,11 +11,11 @@
 //    sums are combined by a TRANSPOSED xor-butterfly (each step halves the number of live values: 8 SHFL
 //    for 6 values instead of 30), the clearance minimum by one REDUX.MIN on an order-preserving integer
 //    key.  Fixed order, no atomics: bit-reproducible.
-//  * When a group spans several warps (L > 32), warps 1.. post their partial sums to shared memory and
-//    warp 0 alone adds them, integrates BOTH agents at once (agent a on lanes 0-15, agent b on lanes
-//    16-31), accumulates the costs and publishes the new state; the other warps pick it up after a named
-//    barrier.  Split arrive / sync barriers and parity double-buffering: one round trip per step, and the
-//    cost arithmetic runs after the state has been published.
+//  * When a group spans several warps (L >= 64) its W = L/32 sweep warps post their partial sums to shared
+//    memory and a dedicated EPILOGUE WARP of the group adds them, integrates BOTH agents at once (agent a on
+//    lanes 0-15, agent b on lanes 16-31), publishes the new state and only then accumulates the costs; the
+//    sweep warps pick the state up after a named barrier.  Split arrive / sync barriers and parity double-
+//    buffering: one round trip per step; what does not need the sums is computed before the wait.
 //
 // Shares nothing with oracle/.
 #pragma once
@@ -186,20 +186,28 @@ struct AgentX2 {
         for (int i = 0; i < 3; ++i) { p[i] = s[i]; v[i] = s[3 + i]; ap[i] = 0.0f; }
         ca.init(norm3f(goal[0] - p[0], goal[1] - p[1], goal[2] - p[2]));
     }
-    // state update only (the critical path): returns the net force for the cost part
-    __device__ __forceinline__ void integrate(const RolloutX2Params& P, float bx, float by, float bz,
-                                              float& fx, float& fy, float& fz, float& ex, float& ey, float& ez) {
+    // Part of the state update that does not need the sphere sums (runs while the sums are still in flight):
+    // e = goal - p, 1/|v| (MUFU.RSQ + Newton), |v|, and the attractor f_a = k_att e - k_damp v (Eq. 7).
+    float ex, ey, ez, inv, nv, fax, fay, faz;
+    __device__ __forceinline__ void pre(const RolloutX2Params& P) {
         ex = P.goal[0] - p[0]; ey = P.goal[1] - p[1]; ez = P.goal[2] - p[2];
-        cf_force_static(P.k_circ, bx, by, bz, v[0], v[1], v[2], fx, fy, fz);
-        fx = fmaf(P.k_att, ex, fmaf(-P.k_damp, v[0], fx));             // Eq. 6-7
-        fy = fmaf(P.k_att, ey, fmaf(-P.k_damp, v[1], fy));
-        fz = fmaf(P.k_att, ez, fmaf(-P.k_damp, v[2], fz));
-        v[0] = fmaf(P.c_lin, fx, v[0]); v[1] = fmaf(P.c_lin, fy, v[1]); v[2] = fmaf(P.c_lin, fz, v[2]);   // Eq. 9-10
-        p[0] = fmaf(P.dt, v[0], p[0]); p[1] = fmaf(P.dt, v[1], p[1]); p[2] = fmaf(P.dt, v[2], p[2]);      // Eq. 11
+        const float n2 = fmaf(v[0], v[0], fmaf(v[1], v[1], fmaf(v[2], v[2], kTiny)));
+        inv = rsqrt_approx(n2);
+        inv = inv * fmaf(-0.5f * n2 * inv, inv, 1.5f);
+        nv = n2 * inv;
+        fax = fmaf(P.k_att, ex, -P.k_damp * v[0]); fay = fmaf(P.k_att, ey, -P.k_damp * v[1]); faz = fmaf(P.k_att, ez, -P.k_damp * v[2]);
+    }
+    // The critical path once the sums B are known: f_r = k_f [((B.v)/|v|) v - |v| B] (BAC-CAB form of Eq. 2-3),
+    // f = f_a + f_r (Eq. 6), v += vel_factor dt inv_mass f (Eq. 9-10), p += dt v (Eq. 11).
+    __device__ __forceinline__ void post(const RolloutX2Params& P, float bx, float by, float bz, float& fx, float& fy, float& fz) {
+        const float A = fmaf(bx, v[0], fmaf(by, v[1], bz * v[2]));
+        const float c1 = P.k_circ * inv * A, c2 = -P.k_circ * nv;
+        fx = fmaf(c1, v[0], fmaf(c2, bx, fax)); fy = fmaf(c1, v[1], fmaf(c2, by, fay)); fz = fmaf(c1, v[2], fmaf(c2, bz, faz));
+        v[0] = fmaf(P.c_lin, fx, v[0]); v[1] = fmaf(P.c_lin, fy, v[1]); v[2] = fmaf(P.c_lin, fz, v[2]);
+        p[0] = fmaf(P.dt, v[0], p[0]); p[1] = fmaf(P.dt, v[1], p[1]); p[2] = fmaf(P.dt, v[2], p[2]);
     }
     // costs of the pose the step started from (uses e = goal - p_old and that pose's clearance) and of the move
-    __device__ __forceinline__ void costs(const RolloutX2Params& P, int k, float dmin, float fx, float fy, float fz,
-                                          float ex, float ey, float ez) {
+    __device__ __forceinline__ void costs(const RolloutX2Params& P, int k, float dmin, float fx, float fy, float fz) {
         ca.pose(norm3f(ex, ey, ez), dmin, P.rcg, P.rco);
         if (k >= 2) {                                                   // third difference = vf dt^2 (a_k - a_{k-1})
             float jx = fx - ap[0], jy = fy - ap[1], jz = fz - ap[2];
@@ -233,18 +241,80 @@ struct AgentX2 {
 };
 
 // ---------------------------------------------------------------------------------------------
-// group body, L >= 32: warp 0 of the group is the epilogue warp
+// warp-level combine shared by the L >= 32 bodies: per-lane partials -> (X, Y, Z, D) of the agent owned by
+// this lane's half (NA == 2: lanes 0-15 agent 0, lanes 16-31 agent 1; NA == 1: the one agent on all lanes)
 // ---------------------------------------------------------------------------------------------
-// shared exchange area per group: part[2][W][NA] float4 (x, y, z, dmin), state[2][NA][2] float4 (p,0),(v,0)
+template <int NA>
+__device__ __forceinline__ void warp_combine(const X2Acc<NA>& acc, int lane, float& X, float& Y, float& Z, float& D) {
+    float x[NA], y[NA], z[NA], dm[NA];
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        float lo, hi;
+        upk2(acc.bx[a], lo, hi); x[a] = lo + hi;
+        upk2(acc.by[a], lo, hi); y[a] = lo + hi;
+        upk2(acc.bz[a], lo, hi); z[a] = lo + hi;
+        dm[a] = fkey_inv(__reduce_min_sync(0xffffffffu, fkey(acc.dmin[a])));
+    }
+    warp_sum3<NA>(x, y, z, lane, X, Y, Z);
+    D = (NA == 2 && (lane & 16)) ? dm[NA - 1] : dm[0];
+}
+
+// ---------------------------------------------------------------------------------------------
+// group body, L == 32: one warp per group does everything; agent a on lanes 0-15, agent b on lanes 16-31
+// ---------------------------------------------------------------------------------------------
 template <int NA, bool CULL>
-__device__ __forceinline__ void group_rollout_wide(const RolloutX2Params& P, const float4* tA, const float4* tB,
-                                                   int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
+__device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, const float4* tA, const float4* tB,
+                                                   int first_agent, int lane) {
+    const int half = (NA == 2) ? (lane >> 4) : 0;
+    const unsigned full = 0xffffffffu;
+    AgentX2 me;
+    me.init(P.agents_in + 6 * size_t(first_agent + half), P.goal);
+    float p[NA][3], v[NA][3];
+    X2Acc<NA> acc;
+    for (int k = 0; k <= P.steps; ++k) {
+        const bool last = (k == P.steps);                  // pose S+1: distance-only pass
+        if (NA == 2) {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+                p[0][i] = __shfl_sync(full, me.p[i], 0);       v[0][i] = __shfl_sync(full, me.v[i], 0);
+                p[NA - 1][i] = __shfl_sync(full, me.p[i], 16); v[NA - 1][i] = __shfl_sync(full, me.v[i], 16);
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
+        }
+        acc.clear();
+        if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc);
+        else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc);
+        float X, Y, Z, D;
+        warp_combine<NA>(acc, lane, X, Y, Z, D);
+        if (last) {
+            if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.finish(P, first_agent + half, D);
+            return;
+        }
+        float fx, fy, fz;
+        me.pre(P);
+        me.post(P, X, Y, Z, fx, fy, fz);
+        me.costs(P, k, D, fx, fy, fz);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// group bodies, L >= 64: W = L/32 sweep warps + ONE epilogue warp per group.
+// shared exchange area per group: part[2][W][NA] float4 (X, Y, Z, dmin), state[2][NA][2] float4 (p,0), (v,0);
+// both double-buffered by step parity, so one arrive/sync pair per direction and step is race-free:
+//   sweep warp k:    write part[k&1] -> arrive(bar_part) -> sync(bar_state) -> read state[k&1]
+//   epilogue warp k: sync(bar_part) -> read part[k&1] -> integrate -> write state[k&1] -> arrive(bar_state) -> costs
+// ---------------------------------------------------------------------------------------------
+template <int NA, bool CULL>
+__device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, const float4* tA, const float4* tB,
+                                                  int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
     const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
-    const int half = (NA == 2) ? (lane >> 4) : 0;          // which of the group's agents this lane integrates
+    const int half = (NA == 2) ? (lane >> 4) : 0;
     const unsigned full = 0xffffffffu;
     float4* part = xch;                                    // [2][W][NA]
-    float4* state = xch + 2 * W * NA;                      // [2][NA][2]
-    const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta;
+    const float4* state = xch + 2 * W * NA;                // [2][NA][2]
+    const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
     float p[NA][3], v[NA][3];
 #pragma unroll
     for (int a = 0; a < NA; ++a) {
@@ -252,72 +322,59 @@ __device__ __forceinline__ void group_rollout_wide(const RolloutX2Params& P, con
 #pragma unroll
         for (int i = 0; i < 3; ++i) { p[a][i] = s[i]; v[a][i] = s[3 + i]; }
     }
-    AgentX2 me;                                            // warp 0 only: the agent of this lane's half
-    if (wig == 0) me.init(P.agents_in + 6 * size_t(first_agent + half), P.goal);
     X2Acc<NA> acc;
     for (int k = 0; k <= P.steps; ++k) {
-        const bool last = (k == P.steps);                  // pose S+1: distance-only pass
+        const bool last = (k == P.steps);
         acc.clear();
         if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
         else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
-        float x[NA], y[NA], z[NA], dm[NA];
+        float X, Y, Z, D;
+        warp_combine<NA>(acc, lane, X, Y, Z, D);
+        const int par = k & 1;
+        if ((lane & 15) == 0 && (NA == 2 || lane == 0)) part[(par * W + wig) * NA + half] = make_float4(X, Y, Z, D);
+        named_bar_arrive(bar_part, nbar);
+        if (last) return;
+        named_bar_sync(bar_state, nbar);
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
-            float lo, hi;
-            upk2(acc.bx[a], lo, hi); x[a] = lo + hi;
-            upk2(acc.by[a], lo, hi); y[a] = lo + hi;
-            upk2(acc.bz[a], lo, hi); z[a] = lo + hi;
-            dm[a] = fkey_inv(__reduce_min_sync(full, fkey(acc.dmin[a])));
+            const float4 sp = state[(par * NA + a) * 2], sv = state[(par * NA + a) * 2 + 1];
+            p[a][0] = sp.x; p[a][1] = sp.y; p[a][2] = sp.z; v[a][0] = sv.x; v[a][1] = sv.y; v[a][2] = sv.z;
         }
-        float X, Y, Z;
-        warp_sum3<NA>(x, y, z, lane, X, Y, Z);
-        float D = (NA == 2 && half) ? dm[NA - 1] : dm[0];
+    }
+}
+
+template <int NA>
+__device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, int first_agent, int lane,
+                                                    int group_in_cta, float4* xch) {
+    const int W = P.L >> 5;
+    const int half = (NA == 2) ? (lane >> 4) : 0;
+    const float4* part = xch;
+    float4* state = xch + 2 * W * NA;
+    const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
+    AgentX2 me;
+    me.init(P.agents_in + 6 * size_t(first_agent + half), P.goal);
+    for (int k = 0; k <= P.steps; ++k) {
+        const bool last = (k == P.steps);
         const int par = k & 1;
-        if (W > 1) {
-            if (wig != 0) {
-                if ((lane & 15) == 0 && (NA == 2 || lane == 0)) part[(par * W + wig) * NA + half] = make_float4(X, Y, Z, D);
-                named_bar_arrive(bar_part, P.L);
-                if (last) return;
-                named_bar_sync(bar_state, P.L);
-#pragma unroll
-                for (int a = 0; a < NA; ++a) {
-                    const float4 sp = state[(par * NA + a) * 2], sv = state[(par * NA + a) * 2 + 1];
-                    p[a][0] = sp.x; p[a][1] = sp.y; p[a][2] = sp.z; v[a][0] = sv.x; v[a][1] = sv.y; v[a][2] = sv.z;
-                }
-                continue;
-            }
-            named_bar_sync(bar_part, P.L);
-            for (int w = 1; w < W; ++w) {
-                const float4 o = part[(par * W + w) * NA + half];
-                X += o.x; Y += o.y; Z += o.z; D = fminf(D, o.w);
-            }
+        me.pre(P);                                         // everything that does not need the sphere sums
+        named_bar_sync(bar_part, nbar);
+        float4 t = part[(par * W) * NA + half];
+        for (int w = 1; w < W; ++w) {
+            const float4 o = part[(par * W + w) * NA + half];
+            t.x += o.x; t.y += o.y; t.z += o.z; t.w = fminf(t.w, o.w);
         }
-        // epilogue warp: lanes of half h own agent h
         if (last) {
-            if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.finish(P, first_agent + half, D);
+            if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.finish(P, first_agent + half, t.w);
             return;
         }
-        float fx, fy, fz, ex, ey, ez;
-        me.integrate(P, X, Y, Z, fx, fy, fz, ex, ey, ez);
-        if (W > 1) {
-            if ((lane & 15) == 0 && (NA == 2 || lane == 0)) {
-                state[(par * NA + half) * 2] = make_float4(me.p[0], me.p[1], me.p[2], 0.0f);
-                state[(par * NA + half) * 2 + 1] = make_float4(me.v[0], me.v[1], me.v[2], 0.0f);
-            }
-            named_bar_arrive(bar_state, P.L);
+        float fx, fy, fz;
+        me.post(P, t.x, t.y, t.z, fx, fy, fz);
+        if ((lane & 15) == 0 && (NA == 2 || lane == 0)) {
+            state[(par * NA + half) * 2] = make_float4(me.p[0], me.p[1], me.p[2], 0.0f);
+            state[(par * NA + half) * 2 + 1] = make_float4(me.v[0], me.v[1], me.v[2], 0.0f);
         }
-        me.costs(P, k, D, fx, fy, fz, ex, ey, ez);
-        // this warp's own copy of both agents' state
-        if (NA == 2) {
-#pragma unroll
-            for (int i = 0; i < 3; ++i) {
-                p[0][i] = __shfl_sync(full, me.p[i], 0);  v[0][i] = __shfl_sync(full, me.v[i], 0);
-                p[NA - 1][i] = __shfl_sync(full, me.p[i], 16); v[NA - 1][i] = __shfl_sync(full, me.v[i], 16);
-            }
-        } else {
-#pragma unroll
-            for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
-        }
+        named_bar_arrive(bar_state, nbar);
+        me.costs(P, k, t.w, fx, fy, fz);                   // off the critical path: the sweep warps are already running
     }
 }
 
@@ -355,9 +412,10 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
             if (last) { if (lane_in_group == 0) ag[a].finish(P, first_agent + a, dm[a]); continue; }
-            float fx, fy, fz, ex, ey, ez;
-            ag[a].integrate(P, x[a], y[a], z[a], fx, fy, fz, ex, ey, ez);
-            ag[a].costs(P, k, dm[a], fx, fy, fz, ex, ey, ez);
+            float fx, fy, fz;
+            ag[a].pre(P);
+            ag[a].post(P, x[a], y[a], z[a], fx, fy, fz);
+            ag[a].costs(P, k, dm[a], fx, fy, fz);
         }
     }
 }
@@ -365,8 +423,10 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 // ---------------------------------------------------------------------------------------------
 // the kernel: one launch per planning cycle
 // ---------------------------------------------------------------------------------------------
-// AT = agents per group (1 or 2); WIDE = (L >= 32); STAGE 1 = sphere pairs staged in shared memory by TMA
-template <int AT, bool WIDE, bool CULL, int STAGE, int MAXT>
+// AT = agents per group (1 or 2); MODE 0: L < 32 (sub-warp groups), 1: L == 32 (one warp per group),
+// 2: L >= 64 (W sweep warps + one epilogue warp per group; threads [0, G L) sweep, [G L, G L + 32 G) epilogue);
+// STAGE 1 = sphere pairs staged in shared memory by TMA bulk copies
+template <int AT, int MODE, bool CULL, int STAGE, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ RolloutX2Params P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
@@ -390,22 +450,43 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         tA = tile;
         tB = tile + P.n2p;
     }
-    const int group_in_cta = tid >> P.logL;
-    const int lane_in_group = tid & (P.L - 1);
     const int cta_first = blockIdx.x * P.agents_per_cta;
     int cta_end = cta_first + P.agents_per_cta;
     if (cta_end > P.n_agents) cta_end = P.n_agents;
+    constexpr int NA2 = (AT == 2) ? 2 : 1;
+    if (MODE == 2) {
+        const int G = (P.agents_per_cta + AT - 1) / AT;
+        const int W = P.L >> 5;
+        const int n_sweep = G * P.L;
+        const bool is_epi = tid >= n_sweep;
+        const int group_in_cta = is_epi ? ((tid - n_sweep) >> 5) : (tid >> P.logL);
+        const int first = cta_first + group_in_cta * AT;
+        const int na = cta_end - first;
+        float4* xch = reinterpret_cast<float4*>(smem_raw + P.xch_off) + group_in_cta * (2 * W * 2 + 2 * 2 * 2);
+        if (is_epi) {                                      // the epilogue warps never touch the sphere tile
+            if (na <= 0) return;
+            if (AT == 2 && na >= 2) group_epilogue_warp<NA2>(P, first, tid & 31, group_in_cta, xch);
+            else group_epilogue_warp<1>(P, first, tid & 31, group_in_cta, xch);
+            return;
+        }
+        if (STAGE == 1) mbar_wait(bar, 0);
+        if (na <= 0) return;
+        const int lane_in_group = tid & (P.L - 1);
+        if (AT == 2 && na >= 2) group_sweep_warps<NA2, CULL>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
+        else group_sweep_warps<1, CULL>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
+        return;
+    }
+    const int group_in_cta = tid >> P.logL;
+    const int lane_in_group = tid & (P.L - 1);
     const int first = cta_first + group_in_cta * AT;
     const int na = cta_end - first;
     if (STAGE == 1) mbar_wait(bar, 0);
     if (na <= 0) return;
-    if (WIDE) {
-        const int W = P.L >> 5;
-        float4* xch = reinterpret_cast<float4*>(smem_raw + P.xch_off) + group_in_cta * (2 * W * 2 + 2 * 2 * 2);
-        if (AT == 2 && na >= 2) group_rollout_wide<(AT == 2 ? 2 : 1), CULL>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
-        else group_rollout_wide<1, CULL>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
+    if (MODE == 1) {
+        if (AT == 2 && na >= 2) group_rollout_warp<NA2, CULL>(P, tA, tB, first, lane_in_group);
+        else group_rollout_warp<1, CULL>(P, tA, tB, first, lane_in_group);
     } else {
-        if (AT == 2 && na >= 2) group_rollout_narrow<(AT == 2 ? 2 : 1), CULL>(P, tA, tB, first, lane_in_group);
+        if (AT == 2 && na >= 2) group_rollout_narrow<NA2, CULL>(P, tA, tB, first, lane_in_group);
         else group_rollout_narrow<1, CULL>(P, tA, tB, first, lane_in_group);
     }
 }
