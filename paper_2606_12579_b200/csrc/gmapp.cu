@@ -92,12 +92,14 @@ static rollout_fn rollout_kernel(int kind, int at, bool moving, bool cull, int s
 }
 typedef void (*rollout_x2_fn)(const RolloutX2Params);
 static const int kX2SweepThreads = 512;       // sweep threads per CTA; mode 2 adds one epilogue warp per group (<= 672 in all)
+// mode 3 = mode 2 compiled for up to 7 groups (21 warps, 80 registers); mode 2 proper holds <= 4 groups
+// (20 warps = 5 per SM sub-partition, 96 registers), which is what one wave of config 3 needs
 static rollout_x2_fn rollout_x2_kernel(int at, int mode, bool cull, int stage) {
 #define PICKX(A, M, MT)                                                                                              \
     (cull ? (stage ? (rollout_x2_fn)k_rollout_x2<A, M, true, 1, MT> : (rollout_x2_fn)k_rollout_x2<A, M, true, 0, MT>)     \
           : (stage ? (rollout_x2_fn)k_rollout_x2<A, M, false, 1, MT> : (rollout_x2_fn)k_rollout_x2<A, M, false, 0, MT>))
-    if (at == 2) return mode == 2 ? PICKX(2, 2, 672) : (mode == 1 ? PICKX(2, 1, 512) : PICKX(2, 0, 512));
-    return mode == 2 ? PICKX(1, 2, 672) : (mode == 1 ? PICKX(1, 1, 512) : PICKX(1, 0, 512));
+    if (at == 2) return mode == 3 ? PICKX(2, 2, 672) : (mode == 2 ? PICKX(2, 2, 640) : (mode == 1 ? PICKX(2, 1, 512) : PICKX(2, 0, 512)));
+    return mode == 3 ? PICKX(1, 2, 672) : (mode == 2 ? PICKX(1, 2, 640) : (mode == 1 ? PICKX(1, 1, 512) : PICKX(1, 0, 512)));
 #undef PICKX
 }
 static int rollout_max_threads(int kind, int at) { return (kind == GMAPP_MOTOR6 || at == 2) ? 512 : 1024; }
@@ -161,7 +163,7 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
                         if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
                     }
     for (int at = 1; at <= 2; ++at)
-        for (int md = 0; md < 3; ++md)
+        for (int md = 0; md < 4; ++md)
             for (int cu = 0; cu < 2; ++cu)
                 for (int st = 0; st < 2; ++st) {
                     e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, md, cu, st),
@@ -385,7 +387,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
         if (L > cap) L = cap;
         if (L > 32 && G > 7) L = 32;                              // two named barriers per multi-warp group
     }
-    const int mode = L >= 64 ? 2 : (L == 32 ? 1 : 0);
+    const int mode = L >= 64 ? (G <= 4 ? 2 : 3) : (L == 32 ? 1 : 0);
     const int n2p = n2 > 0 ? round_up(n2, L) : 0;
     const int cull = (t && t->cull >= 0) ? t->cull : 0;
     // dynamic shared memory: [0,64) mbarrier; [64, 64+4 KB) cross-warp exchange; sphere-pair tile at 4224
@@ -419,7 +421,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     P.w_goal = g->w_goal; P.w_obs = g->w_obs; P.w_path = g->w_path; P.w_smooth = g->w_smooth; P.a_max = g->a_max;
     P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
     P.tile_off = tile_off; P.xch_off = xch_off;
-    const int block = mode == 2 ? G * L + 32 * G : round_up(G * L, 32);
+    const int block = mode >= 2 ? G * L + 32 * G : round_up(G * L, 32);
     const int smem = tile_off + (stage == 1 ? (int)tile_bytes : 0);
     rollout_x2_fn fn = rollout_x2_kernel(at, mode, cull != 0, stage);
     fn<<<grid, block, smem, st>>>(P);
