@@ -35,9 +35,10 @@ FLOP_PER_PAIR = 35.0
 # FP32 peak from the guide's unit counts and clock: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz
 NOMINAL_SMS, LANES_PER_SM, MAX_GHZ = 148, 128, 1.965
 PEAK_TFLOPS = NOMINAL_SMS * LANES_PER_SM * 2 * MAX_GHZ / 1e3
-# dram__bytes_read.sum + dram__bytes_write.sum of one rollout launch from the committed ncu capture
-# (profiles/); None until a capture exists
-TRAFFIC_BYTES_PER_LAUNCH = None
+# dram__bytes_read.sum + dram__bytes_write.sum of one config-3 rollout launch from the committed ncu capture
+# (profiles/r01_rollout_x2_full.md): 130.6 KB read + 0 B written (algorithmic: 64 KB spheres + 24 KB agents in,
+# 36 KB results out, which stay in L2).  Only valid for the config-3 workload.
+TRAFFIC_BYTES_PER_LAUNCH = {"config3": 130560}
 
 
 def parse_args():
@@ -280,6 +281,19 @@ def run_ours(args):
     bf_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in rev]))
     info_bf = ctx.launch_info()
     achieved = pairs_local * FLOP_PER_PAIR / (bf_ms * 1e-3) / 1e12
+    # ---- the warp-vote variant (cull=1: the force math is skipped where no lane's pair is inside r_d; results
+    # are bit-identical).  Reported beside the headline, never as the roofline numerator.
+    ctx.set_tuning(**{**tune, "cull": 1})
+    for _ in range(3):
+        ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
+    torch.cuda.synchronize(dev)
+    for i in range(K):
+        flush.zero_()
+        rev[i][0].record()
+        ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
+        rev[i][1].record()
+    torch.cuda.synchronize(dev)
+    cull_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in rev]))
     ctx.set_tuning(**tune)
     peak_meas = ctx.measure_fp32_peak(False)
     peak_meas_x2 = ctx.measure_fp32_peak(True)
@@ -327,13 +341,16 @@ def run_ours(args):
                     "call": "gmapp_plan_cycle_host (host spheres + agents in, best index out)"},
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_TFLOPS, "unit": "TFLOP/s",
-                         "frac": achieved / PEAK_TFLOPS, "traffic": TRAFFIC_BYTES_PER_LAUNCH,
+                         "frac": achieved / PEAK_TFLOPS, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.config) if world == 1 else None,
                          "kernel": "k_rollout (branch-free variant, cull=0)", "kernel_ms": bf_ms,
                          "flop_per_pair": FLOP_PER_PAIR, "pairs_per_launch": pairs_local,
                          "peak_how": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (guide unit counts, max clock)",
                          "peak_measured_ffma_tflops": peak_meas, "peak_measured_ffma2_tflops": peak_meas_x2,
                          "frac_of_measured_ffma": achieved / peak_meas if peak_meas else None,
                          "launch": info_bf},
+            "cull_variant": {"kernel_ms": cull_ms, "interactions_per_s": pairs_local / (cull_ms * 1e-3),
+                             "note": "same kernel with the warp-vote skip of the force math (tuning cull=1); "
+                                     "bit-identical results; not used for the roofline"},
             "clocks": sampler.summary(),
         }
         if world == 1 and not args.no_cpu_baseline:
