@@ -102,7 +102,7 @@ class ClockSampler:
                         self.reasons.add(nm)
             except Exception:
                 pass
-            self._stop.wait(0.01)
+            self._stop.wait(0.002)
 
     def __enter__(self):
         if self.ok:
@@ -135,11 +135,16 @@ def oracle_rate(scene, target_seconds: float):
     t_probe = max(time.perf_counter() - t0, 1e-4)
     n = int(min(n_all, max(probe, (target_seconds / t_probe) * probe)))
     n = max(cores, (n // cores) * cores) if n >= cores else n
+    # when the whole workload takes less than the target, repeat it so the sample is still ~target seconds of CPU work
+    t_est = t_probe * n / probe
+    reps = int(max(1, min(50, round(target_seconds / max(t_est, 1e-3))))) if n == n_all else 1
     t0 = time.perf_counter()
-    oracle.rollout_scene(scene, threads=cores, agent_slice=slice(0, n))
+    for _ in range(reps):
+        oracle.rollout_scene(scene, threads=cores, agent_slice=slice(0, n))
     dt = time.perf_counter() - t0
-    pairs = float(n) * scene.n_spheres * scene.steps
-    sample = f"first {n} of {n_all} agents x {scene.n_spheres} spheres x {scene.steps} steps, OpenMP over agents"
+    pairs = float(n) * scene.n_spheres * scene.steps * reps
+    sample = (f"first {n} of {n_all} agents x {scene.n_spheres} spheres x {scene.steps} steps, OpenMP over agents"
+              + (f", repeated {reps}x" if reps > 1 else ""))
     return pairs / dt, cores, sample, dt
 
 
