@@ -98,6 +98,7 @@ static rollout_x2_fn rollout_x2_kernel(int at, int mode, bool cull, int stage) {
 #define PICKX(A, M, MT)                                                                                              \
     (cull ? (stage ? (rollout_x2_fn)k_rollout_x2<A, M, true, 1, MT> : (rollout_x2_fn)k_rollout_x2<A, M, true, 0, MT>)     \
           : (stage ? (rollout_x2_fn)k_rollout_x2<A, M, false, 1, MT> : (rollout_x2_fn)k_rollout_x2<A, M, false, 0, MT>))
+    if (mode == 4) return PICKX(2, 4, 512);
     if (at == 2) return mode == 3 ? PICKX(2, 2, 672) : (mode == 2 ? PICKX(2, 2, 640) : (mode == 1 ? PICKX(2, 1, 512) : PICKX(2, 0, 512)));
     return mode == 3 ? PICKX(1, 2, 672) : (mode == 2 ? PICKX(1, 2, 640) : (mode == 1 ? PICKX(1, 1, 512) : PICKX(1, 0, 512)));
 #undef PICKX
@@ -163,7 +164,7 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
                         if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
                     }
     for (int at = 1; at <= 2; ++at)
-        for (int md = 0; md < 4; ++md)
+        for (int md = 0; md < 5; ++md)
             for (int cu = 0; cu < 2; ++cu)
                 for (int st = 0; st < 2; ++st) {
                     e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, md, cu, st),
@@ -371,13 +372,18 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     const int grid = (n_agents + A - 1) / A;
     int at = A >= 2 ? 2 : 1;
     if (t && t->agents_per_thread) at = t->agents_per_thread;
-    const int G = (A + at - 1) / at;                              // groups per CTA
+    int G = (A + at - 1) / at;                                    // groups per CTA
     const int tmax = kX2SweepThreads;
-    if (G > tmax) return fail(c, GMAPP_ECAPACITY, "rollout: %s%ld agent groups per CTA exceed %ld threads", "", G, tmax);
     const int ns = c->n_spheres;
     const int n2 = (ns + 1) / 2;
+    // more than two agents per warp: every warp walks a block of agents in chunks of two (mode 4)
+    const bool chunked = A > 32 && n2 >= 32 && at == 2 && !(t && t->lanes_per_agent && t->lanes_per_agent != 32);
+    if (chunked && A > 1024) return fail(c, GMAPP_ECAPACITY, "rollout: %s%ld agents per CTA exceed the 1024 state records", "", A);
+    if (!chunked && G > tmax) return fail(c, GMAPP_ECAPACITY, "rollout: %s%ld agent groups per CTA exceed %ld threads", "", G, tmax);
     int L;
-    if (t && t->lanes_per_agent) {
+    if (chunked) {
+        L = 32; G = tmax / 32;
+    } else if (t && t->lanes_per_agent) {
         L = t->lanes_per_agent;
         if (G * L > tmax) return fail(c, GMAPP_EINVAL, "rollout: lanes_per_agent %s%ld x %ld groups exceeds the thread limit", "", L, G);
         if (L > 32 && G > 7) return fail(c, GMAPP_EINVAL, "rollout: lanes_per_agent > 32 allows at most 7 groups per CTA, need %s%ld", "", G);
@@ -387,11 +393,12 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
         if (L > cap) L = cap;
         if (L > 32 && G > 7) L = 32;                              // two named barriers per multi-warp group
     }
-    const int mode = L >= 64 ? (G <= 4 ? 2 : 3) : (L == 32 ? 1 : 0);
+    const int mode = chunked ? 4 : (L >= 64 ? (G <= 4 ? 2 : 3) : (L == 32 ? 1 : 0));
     const int n2p = n2 > 0 ? round_up(n2, L) : 0;
     const int cull = (t && t->cull >= 0) ? t->cull : 0;
     // dynamic shared memory: [0,64) mbarrier; [64, 64+4 KB) cross-warp exchange; sphere-pair tile at 4224
-    const int xch_off = 64, tile_off = 4224;
+    const int xch_off = 64, rec_off = 4224;
+    const int tile_off = rec_off + (chunked ? round_up(A * 24 * 4, 128) : 0);      // mode 4: 24-word state record per agent
     const size_t tile_bytes = (size_t)n2p * 32;
     const bool fits = tile_off + tile_bytes <= (size_t)c->smem_optin;
     int stage = fits ? 1 : 0;
@@ -420,8 +427,8 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     P.rco = g->r_cost_obs > 0.0f ? g->r_cost_obs : g->r_influence;
     P.w_goal = g->w_goal; P.w_obs = g->w_obs; P.w_path = g->w_path; P.w_smooth = g->w_smooth; P.a_max = g->a_max;
     P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
-    P.tile_off = tile_off; P.xch_off = xch_off;
-    const int block = mode >= 2 ? G * L + 32 * G : round_up(G * L, 32);
+    P.tile_off = tile_off; P.xch_off = xch_off; P.rec_off = rec_off;
+    const int block = mode == 4 ? tmax : (mode >= 2 ? G * L + 32 * G : round_up(G * L, 32));
     const int smem = tile_off + (stage == 1 ? (int)tile_bytes : 0);
     rollout_x2_fn fn = rollout_x2_kernel(at, mode, cull != 0, stage);
     fn<<<grid, block, smem, st>>>(P);

@@ -67,6 +67,7 @@ struct RolloutX2Params {
     int* collided;            // [n]
     int tile_off;             // byte offset of the sphere tile in dynamic shared memory
     int xch_off;              // byte offset of the cross-warp exchange area
+    int rec_off;              // byte offset of the per-agent state records (mode 4)
 };
 
 // per-lane partial sums of NA agents over the lane's sphere pairs (both halves of a pair kept apart)
@@ -305,6 +306,82 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
 }
 
 // ---------------------------------------------------------------------------------------------
+// many agents per CTA (more than two per warp): every warp owns a contiguous block of the CTA's agents and
+// walks it in chunks of two inside each step; the persistent per-agent state (24 words) lives in a
+// warp-private shared-memory record between visits.  No cross-warp traffic, no barriers, all warps busy.
+// ---------------------------------------------------------------------------------------------
+constexpr int kAgentRecWords = 24;      // p3 v3 ap3 | sumG cG sumO cO sumV cV sumJ cJ minclr d1 collided | pad
+__device__ __forceinline__ void agent_store(const AgentX2& a, float* r) {
+    r[0] = a.p[0]; r[1] = a.p[1]; r[2] = a.p[2]; r[3] = a.v[0]; r[4] = a.v[1]; r[5] = a.v[2];
+    r[6] = a.ap[0]; r[7] = a.ap[1]; r[8] = a.ap[2];
+    r[9] = a.ca.sumG; r[10] = a.ca.cG; r[11] = a.ca.sumO; r[12] = a.ca.cO; r[13] = a.ca.sumV; r[14] = a.ca.cV;
+    r[15] = a.ca.sumJ; r[16] = a.ca.cJ; r[17] = a.ca.minclr; r[18] = a.ca.d1; r[19] = __int_as_float(a.ca.collided);
+}
+__device__ __forceinline__ void agent_load(AgentX2& a, const float* r) {
+    a.p[0] = r[0]; a.p[1] = r[1]; a.p[2] = r[2]; a.v[0] = r[3]; a.v[1] = r[4]; a.v[2] = r[5];
+    a.ap[0] = r[6]; a.ap[1] = r[7]; a.ap[2] = r[8];
+    a.ca.sumG = r[9]; a.ca.cG = r[10]; a.ca.sumO = r[11]; a.ca.cO = r[12]; a.ca.sumV = r[13]; a.ca.cV = r[14];
+    a.ca.sumJ = r[15]; a.ca.cJ = r[16]; a.ca.minclr = r[17]; a.ca.d1 = r[18]; a.ca.collided = __float_as_int(r[19]);
+}
+
+template <int NA, bool CULL>
+__device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float4* tA, const float4* tB, int agent0,
+                                           int lane, int k, float* rec0) {
+    const int half = (NA == 2) ? (lane >> 4) : 0;
+    const unsigned full = 0xffffffffu;
+    float* rec = rec0 + half * kAgentRecWords;
+    AgentX2 me;
+    agent_load(me, rec);
+    float p[NA][3], v[NA][3];
+    if (NA == 2) {
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            p[0][i] = __shfl_sync(full, me.p[i], 0);       v[0][i] = __shfl_sync(full, me.v[i], 0);
+            p[NA - 1][i] = __shfl_sync(full, me.p[i], 16); v[NA - 1][i] = __shfl_sync(full, me.v[i], 16);
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
+    }
+    const bool last = (k == P.steps);
+    X2Acc<NA> acc;
+    acc.clear();
+    if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc);
+    else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc);
+    float X, Y, Z, D;
+    warp_combine<NA>(acc, lane, X, Y, Z, D);
+    const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
+    if (last) {
+        if (writer) me.finish(P, agent0 + half, D);
+        return;
+    }
+    float fx, fy, fz;
+    me.pre(P);
+    me.post(P, X, Y, Z, fx, fy, fz);
+    me.costs(P, k, D, fx, fy, fz);
+    __syncwarp();                                         // every lane has read the record before it is rewritten
+    if (writer) agent_store(me, rec);
+    __syncwarp();
+}
+
+template <bool CULL>
+__device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, const float4* tA, const float4* tB,
+                                                    int first_agent, int n_mine, int lane, float* recs) {
+    // records of this warp's agents: recs[i * kAgentRecWords], i < n_mine
+    for (int i = lane; i < n_mine; i += 32) {
+        AgentX2 a;
+        a.init(P.agents_in + 6 * size_t(first_agent + i), P.goal);
+        agent_store(a, recs + i * kAgentRecWords);
+    }
+    __syncwarp();
+    for (int k = 0; k <= P.steps; ++k) {
+        int i = 0;
+        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL>(P, tA, tB, first_agent + i, lane, k, recs + i * kAgentRecWords);
+        if (i < n_mine) chunk_step<1, CULL>(P, tA, tB, first_agent + i, lane, k, recs + i * kAgentRecWords);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // group bodies, L >= 64: W = L/32 sweep warps + ONE epilogue warp per group.
 // shared exchange area per group: part[2][W][NA] float4 (X, Y, Z, dmin), state[2][NA][2] float4 (p,0), (v,0);
 // both double-buffered by step parity, so one arrive/sync pair per direction and step is race-free:
@@ -430,6 +507,7 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 // ---------------------------------------------------------------------------------------------
 // AT = agents per group (1 or 2); MODE 0: L < 32 (sub-warp groups), 1: L == 32 (one warp per group),
 // 2: L >= 64 (W sweep warps + one epilogue warp per group; threads [0, G L) sweep, [G L, G L + 32 G) epilogue);
+// 4: many agents per CTA, each warp walks its block of agents in chunks of two (state records in shared memory);
 // STAGE 1 = sphere pairs staged in shared memory by TMA bulk copies
 template <int AT, int MODE, bool CULL, int STAGE, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ RolloutX2Params P) {
@@ -479,6 +557,17 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         const int lane_in_group = tid & (P.L - 1);
         if (AT == 2 && na >= 2) group_sweep_warps<NA2, CULL>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
         else group_sweep_warps<1, CULL>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
+        return;
+    }
+    if (MODE == 4) {
+        // balanced contiguous split of the CTA's agents over its warps
+        const int nw = blockDim.x >> 5, w = tid >> 5, n_cta = cta_end - cta_first;
+        const int base = n_cta / nw, rem = n_cta % nw;
+        const int start = w * base + (w < rem ? w : rem), n_mine = base + (w < rem ? 1 : 0);
+        if (STAGE == 1) mbar_wait(bar, 0);
+        if (n_mine <= 0) return;
+        float* recs = reinterpret_cast<float*>(smem_raw + P.rec_off) + start * kAgentRecWords;
+        warp_rollout_chunks<CULL>(P, tA, tB, cta_first + start, n_mine, tid & 31, recs);
         return;
     }
     const int group_in_cta = tid >> P.logL;

@@ -291,6 +291,7 @@ def test_pose6_large_rotation_fast_twist(api, ctx, orc):
     dict(max_ctas=5), dict(max_ctas=5, cull=1, agents_per_thread=1),
     dict(scalar_path=1), dict(scalar_path=1, lanes_per_agent=128, agents_per_thread=2, cull=1),
     dict(lanes_per_agent=512, agents_per_thread=1), dict(lanes_per_agent=1, agents_per_thread=2, max_ctas=3),
+    dict(max_ctas=1), dict(max_ctas=1, cull=1, stage=0),      # > 32 agents per CTA: chunked warps (mode 4)
 ], ids=lambda t: "-".join(f"{k[:4]}{v}" for k, v in t.items()))
 def test_launch_variants_match_oracle(api, ctx, orc, tuning):
     try:
