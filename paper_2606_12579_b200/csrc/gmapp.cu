@@ -9,6 +9,7 @@
 #include "../../include/gmapp.h"
 #include "gmapp_kernels.cuh"
 #include "gmapp_rollout_x2.cuh"
+#include "gmapp_rollout_wide.cuh"
 
 using namespace gmapp;
 
@@ -90,6 +91,17 @@ static rollout_fn rollout_kernel(int kind, int at, bool moving, bool cull, int s
     return PICK(0, 1, 1024);
 #undef PICK
 }
+// multi-warp groups with an epilogue warp, scalar pair math: 6D agents (static or moving spheres), 3D agents over moving spheres
+static rollout_fn rollout_wide_kernel(int kind, int at, bool moving, bool cull, int stage) {
+#define PICKW(K, A, M)                                                                                          \
+    (cull ? (stage ? (rollout_fn)k_rollout_wide<K, A, M, true, 1> : (rollout_fn)k_rollout_wide<K, A, M, true, 0>)    \
+          : (stage ? (rollout_fn)k_rollout_wide<K, A, M, false, 1> : (rollout_fn)k_rollout_wide<K, A, M, false, 0>))
+    if (kind == GMAPP_MOTOR6) return moving ? PICKW(1, 1, true) : PICKW(1, 1, false);
+    if (at == 2) return PICKW(0, 2, true);
+    return PICKW(0, 1, true);
+#undef PICKW
+}
+
 typedef void (*rollout_x2_fn)(const RolloutX2Params);
 static const int kX2SweepThreads = 512;       // sweep threads per CTA; mode 2 adds one epilogue warp per group (<= 672 in all)
 // mode 3 = mode 2 compiled for up to 7 groups (21 warps, 80 registers); mode 2 proper holds <= 4 groups
@@ -160,6 +172,15 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
                 for (int cu = 0; cu < 2; ++cu)
                     for (int st = 0; st < 2; ++st) {
                         e = cudaFuncSetAttribute((const void*)rollout_kernel(kind, at, mv, cu, st),
+                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
+                        if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
+                    }
+    for (int kind = 0; kind < 2; ++kind)
+        for (int at = 1; at <= (kind == 0 ? 2 : 1); ++at)
+            for (int mv = (kind == 0 ? 1 : 0); mv < 2; ++mv)
+                for (int cu = 0; cu < 2; ++cu)
+                    for (int st = 0; st < 2; ++st) {
+                        e = cudaFuncSetAttribute((const void*)rollout_wide_kernel(kind, at, mv, cu, st),
                                                  cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
                         if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
                     }
@@ -493,7 +514,16 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
     P.a_max = g->a_max; P.vel_factor = g->vel_factor;
     P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
     P.tile_off = cfg.tile_off; P.red_off = cfg.red_off;
-    rollout_fn fn = rollout_kernel(kind, cfg.at, c->moving, cfg.cull != 0, cfg.stage);
+    // few agents per CTA and many lanes per agent: sweep warps + one epilogue warp per group (gmapp_rollout_wide.cuh)
+    const bool scalar_forced = c->has_tuning && c->tuning.scalar_path;
+    const bool wide = !scalar_forced && (kind == GMAPP_MOTOR6 || c->moving) && cfg.groups <= 4 && cfg.L >= 64;
+    if (wide) {
+        while (cfg.groups * cfg.L > 512) cfg.L >>= 1;            // n_pad stays a multiple of the smaller L
+        P.L = cfg.L; P.logL = ilog2(cfg.L);
+        cfg.block = cfg.groups * cfg.L + 32 * cfg.groups;
+    }
+    rollout_fn fn = wide ? rollout_wide_kernel(kind, cfg.at, c->moving, cfg.cull != 0, cfg.stage)
+                         : rollout_kernel(kind, cfg.at, c->moving, cfg.cull != 0, cfg.stage);
     fn<<<cfg.grid, cfg.block, cfg.smem, st>>>(P);
     CUDA_TRY(c, cudaGetLastError());
     ++launches;

@@ -1,0 +1,315 @@
+// gmapp_rollout_wide.cuh -- rollout kernel for MOVING spheres and 6D motor agents when a group of lanes spans
+// several warps (L >= 64, <= 4 groups per CTA: the few-agents / many-spheres shape of config 4).
+//
+// Same machine mapping as the multi-warp mode of gmapp_rollout_x2.cuh: W = L/32 sweep warps per group evaluate the
+// pair sums (scalar FP32 pair math of gmapp_kernels.cuh: per-pair relative velocity for moving spheres), combine
+// them inside the warp (transposed butterfly + REDUX.MIN) and post them to shared memory; ONE epilogue warp per
+// group adds the W partials, updates the agent(s) and publishes (p, world velocity) for the next sweep.  The 6D
+// update is split so that everything that does not need the sphere sums -- the SE(3) log map of Eq. 8, the
+// torque, the rotor increment exp(dt w), the new rotor -- runs BEFORE the epilogue warp waits for the sums; after
+// the wait only R^T f_r, the new twist, the translation of exp(dt v) and two rotations remain (Eq. 9-11).
+// In the scalar kernel the whole 6D update ran redundantly on every lane of the group and took 60 % of the time.
+//
+// Shares nothing with oracle/.
+#pragma once
+#include "gmapp_rollout_x2.cuh"
+
+namespace gmapp {
+
+template <int NA>
+__device__ __forceinline__ void warp_combine(const StaticAcc<NA>& acc, int lane, float& X, float& Y, float& Z, float& D) {
+    float x[NA], y[NA], z[NA], dm[NA];
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        x[a] = acc.bx[a]; y[a] = acc.by[a]; z[a] = acc.bz[a];
+        dm[a] = fkey_inv(__reduce_min_sync(0xffffffffu, fkey(acc.dmin[a])));
+    }
+    warp_sum3<NA>(x, y, z, lane, X, Y, Z);
+    D = (NA == 2 && (lane & 16)) ? dm[NA - 1] : dm[0];
+}
+
+// ---------------------------------------------------------------------------------------------
+// epilogue-side agent models.  Interface: init, pre (no sums needed), post (sums known -> new state, pub[6] =
+// position and WORLD linear velocity for the sweep warps), costs, finish.
+// ---------------------------------------------------------------------------------------------
+template <bool MOVING>
+struct EpiPoint3 {
+    float p[3], v[3], ap[3], pub[6];
+    float ex, ey, ez, inv, nv, fax, fay, faz, fx, fy, fz;
+    CostAcc ca;
+    __device__ __forceinline__ void init(const RolloutParams& P, int i) {
+        const float* s = P.agents_in + 6 * size_t(i);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { p[c] = s[c]; v[c] = s[3 + c]; ap[c] = 0.0f; pub[c] = p[c]; pub[3 + c] = v[c]; }
+        ca.init(norm3f(P.goal[0] - p[0], P.goal[1] - p[1], P.goal[2] - p[2]));
+    }
+    __device__ __forceinline__ void pre(const RolloutParams& P) {
+        ex = P.goal[0] - p[0]; ey = P.goal[1] - p[1]; ez = P.goal[2] - p[2];
+        if (!MOVING) {
+            const float n2 = fmaf(v[0], v[0], fmaf(v[1], v[1], fmaf(v[2], v[2], kTiny)));
+            inv = rsqrt_approx(n2);
+            inv = inv * fmaf(-0.5f * n2 * inv, inv, 1.5f);
+            nv = n2 * inv;
+        }
+        fax = fmaf(P.k_att, ex, -P.k_damp * v[0]); fay = fmaf(P.k_att, ey, -P.k_damp * v[1]); faz = fmaf(P.k_att, ez, -P.k_damp * v[2]);
+    }
+    __device__ __forceinline__ void post(const RolloutParams& P, float bx, float by, float bz) {
+        if (MOVING) {                                      // the sweep accumulated the force vector itself
+            fx = fmaf(P.k_circ, bx, fax); fy = fmaf(P.k_circ, by, fay); fz = fmaf(P.k_circ, bz, faz);
+        } else {
+            const float A = fmaf(bx, v[0], fmaf(by, v[1], bz * v[2]));
+            const float c1 = P.k_circ * inv * A, c2 = -P.k_circ * nv;
+            fx = fmaf(c1, v[0], fmaf(c2, bx, fax)); fy = fmaf(c1, v[1], fmaf(c2, by, fay)); fz = fmaf(c1, v[2], fmaf(c2, bz, faz));
+        }
+        v[0] = fmaf(P.c_lin, fx, v[0]); v[1] = fmaf(P.c_lin, fy, v[1]); v[2] = fmaf(P.c_lin, fz, v[2]);   // Eq. 9-10
+        p[0] = fmaf(P.dt, v[0], p[0]); p[1] = fmaf(P.dt, v[1], p[1]); p[2] = fmaf(P.dt, v[2], p[2]);      // Eq. 11
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { pub[c] = p[c]; pub[3 + c] = v[c]; }
+    }
+    __device__ __forceinline__ void costs(const RolloutParams& P, int k, float dmin) {
+        ca.pose(norm3f(ex, ey, ez), dmin, P.rcg, P.rco);
+        if (k >= 2) {
+            float jx = fx - ap[0], jy = fy - ap[1], jz = fz - ap[2];
+            ca.add_jerk(fmaf(jx, jx, fmaf(jy, jy, jz * jz)));
+        }
+        ap[0] = fx; ap[1] = fy; ap[2] = fz;
+        ca.add_len(norm3f(v[0], v[1], v[2]));
+    }
+    __device__ __forceinline__ void finish(const RolloutParams& P, int i, float dmin) {
+        ca.pose(norm3f(P.goal[0] - p[0], P.goal[1] - p[1], P.goal[2] - p[2]), dmin, P.rcg, P.rco);
+        const float cj = P.vel_factor * P.dt * P.dt * P.inv_mass;
+        ca.finish(P, P.dt * ca.sumV, cj * cj * ca.sumJ, P.cost + 5 * size_t(i));
+        P.minclr[i] = ca.minclr;
+        P.collided[i] = ca.collided;
+        if (P.agents_out) {
+            float* o = P.agents_out + 6 * size_t(i);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { o[c] = p[c]; o[3 + c] = v[c]; }
+        }
+    }
+};
+
+template <bool MOVING>
+struct EpiPose6 {
+    Pose6 x;
+    Quat rg; Vec3 pg;
+    float pub[6];
+    // computed by pre(): old position, torque-updated angular velocity, new rotor, exp coefficients, force without f_r
+    Vec3 pos, w_new, phi, fpre, td, dp, dp1, dp2;
+    Quat r_new;
+    float Bc, Cc;
+    CostAcc ca;
+    __device__ __forceinline__ void init(const RolloutParams& P, int i) {
+        x = load_pose6(P.agents_in + 14 * size_t(i));
+        rg = Quat{P.goal[0], P.goal[1], P.goal[2], P.goal[3]};
+        Quat dg = Quat{P.goal[4], P.goal[5], P.goal[6], P.goal[7]};
+        motor_normalise(rg, dg);
+        pg = motor_translation(rg, dg);
+        ca.init(norm3f(pg.x - x.p.x, pg.y - x.p.y, pg.z - x.p.z));
+        dp1 = v3(0, 0, 0); dp2 = v3(0, 0, 0);
+        const Vec3 pdot = qrot(x.r, x.nu);
+        pub[0] = x.p.x; pub[1] = x.p.y; pub[2] = x.p.z; pub[3] = pdot.x; pub[4] = pdot.y; pub[5] = pdot.z;
+    }
+    // Eq. 8 log map, torque, w update, rotation part of exp(dt v), new rotor: none of it needs the sphere sums
+    __device__ __forceinline__ void pre(const RolloutParams& P) {
+        pos = x.p;
+        const Quat qrel = qmul(qconj(x.r), rg);
+        const Vec3 trel = qrot_inv(x.r, pg - pos);
+        Vec3 ew, ev;
+        se3_log_from_quat(qrel, trel, ew, ev);
+        const Vec3 tau = fma3(P.k_att_rot, ew, (-P.k_damp_rot) * x.w);
+        fpre = fma3(P.k_att, ev, (-P.k_damp) * x.nu);
+        w_new = fma3(P.c_rot, tau, x.w);                                   // Eq. 9-10, rotational block
+        phi = P.dt * w_new;
+        float ch, sh_over_th;
+        se3_exp_coeffs(phi, ch, sh_over_th, Bc, Cc);
+        const Quat rd = Quat{ch, sh_over_th * phi.x, sh_over_th * phi.y, sh_over_th * phi.z};
+        r_new = qmul(x.r, rd);                                             // Eq. 11, rotor part of M <- M exp(dt v)
+        Quat dz = Quat{0, 0, 0, 0};
+        motor_normalise(r_new, dz);
+    }
+    __device__ __forceinline__ void post(const RolloutParams& P, float bx, float by, float bz) {
+        Vec3 fr;
+        if (MOVING) fr = P.k_circ * v3(bx, by, bz);
+        else cf_force_static(P.k_circ, bx, by, bz, pub[3], pub[4], pub[5], fr.x, fr.y, fr.z);
+        const Vec3 f = fpre + qrot_inv(x.r, fr);                           // Eq. 6 in the body frame (reading G18)
+        x.nu = fma3(P.c_lin, f, x.nu);                                     // Eq. 9-10, linear block
+        const Vec3 rho = P.dt * x.nu;
+        const Vec3 wr = cross(phi, rho);
+        const Vec3 wwr = cross(phi, wr);
+        td = fma3(Cc, wwr, fma3(Bc, wr, rho));                             // translation of exp(dt v)
+        dp = qrot(x.r, td);                                                // world displacement p_new - p
+        x.p = x.p + dp;
+        x.r = r_new;
+        x.w = w_new;
+        const Vec3 pdot = qrot(x.r, x.nu);                                 // world linear velocity for the next sweep
+        pub[0] = x.p.x; pub[1] = x.p.y; pub[2] = x.p.z; pub[3] = pdot.x; pub[4] = pdot.y; pub[5] = pdot.z;
+    }
+    __device__ __forceinline__ void costs(const RolloutParams& P, int k, float dmin) {
+        ca.pose(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z), dmin, P.rcg, P.rco);
+        ca.add_len(norm3f(td.x, td.y, td.z));
+        if (k >= 2) {
+            const Vec3 t3 = dp - 2.0f * dp1 + dp2;                         // p4 - 3 p3 + 3 p2 - p1 from displacements
+            ca.add_jerk(dot(t3, t3));
+        }
+        dp2 = dp1; dp1 = dp;
+    }
+    __device__ __forceinline__ void finish(const RolloutParams& P, int i, float dmin) {
+        ca.pose(norm3f(pg.x - x.p.x, pg.y - x.p.y, pg.z - x.p.z), dmin, P.rcg, P.rco);
+        ca.finish(P, ca.sumV, ca.sumJ, P.cost + 5 * size_t(i));
+        P.minclr[i] = ca.minclr;
+        P.collided[i] = ca.collided;
+        if (P.agents_out) {
+            float* o = P.agents_out + 14 * size_t(i);
+            const Vec3 rv = v3(x.r.x, x.r.y, x.r.z);
+            const Vec3 dv = 0.5f * (fma3(x.r.w, x.p, cross(x.p, rv)));    // dual part d = (1/2) (0, p) (x) r
+            o[0] = x.r.w; o[1] = x.r.x; o[2] = x.r.y; o[3] = x.r.z;
+            o[4] = -0.5f * dot(x.p, rv); o[5] = dv.x; o[6] = dv.y; o[7] = dv.z;
+            o[8] = x.w.x; o[9] = x.w.y; o[10] = x.w.z; o[11] = x.nu.x; o[12] = x.nu.y; o[13] = x.nu.z;
+        }
+    }
+};
+
+// ---------------------------------------------------------------------------------------------
+// group bodies (protocol and hazard argument as in gmapp_rollout_x2.cuh, multi-warp mode)
+// exchange area per group: part[2][W][NA] float4, state[2][NA][2] float4
+// ---------------------------------------------------------------------------------------------
+template <int NA, bool MOVING, bool CULL>
+__device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const float4* sph, const float4* svel,
+                                                 int lane_in_group, int group_in_cta, float4* xch) {
+    const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
+    const int half = (NA == 2) ? (lane >> 4) : 0;
+    const unsigned full = 0xffffffffu;
+    float4* part = xch;
+    const float4* state = xch + 2 * W * NA;
+    const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
+    float p[NA][3], v[NA][3];
+    // initial (p, world velocity) comes from the epilogue warp too (6D: needs the motor algebra): step "-1" hand-over
+    named_bar_sync(bar_state, nbar);
+#pragma unroll
+    for (int a = 0; a < NA; ++a) {
+        const float4 sp = state[(1 * NA + a) * 2], sv = state[(1 * NA + a) * 2 + 1];
+        p[a][0] = sp.x; p[a][1] = sp.y; p[a][2] = sp.z; v[a][0] = sv.x; v[a][1] = sv.y; v[a][2] = sv.z;
+    }
+    StaticAcc<NA> acc;
+    for (int k = 0; k <= P.steps; ++k) {
+        const bool last = (k == P.steps);
+        const float tk = float(k) * P.dt;
+        acc.clear();
+        if (!last) sphere_sweep<NA, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc);
+        else       sphere_sweep<NA, MOVING, false, false>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc);
+        float X, Y, Z, D;
+        warp_combine<NA>(acc, lane, X, Y, Z, D);
+        const int par = k & 1;
+        if ((lane & 15) == 0 && (NA == 2 || lane == 0)) part[(par * W + wig) * NA + half] = make_float4(X, Y, Z, D);
+        named_bar_arrive(bar_part, nbar);
+        if (last) return;
+        named_bar_sync(bar_state, nbar);
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            const float4 sp = state[(par * NA + a) * 2], sv = state[(par * NA + a) * 2 + 1];
+            p[a][0] = sp.x; p[a][1] = sp.y; p[a][2] = sp.z; v[a][0] = sv.x; v[a][1] = sv.y; v[a][2] = sv.z;
+        }
+    }
+}
+
+template <class Model, int NA>
+__device__ __forceinline__ void wide_epilogue_warp(const RolloutParams& P, int first_agent, int lane,
+                                                   int group_in_cta, float4* xch) {
+    const int W = P.L >> 5;
+    const int half = (NA == 2) ? (lane >> 4) : 0;
+    const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
+    const float4* part = xch;
+    float4* state = xch + 2 * W * NA;
+    const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
+    Model me;
+    me.init(P, first_agent + half);
+    // hand the start state to the sweep warps through the parity-1 buffer (step 0 publishes into parity 0)
+    if (writer) {
+        state[(1 * NA + half) * 2] = make_float4(me.pub[0], me.pub[1], me.pub[2], 0.0f);
+        state[(1 * NA + half) * 2 + 1] = make_float4(me.pub[3], me.pub[4], me.pub[5], 0.0f);
+    }
+    named_bar_arrive(bar_state, nbar);
+    for (int k = 0; k <= P.steps; ++k) {
+        const bool last = (k == P.steps);
+        const int par = k & 1;
+        if (!last) me.pre(P);
+        named_bar_sync(bar_part, nbar);
+        float4 t = part[(par * W) * NA + half];
+        for (int w = 1; w < W; ++w) {
+            const float4 o = part[(par * W + w) * NA + half];
+            t.x += o.x; t.y += o.y; t.z += o.z; t.w = fminf(t.w, o.w);
+        }
+        if (last) {
+            if (writer) me.finish(P, first_agent + half, t.w);
+            return;
+        }
+        me.post(P, t.x, t.y, t.z);
+        if (writer) {
+            state[(par * NA + half) * 2] = make_float4(me.pub[0], me.pub[1], me.pub[2], 0.0f);
+            state[(par * NA + half) * 2 + 1] = make_float4(me.pub[3], me.pub[4], me.pub[5], 0.0f);
+        }
+        named_bar_arrive(bar_state, nbar);
+        me.costs(P, k, t.w);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// the kernel: threads [0, G L) sweep, [G L, G L + 32 G) one epilogue warp per group; G <= 4, L >= 64
+// KIND 0 = 3D point agents (AT 1 or 2 per group), KIND 1 = 6D motor agents (one per group)
+// ---------------------------------------------------------------------------------------------
+template <int KIND, int AT, bool MOVING, bool CULL, int STAGE>
+__global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__ RolloutParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
+    const float4* sph = P.sph;
+    const float4* svel = P.svel;
+    const int tid = threadIdx.x;
+    if (STAGE == 1) {
+        float4* tile = reinterpret_cast<float4*>(smem_raw + P.tile_off);
+        if (tid == 0) { mbar_init(bar, 1); fence_mbar_init(); }
+        __syncthreads();
+        if (tid == 0) {
+            const uint32_t bytes = uint32_t(P.n_pad) * 16u;
+            mbar_arrive_expect_tx(bar, MOVING ? 2u * bytes : bytes);
+            const uint32_t chunk = 32768u;
+            for (uint32_t o = 0; o < bytes; o += chunk) {
+                const uint32_t nb = bytes - o < chunk ? bytes - o : chunk;
+                tma_bulk_g2s(reinterpret_cast<unsigned char*>(tile) + o, reinterpret_cast<const unsigned char*>(P.sph) + o, nb, bar);
+                if (MOVING)
+                    tma_bulk_g2s(reinterpret_cast<unsigned char*>(tile) + bytes + o,
+                                 reinterpret_cast<const unsigned char*>(P.svel) + o, nb, bar);
+            }
+        }
+        sph = tile;
+        svel = tile + P.n_pad;
+    }
+    const int cta_first = blockIdx.x * P.agents_per_cta;
+    int cta_end = cta_first + P.agents_per_cta;
+    if (cta_end > P.n_agents) cta_end = P.n_agents;
+    constexpr int NA2 = (KIND == 0 && AT == 2) ? 2 : 1;
+    constexpr int ATE = (KIND == 0) ? AT : 1;
+    const int G = (P.agents_per_cta + ATE - 1) / ATE;
+    const int W = P.L >> 5;
+    const int n_sweep = G * P.L;
+    const bool is_epi = tid >= n_sweep;
+    const int group_in_cta = is_epi ? ((tid - n_sweep) >> 5) : (tid >> P.logL);
+    const int first = cta_first + group_in_cta * ATE;
+    const int na = cta_end - first;
+    float4* xch = reinterpret_cast<float4*>(smem_raw + P.red_off) + group_in_cta * (2 * W * 2 + 2 * 2 * 2);
+    if (is_epi) {
+        if (na <= 0) return;
+        const int lane = tid & 31;
+        if (KIND == 1) wide_epilogue_warp<EpiPose6<MOVING>, 1>(P, first, lane, group_in_cta, xch);
+        else if (NA2 == 2 && na >= 2) wide_epilogue_warp<EpiPoint3<MOVING>, NA2>(P, first, lane, group_in_cta, xch);
+        else wide_epilogue_warp<EpiPoint3<MOVING>, 1>(P, first, lane, group_in_cta, xch);
+        return;
+    }
+    if (STAGE == 1) mbar_wait(bar, 0);
+    if (na <= 0) return;
+    const int lane_in_group = tid & (P.L - 1);
+    if (NA2 == 2 && na >= 2) wide_sweep_warps<NA2, MOVING, CULL>(P, sph, svel, lane_in_group, group_in_cta, xch);
+    else wide_sweep_warps<1, MOVING, CULL>(P, sph, svel, lane_in_group, group_in_cta, xch);
+}
+
+}  // namespace gmapp
