@@ -147,8 +147,8 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
     ALLOC(c->d_sph_raw, sizeof(float4) * c->cap_spheres);
     ALLOC(c->d_sph_eff, sizeof(float4) * c->cap_spheres);
     ALLOC(c->d_svel, sizeof(float4) * c->cap_spheres);
-    ALLOC(c->d_pairA, sizeof(float4) * (c->cap_spheres / 2));
-    ALLOC(c->d_pairB, sizeof(float4) * (c->cap_spheres / 2));
+    ALLOC(c->d_pairA, sizeof(float4) * (c->cap_spheres / 2) * 4);      // A, B, U, V contiguous
+    c->d_pairB = c->d_pairA + c->cap_spheres / 2;
     ALLOC(c->d_cost, sizeof(float) * 5 * max_agents);
     ALLOC(c->d_minclr, sizeof(float) * max_agents);
     ALLOC(c->d_collided, sizeof(int) * max_agents);
@@ -200,7 +200,7 @@ extern "C" gmapp_status gmapp_destroy(gmapp_ctx* c) {
     if (!c) return GMAPP_OK;
     cudaSetDevice(c->device);
     cudaDeviceSynchronize();
-    cudaFree(c->d_sph_raw); cudaFree(c->d_sph_eff); cudaFree(c->d_svel); cudaFree(c->d_pairA); cudaFree(c->d_pairB);
+    cudaFree(c->d_sph_raw); cudaFree(c->d_sph_eff); cudaFree(c->d_svel); cudaFree(c->d_pairA);
     cudaFree(c->d_cost); cudaFree(c->d_minclr); cudaFree(c->d_collided);
     cudaFree(c->d_agents_stage); cudaFree(c->d_xyzr_stage); cudaFree(c->d_vel_stage);
     cudaFree(c->d_best_idx); cudaFree(c->d_best_cost); cudaFree(c->d_scratch);
@@ -265,12 +265,8 @@ extern "C" gmapp_status gmapp_set_obstacles(gmapp_ctx* c, const float* d_xyzr, c
     c->moving = (d_vel != nullptr) && n > 0;
     c->eff_valid = false;
     c->pair_valid = false;
-    if (!c->moving) {
-        // sphere-pair layout of the packed kernel, for r_agent = 0 (repacked lazily if a rollout asks for another r_agent)
-        gmapp_status s = effective_pairs(c, 0.0f, st, nullptr);
-        if (s != GMAPP_OK) return s;
-    }
-    return GMAPP_OK;
+    // sphere-pair layout of the packed kernels, for r_agent = 0 (repacked lazily if a rollout asks for another r_agent)
+    return effective_pairs(c, 0.0f, st, nullptr);
 }
 
 extern "C" gmapp_status gmapp_set_obstacles_host(gmapp_ctx* c, const float* h_xyzr, const float* h_vel, int n, void* stream) {
@@ -310,7 +306,8 @@ static gmapp_status effective_spheres(gmapp_ctx* c, float r_agent, cudaStream_t 
 static gmapp_status effective_pairs(gmapp_ctx* c, float r_agent, cudaStream_t st, int* launches) {
     if (c->pair_valid && c->pair_r_agent == r_agent) return GMAPP_OK;
     const int n2f = fill_count(c, c->n_spheres) / 2;
-    k_pack_pairs<<<(n2f + 255) / 256, 256, 0, st>>>(c->d_sph_raw, c->n_spheres, n2f, r_agent, c->d_pairA, c->d_pairB);
+    k_pack_pairs<<<(n2f + 255) / 256, 256, 0, st>>>(c->d_sph_raw, c->moving ? c->d_svel : nullptr, c->n_spheres, n2f, r_agent,
+                                                    c->d_pairA, c->cap_spheres / 2);
     CUDA_TRY(c, cudaGetLastError());
     c->pair_valid = true; c->pair_r_agent = r_agent;
     if (launches) ++*launches;
@@ -516,11 +513,19 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
     P.tile_off = cfg.tile_off; P.red_off = cfg.red_off;
     // few agents per CTA and many lanes per agent: sweep warps + one epilogue warp per group (gmapp_rollout_wide.cuh)
     const bool scalar_forced = c->has_tuning && c->tuning.scalar_path;
-    const bool wide = !scalar_forced && (kind == GMAPP_MOTOR6 || c->moving) && cfg.groups <= 4 && cfg.L >= 64;
+    const int n2 = (c->n_spheres + 1) / 2;
+    bool wide = !scalar_forced && (kind == GMAPP_MOTOR6 || c->moving) && cfg.groups <= 4 && cfg.L >= 64 && n2 >= 64;
     if (wide) {
-        while (cfg.groups * cfg.L > 512) cfg.L >>= 1;            // n_pad stays a multiple of the smaller L
+        while (cfg.groups * cfg.L > 512 || cfg.L > pow2_ceil(n2)) cfg.L >>= 1;
         P.L = cfg.L; P.logL = ilog2(cfg.L);
         cfg.block = cfg.groups * cfg.L + 32 * cfg.groups;
+        s = effective_pairs(c, g->r_agent, st, &launches);
+        if (s != GMAPP_OK) return s;
+        P.pairA = c->d_pairA; P.pair_stride = c->cap_spheres / 2; P.n2p = round_up(n2, cfg.L);
+        const size_t tile_bytes = (size_t)P.n2p * 16 * (c->moving ? 4 : 2);
+        const bool fits = cfg.tile_off + tile_bytes <= (size_t)c->smem_optin;
+        if (cfg.stage == 1 && !fits) cfg.stage = 0;
+        cfg.smem = cfg.tile_off + (cfg.stage == 1 ? (int)tile_bytes : 0);
     }
     rollout_fn fn = wide ? rollout_wide_kernel(kind, cfg.at, c->moving, cfg.cull != 0, cfg.stage)
                          : rollout_kernel(kind, cfg.at, c->moving, cfg.cull != 0, cfg.stage);

@@ -33,6 +33,8 @@ struct RolloutParams {
     const float4* sph;        // [n_pad] (cx, cy, cz, r_j + r_a), sentinel-padded
     const float4* svel;       // [n_pad] (ux, uy, uz, 0) or nullptr
     int n_pad;                // multiple of L
+    const float4* pairA;      // sphere-pair arrays A, B, U, V (gmapp_rollout_wide.cuh), pair_stride float4 apart
+    int pair_stride, n2p;     // n2p = sphere pairs padded to a multiple of L
     const float* agents_in;   // [n][6] or [n][14]
     float* agents_out;        // same layout or nullptr
     int n_agents, agents_per_cta;

@@ -2,7 +2,7 @@
 // several warps (L >= 64, <= 4 groups per CTA: the few-agents / many-spheres shape of config 4).
 //
 // Same machine mapping as the multi-warp mode of gmapp_rollout_x2.cuh: W = L/32 sweep warps per group evaluate the
-// pair sums (scalar FP32 pair math of gmapp_kernels.cuh: per-pair relative velocity for moving spheres), combine
+// pair sums (packed f32x2 pair math; per-pair relative velocity for moving spheres), combine
 // them inside the warp (transposed butterfly + REDUX.MIN) and post them to shared memory; ONE epilogue warp per
 // group adds the W partials, updates the agent(s) and publishes (p, world velocity) for the next sweep.  The 6D
 // update is split so that everything that does not need the sphere sums -- the SE(3) log map of Eq. 8, the
@@ -26,6 +26,66 @@ __device__ __forceinline__ void warp_combine(const StaticAcc<NA>& acc, int lane,
     }
     warp_sum3<NA>(x, y, z, lane, X, Y, Z);
     D = (NA == 2 && (lane & 16)) ? dm[NA - 1] : dm[0];
+}
+
+// ---------------------------------------------------------------------------------------------
+// packed f32x2 sweep for MOVING spheres.  Sphere pairs: A = (cx0,cx1,cy0,cy1), B = (cz0,cz1,-R0,-R1) at t = 0,
+// U = (ux0,ux1,uy0,uy1), V = (uz0,uz1,0,0).  Per pair (reading G5/G25): c(t) = c + t u, v_rel = v - u,
+// f_j = w [ (s/|v_rel|) v_rel - |v_rel| d ],  w = s / (d_O |d|^2),  s = d.v_rel, accumulated directly
+// (k_f applied after the sum).  The distance half is the static one.
+// ---------------------------------------------------------------------------------------------
+template <int NA, bool FORCE, bool CULL>
+__device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, const float4* __restrict__ tB,
+                                                const float4* __restrict__ tU, const float4* __restrict__ tV, int n2p,
+                                                int lane, int L, float tk, const float (&p)[NA][3], const float (&v)[NA][3],
+                                                float r_d, float eps, unsigned mask, X2Acc<NA>& acc) {
+    const u64 tiny = bc2(kTiny), half = bc2(0.5f), t2 = bc2(tk);
+#pragma unroll 2
+    for (int j = lane; j < n2p; j += L) {
+        const float4 s0 = tA[j], s1 = tB[j], s2 = tU[j], s3 = tV[j];
+        const u64 ux = pk2(s2.x, s2.y), uy = pk2(s2.z, s2.w), uz = pk2(s3.x, s3.y), nR = pk2(s1.z, s1.w);
+        const u64 cx = fma2(ux, t2, pk2(s0.x, s0.y)), cy = fma2(uy, t2, pk2(s0.z, s0.w)), cz = fma2(uz, t2, pk2(s1.x, s1.y));
+        u64 dx[NA], dy[NA], dz[NA], q[NA];
+        float d0[NA], d1[NA];
+        bool any = false;
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            dx[a] = sub2(cx, bc2(p[a][0])); dy[a] = sub2(cy, bc2(p[a][1])); dz[a] = sub2(cz, bc2(p[a][2]));
+            q[a] = fma2(dx[a], dx[a], fma2(dy[a], dy[a], fma2(dz[a], dz[a], tiny)));
+            float q0, q1; upk2(q[a], q0, q1);
+            const u64 y = pk2(rsqrt_approx(q0), rsqrt_approx(q1));
+            const u64 t = mul2(q[a], y);
+            const u64 hy = mul2(y, half);
+            float t0, t1; upk2(t, t0, t1);
+            const u64 e = pk2(fmaf(-t0, t0, q0), fmaf(-t1, t1, q1));
+            const u64 ds = fma2(hy, e, add2(t, nR));
+            upk2(ds, d0[a], d1[a]);
+            acc.dmin[a] = min3f(acc.dmin[a], d0[a], d1[a]);
+            if (CULL) any = any || (fminf(d0[a], d1[a]) <= r_d);
+        }
+        if (!FORCE) continue;
+        if (CULL) { if (!__any_sync(mask, any)) continue; }
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            const u64 vx = sub2(bc2(v[a][0]), ux), vy = sub2(bc2(v[a][1]), uy), vz = sub2(bc2(v[a][2]), uz);
+            const u64 n2 = fma2(vx, vx, fma2(vy, vy, fma2(vz, vz, tiny)));
+            float m0, m1; upk2(n2, m0, m1);
+            const float i0 = rsqrt_approx(m0), i1 = rsqrt_approx(m1);
+            const u64 inv = pk2(i0, i1), ninv = pk2(-i0, -i1);
+            const u64 nvn = mul2(n2, ninv);                                              // -|v_rel|
+            const u64 den = mul2(pk2(fmaxf(d0[a], eps), fmaxf(d1[a], eps)), q[a]);
+            float n0, n1; upk2(den, n0, n1);
+            float r0 = 0.0f, r1 = 0.0f;
+            if (d0[a] <= r_d) r0 = rcp_approx(n0);
+            if (d1[a] <= r_d) r1 = rcp_approx(n1);
+            const u64 s = fma2(dx[a], vx, fma2(dy[a], vy, mul2(dz[a], vz)));
+            const u64 w = mul2(s, pk2(r0, r1));
+            const u64 c1 = mul2(mul2(w, s), inv), c2 = mul2(w, nvn);
+            acc.bx[a] = fma2(c1, vx, fma2(c2, dx[a], acc.bx[a]));
+            acc.by[a] = fma2(c1, vy, fma2(c2, dy[a], acc.by[a]));
+            acc.bz[a] = fma2(c1, vz, fma2(c2, dz[a], acc.bz[a]));
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -174,8 +234,9 @@ struct EpiPose6 {
 // group bodies (protocol and hazard argument as in gmapp_rollout_x2.cuh, multi-warp mode)
 // exchange area per group: part[2][W][NA] float4, state[2][NA][2] float4
 // ---------------------------------------------------------------------------------------------
+// sweep warps: packed f32x2 sweeps over sphere pairs; tile = A, B (, U, V when MOVING) arrays of n2p float4 each
 template <int NA, bool MOVING, bool CULL>
-__device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const float4* sph, const float4* svel,
+__device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const float4* tile, int astride,
                                                  int lane_in_group, int group_in_cta, float4* xch) {
     const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
     const int half = (NA == 2) ? (lane >> 4) : 0;
@@ -183,21 +244,27 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
     float4* part = xch;
     const float4* state = xch + 2 * W * NA;
     const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
+    const float4* tA = tile; const float4* tB = tile + astride; const float4* tU = tile + 2 * astride; const float4* tV = tile + 3 * astride;
     float p[NA][3], v[NA][3];
-    // initial (p, world velocity) comes from the epilogue warp too (6D: needs the motor algebra): step "-1" hand-over
+    // the start (p, world velocity) comes from the epilogue warp too (6D: needs the motor algebra): parity-1 buffer
     named_bar_sync(bar_state, nbar);
 #pragma unroll
     for (int a = 0; a < NA; ++a) {
         const float4 sp = state[(1 * NA + a) * 2], sv = state[(1 * NA + a) * 2 + 1];
         p[a][0] = sp.x; p[a][1] = sp.y; p[a][2] = sp.z; v[a][0] = sv.x; v[a][1] = sv.y; v[a][2] = sv.z;
     }
-    StaticAcc<NA> acc;
+    X2Acc<NA> acc;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         const float tk = float(k) * P.dt;
         acc.clear();
-        if (!last) sphere_sweep<NA, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc);
-        else       sphere_sweep<NA, MOVING, false, false>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc);
+        if (MOVING) {
+            if (!last) sweep_x2_moving<NA, true, CULL>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc);
+            else       sweep_x2_moving<NA, false, false>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc);
+        } else {
+            if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
+            else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
+        }
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
         const int par = k & 1;
@@ -230,10 +297,10 @@ __device__ __forceinline__ void wide_epilogue_warp(const RolloutParams& P, int f
         state[(1 * NA + half) * 2 + 1] = make_float4(me.pub[3], me.pub[4], me.pub[5], 0.0f);
     }
     named_bar_arrive(bar_state, nbar);
+    me.pre(P);
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         const int par = k & 1;
-        if (!last) me.pre(P);
         named_bar_sync(bar_part, nbar);
         float4 t = part[(par * W) * NA + half];
         for (int w = 1; w < W; ++w) {
@@ -250,7 +317,10 @@ __device__ __forceinline__ void wide_epilogue_warp(const RolloutParams& P, int f
             state[(par * NA + half) * 2 + 1] = make_float4(me.pub[3], me.pub[4], me.pub[5], 0.0f);
         }
         named_bar_arrive(bar_state, nbar);
+        // off the critical path of the sweep warps; the costs of this step and the sum-free part of the next
+        // step sit in one block so their independent instruction chains interleave
         me.costs(P, k, t.w);
+        me.pre(P);
     }
 }
 
@@ -262,27 +332,28 @@ template <int KIND, int AT, bool MOVING, bool CULL, int STAGE>
 __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__ RolloutParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
-    const float4* sph = P.sph;
-    const float4* svel = P.svel;
     const int tid = threadIdx.x;
+    constexpr int NARR = MOVING ? 4 : 2;                    // pair arrays: A, B (, U, V)
+    const float4* tile = P.pairA;                           // STAGE 0: read the pair arrays from global memory / L2
+    int astride = P.pair_stride;
     if (STAGE == 1) {
-        float4* tile = reinterpret_cast<float4*>(smem_raw + P.tile_off);
+        float4* t = reinterpret_cast<float4*>(smem_raw + P.tile_off);
         if (tid == 0) { mbar_init(bar, 1); fence_mbar_init(); }
         __syncthreads();
         if (tid == 0) {
-            const uint32_t bytes = uint32_t(P.n_pad) * 16u;
-            mbar_arrive_expect_tx(bar, MOVING ? 2u * bytes : bytes);
+            const uint32_t bytes = uint32_t(P.n2p) * 16u;
+            mbar_arrive_expect_tx(bar, NARR * bytes);
             const uint32_t chunk = 32768u;
-            for (uint32_t o = 0; o < bytes; o += chunk) {
-                const uint32_t nb = bytes - o < chunk ? bytes - o : chunk;
-                tma_bulk_g2s(reinterpret_cast<unsigned char*>(tile) + o, reinterpret_cast<const unsigned char*>(P.sph) + o, nb, bar);
-                if (MOVING)
-                    tma_bulk_g2s(reinterpret_cast<unsigned char*>(tile) + bytes + o,
-                                 reinterpret_cast<const unsigned char*>(P.svel) + o, nb, bar);
+            for (int r = 0; r < NARR; ++r) {
+                const unsigned char* src = reinterpret_cast<const unsigned char*>(P.pairA + size_t(r) * P.pair_stride);
+                for (uint32_t o = 0; o < bytes; o += chunk) {
+                    const uint32_t nb = bytes - o < chunk ? bytes - o : chunk;
+                    tma_bulk_g2s(reinterpret_cast<unsigned char*>(t) + r * bytes + o, src + o, nb, bar);
+                }
             }
         }
-        sph = tile;
-        svel = tile + P.n_pad;
+        tile = t;
+        astride = P.n2p;
     }
     const int cta_first = blockIdx.x * P.agents_per_cta;
     int cta_end = cta_first + P.agents_per_cta;
@@ -308,8 +379,8 @@ __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__
     if (STAGE == 1) mbar_wait(bar, 0);
     if (na <= 0) return;
     const int lane_in_group = tid & (P.L - 1);
-    if (NA2 == 2 && na >= 2) wide_sweep_warps<NA2, MOVING, CULL>(P, sph, svel, lane_in_group, group_in_cta, xch);
-    else wide_sweep_warps<1, MOVING, CULL>(P, sph, svel, lane_in_group, group_in_cta, xch);
+    if (NA2 == 2 && na >= 2) wide_sweep_warps<NA2, MOVING, CULL>(P, tile, astride, lane_in_group, group_in_cta, xch);
+    else wide_sweep_warps<1, MOVING, CULL>(P, tile, astride, lane_in_group, group_in_cta, xch);
 }
 
 }  // namespace gmapp

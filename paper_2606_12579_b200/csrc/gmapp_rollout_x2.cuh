@@ -585,17 +585,22 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
     }
 }
 
-// pack (xyz, r) -> sphere-pair layout; R = r + r_agent stored negated; sentinel pairs up to n2_fill
-__global__ void k_pack_pairs(const float4* __restrict__ sph_raw, int n, int n2_fill, float r_agent,
-                             float4* __restrict__ pairA, float4* __restrict__ pairB) {
+// pack (xyz, r) [+ velocities] -> sphere-pair arrays A, B (, U, V), `stride` float4 apart; R = r + r_agent stored
+// negated; sentinel pairs (far away, at rest) up to n2_fill
+__global__ void k_pack_pairs(const float4* __restrict__ sph_raw, const float4* __restrict__ svel, int n, int n2_fill,
+                             float r_agent, float4* __restrict__ pairs, int stride) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n2_fill) return;
     const float far = 1.0e18f;
-    float4 s0 = make_float4(far, far, far, 0.0f), s1 = s0;
-    if (2 * j < n) { s0 = sph_raw[2 * j]; s0.w += r_agent; }
-    if (2 * j + 1 < n) { s1 = sph_raw[2 * j + 1]; s1.w += r_agent; }
-    pairA[j] = make_float4(s0.x, s1.x, s0.y, s1.y);
-    pairB[j] = make_float4(s0.z, s1.z, -s0.w, -s1.w);
+    float4 s0 = make_float4(far, far, far, 0.0f), s1 = s0, u0 = make_float4(0, 0, 0, 0), u1 = u0;
+    if (2 * j < n) { s0 = sph_raw[2 * j]; s0.w += r_agent; if (svel) u0 = svel[2 * j]; }
+    if (2 * j + 1 < n) { s1 = sph_raw[2 * j + 1]; s1.w += r_agent; if (svel) u1 = svel[2 * j + 1]; }
+    pairs[j] = make_float4(s0.x, s1.x, s0.y, s1.y);
+    pairs[stride + j] = make_float4(s0.z, s1.z, -s0.w, -s1.w);
+    if (svel) {
+        pairs[2 * stride + j] = make_float4(u0.x, u1.x, u0.y, u1.y);
+        pairs[3 * stride + j] = make_float4(u0.z, u1.z, 0.0f, 0.0f);
+    }
 }
 
 }  // namespace gmapp
