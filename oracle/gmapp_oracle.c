@@ -17,7 +17,8 @@
  * P4 closed-form magnitude, P5 hand-computed single-sphere cases, P6 mirror / rotation / permutation
  * symmetry, P7 Galilean, P8 no-obstacle closed form (matrix power), P9 multi-step golden by hand,
  * P10 SE(3) exp/log vs scipy expm/logm and 6D == 3D reduction, P11 cost closed forms,
- * P12 agent independence, P13 brute-force numpy restatement.
+ * P12 agent independence, P13 brute-force numpy restatement, P14 APF (Eq. 1 under reading N1): hand-computed
+ * single-sphere cases, F = -grad of the Khatib potential, superposition and mirror symmetry.
  * parity unpinned (fixed by DESIGN.md readings only, the paper gives no value to pin them to):
  * G16 (the 1/2 of Eq. 10 is taken as printed), G18 (frame of the 6D repulsion), G19 (N_k = S+1),
  * G23 (default constants), G24 (collision-first selection key).

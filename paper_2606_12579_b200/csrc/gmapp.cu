@@ -106,14 +106,16 @@ typedef void (*rollout_x2_fn)(const RolloutX2Params);
 static const int kX2SweepThreads = 512;       // sweep threads per CTA; mode 2 adds one epilogue warp per group (<= 672 in all)
 // mode 3 = mode 2 compiled for up to 7 groups (21 warps, 80 registers); mode 2 proper holds <= 4 groups
 // (20 warps = 5 per SM sub-partition, 96 registers), which is what one wave of config 3 needs
-static rollout_x2_fn rollout_x2_kernel(int at, int mode, bool cull, int stage) {
-#define PICKX(A, M, MT)                                                                                              \
-    (cull ? (stage ? (rollout_x2_fn)k_rollout_x2<A, M, true, 1, MT> : (rollout_x2_fn)k_rollout_x2<A, M, true, 0, MT>)     \
-          : (stage ? (rollout_x2_fn)k_rollout_x2<A, M, false, 1, MT> : (rollout_x2_fn)k_rollout_x2<A, M, false, 0, MT>))
+static rollout_x2_fn rollout_x2_kernel(int at, int mode, bool cull, int stage, bool apf) {
+#define PICKS(A, M, MT, F)                                                                                                  \
+    (cull ? (stage ? (rollout_x2_fn)k_rollout_x2<A, M, true, 1, MT, F> : (rollout_x2_fn)k_rollout_x2<A, M, true, 0, MT, F>)     \
+          : (stage ? (rollout_x2_fn)k_rollout_x2<A, M, false, 1, MT, F> : (rollout_x2_fn)k_rollout_x2<A, M, false, 0, MT, F>))
+#define PICKX(A, M, MT) (apf ? PICKS(A, M, MT, true) : PICKS(A, M, MT, false))
     if (mode == 4) return PICKX(2, 4, 512);
     if (at == 2) return mode == 3 ? PICKX(2, 2, 672) : (mode == 2 ? PICKX(2, 2, 640) : (mode == 1 ? PICKX(2, 1, 512) : PICKX(2, 0, 512)));
     return mode == 3 ? PICKX(1, 2, 672) : (mode == 2 ? PICKX(1, 2, 640) : (mode == 1 ? PICKX(1, 1, 512) : PICKX(1, 0, 512)));
 #undef PICKX
+#undef PICKS
 }
 static int rollout_max_threads(int kind, int at) { return (kind == GMAPP_MOTOR6 || at == 2) ? 512 : 1024; }
 
@@ -187,11 +189,12 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
     for (int at = 1; at <= 2; ++at)
         for (int md = 0; md < 5; ++md)
             for (int cu = 0; cu < 2; ++cu)
-                for (int st = 0; st < 2; ++st) {
-                    e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, md, cu, st),
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
-                    if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
-                }
+                for (int st = 0; st < 2; ++st)
+                    for (int hf = 0; hf < 2; ++hf) {
+                        e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, md, cu, st, hf != 0),
+                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
+                        if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
+                    }
     *out = c;
     return GMAPP_OK;
 }
@@ -322,7 +325,7 @@ static gmapp_status check_gains(gmapp_ctx* c, const gmapp_gains* g, const char* 
         return fail(c, GMAPP_EINVAL, "%s: need 0 < eps_dist <= r_influence (Alg. 1 lines 6-7)", who);
     if (g->r_agent < 0.0f || g->r_cost_goal < 0.0f || g->r_cost_obs < 0.0f || !(g->a_max > 0.0f))
         return fail(c, GMAPP_EINVAL, "%s: r_agent, r_cost_* must be >= 0 and a_max > 0", who);
-    if (g->heuristic != 0) return fail(c, GMAPP_EINVAL, "%s: only heuristic 0 (circular field / MFI, Eq. 2-3) is built", who);
+    if (g->heuristic != 0 && g->heuristic != 1) return fail(c, GMAPP_EINVAL, "%s: heuristic must be 0 (circular field / MFI, Eq. 2-3) or 1 (APF, Eq. 1)", who);
     return GMAPP_OK;
 }
 
@@ -441,6 +444,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     P.c_lin = g->vel_factor * dt * g->inv_mass;
     P.inv_mass = g->inv_mass; P.vel_factor = g->vel_factor;
     P.r_d = g->r_influence; P.eps = g->eps_dist;
+    P.apf = g->heuristic == 1; P.inv_rd = 1.0f / g->r_influence;
     P.rcg = g->r_cost_goal > 0.0f ? g->r_cost_goal : g->r_influence;
     P.rco = g->r_cost_obs > 0.0f ? g->r_cost_obs : g->r_influence;
     P.w_goal = g->w_goal; P.w_obs = g->w_obs; P.w_path = g->w_path; P.w_smooth = g->w_smooth; P.a_max = g->a_max;
@@ -448,7 +452,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     P.tile_off = tile_off; P.xch_off = xch_off; P.rec_off = rec_off;
     const int block = mode == 4 ? tmax : (mode >= 2 ? G * L + 32 * G : round_up(G * L, 32));
     const int smem = tile_off + (stage == 1 ? (int)tile_bytes : 0);
-    rollout_x2_fn fn = rollout_x2_kernel(at, mode, cull != 0, stage);
+    rollout_x2_fn fn = rollout_x2_kernel(at, mode, cull != 0, stage, g->heuristic == 1);
     fn<<<grid, block, smem, st>>>(P);
     CUDA_TRY(c, cudaGetLastError());
     ++launches;
@@ -505,6 +509,7 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
     P.c_rot = g->vel_factor * dt * g->inv_inertia;
     P.inv_mass = g->inv_mass;
     P.r_d = g->r_influence; P.eps = g->eps_dist;
+    P.apf = g->heuristic == 1; P.inv_rd = 1.0f / g->r_influence;
     P.rcg = g->r_cost_goal > 0.0f ? g->r_cost_goal : g->r_influence;
     P.rco = g->r_cost_obs > 0.0f ? g->r_cost_obs : g->r_influence;
     P.w_goal = g->w_goal; P.w_obs = g->w_obs; P.w_path = g->w_path; P.w_smooth = g->w_smooth;
@@ -591,6 +596,7 @@ extern "C" gmapp_status gmapp_forces(gmapp_ctx* c, gmapp_kind kind, const float*
     P.k_circ = g->k_circ; P.k_att = g->k_att; P.k_damp = g->k_damp;
     P.k_att_rot = g->k_att_rot; P.k_damp_rot = g->k_damp_rot;
     P.r_d = g->r_influence; P.eps = g->eps_dist; P.t_obs = t_obstacles;
+    P.apf = g->heuristic == 1; P.inv_rd = 1.0f / g->r_influence;
     P.f_rep = d_f_rep; P.f_total = d_f_total;
     const int warps_per_block = 8;
     const int grid = (n_agents + warps_per_block - 1) / warps_per_block;

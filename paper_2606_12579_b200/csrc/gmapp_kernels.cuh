@@ -51,6 +51,8 @@ struct RolloutParams {
     float* cost;              // [n][5]
     float* minclr;            // [n]
     int* collided;            // [n]
+    int apf;                  // 1: APF heuristic (Eq. 1) instead of the circular field (Eq. 2-3)
+    float inv_rd;             // 1 / r_d (APF)
     int tile_off;             // byte offset of the sphere tile in dynamic shared memory
     int red_off;              // byte offset of the cross-warp exchange scratch
 };
@@ -79,9 +81,20 @@ __device__ __forceinline__ float pair_distance(float cx, float cy, float cz, flo
     return fmaf(0.5f * y, e, t - R);
 }
 
-template <int NA, bool FORCE, bool CULL>
+// APF (Eq. 1, Khatib form on the clamped surface distance, reading N1):
+// f_j = -k_f (1/d_O - 1/r_d) / d_O^2 * d/|d|; accumulated without k_f; exactly 0 outside r_d
+__device__ __forceinline__ void apf_accumulate(float ds, float q, float dx, float dy, float dz, float r_d, float eps,
+                                               float inv_rd, float& bx, float& by, float& bz) {
+    if (ds <= r_d) {
+        const float ro = rcp_approx(fmaxf(ds, eps));
+        const float m = (inv_rd - ro) * (ro * ro) * rsqrt_approx(q);
+        bx = fmaf(m, dx, bx); by = fmaf(m, dy, by); bz = fmaf(m, dz, bz);
+    }
+}
+
+template <int NA, bool FORCE, bool CULL, bool APF = false>
 __device__ __forceinline__ void pair_static(const float4 s, const float (&p)[NA][3], const float (&v)[NA][3],
-                                            float r_d, float eps, unsigned mask, StaticAcc<NA>& acc) {
+                                            float r_d, float eps, unsigned mask, StaticAcc<NA>& acc, float inv_rd = 0.0f) {
     float dx[NA], dy[NA], dz[NA], q[NA], ds[NA];
     bool any = false;
 #pragma unroll
@@ -92,6 +105,11 @@ __device__ __forceinline__ void pair_static(const float4 s, const float (&p)[NA]
     }
     if (!FORCE) return;
     if (CULL) { if (!__any_sync(mask, any)) return; }
+    if (APF) {
+#pragma unroll
+        for (int a = 0; a < NA; ++a) apf_accumulate(ds[a], q[a], dx[a], dy[a], dz[a], r_d, eps, inv_rd, acc.bx[a], acc.by[a], acc.bz[a]);
+        return;
+    }
 #pragma unroll
     for (int a = 0; a < NA; ++a) {
         float dO = fmaxf(ds[a], eps);
@@ -107,10 +125,10 @@ __device__ __forceinline__ void pair_static(const float4 s, const float (&p)[NA]
 
 // moving spheres: centre advected to obstacle time tk, relative velocity per pair, force accumulated
 // directly:  f_j = w [ (s/|vr|) vr - |vr| d ],  w = s / (dO q),  s = d.vr   (k_f applied after the sum)
-template <int NA, bool FORCE, bool CULL>
+template <int NA, bool FORCE, bool CULL, bool APF = false>
 __device__ __forceinline__ void pair_moving(const float4 s, const float4 su, float tk,
                                             const float (&p)[NA][3], const float (&v)[NA][3],
-                                            float r_d, float eps, unsigned mask, StaticAcc<NA>& acc) {
+                                            float r_d, float eps, unsigned mask, StaticAcc<NA>& acc, float inv_rd = 0.0f) {
     const float cx = fmaf(tk, su.x, s.x), cy = fmaf(tk, su.y, s.y), cz = fmaf(tk, su.z, s.z);
     float dx[NA], dy[NA], dz[NA], q[NA], ds[NA];
     bool any = false;
@@ -122,6 +140,11 @@ __device__ __forceinline__ void pair_moving(const float4 s, const float4 su, flo
     }
     if (!FORCE) return;
     if (CULL) { if (!__any_sync(mask, any)) return; }
+    if (APF) {
+#pragma unroll
+        for (int a = 0; a < NA; ++a) apf_accumulate(ds[a], q[a], dx[a], dy[a], dz[a], r_d, eps, inv_rd, acc.bx[a], acc.by[a], acc.bz[a]);
+        return;
+    }
 #pragma unroll
     for (int a = 0; a < NA; ++a) {
         float vx = v[a][0] - su.x, vy = v[a][1] - su.y, vz = v[a][2] - su.z;
@@ -141,11 +164,11 @@ __device__ __forceinline__ void pair_moving(const float4 s, const float4 su, flo
 }
 
 // One lane's slice of the sphere sum for NA agents at obstacle time tk.
-template <int NA, bool MOVING, bool FORCE, bool CULL>
+template <int NA, bool MOVING, bool FORCE, bool CULL, bool APF = false>
 __device__ __forceinline__ void sphere_sweep(const float4* __restrict__ sph, const float4* __restrict__ svel,
                                              int n_pad, int lane, int L, float tk,
                                              const float (&p)[NA][3], const float (&v)[NA][3],
-                                             float r_d, float eps, unsigned mask, StaticAcc<NA>& acc) {
+                                             float r_d, float eps, unsigned mask, StaticAcc<NA>& acc, float inv_rd = 0.0f) {
     constexpr int U = (NA == 1) ? 4 : 2;
     int j = lane;
     const int step = L * U;
@@ -155,14 +178,14 @@ __device__ __forceinline__ void sphere_sweep(const float4* __restrict__ sph, con
         for (int u = 0; u < U; ++u) { s[u] = sph[j + u * L]; if (MOVING) su[u] = svel[j + u * L]; }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            if (MOVING) pair_moving<NA, FORCE, CULL>(s[u], su[u], tk, p, v, r_d, eps, mask, acc);
-            else        pair_static<NA, FORCE, CULL>(s[u], p, v, r_d, eps, mask, acc);
+            if (MOVING) pair_moving<NA, FORCE, CULL, APF>(s[u], su[u], tk, p, v, r_d, eps, mask, acc, inv_rd);
+            else        pair_static<NA, FORCE, CULL, APF>(s[u], p, v, r_d, eps, mask, acc, inv_rd);
         }
     }
     for (; j < n_pad; j += L) {
         float4 s = sph[j];
-        if (MOVING) pair_moving<NA, FORCE, CULL>(s, svel[j], tk, p, v, r_d, eps, mask, acc);
-        else        pair_static<NA, FORCE, CULL>(s, p, v, r_d, eps, mask, acc);
+        if (MOVING) pair_moving<NA, FORCE, CULL, APF>(s, svel[j], tk, p, v, r_d, eps, mask, acc, inv_rd);
+        else        pair_static<NA, FORCE, CULL, APF>(s, p, v, r_d, eps, mask, acc, inv_rd);
     }
 }
 
@@ -296,13 +319,14 @@ __device__ __forceinline__ void rollout_point3(const RolloutParams& P, const flo
     for (int k = 0; k < P.steps; ++k) {
         const float tk = float(k) * P.dt;
         acc.clear();
-        sphere_sweep<NA, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, mask, acc);
+        if (P.apf) sphere_sweep<NA, MOVING, true, CULL, true>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, mask, acc, P.inv_rd);
+        else sphere_sweep<NA, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, mask, acc);
         group_allreduce<NA>(acc, P.L, lane_in_group, group_in_cta, red, k & 1, mask);
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
             float ex = P.goal[0] - p[a][0], ey = P.goal[1] - p[a][1], ez = P.goal[2] - p[a][2];
             float fx, fy, fz;
-            if (MOVING) { fx = P.k_circ * acc.bx[a]; fy = P.k_circ * acc.by[a]; fz = P.k_circ * acc.bz[a]; }
+            if (MOVING || P.apf) { fx = P.k_circ * acc.bx[a]; fy = P.k_circ * acc.by[a]; fz = P.k_circ * acc.bz[a]; }
             else cf_force_static(P.k_circ, acc.bx[a], acc.by[a], acc.bz[a], v[a][0], v[a][1], v[a][2], fx, fy, fz);
             fx = fmaf(P.k_att, ex, fmaf(-P.k_damp, v[a][0], fx));      // Eq. 6-7
             fy = fmaf(P.k_att, ey, fmaf(-P.k_damp, v[a][1], fy));
@@ -401,10 +425,11 @@ __device__ __forceinline__ void rollout_pose6(const RolloutParams& P, const floa
         p[0][0] = pos.x; p[0][1] = pos.y; p[0][2] = pos.z;
         v[0][0] = pdot.x; v[0][1] = pdot.y; v[0][2] = pdot.z;
         acc.clear();
-        sphere_sweep<1, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, mask, acc);
+        if (P.apf) sphere_sweep<1, MOVING, true, CULL, true>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, mask, acc, P.inv_rd);
+        else sphere_sweep<1, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, mask, acc);
         group_allreduce<1>(acc, P.L, lane_in_group, group_in_cta, red, k & 1, mask);
         Vec3 fr;
-        if (MOVING) fr = P.k_circ * v3(acc.bx[0], acc.by[0], acc.bz[0]);
+        if (MOVING || P.apf) fr = P.k_circ * v3(acc.bx[0], acc.by[0], acc.bz[0]);
         else cf_force_static(P.k_circ, acc.bx[0], acc.by[0], acc.bz[0], pdot.x, pdot.y, pdot.z, fr.x, fr.y, fr.z);
         if (cost_warp) ca.pose(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z), acc.dmin[0], P.rcg, P.rco);
         Vec3 tau, f;
@@ -507,6 +532,7 @@ struct ForceParams {
     const float* agents; int n_agents; int kind;
     float goal[8];
     float k_circ, k_att, k_damp, k_att_rot, k_damp_rot, r_d, eps, t_obs;
+    int apf; float inv_rd;
     float* f_rep; float* f_total;
 };
 
@@ -530,10 +556,11 @@ __global__ void __launch_bounds__(256) k_forces(const __grid_constant__ ForcePar
     }
     StaticAcc<1> acc;
     acc.clear();
-    sphere_sweep<1, MOVING, true, false>(P.sph, P.svel, P.n_pad, lane, 32, P.t_obs, p, v, P.r_d, P.eps, 0xffffffffu, acc);
+    if (P.apf) sphere_sweep<1, MOVING, true, false, true>(P.sph, P.svel, P.n_pad, lane, 32, P.t_obs, p, v, P.r_d, P.eps, 0xffffffffu, acc, P.inv_rd);
+    else sphere_sweep<1, MOVING, true, false>(P.sph, P.svel, P.n_pad, lane, 32, P.t_obs, p, v, P.r_d, P.eps, 0xffffffffu, acc);
     group_allreduce<1>(acc, 32, lane, 0, nullptr, 0, 0xffffffffu);
     Vec3 fr;
-    if (MOVING) fr = P.k_circ * v3(acc.bx[0], acc.by[0], acc.bz[0]);
+    if (MOVING || P.apf) fr = P.k_circ * v3(acc.bx[0], acc.by[0], acc.bz[0]);
     else cf_force_static(P.k_circ, acc.bx[0], acc.by[0], acc.bz[0], v[0][0], v[0][1], v[0][2], fr.x, fr.y, fr.z);
     if (lane != 0) return;
     if (P.f_rep) { float* o = P.f_rep + 3 * size_t(warp); o[0] = fr.x; o[1] = fr.y; o[2] = fr.z; }

@@ -34,18 +34,18 @@ __device__ __forceinline__ void warp_combine(const StaticAcc<NA>& acc, int lane,
 // f_j = w [ (s/|v_rel|) v_rel - |v_rel| d ],  w = s / (d_O |d|^2),  s = d.v_rel, accumulated directly
 // (k_f applied after the sum).  The distance half is the static one.
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool FORCE, bool CULL>
+template <int NA, bool FORCE, bool CULL, bool APF = false>
 __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, const float4* __restrict__ tB,
                                                 const float4* __restrict__ tU, const float4* __restrict__ tV, int n2p,
                                                 int lane, int L, float tk, const float (&p)[NA][3], const float (&v)[NA][3],
-                                                float r_d, float eps, unsigned mask, X2Acc<NA>& acc) {
+                                                float r_d, float eps, unsigned mask, X2Acc<NA>& acc, float inv_rd = 0.0f) {
     const u64 tiny = bc2(kTiny), half = bc2(0.5f), t2 = bc2(tk);
 #pragma unroll 2
     for (int j = lane; j < n2p; j += L) {
         const float4 s0 = tA[j], s1 = tB[j], s2 = tU[j], s3 = tV[j];
         const u64 ux = pk2(s2.x, s2.y), uy = pk2(s2.z, s2.w), uz = pk2(s3.x, s3.y), nR = pk2(s1.z, s1.w);
         const u64 cx = fma2(ux, t2, pk2(s0.x, s0.y)), cy = fma2(uy, t2, pk2(s0.z, s0.w)), cz = fma2(uz, t2, pk2(s1.x, s1.y));
-        u64 dx[NA], dy[NA], dz[NA], q[NA];
+        u64 dx[NA], dy[NA], dz[NA], q[NA], yy[NA];
         float d0[NA], d1[NA];
         bool any = false;
 #pragma unroll
@@ -54,6 +54,7 @@ __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, c
             q[a] = fma2(dx[a], dx[a], fma2(dy[a], dy[a], fma2(dz[a], dz[a], tiny)));
             float q0, q1; upk2(q[a], q0, q1);
             const u64 y = pk2(rsqrt_approx(q0), rsqrt_approx(q1));
+            yy[a] = y;
             const u64 t = mul2(q[a], y);
             const u64 hy = mul2(y, half);
             float t0, t1; upk2(t, t0, t1);
@@ -65,6 +66,20 @@ __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, c
         }
         if (!FORCE) continue;
         if (CULL) { if (!__any_sync(mask, any)) continue; }
+        if (APF) {                                          // Eq. 1 depends on positions only
+#pragma unroll
+            for (int a = 0; a < NA; ++a) {
+                float r0 = 0.0f, r1 = 0.0f;
+                if (d0[a] <= r_d) r0 = rcp_approx(fmaxf(d0[a], eps));
+                if (d1[a] <= r_d) r1 = rcp_approx(fmaxf(d1[a], eps));
+                const u64 ro = pk2(r0, r1);
+                const u64 m = mul2(mul2(sub2(bc2(inv_rd), ro), mul2(ro, ro)), yy[a]);
+                acc.bx[a] = fma2(m, dx[a], acc.bx[a]);
+                acc.by[a] = fma2(m, dy[a], acc.by[a]);
+                acc.bz[a] = fma2(m, dz[a], acc.bz[a]);
+            }
+            continue;
+        }
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
             const u64 vx = sub2(bc2(v[a][0]), ux), vy = sub2(bc2(v[a][1]), uy), vz = sub2(bc2(v[a][2]), uz);
@@ -114,7 +129,7 @@ struct EpiPoint3 {
         fax = fmaf(P.k_att, ex, -P.k_damp * v[0]); fay = fmaf(P.k_att, ey, -P.k_damp * v[1]); faz = fmaf(P.k_att, ez, -P.k_damp * v[2]);
     }
     __device__ __forceinline__ void post(const RolloutParams& P, float bx, float by, float bz) {
-        if (MOVING) {                                      // the sweep accumulated the force vector itself
+        if (MOVING || P.apf) {                             // the sweep accumulated the force vector itself
             fx = fmaf(P.k_circ, bx, fax); fy = fmaf(P.k_circ, by, fay); fz = fmaf(P.k_circ, bz, faz);
         } else {
             const float A = fmaf(bx, v[0], fmaf(by, v[1], bz * v[2]));
@@ -190,7 +205,7 @@ struct EpiPose6 {
     }
     __device__ __forceinline__ void post(const RolloutParams& P, float bx, float by, float bz) {
         Vec3 fr;
-        if (MOVING) fr = P.k_circ * v3(bx, by, bz);
+        if (MOVING || P.apf) fr = P.k_circ * v3(bx, by, bz);
         else cf_force_static(P.k_circ, bx, by, bz, pub[3], pub[4], pub[5], fr.x, fr.y, fr.z);
         const Vec3 f = fpre + qrot_inv(x.r, fr);                           // Eq. 6 in the body frame (reading G18)
         x.nu = fma3(P.c_lin, f, x.nu);                                     // Eq. 9-10, linear block
@@ -259,10 +274,12 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
         const float tk = float(k) * P.dt;
         acc.clear();
         if (MOVING) {
-            if (!last) sweep_x2_moving<NA, true, CULL>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc);
+            if (!last && P.apf) sweep_x2_moving<NA, true, CULL, true>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc, P.inv_rd);
+            else if (!last) sweep_x2_moving<NA, true, CULL>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc);
             else       sweep_x2_moving<NA, false, false>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc);
         } else {
-            if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
+            if (!last && P.apf) sweep_x2<NA, true, CULL, true>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc, P.inv_rd);
+            else if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
             else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
         }
         float X, Y, Z, D;

@@ -68,6 +68,8 @@ struct RolloutX2Params {
     int tile_off;             // byte offset of the sphere tile in dynamic shared memory
     int xch_off;              // byte offset of the cross-warp exchange area
     int rec_off;              // byte offset of the per-agent state records (mode 4)
+    int apf;                  // 1: APF heuristic (Eq. 1) instead of the circular field (Eq. 2-3)
+    float inv_rd;             // 1 / r_d (APF)
 };
 
 // per-lane partial sums of NA agents over the lane's sphere pairs (both halves of a pair kept apart)
@@ -82,16 +84,18 @@ struct X2Acc {
 };
 
 // One lane's slice of the sphere sum: pairs lane, lane+L, ... ; FORCE=false is the distance-only final pass.
-template <int NA, bool FORCE, bool CULL>
+// APF = true: Eq. 1 in the Khatib form on the clamped surface distance (reading N1),
+// f_j = -k_f (1/d_O - 1/r_d) / d_O^2 * d/|d|; the sums then hold the force itself (no velocity factor).
+template <int NA, bool FORCE, bool CULL, bool APF = false>
 __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const float4* __restrict__ tB, int n2p,
                                          int lane, int L, const float (&p)[NA][3], const float (&v)[NA][3],
-                                         float r_d, float eps, unsigned mask, X2Acc<NA>& acc) {
+                                         float r_d, float eps, unsigned mask, X2Acc<NA>& acc, float inv_rd = 0.0f) {
     const u64 tiny = bc2(kTiny), half = bc2(0.5f);
 #pragma unroll kX2Unroll
     for (int j = lane; j < n2p; j += L) {
         const float4 s0 = tA[j], s1 = tB[j];
         const u64 cx = pk2(s0.x, s0.y), cy = pk2(s0.z, s0.w), cz = pk2(s1.x, s1.y), nR = pk2(s1.z, s1.w);
-        u64 dx[NA], dy[NA], dz[NA], q[NA];
+        u64 dx[NA], dy[NA], dz[NA], q[NA], yy[NA];
         float d0[NA], d1[NA];
         bool any = false;
 #pragma unroll
@@ -100,6 +104,7 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
             q[a] = fma2(dx[a], dx[a], fma2(dy[a], dy[a], fma2(dz[a], dz[a], tiny)));
             float q0, q1; upk2(q[a], q0, q1);
             const u64 y = pk2(rsqrt_approx(q0), rsqrt_approx(q1));
+            yy[a] = y;
             const u64 t = mul2(q[a], y);
             const u64 hy = mul2(y, half);
             float t0, t1; upk2(t, t0, t1);
@@ -111,6 +116,20 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
         }
         if (!FORCE) continue;
         if (CULL) { if (!__any_sync(mask, any)) continue; }
+        if (APF) {
+#pragma unroll
+            for (int a = 0; a < NA; ++a) {
+                float r0 = 0.0f, r1 = 0.0f;                                  // 1/d_O inside r_d, else 0 (contributes exactly 0)
+                if (d0[a] <= r_d) r0 = rcp_approx(fmaxf(d0[a], eps));
+                if (d1[a] <= r_d) r1 = rcp_approx(fmaxf(d1[a], eps));
+                const u64 ro = pk2(r0, r1);
+                const u64 m = mul2(mul2(sub2(bc2(inv_rd), ro), mul2(ro, ro)), yy[a]);   // -(1/d_O - 1/r_d)/d_O^2 / |d|
+                acc.bx[a] = fma2(m, dx[a], acc.bx[a]);
+                acc.by[a] = fma2(m, dy[a], acc.by[a]);
+                acc.bz[a] = fma2(m, dz[a], acc.bz[a]);
+            }
+            continue;
+        }
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
             const u64 den = mul2(pk2(fmaxf(d0[a], eps), fmaxf(d1[a], eps)), q[a]);     // d_O * |d|^2
@@ -206,9 +225,13 @@ struct AgentX2 {
     // The critical path once the sums B are known: f_r = k_f [((B.v)/|v|) v - |v| B] (BAC-CAB form of Eq. 2-3),
     // f = f_a + f_r (Eq. 6), v += vel_factor dt inv_mass f (Eq. 9-10), p += dt v (Eq. 11).
     __device__ __forceinline__ void post(const RolloutX2Params& P, float bx, float by, float bz, float& fx, float& fy, float& fz) {
-        const float A = fmaf(bx, v[0], fmaf(by, v[1], bz * v[2]));
-        const float c1 = P.k_circ * inv * A, c2 = -P.k_circ * nv;
-        fx = fmaf(c1, v[0], fmaf(c2, bx, fax)); fy = fmaf(c1, v[1], fmaf(c2, by, fay)); fz = fmaf(c1, v[2], fmaf(c2, bz, faz));
+        if (P.apf) {                                       // Eq. 1: the sums are the force itself
+            fx = fmaf(P.k_circ, bx, fax); fy = fmaf(P.k_circ, by, fay); fz = fmaf(P.k_circ, bz, faz);
+        } else {
+            const float A = fmaf(bx, v[0], fmaf(by, v[1], bz * v[2]));
+            const float c1 = P.k_circ * inv * A, c2 = -P.k_circ * nv;
+            fx = fmaf(c1, v[0], fmaf(c2, bx, fax)); fy = fmaf(c1, v[1], fmaf(c2, by, fay)); fz = fmaf(c1, v[2], fmaf(c2, bz, faz));
+        }
         v[0] = fmaf(P.c_lin, fx, v[0]); v[1] = fmaf(P.c_lin, fy, v[1]); v[2] = fmaf(P.c_lin, fz, v[2]);
         p[0] = fmaf(P.dt, v[0], p[0]); p[1] = fmaf(P.dt, v[1], p[1]); p[2] = fmaf(P.dt, v[2], p[2]);
     }
@@ -268,7 +291,7 @@ __device__ __forceinline__ void warp_combine(const X2Acc<NA>& acc, int lane, flo
 // ---------------------------------------------------------------------------------------------
 // group body, L == 32: one warp per group does everything; agent a on lanes 0-15, agent b on lanes 16-31
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL>
+template <int NA, bool CULL, bool APF>
 __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, const float4* tA, const float4* tB,
                                                    int first_agent, int lane) {
     const int half = (NA == 2) ? (lane >> 4) : 0;
@@ -290,7 +313,7 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
             for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
         }
         acc.clear();
-        if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc);
+        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc, P.inv_rd);
         else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
@@ -324,7 +347,7 @@ __device__ __forceinline__ void agent_load(AgentX2& a, const float* r) {
     a.ca.sumJ = r[15]; a.ca.cJ = r[16]; a.ca.minclr = r[17]; a.ca.d1 = r[18]; a.ca.collided = __float_as_int(r[19]);
 }
 
-template <int NA, bool CULL>
+template <int NA, bool CULL, bool APF>
 __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float4* tA, const float4* tB, int agent0,
                                            int lane, int k, float* rec0) {
     const int half = (NA == 2) ? (lane >> 4) : 0;
@@ -346,7 +369,7 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     const bool last = (k == P.steps);
     X2Acc<NA> acc;
     acc.clear();
-    if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc);
+    if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc, P.inv_rd);
     else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc);
     float X, Y, Z, D;
     warp_combine<NA>(acc, lane, X, Y, Z, D);
@@ -364,7 +387,7 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     __syncwarp();
 }
 
-template <bool CULL>
+template <bool CULL, bool APF>
 __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, const float4* tA, const float4* tB,
                                                     int first_agent, int n_mine, int lane, float* recs) {
     // records of this warp's agents: recs[i * kAgentRecWords], i < n_mine
@@ -376,8 +399,8 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
     __syncwarp();
     for (int k = 0; k <= P.steps; ++k) {
         int i = 0;
-        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL>(P, tA, tB, first_agent + i, lane, k, recs + i * kAgentRecWords);
-        if (i < n_mine) chunk_step<1, CULL>(P, tA, tB, first_agent + i, lane, k, recs + i * kAgentRecWords);
+        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL, APF>(P, tA, tB, first_agent + i, lane, k, recs + i * kAgentRecWords);
+        if (i < n_mine) chunk_step<1, CULL, APF>(P, tA, tB, first_agent + i, lane, k, recs + i * kAgentRecWords);
     }
 }
 
@@ -388,7 +411,7 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
 //   sweep warp k:    write part[k&1] -> arrive(bar_part) -> sync(bar_state) -> read state[k&1]
 //   epilogue warp k: sync(bar_part) -> read part[k&1] -> integrate -> write state[k&1] -> arrive(bar_state) -> costs
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL>
+template <int NA, bool CULL, bool APF>
 __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, const float4* tA, const float4* tB,
                                                   int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
     const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
@@ -408,7 +431,7 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         acc.clear();
-        if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
+        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc, P.inv_rd);
         else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
@@ -463,7 +486,7 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
 // ---------------------------------------------------------------------------------------------
 // group body, L < 32 (several groups per warp): plain butterfly, every lane integrates its group's agents
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL>
+template <int NA, bool CULL, bool APF>
 __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, const float4* tA, const float4* tB,
                                                      int first_agent, int lane_in_group) {
     const unsigned mask = __activemask();
@@ -479,7 +502,7 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 #pragma unroll
             for (int i = 0; i < 3; ++i) { p[a][i] = ag[a].p[i]; v[a][i] = ag[a].v[i]; }
         acc.clear();
-        if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, mask, acc);
+        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, mask, acc, P.inv_rd);
         else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, mask, acc);
         float x[NA], y[NA], z[NA], dm[NA];
 #pragma unroll
@@ -509,7 +532,7 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 // 2: L >= 64 (W sweep warps + one epilogue warp per group; threads [0, G L) sweep, [G L, G L + 32 G) epilogue);
 // 4: many agents per CTA, each warp walks its block of agents in chunks of two (state records in shared memory);
 // STAGE 1 = sphere pairs staged in shared memory by TMA bulk copies
-template <int AT, int MODE, bool CULL, int STAGE, int MAXT>
+template <int AT, int MODE, bool CULL, int STAGE, int MAXT, bool APF>
 __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ RolloutX2Params P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
@@ -555,8 +578,8 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         if (STAGE == 1) mbar_wait(bar, 0);
         if (na <= 0) return;
         const int lane_in_group = tid & (P.L - 1);
-        if (AT == 2 && na >= 2) group_sweep_warps<NA2, CULL>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
-        else group_sweep_warps<1, CULL>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
+        if (AT == 2 && na >= 2) group_sweep_warps<NA2, CULL, APF>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
+        else group_sweep_warps<1, CULL, APF>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
         return;
     }
     if (MODE == 4) {
@@ -567,7 +590,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         if (STAGE == 1) mbar_wait(bar, 0);
         if (n_mine <= 0) return;
         float* recs = reinterpret_cast<float*>(smem_raw + P.rec_off) + start * kAgentRecWords;
-        warp_rollout_chunks<CULL>(P, tA, tB, cta_first + start, n_mine, tid & 31, recs);
+        warp_rollout_chunks<CULL, APF>(P, tA, tB, cta_first + start, n_mine, tid & 31, recs);
         return;
     }
     const int group_in_cta = tid >> P.logL;
@@ -577,11 +600,11 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
     if (STAGE == 1) mbar_wait(bar, 0);
     if (na <= 0) return;
     if (MODE == 1) {
-        if (AT == 2 && na >= 2) group_rollout_warp<NA2, CULL>(P, tA, tB, first, lane_in_group);
-        else group_rollout_warp<1, CULL>(P, tA, tB, first, lane_in_group);
+        if (AT == 2 && na >= 2) group_rollout_warp<NA2, CULL, APF>(P, tA, tB, first, lane_in_group);
+        else group_rollout_warp<1, CULL, APF>(P, tA, tB, first, lane_in_group);
     } else {
-        if (AT == 2 && na >= 2) group_rollout_narrow<NA2, CULL>(P, tA, tB, first, lane_in_group);
-        else group_rollout_narrow<1, CULL>(P, tA, tB, first, lane_in_group);
+        if (AT == 2 && na >= 2) group_rollout_narrow<NA2, CULL, APF>(P, tA, tB, first, lane_in_group);
+        else group_rollout_narrow<1, CULL, APF>(P, tA, tB, first, lane_in_group);
     }
 }
 

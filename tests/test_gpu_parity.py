@@ -282,6 +282,48 @@ def test_pose6_large_rotation_fast_twist(api, ctx, orc):
     _check_rollout(api, ctx, orc, sc, smooth_tol=1e-3, allow_illcond=0.1)
 
 
+# ---------------------------------------------------------------------------------- APF heuristic (Eq. 1, NEXT row N1)
+def _apf(scene, k=1e-4):
+    """Same scene with the APF heuristic; k_f scaled so that (1/dO - 1/r_d)/dO^2 ~ 1e5 gives forces of order 10."""
+    import copy
+    s2 = copy.copy(scene)
+    s2.gains = dict(scene.gains, heuristic=1, k_circ=k)
+    return s2
+
+
+@pytest.mark.parametrize("moving", [False, True], ids=["static", "moving"])
+def test_apf_rollout_point3(api, ctx, orc, moving):
+    sc = _apf(scenes.fast_clutter(moving=moving))
+    g, o = _check_rollout(api, ctx, orc, sc)
+    assert g["info"]["packed_x2"] == (0 if moving else 1)
+    # the heuristic really changes the motion (guards against a silently ignored flag)
+    base = api.run_scene(ctx, scenes.fast_clutter(moving=moving))
+    assert np.abs(base["final"] - g["final"]).max() > 1e-3
+
+
+@pytest.mark.parametrize("tuning", [dict(lanes_per_agent=8, agents_per_thread=2, max_ctas=6), dict(lanes_per_agent=32),
+                                    dict(max_ctas=1, cull=1), dict(scalar_path=1, cull=1)],
+                         ids=lambda t: "-".join(f"{k[:4]}{v}" for k, v in t.items()))
+def test_apf_launch_variants(api, ctx, orc, tuning):
+    try:
+        for moving in (False, True):
+            _check_rollout(api, ctx, orc, _apf(scenes.fast_clutter(moving=moving, n_agents=45, n_spheres=333)), tuning=tuning)
+    finally:
+        ctx.set_tuning(reset=True)
+
+
+def test_apf_rollout_pose6_and_config3(api, ctx, orc):
+    _check_rollout(api, ctx, orc, _apf(scenes.config4(n_agents=32, n_spheres=512, steps=100)), smooth_tol=1e-3)
+    _check_rollout(api, ctx, orc, _apf(scenes.config3(n_agents=300)))
+
+
+@pytest.mark.parametrize("moving", [False, True], ids=["static", "moving"])
+def test_apf_per_step_forces(api, ctx, orc, moving):
+    sc = _apf(scenes.fast_clutter(moving=moving, n_agents=128, n_spheres=700))
+    _check_forces_on_oracle_states(api, ctx, orc, sc, [0, 25, 50, 100])
+    _check_forces_on_oracle_states(api, ctx, orc, _apf(scenes.config4(n_agents=32, n_spheres=512, steps=60)), [0, 30, 60])
+
+
 # ---------------------------------------------------------------------------------- launch variants
 @pytest.mark.parametrize("tuning", [
     dict(lanes_per_agent=8, agents_per_thread=1), dict(lanes_per_agent=32, agents_per_thread=1),

@@ -504,3 +504,63 @@ def test_scenes_are_seeded_and_shaped():
     assert c1.agents.shape == (16, 6) and c1.xyzr.shape == (8, 4) and np.all(c1.agents[:, 3:] == 0)
     c5 = scenes.config5(1024, 4096)
     assert c5.agents.shape == (1024, 6) and c5.steps == 200
+
+
+# ---------------------------------------------------------------------------------- P14: APF (Eq. 1, reading N1)
+def _p14_rows():
+    rows = []
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "p14_apf_single_sphere.txt")):
+        if line.strip() and not line.startswith("#"):
+            t = line.split()
+            rows.append((t[0], [float(x) for x in t[1:4]], float(t[4]), [float(x) for x in t[5:8]]))
+    return rows
+
+
+@pytest.mark.parametrize("row", _p14_rows(), ids=lambda r: r[0])
+def test_P14_apf_hand_computed_single_sphere(orc, row):
+    name, c, r, want = row
+    g = dict(scenes.default_gains(), heuristic=1)
+    for v in ([1.0, 0.0, 0.0], [0.0, 0.0, 0.0], [-0.3, 0.4, 2.0]):        # Eq. 1 has no velocity in it
+        f, ds, gated = orc.pair_force([0, 0, 0], v, c, r, g)
+        assert np.allclose(f, want, rtol=2e-9, atol=1e-9), (name, f, want)
+    assert gated == (name != "C")
+
+
+def test_P14_apf_is_minus_gradient_of_khatib_potential(orc):
+    """Textbook check: F = -grad U with U = (k_f/2)(1/dO - 1/r_d)^2 inside r_d (central differences in FP64)."""
+    g = dict(scenes.default_gains(), heuristic=1, k_circ=0.7)
+    rng = np.random.default_rng(5)
+    c, r = np.array([0.05, -0.02, 0.1]), 0.04
+    def U(p):
+        ds = np.linalg.norm(c - p) - r
+        return 0.0 if ds > g["r_influence"] else 0.5 * g["k_circ"] * (1.0 / max(ds, g["eps_dist"]) - 1.0 / g["r_influence"]) ** 2
+    n_in = 0
+    for _ in range(50):
+        p = c + rng.normal(size=3) * 0.08
+        ds = np.linalg.norm(c - p) - r
+        if not (2e-3 < ds < g["r_influence"] - 1e-3):
+            continue
+        n_in += 1
+        h = 1e-7
+        grad = np.array([(U(p + h * e) - U(p - h * e)) / (2 * h) for e in np.eye(3)])
+        f, _, gated = orc.pair_force(p, [0.2, 0.1, 0.0], c, r, g)
+        assert gated and np.allclose(f, -grad, rtol=1e-5, atol=1e-6)
+        assert np.dot(f, c - p) < 0                                   # repulsion: away from the obstacle
+    assert n_in >= 10
+
+
+def test_P14_apf_rollout_superposition_and_mirror(orc):
+    """APF forces superpose over spheres and mirror with the scene (same O(3) argument as P6)."""
+    sc = scenes.fast_clutter(n_agents=6, n_spheres=40, steps=20)
+    g = dict(sc.gains, heuristic=1)
+    st = sc.agents.astype(np.float64)
+    tot = orc.forces_point3(st, sc.xyzr, None, sc.goal, g)["f_rep"]
+    acc = np.zeros_like(tot)
+    for j in range(sc.n_spheres):
+        acc += orc.forces_point3(st, sc.xyzr[j:j + 1], None, sc.goal, g)["f_rep"]
+    assert np.allclose(tot, acc, rtol=1e-12, atol=1e-12)
+    M = np.diag([1.0, -1.0, 1.0])
+    stm = np.concatenate([st[:, :3] @ M, st[:, 3:] @ M], axis=1)
+    xm = sc.xyzr.astype(np.float64).copy(); xm[:, :3] = xm[:, :3] @ M
+    totm = orc.forces_point3(stm, xm.astype(np.float32), None, (sc.goal @ M).astype(np.float32), g)["f_rep"]
+    assert np.allclose(totm, tot @ M, rtol=1e-12, atol=1e-12)
