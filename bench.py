@@ -303,6 +303,19 @@ def run_ours(args):
     peak_meas = ctx.measure_fp32_peak(False)
     peak_meas_x2 = ctx.measure_fp32_peak(True)
 
+    # ---- planning-cycle latency distribution: 20 warm-ups, 200 timed cycles, host wall clock of
+    # gmapp_rollout + gmapp_best_agent (launch + execution + sync + 12-byte download), spheres resident, no L2 flush
+    for _ in range(20):
+        cycle()
+    lat = []
+    for _ in range(200):
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
+        ctx.best_agent_ex(scene.alpha, scene.prev_best)
+        lat.append((time.perf_counter() - t0) * 1e3)
+    lat = np.array(lat)
+
     # ---- end to end through the C ABI with HOST buffers (sphere + agent upload, 8-byte result download)
     for _ in range(3):
         ctx.plan_cycle_host(kind, h_agents, goal, gains, scene.dt, scene.steps, h_xyzr=scene.xyzr, h_vel=scene.vel,
@@ -339,7 +352,9 @@ def run_ours(args):
                                           "device_p99": float(np.percentile(step_ms, 99)),
                                           "host_p50": float(np.percentile(host_ms, 50)),
                                           "host_p99": float(np.percentile(host_ms, 99)),
-                                          "rollout_kernel_mean": float(roll_ms.mean())},
+                                          "rollout_kernel_mean": float(roll_ms.mean()),
+                                          "host_200_warm": {"p50": float(np.percentile(lat, 50)), "p99": float(np.percentile(lat, 99)),
+                                                            "min": float(lat.min()), "runs": 200}},
             "wall_ms_per_step_incl_flush": wall_ms / K,
             "e2e": {"value": pairs_global * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                     "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_s / K * 1e3,

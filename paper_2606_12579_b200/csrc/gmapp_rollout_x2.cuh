@@ -29,6 +29,9 @@ typedef unsigned long long u64;
 #define GMAPP_X2_UNROLL 4      // sphere-pair iterations unrolled in the sweep (measured best on B200)
 #endif
 constexpr int kX2Unroll = GMAPP_X2_UNROLL;
+#ifndef GMAPP_X2_HALF_INT
+#define GMAPP_X2_HALF_INT 0
+#endif
 
 __device__ __forceinline__ u64 pk2(float lo, float hi) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
 __device__ __forceinline__ void upk2(u64 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
@@ -103,10 +106,13 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
             dx[a] = sub2(cx, bc2(p[a][0])); dy[a] = sub2(cy, bc2(p[a][1])); dz[a] = sub2(cz, bc2(p[a][2]));
             q[a] = fma2(dx[a], dx[a], fma2(dy[a], dy[a], fma2(dz[a], dz[a], tiny)));
             float q0, q1; upk2(q[a], q0, q1);
-            const u64 y = pk2(rsqrt_approx(q0), rsqrt_approx(q1));
+            const float y0 = rsqrt_approx(q0), y1 = rsqrt_approx(q1);
+            const u64 y = pk2(y0, y1);
             yy[a] = y;
             const u64 t = mul2(q[a], y);
-            const u64 hy = mul2(y, half);
+            // y/2 by an exponent decrement on the integer pipe (exact: y is a normal number for every finite q > 0)
+            const u64 hy = GMAPP_X2_HALF_INT ? pk2(__int_as_float(__float_as_int(y0) - 0x00800000), __int_as_float(__float_as_int(y1) - 0x00800000))
+                                             : mul2(y, half);
             float t0, t1; upk2(t, t0, t1);
             const u64 e = pk2(fmaf(-t0, t0, q0), fmaf(-t1, t1, q1));     // Newton residual q - t^2 (exact in the FMA)
             const u64 ds = fma2(hy, e, add2(t, nR));                     // dist - R, dist to ~1 ulp
