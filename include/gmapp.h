@@ -120,6 +120,17 @@ gmapp_status gmapp_set_obstacles_host(gmapp_ctx* ctx, const float* h_xyzr, const
 /* Optional launch tuning for later gmapp_rollout / gmapp_forces calls; NULL restores automatic choice. */
 gmapp_status gmapp_set_tuning(gmapp_ctx* ctx, const gmapp_tuning* tuning);
 
+/* Heterogeneous ensemble ("two agents per heuristic type, each with either a large or small
+ * detection radius"; Alg. 1 takes r_d per agent; one specialised kernel per heuristic,
+ * PAPER.md:262-266).  HOST arrays of n values, any of them NULL (= take the value from `gains`):
+ * h_r_influence[i] = r_d of agent i (> 0), h_k_circ[i] = k_f of agent i, h_heuristic[i] in {0 = circular field /
+ * MFI (Eq. 2-3), 1 = APF (Eq. 1)}.  The arrays are copied before the call returns (it synchronises the stream).
+ * Later gmapp_rollout calls must pass n_agents == n (else EINVAL); they issue one launch per heuristic present,
+ * and the Eq. 17 / 18 radii default to each agent's own r_d.  n = 0 (or all three NULL) restores uniform agents.
+ * gmapp_forces keeps using `gains` alone. */
+gmapp_status gmapp_set_agent_params(gmapp_ctx* ctx, const float* h_r_influence, const float* h_k_circ,
+                                    const int32_t* h_heuristic, int n, void* cuda_stream);
+
 /* One planning cycle: roll n_agents agents forward `steps` steps of size dt from the
  * states in d_agents (layout by `kind`), through Eq. 2-3, 6-11, accumulating Eq. 16-20 over the
  * steps+1 poses.  Final states are written to d_agents_out (same layout; may alias d_agents; may be

@@ -44,24 +44,16 @@ class gmapp_launch_info(C.Structure):
 
 
 EXPORTS = ["gmapp_default_gains", "gmapp_create", "gmapp_destroy", "gmapp_set_obstacles",
-           "gmapp_set_obstacles_host", "gmapp_set_tuning", "gmapp_rollout", "gmapp_best_agent", "gmapp_best_agent_ex",
+           "gmapp_set_obstacles_host", "gmapp_set_tuning", "gmapp_set_agent_params", "gmapp_rollout", "gmapp_best_agent", "gmapp_best_agent_ex",
            "gmapp_forces",
            "gmapp_get_results", "gmapp_plan_cycle_host", "gmapp_get_launch_info", "gmapp_measure_fp32_peak",
            "gmapp_sm_count", "gmapp_last_error"]
 
 
-def nvcc_command(out: str = _SO, extra=()):
-    return ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-            "-Xcompiler", "-fPIC", "-shared", "-I", _INCLUDE, *extra, "-o", out, os.path.join(_CSRC, "gmapp.cu")]
-
-
 def build(force: bool = False) -> str:
-    """Compile libgmapp.so in-tree for sm_100a (nvcc cross-compiles without a GPU)."""
-    srcs = [os.path.join(_CSRC, f) for f in os.listdir(_CSRC)] + [os.path.join(_INCLUDE, "gmapp.h")]
-    newest = max(os.path.getmtime(f) for f in srcs)
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < newest:
-        subprocess.check_call(nvcc_command())
-    return _SO
+    """Compile libgmapp.so in-tree for sm_100a (paper_2606_12579_b200/build_lib.py; nvcc cross-compiles without a GPU)."""
+    from . import build_lib
+    return build_lib.build(force=force)
 
 
 def _load():
@@ -76,6 +68,7 @@ def _load():
     lib.gmapp_set_obstacles.argtypes = [vp, vp, vp, C.c_int, vp]
     lib.gmapp_set_obstacles_host.argtypes = [vp, vp, vp, C.c_int, vp]
     lib.gmapp_set_tuning.argtypes = [vp, C.POINTER(gmapp_tuning)]
+    lib.gmapp_set_agent_params.argtypes = [vp, vp, vp, vp, C.c_int, vp]
     lib.gmapp_rollout.argtypes = [vp, C.c_int, vp, vp, C.c_int, fp, C.POINTER(gmapp_gains), C.c_float, C.c_int, vp]
     lib.gmapp_best_agent.argtypes = [vp, C.c_float, C.c_int, ip, fp, vp]
     lib.gmapp_best_agent_ex.argtypes = [vp, C.c_float, C.c_int, ip, fp, ip, vp]
@@ -198,6 +191,17 @@ class Context:
             return
         t = gmapp_tuning(lanes_per_agent, agents_per_thread, cull, stage, max_ctas, scalar_path)
         self._check(_lib.gmapp_set_tuning(self._h, C.byref(t)))
+
+    def set_agent_params(self, r_influence=None, k_circ=None, heuristic=None, n=None, stream=None):
+        """Per-agent detection radius / gain / heuristic (host arrays, any None); all None or n == 0 clears."""
+        arrs = [None if a is None else np.ascontiguousarray(a, dtype=dt)
+                for a, dt in ((r_influence, np.float32), (k_circ, np.float32), (heuristic, np.int32))]
+        if n is None:
+            n = max([a.shape[0] for a in arrs if a is not None], default=0)
+        for a in arrs:
+            assert a is None or a.shape[0] >= n
+        ptrs = [None if a is None else a.ctypes.data_as(C.c_void_p) for a in arrs]
+        self._check(_lib.gmapp_set_agent_params(self._h, ptrs[0], ptrs[1], ptrs[2], int(n), _stream(stream)))
 
     def rollout(self, kind, d_agents, d_agents_out, goal, gains, dt, steps, n_agents=None, stream=None):
         n = int(d_agents.shape[0]) if n_agents is None else n_agents

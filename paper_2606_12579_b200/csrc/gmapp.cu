@@ -6,10 +6,11 @@
 #include <stdlib.h>
 #include <string.h>
 
+#define GMAPP_MAIN_TU
 #include "../../include/gmapp.h"
 #include "gmapp_kernels.cuh"
 #include "gmapp_rollout_x2.cuh"
-#include "gmapp_rollout_wide.cuh"
+#include "gmapp_tables.h"
 
 using namespace gmapp;
 
@@ -38,6 +39,14 @@ struct gmapp_ctx {
     float* d_vel_stage = nullptr;        // [max_spheres][3]
     float* h_pinned = nullptr;           // spheres*7 + agents*14 floats
     size_t h_pinned_floats = 0;
+    // heterogeneous ensemble (gmapp_set_agent_params): per-agent r_d, k_f, and agent indices grouped by heuristic
+    float* d_ap_rd = nullptr; float* d_ap_kf = nullptr; int* d_ap_idx = nullptr;
+    float* h_ap = nullptr;               // pinned staging: 3 * max_agents words
+    int ap_n = 0;                        // 0: not set
+    bool ap_has_rd = false, ap_has_kf = false, ap_has_h = false;
+    int ap_count[2] = {0, 0};            // agents per heuristic; d_ap_idx holds class 0 first, then class 1
+    float ap_min_rd = 0.0f;
+    const int* sub_idx = nullptr;        // the sub-launch being issued (one per heuristic)
     int* d_best_idx = nullptr; float* d_best_cost = nullptr;
     int* h_best = nullptr;               // pinned: {idx, cost bits}
     float* d_scratch = nullptr;
@@ -78,7 +87,6 @@ extern "C" void gmapp_default_gains(gmapp_gains* g) {
 // ---------------------------------------------------------------------------------------------
 // kernel table
 // ---------------------------------------------------------------------------------------------
-typedef void (*rollout_fn)(const RolloutParams);
 // index: kind(2) x at(2: AT=1,2) x moving(2) x cull(2) x stage(2)
 static rollout_fn rollout_kernel(int kind, int at, bool moving, bool cull, int stage) {
 #define PICK(K, A, MT)                                                                            \
@@ -91,31 +99,12 @@ static rollout_fn rollout_kernel(int kind, int at, bool moving, bool cull, int s
     return PICK(0, 1, 1024);
 #undef PICK
 }
-// multi-warp groups with an epilogue warp, scalar pair math: 6D agents (static or moving spheres), 3D agents over moving spheres
-static rollout_fn rollout_wide_kernel(int kind, int at, bool moving, bool cull, int stage) {
-#define PICKW(K, A, M)                                                                                          \
-    (cull ? (stage ? (rollout_fn)k_rollout_wide<K, A, M, true, 1> : (rollout_fn)k_rollout_wide<K, A, M, true, 0>)    \
-          : (stage ? (rollout_fn)k_rollout_wide<K, A, M, false, 1> : (rollout_fn)k_rollout_wide<K, A, M, false, 0>))
-    if (kind == GMAPP_MOTOR6) return moving ? PICKW(1, 1, true) : PICKW(1, 1, false);
-    if (at == 2) return PICKW(0, 2, true);
-    return PICKW(0, 1, true);
-#undef PICKW
-}
-
-typedef void (*rollout_x2_fn)(const RolloutX2Params);
 static const int kX2SweepThreads = 512;       // sweep threads per CTA; mode 2 adds one epilogue warp per group (<= 672 in all)
-// mode 3 = mode 2 compiled for up to 7 groups (21 warps, 80 registers); mode 2 proper holds <= 4 groups
-// (20 warps = 5 per SM sub-partition, 96 registers), which is what one wave of config 3 needs
 static rollout_x2_fn rollout_x2_kernel(int at, int mode, bool cull, int stage, bool apf) {
-#define PICKS(A, M, MT, F)                                                                                                  \
-    (cull ? (stage ? (rollout_x2_fn)k_rollout_x2<A, M, true, 1, MT, F> : (rollout_x2_fn)k_rollout_x2<A, M, true, 0, MT, F>)     \
-          : (stage ? (rollout_x2_fn)k_rollout_x2<A, M, false, 1, MT, F> : (rollout_x2_fn)k_rollout_x2<A, M, false, 0, MT, F>))
-#define PICKX(A, M, MT) (apf ? PICKS(A, M, MT, true) : PICKS(A, M, MT, false))
-    if (mode == 4) return PICKX(2, 4, 512);
-    if (at == 2) return mode == 3 ? PICKX(2, 2, 672) : (mode == 2 ? PICKX(2, 2, 640) : (mode == 1 ? PICKX(2, 1, 512) : PICKX(2, 0, 512)));
-    return mode == 3 ? PICKX(1, 2, 672) : (mode == 2 ? PICKX(1, 2, 640) : (mode == 1 ? PICKX(1, 1, 512) : PICKX(1, 0, 512)));
-#undef PICKX
-#undef PICKS
+    return apf ? gmapp::rollout_x2_kernel_apf(at, mode, cull, stage) : gmapp::rollout_x2_kernel_cf(at, mode, cull, stage);
+}
+static rollout_fn rollout_wide_kernel(int kind, int at, bool moving, bool cull, int stage, bool apf) {
+    return gmapp::rollout_wide_kernel_tu(kind, at, moving, cull, stage, apf);
 }
 static int rollout_max_threads(int kind, int at) { return (kind == GMAPP_MOTOR6 || at == 2) ? 512 : 1024; }
 
@@ -157,12 +146,16 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
     ALLOC(c->d_agents_stage, sizeof(float) * 14 * max_agents);
     ALLOC(c->d_xyzr_stage, sizeof(float) * 4 * c->cap_spheres);
     ALLOC(c->d_vel_stage, sizeof(float) * 3 * c->cap_spheres);
+    ALLOC(c->d_ap_rd, sizeof(float) * max_agents);
+    ALLOC(c->d_ap_kf, sizeof(float) * max_agents);
+    ALLOC(c->d_ap_idx, sizeof(int) * max_agents);
     ALLOC(c->d_best_idx, sizeof(int) * 2);
     ALLOC(c->d_best_cost, sizeof(float));
     ALLOC(c->d_scratch, sizeof(float) * 64);
 #undef ALLOC
     if ((e = cudaMallocHost((void**)&c->h_pinned, sizeof(float) * hp)) != cudaSuccess ||
         (e = cudaMallocHost((void**)&c->h_best, sizeof(int) * 4)) != cudaSuccess ||
+        (e = cudaMallocHost((void**)&c->h_ap, sizeof(float) * 3 * (size_t)max_agents)) != cudaSuccess ||
         (e = cudaEventCreate(&c->ev0)) != cudaSuccess || (e = cudaEventCreate(&c->ev1)) != cudaSuccess) {
         gmapp_destroy(c);
         return fail(nullptr, GMAPP_ECUDA, "pinned / event allocation: %s", cudaGetErrorString(e));
@@ -180,21 +173,19 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
     for (int kind = 0; kind < 2; ++kind)
         for (int at = 1; at <= (kind == 0 ? 2 : 1); ++at)
             for (int mv = (kind == 0 ? 1 : 0); mv < 2; ++mv)
-                for (int cu = 0; cu < 2; ++cu)
-                    for (int st = 0; st < 2; ++st) {
-                        e = cudaFuncSetAttribute((const void*)rollout_wide_kernel(kind, at, mv, cu, st),
-                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
-                        if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
-                    }
+                for (int cu = 0; cu < 8; ++cu) {
+                    e = cudaFuncSetAttribute((const void*)rollout_wide_kernel(kind, at, mv, cu & 1, (cu >> 1) & 1, (cu >> 2) != 0),
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
+                    if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
+                }
     for (int at = 1; at <= 2; ++at)
         for (int md = 0; md < 5; ++md)
-            for (int cu = 0; cu < 2; ++cu)
-                for (int st = 0; st < 2; ++st)
-                    for (int hf = 0; hf < 2; ++hf) {
-                        e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, md, cu, st, hf != 0),
-                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
-                        if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
-                    }
+            for (int cu = 0; cu < 4; ++cu)
+                for (int hf = 0; hf < 2; ++hf) {
+                    e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, md, cu & 1, cu >> 1, hf != 0),
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
+                    if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
+                }
     *out = c;
     return GMAPP_OK;
 }
@@ -207,6 +198,8 @@ extern "C" gmapp_status gmapp_destroy(gmapp_ctx* c) {
     cudaFree(c->d_cost); cudaFree(c->d_minclr); cudaFree(c->d_collided);
     cudaFree(c->d_agents_stage); cudaFree(c->d_xyzr_stage); cudaFree(c->d_vel_stage);
     cudaFree(c->d_best_idx); cudaFree(c->d_best_cost); cudaFree(c->d_scratch);
+    cudaFree(c->d_ap_rd); cudaFree(c->d_ap_kf); cudaFree(c->d_ap_idx);
+    if (c->h_ap) cudaFreeHost(c->h_ap);
     if (c->h_pinned) cudaFreeHost(c->h_pinned);
     if (c->h_best) cudaFreeHost(c->h_best);
     if (c->ev0) cudaEventDestroy(c->ev0);
@@ -330,6 +323,47 @@ static gmapp_status check_gains(gmapp_ctx* c, const gmapp_gains* g, const char* 
 }
 
 // ---------------------------------------------------------------------------------------------
+// heterogeneous ensemble: per-agent detection radius, gain and heuristic
+// ---------------------------------------------------------------------------------------------
+extern "C" gmapp_status gmapp_set_agent_params(gmapp_ctx* c, const float* h_r_influence, const float* h_k_circ,
+                                               const int32_t* h_heuristic, int n, void* stream) {
+    if (!c) return GMAPP_EINVAL;
+    if (n < 0) return fail(c, GMAPP_EINVAL, "set_agent_params: n < 0%s");
+    if (n > c->max_agents) return fail(c, GMAPP_ECAPACITY, "set_agent_params: n = %s%ld exceeds max_agents = %ld", "", n, c->max_agents);
+    if (n == 0 || (!h_r_influence && !h_k_circ && !h_heuristic)) { c->ap_n = 0; return GMAPP_OK; }
+    float min_rd = INFINITY;
+    for (int i = 0; i < n; ++i) {
+        if (h_r_influence) {
+            if (!isfinite(h_r_influence[i]) || !(h_r_influence[i] > 0.0f)) return fail(c, GMAPP_EINVAL, "set_agent_params: r_influence[%s%ld] must be finite and > 0", "", i);
+            if (h_r_influence[i] < min_rd) min_rd = h_r_influence[i];
+        }
+        if (h_k_circ && !isfinite(h_k_circ[i])) return fail(c, GMAPP_EINVAL, "set_agent_params: k_circ[%s%ld] is not finite", "", i);
+        if (h_heuristic && h_heuristic[i] != 0 && h_heuristic[i] != 1) return fail(c, GMAPP_EINVAL, "set_agent_params: heuristic[%s%ld] must be 0 or 1", "", i);
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaStreamSynchronize(st));          // the pinned staging may still be in flight from an earlier call
+    float* hrd = c->h_ap; float* hkf = c->h_ap + c->max_agents; int* hidx = (int*)(c->h_ap + 2 * (size_t)c->max_agents);
+    c->ap_count[0] = c->ap_count[1] = 0;
+    if (h_heuristic) {                               // stable grouping: circular-field agents first, then APF agents
+        int k = 0;
+        for (int h = 0; h < 2; ++h)
+            for (int i = 0; i < n; ++i) if (h_heuristic[i] == h) { hidx[k++] = i; ++c->ap_count[h]; }
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_ap_idx, hidx, sizeof(int) * n, cudaMemcpyHostToDevice, st));
+    }
+    if (h_r_influence) {
+        memcpy(hrd, h_r_influence, sizeof(float) * n);
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_ap_rd, hrd, sizeof(float) * n, cudaMemcpyHostToDevice, st));
+    }
+    if (h_k_circ) {
+        memcpy(hkf, h_k_circ, sizeof(float) * n);
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_ap_kf, hkf, sizeof(float) * n, cudaMemcpyHostToDevice, st));
+    }
+    c->ap_n = n; c->ap_has_rd = h_r_influence != nullptr; c->ap_has_kf = h_k_circ != nullptr; c->ap_has_h = h_heuristic != nullptr;
+    c->ap_min_rd = min_rd;
+    return GMAPP_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
 // launch selection
 // ---------------------------------------------------------------------------------------------
 struct LaunchCfg { int at, L, groups, block, grid, agents_per_cta, stage, cull, n_pad, smem, tile_off, red_off; };
@@ -444,14 +478,19 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     P.c_lin = g->vel_factor * dt * g->inv_mass;
     P.inv_mass = g->inv_mass; P.vel_factor = g->vel_factor;
     P.r_d = g->r_influence; P.eps = g->eps_dist;
-    P.apf = g->heuristic == 1; P.inv_rd = 1.0f / g->r_influence;
+    P.apf = g->heuristic == 1;
     P.rcg = g->r_cost_goal > 0.0f ? g->r_cost_goal : g->r_influence;
     P.rco = g->r_cost_obs > 0.0f ? g->r_cost_obs : g->r_influence;
+    P.rcg_is_rd = !(g->r_cost_goal > 0.0f); P.rco_is_rd = !(g->r_cost_obs > 0.0f);
     P.w_goal = g->w_goal; P.w_obs = g->w_obs; P.w_path = g->w_path; P.w_smooth = g->w_smooth; P.a_max = g->a_max;
     P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
+    P.agent_idx = c->sub_idx;
+    P.rd_arr = (c->ap_n > 0 && c->ap_has_rd) ? c->d_ap_rd : nullptr;
+    P.kf_arr = (c->ap_n > 0 && c->ap_has_kf) ? c->d_ap_kf : nullptr;
     P.tile_off = tile_off; P.xch_off = xch_off; P.rec_off = rec_off;
     const int block = mode == 4 ? tmax : (mode >= 2 ? G * L + 32 * G : round_up(G * L, 32));
     const int smem = tile_off + (stage == 1 ? (int)tile_bytes : 0);
+    P.stage = stage;
     rollout_x2_fn fn = rollout_x2_kernel(at, mode, cull != 0, stage, g->heuristic == 1);
     fn<<<grid, block, smem, st>>>(P);
     CUDA_TRY(c, cudaGetLastError());
@@ -470,6 +509,9 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
 // ---------------------------------------------------------------------------------------------
 // rollout
 // ---------------------------------------------------------------------------------------------
+static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_agents, float* d_agents_out, int n_agents,
+                                const float* goal, const gmapp_gains* g, float dt, int steps, cudaStream_t stream);
+
 extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float* d_agents, float* d_agents_out,
                                       int n_agents, const float* goal, const gmapp_gains* g, float dt, int steps,
                                       void* stream) {
@@ -484,6 +526,43 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
     if (s != GMAPP_OK) return s;
     const int ng = kind == GMAPP_POINT3 ? 3 : 8;
     for (int i = 0; i < ng; ++i) if (!isfinite(goal[i])) return fail(c, GMAPP_EINVAL, "rollout: non-finite goal%s");
+    c->sub_idx = nullptr;
+    if (c->ap_n > 0) {
+        // heterogeneous ensemble: one launch per heuristic over that heuristic's agents (the paper runs one
+        // specialised kernel per heuristic), per-agent r_d / k_f read inside the kernels
+        if (c->ap_n != n_agents) return fail(c, GMAPP_EINVAL, "rollout: gmapp_set_agent_params was given %s%ld agents, the rollout %ld", "", c->ap_n, n_agents);
+        if (c->ap_has_rd && g->eps_dist > c->ap_min_rd) return fail(c, GMAPP_EINVAL, "rollout: need eps_dist <= every per-agent r_influence%s");
+        if (c->ap_has_h) {
+            int total = 0;
+            gmapp_launch_info first; memset(&first, 0, sizeof first);
+            const int* idx = c->d_ap_idx;
+            for (int h = 0; h < 2; ++h) {
+                const int nh = c->ap_count[h];
+                if (nh > 0) {
+                    gmapp_gains gh = *g; gh.heuristic = h;
+                    c->sub_idx = idx;
+                    s = rollout_sub(c, kind, d_agents, d_agents_out, nh, goal, &gh, dt, steps, (cudaStream_t)stream);
+                    c->sub_idx = nullptr;
+                    if (s != GMAPP_OK) return s;
+                    total += c->info.kernels_launched;
+                }
+                idx += nh;
+            }
+            c->info.kernels_launched = total;
+            c->last_n_agents = n_agents;
+            return GMAPP_OK;
+        }
+    }
+    s = rollout_sub(c, kind, d_agents, d_agents_out, n_agents, goal, g, dt, steps, (cudaStream_t)stream);
+    c->last_n_agents = n_agents;
+    return s;
+}
+
+// one launch over n_agents agents (all of them, or the agents c->sub_idx lists)
+static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_agents, float* d_agents_out, int n_agents,
+                                const float* goal, const gmapp_gains* g, float dt, int steps, cudaStream_t stream) {
+    gmapp_status s;
+    const int ng = kind == GMAPP_POINT3 ? 3 : 8;
     if (kind == GMAPP_POINT3 && !c->moving && !(c->has_tuning && c->tuning.scalar_path))
         return launch_rollout_x2(c, d_agents, d_agents_out, n_agents, goal, g, dt, steps, (cudaStream_t)stream);
     LaunchCfg cfg;
@@ -509,12 +588,16 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
     P.c_rot = g->vel_factor * dt * g->inv_inertia;
     P.inv_mass = g->inv_mass;
     P.r_d = g->r_influence; P.eps = g->eps_dist;
-    P.apf = g->heuristic == 1; P.inv_rd = 1.0f / g->r_influence;
+    P.apf = g->heuristic == 1;
     P.rcg = g->r_cost_goal > 0.0f ? g->r_cost_goal : g->r_influence;
     P.rco = g->r_cost_obs > 0.0f ? g->r_cost_obs : g->r_influence;
+    P.rcg_is_rd = !(g->r_cost_goal > 0.0f); P.rco_is_rd = !(g->r_cost_obs > 0.0f);
     P.w_goal = g->w_goal; P.w_obs = g->w_obs; P.w_path = g->w_path; P.w_smooth = g->w_smooth;
     P.a_max = g->a_max; P.vel_factor = g->vel_factor;
     P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
+    P.agent_idx = c->sub_idx;
+    P.rd_arr = (c->ap_n > 0 && c->ap_has_rd) ? c->d_ap_rd : nullptr;
+    P.kf_arr = (c->ap_n > 0 && c->ap_has_kf) ? c->d_ap_kf : nullptr;
     P.tile_off = cfg.tile_off; P.red_off = cfg.red_off;
     // few agents per CTA and many lanes per agent: sweep warps + one epilogue warp per group (gmapp_rollout_wide.cuh)
     const bool scalar_forced = c->has_tuning && c->tuning.scalar_path;
@@ -532,7 +615,8 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
         if (cfg.stage == 1 && !fits) cfg.stage = 0;
         cfg.smem = cfg.tile_off + (cfg.stage == 1 ? (int)tile_bytes : 0);
     }
-    rollout_fn fn = wide ? rollout_wide_kernel(kind, cfg.at, c->moving, cfg.cull != 0, cfg.stage)
+    P.stage = cfg.stage;
+    rollout_fn fn = wide ? rollout_wide_kernel(kind, cfg.at, c->moving, cfg.cull != 0, cfg.stage, g->heuristic == 1)
                          : rollout_kernel(kind, cfg.at, c->moving, cfg.cull != 0, cfg.stage);
     fn<<<cfg.grid, cfg.block, cfg.smem, st>>>(P);
     CUDA_TRY(c, cudaGetLastError());

@@ -52,10 +52,19 @@ struct RolloutParams {
     float* minclr;            // [n]
     int* collided;            // [n]
     int apf;                  // 1: APF heuristic (Eq. 1) instead of the circular field (Eq. 2-3)
-    float inv_rd;             // 1 / r_d (APF)
+    // heterogeneous ensemble (gmapp_set_agent_params): all nullable
+    const int* agent_idx;     // [n_agents] this launch's agents as indices into the caller's arrays
+    const float* rd_arr;      // per-agent detection radius r_d, indexed by the caller's agent index
+    const float* kf_arr;      // per-agent gain k_f
+    int rcg_is_rd, rco_is_rd; // Eq. 17 / 18 radii default to the agent's own r_d
+    int stage;                // gmapp_rollout_wide.cuh: 1 = pair arrays staged in shared memory (run-time choice)
     int tile_off;             // byte offset of the sphere tile in dynamic shared memory
     int red_off;              // byte offset of the cross-warp exchange scratch
 };
+
+__device__ __forceinline__ int agent_gid(const RolloutParams& P, int i) { return P.agent_idx ? P.agent_idx[i] : i; }
+__device__ __forceinline__ float agent_rd(const RolloutParams& P, int gid) { return P.rd_arr ? P.rd_arr[gid] : P.r_d; }
+__device__ __forceinline__ float agent_kf(const RolloutParams& P, int gid) { return P.kf_arr ? P.kf_arr[gid] : P.k_circ; }
 
 // ---------------------------------------------------------------------------------------------
 // per-pair math
@@ -84,30 +93,30 @@ __device__ __forceinline__ float pair_distance(float cx, float cy, float cz, flo
 // APF (Eq. 1, Khatib form on the clamped surface distance, reading N1):
 // f_j = -k_f (1/d_O - 1/r_d) / d_O^2 * d/|d|; accumulated without k_f; exactly 0 outside r_d
 __device__ __forceinline__ void apf_accumulate(float ds, float q, float dx, float dy, float dz, float r_d, float eps,
-                                               float inv_rd, float& bx, float& by, float& bz) {
+                                               float& bx, float& by, float& bz) {
     if (ds <= r_d) {
         const float ro = rcp_approx(fmaxf(ds, eps));
-        const float m = (inv_rd - ro) * (ro * ro) * rsqrt_approx(q);
+        const float m = (rcp_approx(r_d) - ro) * (ro * ro) * rsqrt_approx(q);
         bx = fmaf(m, dx, bx); by = fmaf(m, dy, by); bz = fmaf(m, dz, bz);
     }
 }
 
 template <int NA, bool FORCE, bool CULL, bool APF = false>
 __device__ __forceinline__ void pair_static(const float4 s, const float (&p)[NA][3], const float (&v)[NA][3],
-                                            float r_d, float eps, unsigned mask, StaticAcc<NA>& acc, float inv_rd = 0.0f) {
+                                            const float (&rd)[NA], float eps, unsigned mask, StaticAcc<NA>& acc) {
     float dx[NA], dy[NA], dz[NA], q[NA], ds[NA];
     bool any = false;
 #pragma unroll
     for (int a = 0; a < NA; ++a) {
         ds[a] = pair_distance(s.x, s.y, s.z, s.w, p[a][0], p[a][1], p[a][2], dx[a], dy[a], dz[a], q[a]);
         acc.dmin[a] = fminf(acc.dmin[a], ds[a]);
-        any = any || (ds[a] <= r_d);
+        any = any || (ds[a] <= rd[a]);
     }
     if (!FORCE) return;
     if (CULL) { if (!__any_sync(mask, any)) return; }
     if (APF) {
 #pragma unroll
-        for (int a = 0; a < NA; ++a) apf_accumulate(ds[a], q[a], dx[a], dy[a], dz[a], r_d, eps, inv_rd, acc.bx[a], acc.by[a], acc.bz[a]);
+        for (int a = 0; a < NA; ++a) apf_accumulate(ds[a], q[a], dx[a], dy[a], dz[a], rd[a], eps, acc.bx[a], acc.by[a], acc.bz[a]);
         return;
     }
 #pragma unroll
@@ -115,7 +124,7 @@ __device__ __forceinline__ void pair_static(const float4 s, const float (&p)[NA]
         float dO = fmaxf(ds[a], eps);
         float sv = fmaf(dx[a], v[a][0], fmaf(dy[a], v[a][1], dz[a] * v[a][2]));
         float w = sv * rcp_approx(dO * q[a]);
-        if (ds[a] <= r_d) {
+        if (ds[a] <= rd[a]) {
             acc.bx[a] = fmaf(w, dx[a], acc.bx[a]);
             acc.by[a] = fmaf(w, dy[a], acc.by[a]);
             acc.bz[a] = fmaf(w, dz[a], acc.bz[a]);
@@ -128,7 +137,7 @@ __device__ __forceinline__ void pair_static(const float4 s, const float (&p)[NA]
 template <int NA, bool FORCE, bool CULL, bool APF = false>
 __device__ __forceinline__ void pair_moving(const float4 s, const float4 su, float tk,
                                             const float (&p)[NA][3], const float (&v)[NA][3],
-                                            float r_d, float eps, unsigned mask, StaticAcc<NA>& acc, float inv_rd = 0.0f) {
+                                            const float (&rd)[NA], float eps, unsigned mask, StaticAcc<NA>& acc) {
     const float cx = fmaf(tk, su.x, s.x), cy = fmaf(tk, su.y, s.y), cz = fmaf(tk, su.z, s.z);
     float dx[NA], dy[NA], dz[NA], q[NA], ds[NA];
     bool any = false;
@@ -136,13 +145,13 @@ __device__ __forceinline__ void pair_moving(const float4 s, const float4 su, flo
     for (int a = 0; a < NA; ++a) {
         ds[a] = pair_distance(cx, cy, cz, s.w, p[a][0], p[a][1], p[a][2], dx[a], dy[a], dz[a], q[a]);
         acc.dmin[a] = fminf(acc.dmin[a], ds[a]);
-        any = any || (ds[a] <= r_d);
+        any = any || (ds[a] <= rd[a]);
     }
     if (!FORCE) return;
     if (CULL) { if (!__any_sync(mask, any)) return; }
     if (APF) {
 #pragma unroll
-        for (int a = 0; a < NA; ++a) apf_accumulate(ds[a], q[a], dx[a], dy[a], dz[a], r_d, eps, inv_rd, acc.bx[a], acc.by[a], acc.bz[a]);
+        for (int a = 0; a < NA; ++a) apf_accumulate(ds[a], q[a], dx[a], dy[a], dz[a], rd[a], eps, acc.bx[a], acc.by[a], acc.bz[a]);
         return;
     }
 #pragma unroll
@@ -155,7 +164,7 @@ __device__ __forceinline__ void pair_moving(const float4 s, const float4 su, flo
         float sv = fmaf(dx[a], vx, fmaf(dy[a], vy, dz[a] * vz));
         float w = sv * rcp_approx(dO * q[a]);
         float c1 = w * sv * inv, c2 = -w * nv;
-        if (ds[a] <= r_d) {
+        if (ds[a] <= rd[a]) {
             acc.bx[a] = fmaf(c1, vx, fmaf(c2, dx[a], acc.bx[a]));
             acc.by[a] = fmaf(c1, vy, fmaf(c2, dy[a], acc.by[a]));
             acc.bz[a] = fmaf(c1, vz, fmaf(c2, dz[a], acc.bz[a]));
@@ -168,7 +177,7 @@ template <int NA, bool MOVING, bool FORCE, bool CULL, bool APF = false>
 __device__ __forceinline__ void sphere_sweep(const float4* __restrict__ sph, const float4* __restrict__ svel,
                                              int n_pad, int lane, int L, float tk,
                                              const float (&p)[NA][3], const float (&v)[NA][3],
-                                             float r_d, float eps, unsigned mask, StaticAcc<NA>& acc, float inv_rd = 0.0f) {
+                                             const float (&rd)[NA], float eps, unsigned mask, StaticAcc<NA>& acc) {
     constexpr int U = (NA == 1) ? 4 : 2;
     int j = lane;
     const int step = L * U;
@@ -178,14 +187,14 @@ __device__ __forceinline__ void sphere_sweep(const float4* __restrict__ sph, con
         for (int u = 0; u < U; ++u) { s[u] = sph[j + u * L]; if (MOVING) su[u] = svel[j + u * L]; }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            if (MOVING) pair_moving<NA, FORCE, CULL, APF>(s[u], su[u], tk, p, v, r_d, eps, mask, acc, inv_rd);
-            else        pair_static<NA, FORCE, CULL, APF>(s[u], p, v, r_d, eps, mask, acc, inv_rd);
+            if (MOVING) pair_moving<NA, FORCE, CULL, APF>(s[u], su[u], tk, p, v, rd, eps, mask, acc);
+            else        pair_static<NA, FORCE, CULL, APF>(s[u], p, v, rd, eps, mask, acc);
         }
     }
     for (; j < n_pad; j += L) {
         float4 s = sph[j];
-        if (MOVING) pair_moving<NA, FORCE, CULL, APF>(s, svel[j], tk, p, v, r_d, eps, mask, acc, inv_rd);
-        else        pair_static<NA, FORCE, CULL, APF>(s, p, v, r_d, eps, mask, acc, inv_rd);
+        if (MOVING) pair_moving<NA, FORCE, CULL, APF>(s, svel[j], tk, p, v, rd, eps, mask, acc);
+        else        pair_static<NA, FORCE, CULL, APF>(s, p, v, rd, eps, mask, acc);
     }
 }
 
@@ -300,10 +309,12 @@ template <int NA, bool MOVING, bool CULL>
 __device__ __forceinline__ void rollout_point3(const RolloutParams& P, const float4* sph, const float4* svel,
                                                int first_agent, int lane_in_group, int group_in_cta, float* red) {
     const unsigned mask = __activemask();      // lanes of this warp on this code path (sub-warp groups may differ)
-    float p[NA][3], v[NA][3];
+    float p[NA][3], v[NA][3], rd[NA], kf[NA];
+    int gid[NA];
 #pragma unroll
     for (int a = 0; a < NA; ++a) {
-        const float* s = P.agents_in + 6 * size_t(first_agent + a);
+        gid[a] = agent_gid(P, first_agent + a); rd[a] = agent_rd(P, gid[a]); kf[a] = agent_kf(P, gid[a]);
+        const float* s = P.agents_in + 6 * size_t(gid[a]);
 #pragma unroll
         for (int i = 0; i < 3; ++i) { p[a][i] = s[i]; v[a][i] = s[3 + i]; }
     }
@@ -319,20 +330,20 @@ __device__ __forceinline__ void rollout_point3(const RolloutParams& P, const flo
     for (int k = 0; k < P.steps; ++k) {
         const float tk = float(k) * P.dt;
         acc.clear();
-        if (P.apf) sphere_sweep<NA, MOVING, true, CULL, true>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, mask, acc, P.inv_rd);
-        else sphere_sweep<NA, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, mask, acc);
+        if (P.apf) sphere_sweep<NA, MOVING, true, CULL, true>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
+        else sphere_sweep<NA, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
         group_allreduce<NA>(acc, P.L, lane_in_group, group_in_cta, red, k & 1, mask);
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
             float ex = P.goal[0] - p[a][0], ey = P.goal[1] - p[a][1], ez = P.goal[2] - p[a][2];
             float fx, fy, fz;
-            if (MOVING || P.apf) { fx = P.k_circ * acc.bx[a]; fy = P.k_circ * acc.by[a]; fz = P.k_circ * acc.bz[a]; }
-            else cf_force_static(P.k_circ, acc.bx[a], acc.by[a], acc.bz[a], v[a][0], v[a][1], v[a][2], fx, fy, fz);
+            if (MOVING || P.apf) { fx = kf[a] * acc.bx[a]; fy = kf[a] * acc.by[a]; fz = kf[a] * acc.bz[a]; }
+            else cf_force_static(kf[a], acc.bx[a], acc.by[a], acc.bz[a], v[a][0], v[a][1], v[a][2], fx, fy, fz);
             fx = fmaf(P.k_att, ex, fmaf(-P.k_damp, v[a][0], fx));      // Eq. 6-7
             fy = fmaf(P.k_att, ey, fmaf(-P.k_damp, v[a][1], fy));
             fz = fmaf(P.k_att, ez, fmaf(-P.k_damp, v[a][2], fz));
             if (cost_warp) {
-                ca[a].pose(norm3f(ex, ey, ez), acc.dmin[a], P.rcg, P.rco);
+                ca[a].pose(norm3f(ex, ey, ez), acc.dmin[a], P.rcg_is_rd ? rd[a] : P.rcg, P.rco_is_rd ? rd[a] : P.rco);
                 if (k >= 2) {                                          // third difference = vf dt^2 (a_k - a_{k-1})
                     float jx = fx - ap[a][0], jy = fy - ap[a][1], jz = fz - ap[a][2];
                     ca[a].add_jerk(fmaf(jx, jx, fmaf(jy, jy, jz * jz)));
@@ -351,13 +362,14 @@ __device__ __forceinline__ void rollout_point3(const RolloutParams& P, const flo
     // final pose: distance-only pass
     acc.clear();
     sphere_sweep<NA, MOVING, false, false>(sph, svel, P.n_pad, lane_in_group, P.L, float(P.steps) * P.dt, p, v,
-                                           P.r_d, P.eps, mask, acc);
+                                           rd, P.eps, mask, acc);
     group_allreduce<NA>(acc, P.L, lane_in_group, group_in_cta, red, P.steps & 1, mask);
     if (lane_in_group == 0) {
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
-            const int i = first_agent + a;
-            ca[a].pose(norm3f(P.goal[0] - p[a][0], P.goal[1] - p[a][1], P.goal[2] - p[a][2]), acc.dmin[a], P.rcg, P.rco);
+            const int i = gid[a];
+            ca[a].pose(norm3f(P.goal[0] - p[a][0], P.goal[1] - p[a][1], P.goal[2] - p[a][2]), acc.dmin[a],
+                       P.rcg_is_rd ? rd[a] : P.rcg, P.rco_is_rd ? rd[a] : P.rco);
             // sumJ holds sum |f_k - f_{k-1}|^2; a = inv_mass f; third difference = vel_factor dt^2 (a_k - a_{k-1})
             float cj = P.vel_factor * P.dt * P.dt * P.inv_mass;
             ca[a].finish(P, P.dt * ca[a].sumV, cj * cj * ca[a].sumJ, P.cost + 5 * size_t(i));
@@ -407,6 +419,11 @@ template <bool MOVING, bool CULL>
 __device__ __forceinline__ void rollout_pose6(const RolloutParams& P, const float4* sph, const float4* svel,
                                               int agent, int lane_in_group, int group_in_cta, float* red) {
     const unsigned mask = __activemask();
+    const int gid = agent_gid(P, agent);
+    float rd[1] = {agent_rd(P, gid)};
+    const float kf = agent_kf(P, gid);
+    const float rcg = P.rcg_is_rd ? rd[0] : P.rcg, rco = P.rco_is_rd ? rd[0] : P.rco;
+    agent = gid;
     Pose6 x = load_pose6(P.agents_in + 14 * size_t(agent));
     Quat rg = Quat{P.goal[0], P.goal[1], P.goal[2], P.goal[3]}, dg = Quat{P.goal[4], P.goal[5], P.goal[6], P.goal[7]};
     motor_normalise(rg, dg);
@@ -425,13 +442,13 @@ __device__ __forceinline__ void rollout_pose6(const RolloutParams& P, const floa
         p[0][0] = pos.x; p[0][1] = pos.y; p[0][2] = pos.z;
         v[0][0] = pdot.x; v[0][1] = pdot.y; v[0][2] = pdot.z;
         acc.clear();
-        if (P.apf) sphere_sweep<1, MOVING, true, CULL, true>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, mask, acc, P.inv_rd);
-        else sphere_sweep<1, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, mask, acc);
+        if (P.apf) sphere_sweep<1, MOVING, true, CULL, true>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
+        else sphere_sweep<1, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
         group_allreduce<1>(acc, P.L, lane_in_group, group_in_cta, red, k & 1, mask);
         Vec3 fr;
-        if (MOVING || P.apf) fr = P.k_circ * v3(acc.bx[0], acc.by[0], acc.bz[0]);
-        else cf_force_static(P.k_circ, acc.bx[0], acc.by[0], acc.bz[0], pdot.x, pdot.y, pdot.z, fr.x, fr.y, fr.z);
-        if (cost_warp) ca.pose(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z), acc.dmin[0], P.rcg, P.rco);
+        if (MOVING || P.apf) fr = kf * v3(acc.bx[0], acc.by[0], acc.bz[0]);
+        else cf_force_static(kf, acc.bx[0], acc.by[0], acc.bz[0], pdot.x, pdot.y, pdot.z, fr.x, fr.y, fr.z);
+        if (cost_warp) ca.pose(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z), acc.dmin[0], rcg, rco);
         Vec3 tau, f;
         pose6_wrench(P, x, pos, rg, pg, fr, tau, f);
         x.w = fma3(P.c_rot, tau, x.w);                    // Eq. 9-10
@@ -457,10 +474,10 @@ __device__ __forceinline__ void rollout_pose6(const RolloutParams& P, const floa
     v[0][0] = v[0][1] = v[0][2] = 0.0f;
     acc.clear();
     sphere_sweep<1, MOVING, false, false>(sph, svel, P.n_pad, lane_in_group, P.L, float(P.steps) * P.dt, p, v,
-                                          P.r_d, P.eps, mask, acc);
+                                          rd, P.eps, mask, acc);
     group_allreduce<1>(acc, P.L, lane_in_group, group_in_cta, red, P.steps & 1, mask);
     if (lane_in_group == 0) {
-        ca.pose(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z), acc.dmin[0], P.rcg, P.rco);
+        ca.pose(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z), acc.dmin[0], rcg, rco);
         ca.finish(P, ca.sumV, ca.sumJ, P.cost + 5 * size_t(agent));
         P.minclr[agent] = ca.minclr;
         P.collided[agent] = ca.collided;
@@ -556,8 +573,9 @@ __global__ void __launch_bounds__(256) k_forces(const __grid_constant__ ForcePar
     }
     StaticAcc<1> acc;
     acc.clear();
-    if (P.apf) sphere_sweep<1, MOVING, true, false, true>(P.sph, P.svel, P.n_pad, lane, 32, P.t_obs, p, v, P.r_d, P.eps, 0xffffffffu, acc, P.inv_rd);
-    else sphere_sweep<1, MOVING, true, false>(P.sph, P.svel, P.n_pad, lane, 32, P.t_obs, p, v, P.r_d, P.eps, 0xffffffffu, acc);
+    const float rd[1] = {P.r_d};
+    if (P.apf) sphere_sweep<1, MOVING, true, false, true>(P.sph, P.svel, P.n_pad, lane, 32, P.t_obs, p, v, rd, P.eps, 0xffffffffu, acc);
+    else sphere_sweep<1, MOVING, true, false>(P.sph, P.svel, P.n_pad, lane, 32, P.t_obs, p, v, rd, P.eps, 0xffffffffu, acc);
     group_allreduce<1>(acc, 32, lane, 0, nullptr, 0, 0xffffffffu);
     Vec3 fr;
     if (MOVING || P.apf) fr = P.k_circ * v3(acc.bx[0], acc.by[0], acc.bz[0]);
@@ -583,6 +601,7 @@ __global__ void __launch_bounds__(256) k_forces(const __grid_constant__ ForcePar
     }
 }
 
+#ifdef GMAPP_MAIN_TU      // non-template kernels: compiled once, in gmapp.cu
 // ---------------------------------------------------------------------------------------------
 // obstacle packing: (xyz, r) [+ vel] -> float4 arrays, R = r + r_a, sentinel padding to n_cap
 // ---------------------------------------------------------------------------------------------
@@ -650,6 +669,8 @@ __global__ void __launch_bounds__(1024) k_best_agent(const float* __restrict__ c
         }
     }
 }
+
+#endif  // GMAPP_MAIN_TU
 
 // ---------------------------------------------------------------------------------------------
 // FP32 peak microkernel: 8 independent FMA chains per thread, register only

@@ -34,11 +34,11 @@ __device__ __forceinline__ void warp_combine(const StaticAcc<NA>& acc, int lane,
 // f_j = w [ (s/|v_rel|) v_rel - |v_rel| d ],  w = s / (d_O |d|^2),  s = d.v_rel, accumulated directly
 // (k_f applied after the sum).  The distance half is the static one.
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool FORCE, bool CULL, bool APF = false>
+template <int NA, bool FORCE, bool CULL, bool APF = false, class RD = RdSel<NA, false>>
 __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, const float4* __restrict__ tB,
                                                 const float4* __restrict__ tU, const float4* __restrict__ tV, int n2p,
                                                 int lane, int L, float tk, const float (&p)[NA][3], const float (&v)[NA][3],
-                                                float r_d, float eps, unsigned mask, X2Acc<NA>& acc, float inv_rd = 0.0f) {
+                                                const RD& rd, float eps, unsigned mask, X2Acc<NA>& acc) {
     const u64 tiny = bc2(kTiny), half = bc2(0.5f), t2 = bc2(tk);
 #pragma unroll 2
     for (int j = lane; j < n2p; j += L) {
@@ -62,7 +62,7 @@ __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, c
             const u64 ds = fma2(hy, e, add2(t, nR));
             upk2(ds, d0[a], d1[a]);
             acc.dmin[a] = min3f(acc.dmin[a], d0[a], d1[a]);
-            if (CULL) any = any || (fminf(d0[a], d1[a]) <= r_d);
+            if (CULL) any = any || (fminf(d0[a], d1[a]) <= rd.get(a));
         }
         if (!FORCE) continue;
         if (CULL) { if (!__any_sync(mask, any)) continue; }
@@ -70,10 +70,10 @@ __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, c
 #pragma unroll
             for (int a = 0; a < NA; ++a) {
                 float r0 = 0.0f, r1 = 0.0f;
-                if (d0[a] <= r_d) r0 = rcp_approx(fmaxf(d0[a], eps));
-                if (d1[a] <= r_d) r1 = rcp_approx(fmaxf(d1[a], eps));
+                if (d0[a] <= rd.get(a)) r0 = rcp_approx(fmaxf(d0[a], eps));
+                if (d1[a] <= rd.get(a)) r1 = rcp_approx(fmaxf(d1[a], eps));
                 const u64 ro = pk2(r0, r1);
-                const u64 m = mul2(mul2(sub2(bc2(inv_rd), ro), mul2(ro, ro)), yy[a]);
+                const u64 m = mul2(mul2(sub2(bc2(rcp_approx(rd.get(a))), ro), mul2(ro, ro)), yy[a]);
                 acc.bx[a] = fma2(m, dx[a], acc.bx[a]);
                 acc.by[a] = fma2(m, dy[a], acc.by[a]);
                 acc.bz[a] = fma2(m, dz[a], acc.bz[a]);
@@ -91,8 +91,8 @@ __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, c
             const u64 den = mul2(pk2(fmaxf(d0[a], eps), fmaxf(d1[a], eps)), q[a]);
             float n0, n1; upk2(den, n0, n1);
             float r0 = 0.0f, r1 = 0.0f;
-            if (d0[a] <= r_d) r0 = rcp_approx(n0);
-            if (d1[a] <= r_d) r1 = rcp_approx(n1);
+            if (d0[a] <= rd.get(a)) r0 = rcp_approx(n0);
+            if (d1[a] <= rd.get(a)) r1 = rcp_approx(n1);
             const u64 s = fma2(dx[a], vx, fma2(dy[a], vy, mul2(dz[a], vz)));
             const u64 w = mul2(s, pk2(r0, r1));
             const u64 c1 = mul2(mul2(w, s), inv), c2 = mul2(w, nvn);
@@ -107,20 +107,25 @@ __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, c
 // epilogue-side agent models.  Interface: init, pre (no sums needed), post (sums known -> new state, pub[6] =
 // position and WORLD linear velocity for the sweep warps), costs, finish.
 // ---------------------------------------------------------------------------------------------
-template <bool MOVING>
+// DIRECT: the sums are the force itself (moving spheres or APF); else the BAC-CAB assembly of Eq. 2-3
+template <bool DIRECT>
 struct EpiPoint3 {
     float p[3], v[3], ap[3], pub[6];
     float ex, ey, ez, inv, nv, fax, fay, faz, fx, fy, fz;
+    int gid; float rd, kf;
     CostAcc ca;
+    __device__ __forceinline__ float rcg(const RolloutParams& P) const { return P.rcg_is_rd ? rd : P.rcg; }
+    __device__ __forceinline__ float rco(const RolloutParams& P) const { return P.rco_is_rd ? rd : P.rco; }
     __device__ __forceinline__ void init(const RolloutParams& P, int i) {
-        const float* s = P.agents_in + 6 * size_t(i);
+        gid = agent_gid(P, i); rd = agent_rd(P, gid); kf = agent_kf(P, gid);
+        const float* s = P.agents_in + 6 * size_t(gid);
 #pragma unroll
         for (int c = 0; c < 3; ++c) { p[c] = s[c]; v[c] = s[3 + c]; ap[c] = 0.0f; pub[c] = p[c]; pub[3 + c] = v[c]; }
         ca.init(norm3f(P.goal[0] - p[0], P.goal[1] - p[1], P.goal[2] - p[2]));
     }
     __device__ __forceinline__ void pre(const RolloutParams& P) {
         ex = P.goal[0] - p[0]; ey = P.goal[1] - p[1]; ez = P.goal[2] - p[2];
-        if (!MOVING) {
+        if (!DIRECT) {
             const float n2 = fmaf(v[0], v[0], fmaf(v[1], v[1], fmaf(v[2], v[2], kTiny)));
             inv = rsqrt_approx(n2);
             inv = inv * fmaf(-0.5f * n2 * inv, inv, 1.5f);
@@ -129,11 +134,11 @@ struct EpiPoint3 {
         fax = fmaf(P.k_att, ex, -P.k_damp * v[0]); fay = fmaf(P.k_att, ey, -P.k_damp * v[1]); faz = fmaf(P.k_att, ez, -P.k_damp * v[2]);
     }
     __device__ __forceinline__ void post(const RolloutParams& P, float bx, float by, float bz) {
-        if (MOVING || P.apf) {                             // the sweep accumulated the force vector itself
-            fx = fmaf(P.k_circ, bx, fax); fy = fmaf(P.k_circ, by, fay); fz = fmaf(P.k_circ, bz, faz);
+        if (DIRECT) {                                      // the sweep accumulated the force vector itself
+            fx = fmaf(kf, bx, fax); fy = fmaf(kf, by, fay); fz = fmaf(kf, bz, faz);
         } else {
             const float A = fmaf(bx, v[0], fmaf(by, v[1], bz * v[2]));
-            const float c1 = P.k_circ * inv * A, c2 = -P.k_circ * nv;
+            const float c1 = kf * inv * A, c2 = -kf * nv;
             fx = fmaf(c1, v[0], fmaf(c2, bx, fax)); fy = fmaf(c1, v[1], fmaf(c2, by, fay)); fz = fmaf(c1, v[2], fmaf(c2, bz, faz));
         }
         v[0] = fmaf(P.c_lin, fx, v[0]); v[1] = fmaf(P.c_lin, fy, v[1]); v[2] = fmaf(P.c_lin, fz, v[2]);   // Eq. 9-10
@@ -142,7 +147,7 @@ struct EpiPoint3 {
         for (int c = 0; c < 3; ++c) { pub[c] = p[c]; pub[3 + c] = v[c]; }
     }
     __device__ __forceinline__ void costs(const RolloutParams& P, int k, float dmin) {
-        ca.pose(norm3f(ex, ey, ez), dmin, P.rcg, P.rco);
+        ca.pose(norm3f(ex, ey, ez), dmin, rcg(P), rco(P));
         if (k >= 2) {
             float jx = fx - ap[0], jy = fy - ap[1], jz = fz - ap[2];
             ca.add_jerk(fmaf(jx, jx, fmaf(jy, jy, jz * jz)));
@@ -150,8 +155,9 @@ struct EpiPoint3 {
         ap[0] = fx; ap[1] = fy; ap[2] = fz;
         ca.add_len(norm3f(v[0], v[1], v[2]));
     }
-    __device__ __forceinline__ void finish(const RolloutParams& P, int i, float dmin) {
-        ca.pose(norm3f(P.goal[0] - p[0], P.goal[1] - p[1], P.goal[2] - p[2]), dmin, P.rcg, P.rco);
+    __device__ __forceinline__ void finish(const RolloutParams& P, float dmin) {
+        const int i = gid;
+        ca.pose(norm3f(P.goal[0] - p[0], P.goal[1] - p[1], P.goal[2] - p[2]), dmin, rcg(P), rco(P));
         const float cj = P.vel_factor * P.dt * P.dt * P.inv_mass;
         ca.finish(P, P.dt * ca.sumV, cj * cj * ca.sumJ, P.cost + 5 * size_t(i));
         P.minclr[i] = ca.minclr;
@@ -164,7 +170,7 @@ struct EpiPoint3 {
     }
 };
 
-template <bool MOVING>
+template <bool DIRECT>
 struct EpiPose6 {
     Pose6 x;
     Quat rg; Vec3 pg;
@@ -173,9 +179,13 @@ struct EpiPose6 {
     Vec3 pos, w_new, phi, fpre, td, dp, dp1, dp2;
     Quat r_new;
     float Bc, Cc;
+    int gid; float rd, kf;
     CostAcc ca;
+    __device__ __forceinline__ float rcg(const RolloutParams& P) const { return P.rcg_is_rd ? rd : P.rcg; }
+    __device__ __forceinline__ float rco(const RolloutParams& P) const { return P.rco_is_rd ? rd : P.rco; }
     __device__ __forceinline__ void init(const RolloutParams& P, int i) {
-        x = load_pose6(P.agents_in + 14 * size_t(i));
+        gid = agent_gid(P, i); rd = agent_rd(P, gid); kf = agent_kf(P, gid);
+        x = load_pose6(P.agents_in + 14 * size_t(gid));
         rg = Quat{P.goal[0], P.goal[1], P.goal[2], P.goal[3]};
         Quat dg = Quat{P.goal[4], P.goal[5], P.goal[6], P.goal[7]};
         motor_normalise(rg, dg);
@@ -205,8 +215,8 @@ struct EpiPose6 {
     }
     __device__ __forceinline__ void post(const RolloutParams& P, float bx, float by, float bz) {
         Vec3 fr;
-        if (MOVING || P.apf) fr = P.k_circ * v3(bx, by, bz);
-        else cf_force_static(P.k_circ, bx, by, bz, pub[3], pub[4], pub[5], fr.x, fr.y, fr.z);
+        if (DIRECT) fr = kf * v3(bx, by, bz);
+        else cf_force_static(kf, bx, by, bz, pub[3], pub[4], pub[5], fr.x, fr.y, fr.z);
         const Vec3 f = fpre + qrot_inv(x.r, fr);                           // Eq. 6 in the body frame (reading G18)
         x.nu = fma3(P.c_lin, f, x.nu);                                     // Eq. 9-10, linear block
         const Vec3 rho = P.dt * x.nu;
@@ -221,7 +231,7 @@ struct EpiPose6 {
         pub[0] = x.p.x; pub[1] = x.p.y; pub[2] = x.p.z; pub[3] = pdot.x; pub[4] = pdot.y; pub[5] = pdot.z;
     }
     __device__ __forceinline__ void costs(const RolloutParams& P, int k, float dmin) {
-        ca.pose(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z), dmin, P.rcg, P.rco);
+        ca.pose(norm3f(pg.x - pos.x, pg.y - pos.y, pg.z - pos.z), dmin, rcg(P), rco(P));
         ca.add_len(norm3f(td.x, td.y, td.z));
         if (k >= 2) {
             const Vec3 t3 = dp - 2.0f * dp1 + dp2;                         // p4 - 3 p3 + 3 p2 - p1 from displacements
@@ -229,8 +239,9 @@ struct EpiPose6 {
         }
         dp2 = dp1; dp1 = dp;
     }
-    __device__ __forceinline__ void finish(const RolloutParams& P, int i, float dmin) {
-        ca.pose(norm3f(pg.x - x.p.x, pg.y - x.p.y, pg.z - x.p.z), dmin, P.rcg, P.rco);
+    __device__ __forceinline__ void finish(const RolloutParams& P, float dmin) {
+        const int i = gid;
+        ca.pose(norm3f(pg.x - x.p.x, pg.y - x.p.y, pg.z - x.p.z), dmin, rcg(P), rco(P));
         ca.finish(P, ca.sumV, ca.sumJ, P.cost + 5 * size_t(i));
         P.minclr[i] = ca.minclr;
         P.collided[i] = ca.collided;
@@ -250,8 +261,8 @@ struct EpiPose6 {
 // exchange area per group: part[2][W][NA] float4, state[2][NA][2] float4
 // ---------------------------------------------------------------------------------------------
 // sweep warps: packed f32x2 sweeps over sphere pairs; tile = A, B (, U, V when MOVING) arrays of n2p float4 each
-template <int NA, bool MOVING, bool CULL>
-__device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const float4* tile, int astride,
+template <int NA, bool MOVING, bool CULL, bool APF, bool PER>
+__device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const float4* tile, int astride, int first_agent,
                                                  int lane_in_group, int group_in_cta, float4* xch) {
     const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
     const int half = (NA == 2) ? (lane >> 4) : 0;
@@ -261,6 +272,9 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
     const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
     const float4* tA = tile; const float4* tB = tile + astride; const float4* tU = tile + 2 * astride; const float4* tV = tile + 3 * astride;
     float p[NA][3], v[NA][3];
+    RdSel<NA, PER> rd; rd.u = P.r_d;
+#pragma unroll
+    for (int a = 0; a < NA; ++a) rd.v[a] = agent_rd(P, agent_gid(P, first_agent + a));
     // the start (p, world velocity) comes from the epilogue warp too (6D: needs the motor algebra): parity-1 buffer
     named_bar_sync(bar_state, nbar);
 #pragma unroll
@@ -274,13 +288,11 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
         const float tk = float(k) * P.dt;
         acc.clear();
         if (MOVING) {
-            if (!last && P.apf) sweep_x2_moving<NA, true, CULL, true>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc, P.inv_rd);
-            else if (!last) sweep_x2_moving<NA, true, CULL>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc);
-            else       sweep_x2_moving<NA, false, false>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, P.r_d, P.eps, full, acc);
+            if (!last) sweep_x2_moving<NA, true, CULL, APF>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
+            else       sweep_x2_moving<NA, false, false>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
         } else {
-            if (!last && P.apf) sweep_x2<NA, true, CULL, true>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc, P.inv_rd);
-            else if (!last) sweep_x2<NA, true, CULL>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
-            else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
+            if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
+            else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
         }
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
@@ -325,7 +337,7 @@ __device__ __forceinline__ void wide_epilogue_warp(const RolloutParams& P, int f
             t.x += o.x; t.y += o.y; t.z += o.z; t.w = fminf(t.w, o.w);
         }
         if (last) {
-            if (writer) me.finish(P, first_agent + half, t.w);
+            if (writer) me.finish(P, t.w);
             return;
         }
         me.post(P, t.x, t.y, t.z);
@@ -345,13 +357,13 @@ __device__ __forceinline__ void wide_epilogue_warp(const RolloutParams& P, int f
 // the kernel: threads [0, G L) sweep, [G L, G L + 32 G) one epilogue warp per group; G <= 4, L >= 64
 // KIND 0 = 3D point agents (AT 1 or 2 per group), KIND 1 = 6D motor agents (one per group)
 // ---------------------------------------------------------------------------------------------
-template <int KIND, int AT, bool MOVING, bool CULL, int STAGE>
+template <int KIND, int AT, bool MOVING, bool CULL, int STAGE, bool APF>
 __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__ RolloutParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
     const int tid = threadIdx.x;
     constexpr int NARR = MOVING ? 4 : 2;                    // pair arrays: A, B (, U, V)
-    const float4* tile = P.pairA;                           // STAGE 0: read the pair arrays from global memory / L2
+    const float4* tile = P.pairA;                           // stage 0: read the pair arrays from global memory / L2
     int astride = P.pair_stride;
     if (STAGE == 1) {
         float4* t = reinterpret_cast<float4*>(smem_raw + P.tile_off);
@@ -388,16 +400,16 @@ __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__
     if (is_epi) {
         if (na <= 0) return;
         const int lane = tid & 31;
-        if (KIND == 1) wide_epilogue_warp<EpiPose6<MOVING>, 1>(P, first, lane, group_in_cta, xch);
-        else if (NA2 == 2 && na >= 2) wide_epilogue_warp<EpiPoint3<MOVING>, NA2>(P, first, lane, group_in_cta, xch);
-        else wide_epilogue_warp<EpiPoint3<MOVING>, 1>(P, first, lane, group_in_cta, xch);
+        if (KIND == 1) wide_epilogue_warp<EpiPose6<(MOVING || APF)>, 1>(P, first, lane, group_in_cta, xch);
+        else if (NA2 == 2 && na >= 2) wide_epilogue_warp<EpiPoint3<(MOVING || APF)>, NA2>(P, first, lane, group_in_cta, xch);
+        else wide_epilogue_warp<EpiPoint3<(MOVING || APF)>, 1>(P, first, lane, group_in_cta, xch);
         return;
     }
     if (STAGE == 1) mbar_wait(bar, 0);
     if (na <= 0) return;
     const int lane_in_group = tid & (P.L - 1);
-    if (NA2 == 2 && na >= 2) wide_sweep_warps<NA2, MOVING, CULL>(P, tile, astride, lane_in_group, group_in_cta, xch);
-    else wide_sweep_warps<1, MOVING, CULL>(P, tile, astride, lane_in_group, group_in_cta, xch);
+    if (NA2 == 2 && na >= 2) { if (P.rd_arr) wide_sweep_warps<NA2, MOVING, CULL, APF, true>(P, tile, astride, first, lane_in_group, group_in_cta, xch); else wide_sweep_warps<NA2, MOVING, CULL, APF, false>(P, tile, astride, first, lane_in_group, group_in_cta, xch); }
+    else { if (P.rd_arr) wide_sweep_warps<1, MOVING, CULL, APF, true>(P, tile, astride, first, lane_in_group, group_in_cta, xch); else wide_sweep_warps<1, MOVING, CULL, APF, false>(P, tile, astride, first, lane_in_group, group_in_cta, xch); }
 }
 
 }  // namespace gmapp

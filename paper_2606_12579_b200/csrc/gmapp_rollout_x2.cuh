@@ -71,8 +71,26 @@ struct RolloutX2Params {
     int tile_off;             // byte offset of the sphere tile in dynamic shared memory
     int xch_off;              // byte offset of the cross-warp exchange area
     int rec_off;              // byte offset of the per-agent state records (mode 4)
+    int stage;                // 1: sphere pairs staged in shared memory by TMA bulk copies; 0: read through L1/L2
     int apf;                  // 1: APF heuristic (Eq. 1) instead of the circular field (Eq. 2-3)
-    float inv_rd;             // 1 / r_d (APF)
+    // heterogeneous ensemble (gmapp_set_agent_params): all nullable
+    const int* agent_idx;     // [n_agents] this launch's agents as indices into the caller's arrays (one launch per heuristic)
+    const float* rd_arr;      // per-agent detection radius r_d, indexed by the caller's agent index
+    const float* kf_arr;      // per-agent gain k_f
+    int rcg_is_rd, rco_is_rd; // Eq. 17 / 18 radii default to the agent's own r_d
+};
+
+__device__ __forceinline__ int agent_gid(const RolloutX2Params& P, int i) { return P.agent_idx ? P.agent_idx[i] : i; }
+__device__ __forceinline__ float agent_rd(const RolloutX2Params& P, int gid) { return P.rd_arr ? P.rd_arr[gid] : P.r_d; }
+
+// Detection radius seen by the sweeps: PER = false -> the uniform r_d of the launch (a kernel parameter, so it stays
+// in a uniform register and costs no vector-register read in the gate compare); PER = true -> per-agent values
+// (gmapp_set_agent_params).  Chosen once per kernel by a top-level branch, not inside the loops.
+template <int NA, bool PER>
+struct RdSel {
+    float v[NA];
+    float u;
+    __device__ __forceinline__ float get(int a) const { return PER ? v[a] : u; }
 };
 
 // per-lane partial sums of NA agents over the lane's sphere pairs (both halves of a pair kept apart)
@@ -89,10 +107,10 @@ struct X2Acc {
 // One lane's slice of the sphere sum: pairs lane, lane+L, ... ; FORCE=false is the distance-only final pass.
 // APF = true: Eq. 1 in the Khatib form on the clamped surface distance (reading N1),
 // f_j = -k_f (1/d_O - 1/r_d) / d_O^2 * d/|d|; the sums then hold the force itself (no velocity factor).
-template <int NA, bool FORCE, bool CULL, bool APF = false>
+template <int NA, bool FORCE, bool CULL, bool APF = false, class RD = RdSel<NA, false>>
 __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const float4* __restrict__ tB, int n2p,
                                          int lane, int L, const float (&p)[NA][3], const float (&v)[NA][3],
-                                         float r_d, float eps, unsigned mask, X2Acc<NA>& acc, float inv_rd = 0.0f) {
+                                         const RD& rd, float eps, unsigned mask, X2Acc<NA>& acc) {
     const u64 tiny = bc2(kTiny), half = bc2(0.5f);
 #pragma unroll kX2Unroll
     for (int j = lane; j < n2p; j += L) {
@@ -118,7 +136,7 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
             const u64 ds = fma2(hy, e, add2(t, nR));                     // dist - R, dist to ~1 ulp
             upk2(ds, d0[a], d1[a]);
             acc.dmin[a] = min3f(acc.dmin[a], d0[a], d1[a]);
-            if (CULL) any = any || (fminf(d0[a], d1[a]) <= r_d);
+            if (CULL) any = any || (fminf(d0[a], d1[a]) <= rd.get(a));
         }
         if (!FORCE) continue;
         if (CULL) { if (!__any_sync(mask, any)) continue; }
@@ -126,10 +144,10 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
 #pragma unroll
             for (int a = 0; a < NA; ++a) {
                 float r0 = 0.0f, r1 = 0.0f;                                  // 1/d_O inside r_d, else 0 (contributes exactly 0)
-                if (d0[a] <= r_d) r0 = rcp_approx(fmaxf(d0[a], eps));
-                if (d1[a] <= r_d) r1 = rcp_approx(fmaxf(d1[a], eps));
+                if (d0[a] <= rd.get(a)) r0 = rcp_approx(fmaxf(d0[a], eps));
+                if (d1[a] <= rd.get(a)) r1 = rcp_approx(fmaxf(d1[a], eps));
                 const u64 ro = pk2(r0, r1);
-                const u64 m = mul2(mul2(sub2(bc2(inv_rd), ro), mul2(ro, ro)), yy[a]);   // -(1/d_O - 1/r_d)/d_O^2 / |d|
+                const u64 m = mul2(mul2(sub2(bc2(rcp_approx(rd.get(a))), ro), mul2(ro, ro)), yy[a]);   // -(1/d_O - 1/r_d)/d_O^2 / |d|
                 acc.bx[a] = fma2(m, dx[a], acc.bx[a]);
                 acc.by[a] = fma2(m, dy[a], acc.by[a]);
                 acc.bz[a] = fma2(m, dz[a], acc.bz[a]);
@@ -141,8 +159,8 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
             const u64 den = mul2(pk2(fmaxf(d0[a], eps), fmaxf(d1[a], eps)), q[a]);     // d_O * |d|^2
             float n0, n1; upk2(den, n0, n1);
             float r0 = 0.0f, r1 = 0.0f;
-            if (d0[a] <= r_d) r0 = rcp_approx(n0);                       // Alg. 1 line 7: outside r_d contributes 0
-            if (d1[a] <= r_d) r1 = rcp_approx(n1);
+            if (d0[a] <= rd.get(a)) r0 = rcp_approx(n0);                     // Alg. 1 line 7: outside r_d contributes 0
+            if (d1[a] <= rd.get(a)) r1 = rcp_approx(n1);
             const u64 s = fma2(dx[a], bc2(v[a][0]), fma2(dy[a], bc2(v[a][1]), mul2(dz[a], bc2(v[a][2]))));
             const u64 w = mul2(s, pk2(r0, r1));
             acc.bx[a] = fma2(w, dx[a], acc.bx[a]);
@@ -211,12 +229,20 @@ __device__ __forceinline__ void subwarp_allreduce(float (&x)[NA], float (&y)[NA]
 // One agent's per-step state update and cost accumulation (Eq. 6-11, 17-20), executed by the lane(s) that own it.
 struct AgentX2 {
     float p[3], v[3], ap[3];
+    int gid;                  // index of this agent in the caller's arrays
+    float rd, kf;             // its detection radius and gain (uniform unless gmapp_set_agent_params was called)
     CostAcc ca;
-    __device__ __forceinline__ void init(const float* s, const float* goal) {
+    __device__ __forceinline__ void init(const RolloutX2Params& P, int i) {
+        gid = agent_gid(P, i);
+        rd = agent_rd(P, gid);
+        kf = P.kf_arr ? P.kf_arr[gid] : P.k_circ;
+        const float* s = P.agents_in + 6 * size_t(gid);
 #pragma unroll
-        for (int i = 0; i < 3; ++i) { p[i] = s[i]; v[i] = s[3 + i]; ap[i] = 0.0f; }
-        ca.init(norm3f(goal[0] - p[0], goal[1] - p[1], goal[2] - p[2]));
+        for (int c = 0; c < 3; ++c) { p[c] = s[c]; v[c] = s[3 + c]; ap[c] = 0.0f; }
+        ca.init(norm3f(P.goal[0] - p[0], P.goal[1] - p[1], P.goal[2] - p[2]));
     }
+    __device__ __forceinline__ float rcg(const RolloutX2Params& P) const { return P.rcg_is_rd ? rd : P.rcg; }
+    __device__ __forceinline__ float rco(const RolloutX2Params& P) const { return P.rco_is_rd ? rd : P.rco; }
     // Part of the state update that does not need the sphere sums (runs while the sums are still in flight):
     // e = goal - p, 1/|v| (MUFU.RSQ + Newton), |v|, and the attractor f_a = k_att e - k_damp v (Eq. 7).
     float ex, ey, ez, inv, nv, fax, fay, faz;
@@ -230,12 +256,13 @@ struct AgentX2 {
     }
     // The critical path once the sums B are known: f_r = k_f [((B.v)/|v|) v - |v| B] (BAC-CAB form of Eq. 2-3),
     // f = f_a + f_r (Eq. 6), v += vel_factor dt inv_mass f (Eq. 9-10), p += dt v (Eq. 11).
+    template <bool APF>
     __device__ __forceinline__ void post(const RolloutX2Params& P, float bx, float by, float bz, float& fx, float& fy, float& fz) {
-        if (P.apf) {                                       // Eq. 1: the sums are the force itself
-            fx = fmaf(P.k_circ, bx, fax); fy = fmaf(P.k_circ, by, fay); fz = fmaf(P.k_circ, bz, faz);
+        if (APF) {                                         // Eq. 1: the sums are the force itself
+            fx = fmaf(kf, bx, fax); fy = fmaf(kf, by, fay); fz = fmaf(kf, bz, faz);
         } else {
             const float A = fmaf(bx, v[0], fmaf(by, v[1], bz * v[2]));
-            const float c1 = P.k_circ * inv * A, c2 = -P.k_circ * nv;
+            const float c1 = kf * inv * A, c2 = -kf * nv;
             fx = fmaf(c1, v[0], fmaf(c2, bx, fax)); fy = fmaf(c1, v[1], fmaf(c2, by, fay)); fz = fmaf(c1, v[2], fmaf(c2, bz, faz));
         }
         v[0] = fmaf(P.c_lin, fx, v[0]); v[1] = fmaf(P.c_lin, fy, v[1]); v[2] = fmaf(P.c_lin, fz, v[2]);
@@ -243,7 +270,7 @@ struct AgentX2 {
     }
     // costs of the pose the step started from (uses e = goal - p_old and that pose's clearance) and of the move
     __device__ __forceinline__ void costs(const RolloutX2Params& P, int k, float dmin, float fx, float fy, float fz) {
-        ca.pose(norm3f(ex, ey, ez), dmin, P.rcg, P.rco);
+        ca.pose(norm3f(ex, ey, ez), dmin, rcg(P), rco(P));
         if (k >= 2) {                                                   // third difference = vf dt^2 (a_k - a_{k-1})
             float jx = fx - ap[0], jy = fy - ap[1], jz = fz - ap[2];
             ca.add_jerk(fmaf(jx, jx, fmaf(jy, jy, jz * jz)));
@@ -251,8 +278,9 @@ struct AgentX2 {
         ap[0] = fx; ap[1] = fy; ap[2] = fz;
         ca.add_len(norm3f(v[0], v[1], v[2]));                           // |p_new - p| = dt |v_new|
     }
-    __device__ __forceinline__ void finish(const RolloutX2Params& P, int i, float dmin_final) {
-        ca.pose(norm3f(P.goal[0] - p[0], P.goal[1] - p[1], P.goal[2] - p[2]), dmin_final, P.rcg, P.rco);
+    __device__ __forceinline__ void finish(const RolloutX2Params& P, float dmin_final) {
+        const int i = gid;
+        ca.pose(norm3f(P.goal[0] - p[0], P.goal[1] - p[1], P.goal[2] - p[2]), dmin_final, rcg(P), rco(P));
         const float cj = P.vel_factor * P.dt * P.dt * P.inv_mass;
         const float Nk = float(P.steps) + 1.0f;
         const float Lp = P.dt * ca.sumV, J = cj * cj * ca.sumJ, d1 = ca.d1;
@@ -297,14 +325,17 @@ __device__ __forceinline__ void warp_combine(const X2Acc<NA>& acc, int lane, flo
 // ---------------------------------------------------------------------------------------------
 // group body, L == 32: one warp per group does everything; agent a on lanes 0-15, agent b on lanes 16-31
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL, bool APF>
+template <int NA, bool CULL, bool APF, bool PER>
 __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, const float4* tA, const float4* tB,
                                                    int first_agent, int lane) {
     const int half = (NA == 2) ? (lane >> 4) : 0;
     const unsigned full = 0xffffffffu;
     AgentX2 me;
-    me.init(P.agents_in + 6 * size_t(first_agent + half), P.goal);
+    me.init(P, first_agent + half);
     float p[NA][3], v[NA][3];
+    RdSel<NA, PER> rd; rd.u = P.r_d;
+    rd.v[0] = __shfl_sync(full, me.rd, 0);
+    if (NA == 2) rd.v[NA - 1] = __shfl_sync(full, me.rd, 16);
     X2Acc<NA> acc;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);                  // pose S+1: distance-only pass
@@ -319,17 +350,17 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
             for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
         }
         acc.clear();
-        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc, P.inv_rd);
-        else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc);
+        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane, 32, p, v, rd, P.eps, full, acc);
+        else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane, 32, p, v, rd, P.eps, full, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
         if (last) {
-            if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.finish(P, first_agent + half, D);
+            if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.finish(P, D);
             return;
         }
         float fx, fy, fz;
         me.pre(P);
-        me.post(P, X, Y, Z, fx, fy, fz);
+        me.template post<APF>(P, X, Y, Z, fx, fy, fz);
         me.costs(P, k, D, fx, fy, fz);
     }
 }
@@ -339,21 +370,23 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
 // walks it in chunks of two inside each step; the persistent per-agent state (24 words) lives in a
 // warp-private shared-memory record between visits.  No cross-warp traffic, no barriers, all warps busy.
 // ---------------------------------------------------------------------------------------------
-constexpr int kAgentRecWords = 24;      // p3 v3 ap3 | sumG cG sumO cO sumV cV sumJ cJ minclr d1 collided | pad
+constexpr int kAgentRecWords = 24;      // p3 v3 ap3 | sumG cG sumO cO sumV cV sumJ cJ minclr d1 collided | gid rd kf | pad
 __device__ __forceinline__ void agent_store(const AgentX2& a, float* r) {
     r[0] = a.p[0]; r[1] = a.p[1]; r[2] = a.p[2]; r[3] = a.v[0]; r[4] = a.v[1]; r[5] = a.v[2];
     r[6] = a.ap[0]; r[7] = a.ap[1]; r[8] = a.ap[2];
     r[9] = a.ca.sumG; r[10] = a.ca.cG; r[11] = a.ca.sumO; r[12] = a.ca.cO; r[13] = a.ca.sumV; r[14] = a.ca.cV;
     r[15] = a.ca.sumJ; r[16] = a.ca.cJ; r[17] = a.ca.minclr; r[18] = a.ca.d1; r[19] = __int_as_float(a.ca.collided);
+    r[20] = __int_as_float(a.gid); r[21] = a.rd; r[22] = a.kf;
 }
 __device__ __forceinline__ void agent_load(AgentX2& a, const float* r) {
     a.p[0] = r[0]; a.p[1] = r[1]; a.p[2] = r[2]; a.v[0] = r[3]; a.v[1] = r[4]; a.v[2] = r[5];
     a.ap[0] = r[6]; a.ap[1] = r[7]; a.ap[2] = r[8];
     a.ca.sumG = r[9]; a.ca.cG = r[10]; a.ca.sumO = r[11]; a.ca.cO = r[12]; a.ca.sumV = r[13]; a.ca.cV = r[14];
     a.ca.sumJ = r[15]; a.ca.cJ = r[16]; a.ca.minclr = r[17]; a.ca.d1 = r[18]; a.ca.collided = __float_as_int(r[19]);
+    a.gid = __float_as_int(r[20]); a.rd = r[21]; a.kf = r[22];
 }
 
-template <int NA, bool CULL, bool APF>
+template <int NA, bool CULL, bool APF, bool PER>
 __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float4* tA, const float4* tB, int agent0,
                                            int lane, int k, float* rec0) {
     const int half = (NA == 2) ? (lane >> 4) : 0;
@@ -362,51 +395,54 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     AgentX2 me;
     agent_load(me, rec);
     float p[NA][3], v[NA][3];
+    RdSel<NA, PER> rd; rd.u = P.r_d;
     if (NA == 2) {
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
             p[0][i] = __shfl_sync(full, me.p[i], 0);       v[0][i] = __shfl_sync(full, me.v[i], 0);
             p[NA - 1][i] = __shfl_sync(full, me.p[i], 16); v[NA - 1][i] = __shfl_sync(full, me.v[i], 16);
         }
+        rd.v[0] = __shfl_sync(full, me.rd, 0); rd.v[NA - 1] = __shfl_sync(full, me.rd, 16);
     } else {
 #pragma unroll
         for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
+        rd.v[0] = me.rd;
     }
     const bool last = (k == P.steps);
     X2Acc<NA> acc;
     acc.clear();
-    if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc, P.inv_rd);
-    else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane, 32, p, v, P.r_d, P.eps, full, acc);
+    if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane, 32, p, v, rd, P.eps, full, acc);
+    else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane, 32, p, v, rd, P.eps, full, acc);
     float X, Y, Z, D;
     warp_combine<NA>(acc, lane, X, Y, Z, D);
     const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
     if (last) {
-        if (writer) me.finish(P, agent0 + half, D);
+        if (writer) me.finish(P, D);
         return;
     }
     float fx, fy, fz;
     me.pre(P);
-    me.post(P, X, Y, Z, fx, fy, fz);
+    me.template post<APF>(P, X, Y, Z, fx, fy, fz);
     me.costs(P, k, D, fx, fy, fz);
     __syncwarp();                                         // every lane has read the record before it is rewritten
     if (writer) agent_store(me, rec);
     __syncwarp();
 }
 
-template <bool CULL, bool APF>
+template <bool CULL, bool APF, bool PER>
 __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, const float4* tA, const float4* tB,
                                                     int first_agent, int n_mine, int lane, float* recs) {
     // records of this warp's agents: recs[i * kAgentRecWords], i < n_mine
     for (int i = lane; i < n_mine; i += 32) {
         AgentX2 a;
-        a.init(P.agents_in + 6 * size_t(first_agent + i), P.goal);
+        a.init(P, first_agent + i);
         agent_store(a, recs + i * kAgentRecWords);
     }
     __syncwarp();
     for (int k = 0; k <= P.steps; ++k) {
         int i = 0;
-        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL, APF>(P, tA, tB, first_agent + i, lane, k, recs + i * kAgentRecWords);
-        if (i < n_mine) chunk_step<1, CULL, APF>(P, tA, tB, first_agent + i, lane, k, recs + i * kAgentRecWords);
+        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL, APF, PER>(P, tA, tB, first_agent + i, lane, k, recs + i * kAgentRecWords);
+        if (i < n_mine) chunk_step<1, CULL, APF, PER>(P, tA, tB, first_agent + i, lane, k, recs + i * kAgentRecWords);
     }
 }
 
@@ -417,7 +453,7 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
 //   sweep warp k:    write part[k&1] -> arrive(bar_part) -> sync(bar_state) -> read state[k&1]
 //   epilogue warp k: sync(bar_part) -> read part[k&1] -> integrate -> write state[k&1] -> arrive(bar_state) -> costs
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL, bool APF>
+template <int NA, bool CULL, bool APF, bool PER>
 __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, const float4* tA, const float4* tB,
                                                   int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
     const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
@@ -427,9 +463,12 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
     const float4* state = xch + 2 * W * NA;                // [2][NA][2]
     const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
     float p[NA][3], v[NA][3];
+    RdSel<NA, PER> rd; rd.u = P.r_d;
 #pragma unroll
     for (int a = 0; a < NA; ++a) {
-        const float* s = P.agents_in + 6 * size_t(first_agent + a);
+        const int gid = agent_gid(P, first_agent + a);
+        const float* s = P.agents_in + 6 * size_t(gid);
+        rd.v[a] = agent_rd(P, gid);
 #pragma unroll
         for (int i = 0; i < 3; ++i) { p[a][i] = s[i]; v[a][i] = s[3 + i]; }
     }
@@ -437,8 +476,8 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         acc.clear();
-        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc, P.inv_rd);
-        else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, full, acc);
+        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
+        else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
         const int par = k & 1;
@@ -454,7 +493,7 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
     }
 }
 
-template <int NA>
+template <int NA, bool APF>
 __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, int first_agent, int lane,
                                                     int group_in_cta, float4* xch) {
     const int W = P.L >> 5;
@@ -463,7 +502,7 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
     float4* state = xch + 2 * W * NA;
     const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
     AgentX2 me;
-    me.init(P.agents_in + 6 * size_t(first_agent + half), P.goal);
+    me.init(P, first_agent + half);
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         const int par = k & 1;
@@ -475,11 +514,11 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
             t.x += o.x; t.y += o.y; t.z += o.z; t.w = fminf(t.w, o.w);
         }
         if (last) {
-            if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.finish(P, first_agent + half, t.w);
+            if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.finish(P, t.w);
             return;
         }
         float fx, fy, fz;
-        me.post(P, t.x, t.y, t.z, fx, fy, fz);
+        me.template post<APF>(P, t.x, t.y, t.z, fx, fy, fz);
         if ((lane & 15) == 0 && (NA == 2 || lane == 0)) {
             state[(par * NA + half) * 2] = make_float4(me.p[0], me.p[1], me.p[2], 0.0f);
             state[(par * NA + half) * 2 + 1] = make_float4(me.v[0], me.v[1], me.v[2], 0.0f);
@@ -492,14 +531,15 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
 // ---------------------------------------------------------------------------------------------
 // group body, L < 32 (several groups per warp): plain butterfly, every lane integrates its group's agents
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL, bool APF>
+template <int NA, bool CULL, bool APF, bool PER>
 __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, const float4* tA, const float4* tB,
                                                      int first_agent, int lane_in_group) {
     const unsigned mask = __activemask();
     AgentX2 ag[NA];
     float p[NA][3], v[NA][3];
+    RdSel<NA, PER> rd; rd.u = P.r_d;
 #pragma unroll
-    for (int a = 0; a < NA; ++a) ag[a].init(P.agents_in + 6 * size_t(first_agent + a), P.goal);
+    for (int a = 0; a < NA; ++a) { ag[a].init(P, first_agent + a); rd.v[a] = ag[a].rd; }
     X2Acc<NA> acc;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
@@ -508,8 +548,8 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 #pragma unroll
             for (int i = 0; i < 3; ++i) { p[a][i] = ag[a].p[i]; v[a][i] = ag[a].v[i]; }
         acc.clear();
-        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, mask, acc, P.inv_rd);
-        else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, P.r_d, P.eps, mask, acc);
+        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane_in_group, P.L, p, v, rd, P.eps, mask, acc);
+        else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, rd, P.eps, mask, acc);
         float x[NA], y[NA], z[NA], dm[NA];
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
@@ -522,10 +562,10 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
         subwarp_allreduce<NA>(x, y, z, dm, P.L, mask);
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
-            if (last) { if (lane_in_group == 0) ag[a].finish(P, first_agent + a, dm[a]); continue; }
+            if (last) { if (lane_in_group == 0) ag[a].finish(P, dm[a]); continue; }
             float fx, fy, fz;
             ag[a].pre(P);
-            ag[a].post(P, x[a], y[a], z[a], fx, fy, fz);
+            ag[a].template post<APF>(P, x[a], y[a], z[a], fx, fy, fz);
             ag[a].costs(P, k, dm[a], fx, fy, fz);
         }
     }
@@ -537,7 +577,8 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 // AT = agents per group (1 or 2); MODE 0: L < 32 (sub-warp groups), 1: L == 32 (one warp per group),
 // 2: L >= 64 (W sweep warps + one epilogue warp per group; threads [0, G L) sweep, [G L, G L + 32 G) epilogue);
 // 4: many agents per CTA, each warp walks its block of agents in chunks of two (state records in shared memory);
-// STAGE 1 = sphere pairs staged in shared memory by TMA bulk copies
+// STAGE 1 = sphere pairs staged in shared memory by TMA bulk copies (a template parameter on purpose: as a run-time
+// choice the tile pointers become generic and every LDS turns into a generic LD, measured 10 % slower)
 template <int AT, int MODE, bool CULL, int STAGE, int MAXT, bool APF>
 __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ RolloutX2Params P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -577,15 +618,15 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         float4* xch = reinterpret_cast<float4*>(smem_raw + P.xch_off) + group_in_cta * (2 * W * 2 + 2 * 2 * 2);
         if (is_epi) {                                      // the epilogue warps never touch the sphere tile
             if (na <= 0) return;
-            if (AT == 2 && na >= 2) group_epilogue_warp<NA2>(P, first, tid & 31, group_in_cta, xch);
-            else group_epilogue_warp<1>(P, first, tid & 31, group_in_cta, xch);
+            if (AT == 2 && na >= 2) group_epilogue_warp<NA2, APF>(P, first, tid & 31, group_in_cta, xch);
+            else group_epilogue_warp<1, APF>(P, first, tid & 31, group_in_cta, xch);
             return;
         }
         if (STAGE == 1) mbar_wait(bar, 0);
         if (na <= 0) return;
         const int lane_in_group = tid & (P.L - 1);
-        if (AT == 2 && na >= 2) group_sweep_warps<NA2, CULL, APF>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
-        else group_sweep_warps<1, CULL, APF>(P, tA, tB, first, lane_in_group, group_in_cta, xch);
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_sweep_warps<NA2, CULL, APF, true>(P, tA, tB, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<NA2, CULL, APF, false>(P, tA, tB, first, lane_in_group, group_in_cta, xch); }
+        else { if (P.rd_arr) group_sweep_warps<1, CULL, APF, true>(P, tA, tB, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<1, CULL, APF, false>(P, tA, tB, first, lane_in_group, group_in_cta, xch); }
         return;
     }
     if (MODE == 4) {
@@ -596,7 +637,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         if (STAGE == 1) mbar_wait(bar, 0);
         if (n_mine <= 0) return;
         float* recs = reinterpret_cast<float*>(smem_raw + P.rec_off) + start * kAgentRecWords;
-        warp_rollout_chunks<CULL, APF>(P, tA, tB, cta_first + start, n_mine, tid & 31, recs);
+        { if (P.rd_arr) warp_rollout_chunks<CULL, APF, true>(P, tA, tB, cta_first + start, n_mine, tid & 31, recs); else warp_rollout_chunks<CULL, APF, false>(P, tA, tB, cta_first + start, n_mine, tid & 31, recs); }
         return;
     }
     const int group_in_cta = tid >> P.logL;
@@ -606,14 +647,15 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
     if (STAGE == 1) mbar_wait(bar, 0);
     if (na <= 0) return;
     if (MODE == 1) {
-        if (AT == 2 && na >= 2) group_rollout_warp<NA2, CULL, APF>(P, tA, tB, first, lane_in_group);
-        else group_rollout_warp<1, CULL, APF>(P, tA, tB, first, lane_in_group);
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_warp<NA2, CULL, APF, true>(P, tA, tB, first, lane_in_group); else group_rollout_warp<NA2, CULL, APF, false>(P, tA, tB, first, lane_in_group); }
+        else { if (P.rd_arr) group_rollout_warp<1, CULL, APF, true>(P, tA, tB, first, lane_in_group); else group_rollout_warp<1, CULL, APF, false>(P, tA, tB, first, lane_in_group); }
     } else {
-        if (AT == 2 && na >= 2) group_rollout_narrow<NA2, CULL, APF>(P, tA, tB, first, lane_in_group);
-        else group_rollout_narrow<1, CULL, APF>(P, tA, tB, first, lane_in_group);
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_narrow<NA2, CULL, APF, true>(P, tA, tB, first, lane_in_group); else group_rollout_narrow<NA2, CULL, APF, false>(P, tA, tB, first, lane_in_group); }
+        else { if (P.rd_arr) group_rollout_narrow<1, CULL, APF, true>(P, tA, tB, first, lane_in_group); else group_rollout_narrow<1, CULL, APF, false>(P, tA, tB, first, lane_in_group); }
     }
 }
 
+#ifdef GMAPP_MAIN_TU
 // pack (xyz, r) [+ velocities] -> sphere-pair arrays A, B (, U, V), `stride` float4 apart; R = r + r_agent stored
 // negated; sentinel pairs (far away, at rest) up to n2_fill
 __global__ void k_pack_pairs(const float4* __restrict__ sph_raw, const float4* __restrict__ svel, int n, int n2_fill,
@@ -631,5 +673,7 @@ __global__ void k_pack_pairs(const float4* __restrict__ sph_raw, const float4* _
         pairs[3 * stride + j] = make_float4(u0.z, u1.z, 0.0f, 0.0f);
     }
 }
+
+#endif  // GMAPP_MAIN_TU
 
 }  // namespace gmapp

@@ -324,6 +324,91 @@ def test_apf_per_step_forces(api, ctx, orc, moving):
     _check_forces_on_oracle_states(api, ctx, orc, _apf(scenes.config4(n_agents=32, n_spheres=512, steps=60)), [0, 30, 60])
 
 
+# ---------------------------------------------------------------------------------- heterogeneous ensemble (NEXT row N2)
+def _ensemble_classes(n):
+    """The paper's set-up: per heuristic, agents with a large and a small detection radius."""
+    classes = [dict(heuristic=0, r_influence=0.15, k_circ=1.0), dict(heuristic=0, r_influence=0.08, k_circ=1.5),
+               dict(heuristic=1, r_influence=0.15, k_circ=1e-4), dict(heuristic=1, r_influence=0.08, k_circ=2e-4)]
+    which = (np.arange(n) * 7 + 3) % 4                  # interleaved, so every CTA / group mixes classes
+    return classes, which
+
+
+def _check_ensemble(api, ctx, orc, scene, tuning=None, smooth_tol=COST_TOL):
+    import copy
+    n = scene.n_agents
+    classes, which = _ensemble_classes(n)
+    rd = np.array([classes[w]["r_influence"] for w in which], np.float32)
+    kf = np.array([classes[w]["k_circ"] for w in which], np.float32)
+    hh = np.array([classes[w]["heuristic"] for w in which], np.int32)
+    try:
+        ctx.set_agent_params(rd, kf, hh)
+        g = api.run_scene(ctx, scene, tuning=tuning)
+    finally:
+        ctx.set_agent_params(n=0)
+        ctx.set_tuning(reset=True)
+    assert np.all(np.isfinite(g["final"])) and np.all(np.isfinite(g["cost"]))
+    cost_o = np.zeros((n, 5)); col_o = np.zeros(n, np.int32)
+    for k, cl in enumerate(classes):
+        idx = np.where(which == k)[0]
+        sc = copy.copy(scene)
+        sc.gains = dict(scene.gains, heuristic=cl["heuristic"], r_influence=float(np.float32(cl["r_influence"])),
+                        k_circ=float(np.float32(cl["k_circ"])))
+        o = orc.rollout_scene(sc, threads=8, agent_slice=idx)
+        if scene.kind == scenes.KIND_POINT3:
+            perr = np.abs(g["final"][idx, :3].astype(np.float64) - o["final"][:, :3]).max(axis=1)
+        else:
+            perr = np.abs(api.state14_to_pose(g["final"][idx])[1] - o["p"]).max(axis=1)
+        assert perr.max() <= POS_TOL, (k, perr.max())
+        ctol = COST_TOL + 2.0 * perr / cl["r_influence"]
+        cerr = np.abs(g["cost"][idx].astype(np.float64) - o["cost"])
+        assert np.all(cerr[:, 1:4] <= ctol[:, None]) and np.all(cerr[:, 4] <= smooth_tol + ctol), (k, cerr.max(axis=0))
+        waive = o["margins"][:, 2] < 1e-6 * cl["r_influence"]
+        assert np.array_equal(g["collided"][idx][~waive], o["collided"][~waive])
+        cost_o[idx] = o["cost"]; col_o[idx] = o["collided"]
+    # selection over the whole ensemble: exact on the GPU's own numbers, and against the oracle's up to the cost gap
+    want_self, _ = orc.best_agent(g["cost"].astype(np.float64), g["collided"], scene.alpha, scene.prev_best)
+    assert g["best"] == want_self
+    want, want_cost = orc.best_agent(cost_o, col_o, scene.alpha, scene.prev_best)
+    assert g["best"] == want or abs(cost_o[g["best"], 0] - want_cost) <= 1e-6 * abs(want_cost)
+    return g
+
+
+@pytest.mark.parametrize("tuning", [None, dict(lanes_per_agent=32), dict(lanes_per_agent=8, agents_per_thread=2, max_ctas=5),
+                                    dict(max_ctas=1, cull=1), dict(scalar_path=1), dict(lanes_per_agent=128, agents_per_thread=2, max_ctas=9)],
+                         ids=lambda t: "auto" if t is None else "-".join(f"{k[:4]}{v}" for k, v in t.items()))
+def test_heterogeneous_ensemble_point3(api, ctx, orc, tuning):
+    for moving in (False, True):
+        g = _check_ensemble(api, ctx, orc, scenes.fast_clutter(moving=moving, n_agents=90, n_spheres=333), tuning=tuning)
+        assert g["info"]["kernels_launched"] == 2            # one launch per heuristic
+
+
+def test_heterogeneous_ensemble_pose6_and_clutter(api, ctx, orc):
+    _check_ensemble(api, ctx, orc, scenes.config4(n_agents=32, n_spheres=512, steps=100), smooth_tol=1e-3)
+    _check_ensemble(api, ctx, orc, scenes.config3(n_agents=300))
+
+
+def test_agent_params_errors_and_reset(api, ctx, orc):
+    sc = scenes.fast_clutter(n_agents=20, n_spheres=50, steps=10)
+    base = api.run_scene(ctx, sc)
+    with pytest.raises(api.GmappError) as e:
+        ctx.set_agent_params(heuristic=np.full(20, 3, np.int32))
+    assert e.value.status == api.GMAPP_EINVAL
+    with pytest.raises(api.GmappError):
+        ctx.set_agent_params(r_influence=np.zeros(20, np.float32))
+    ctx.set_agent_params(r_influence=np.full(19, 0.1, np.float32))
+    with pytest.raises(api.GmappError) as e:                  # 19 parameters, 20 agents
+        api.run_scene(ctx, sc)
+    assert e.value.status == api.GMAPP_EINVAL
+    # uniform arrays reproduce the uniform rollout bit for bit; clearing restores it
+    ctx.set_agent_params(r_influence=np.full(20, sc.gains["r_influence"], np.float32),
+                         k_circ=np.full(20, sc.gains["k_circ"], np.float32), heuristic=np.zeros(20, np.int32))
+    same = api.run_scene(ctx, sc)
+    assert np.array_equal(same["final"], base["final"]) and np.array_equal(same["cost"], base["cost"])
+    ctx.set_agent_params(n=0)
+    again = api.run_scene(ctx, sc)
+    assert np.array_equal(again["final"], base["final"])
+
+
 # ---------------------------------------------------------------------------------- launch variants
 @pytest.mark.parametrize("tuning", [
     dict(lanes_per_agent=8, agents_per_thread=1), dict(lanes_per_agent=32, agents_per_thread=1),
