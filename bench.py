@@ -277,6 +277,8 @@ def run_ours(args):
         ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
     rev = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(K)]
     torch.cuda.synchronize(dev)
+    sampler2 = ClockSampler(local_rank)               # clocks under the roofline loop as well
+    sampler2.__enter__()
     for i in range(K):
         flush.zero_()
         rev[i][0].record()
@@ -315,6 +317,21 @@ def run_ours(args):
         ctx.best_agent_ex(scene.alpha, scene.prev_best)
         lat.append((time.perf_counter() - t0) * 1e3)
     lat = np.array(lat)
+    sampler2.__exit__()
+    sampler.samples += sampler2.samples; sampler.reasons |= sampler2.reasons
+
+    # ---- closed-loop re-planning (gmapp_replan): cycles chained on the device, no host synchronisation inside
+    n_cyc, exec_steps = 50, max(1, scene.steps // 10)
+    d_loop = d_agents.clone()
+    ctx.replan(kind, d_loop, goal, gains, scene.dt, scene.steps, exec_steps, 3)
+    torch.cuda.synchronize(dev)
+    d_loop.copy_(d_agents)
+    rp0, rp1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    rp0.record()
+    ctx.replan(kind, d_loop, goal, gains, scene.dt, scene.steps, exec_steps, n_cyc)
+    rp1.record()
+    torch.cuda.synchronize(dev)
+    replan_ms = rp0.elapsed_time(rp1) / n_cyc
 
     # ---- end to end through the C ABI with HOST buffers (sphere + agent upload, 8-byte result download)
     for _ in range(3):
@@ -368,6 +385,9 @@ def run_ours(args):
                          "peak_measured_ffma_tflops": peak_meas, "peak_measured_ffma2_tflops": peak_meas_x2,
                          "frac_of_measured_ffma": achieved / peak_meas if peak_meas else None,
                          "launch": info_bf},
+            "replan": {"ms_per_cycle": replan_ms, "cycles_per_s": 1e3 / replan_ms, "cycles": n_cyc, "exec_steps": exec_steps,
+                       "note": "gmapp_replan: rollout + selection + restart chained on the device (the paper's control "
+                               "loop runs at ~100 Hz, PAPER.md:47)"},
             "cull_variant": {"kernel_ms": cull_ms, "interactions_per_s": pairs_local / (cull_ms * 1e-3),
                              "note": "same kernel with the warp-vote skip of the force math (tuning cull=1); "
                                      "bit-identical results; not used for the roofline"},

@@ -142,6 +142,21 @@ gmapp_status gmapp_rollout(gmapp_ctx* ctx, gmapp_kind kind, const float* d_agent
                            int n_agents, const float* goal, const gmapp_gains* gains, float dt, int steps,
                            void* cuda_stream);
 
+/* Closed-loop re-planning (Fig. 2 steps 3-5: the planner re-plans from the robot's state while
+ * the control thread follows the best agent).  n_cycles planning cycles are chained ON THE DEVICE, nothing
+ * synchronises: cycle c rolls all agents `steps` steps from d_agents (obstacles at time c * exec_steps * dt),
+ * selects the best agent with hysteresis against the previous cycle's winner (prev_best for the first cycle, < 0 =
+ * none), takes that agent's state after exec_steps steps as the robot's new state -- following the winning
+ * agent's own control law for exec_steps steps IS that agent's rollout truncated there -- and restarts every agent
+ * from it (ensemble diversity then comes from gmapp_set_agent_params).  d_agents [n][6|14] is read and overwritten
+ * (after the call it holds the last robot state, replicated); d_path_out [n_cycles][6|14] (nullable) receives the
+ * robot state after each cycle, d_best_out [n_cycles] int32 (nullable) the winners.  Asynchronous on the stream;
+ * capturable in a CUDA graph.  Errors: EINVAL for NULL / n_cycles < 1 / exec_steps outside 1..steps, plus every
+ * error of gmapp_rollout. */
+gmapp_status gmapp_replan(gmapp_ctx* ctx, gmapp_kind kind, float* d_agents, int n_agents, const float* goal,
+                          const gmapp_gains* gains, float dt, int steps, int exec_steps, float alpha, int prev_best,
+                          int n_cycles, float* d_path_out, int32_t* d_best_out, void* cuda_stream);
+
 /* Agent selection: lexicographic argmin of (collided, C_i, i) over the last rollout;
  * with prev_best >= 0 the incumbent keeps its place unless the challenger is collision-free while the
  * incumbent collided, or the flags are equal and C_best < alpha * C_prev.  A NaN cost ranks last.

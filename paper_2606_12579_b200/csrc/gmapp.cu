@@ -47,6 +47,10 @@ struct gmapp_ctx {
     int ap_count[2] = {0, 0};            // agents per heuristic; d_ap_idx holds class 0 first, then class 1
     float ap_min_rd = 0.0f;
     const int* sub_idx = nullptr;        // the sub-launch being issued (one per heuristic)
+    // closed-loop re-planning (gmapp_replan)
+    float* d_snap = nullptr;             // [max_agents][14]
+    int* d_prev = nullptr;               // incumbent on the device
+    float roll_t0 = 0.0f; float* roll_snap = nullptr; int roll_snap_step = 0;
     int* d_best_idx = nullptr; float* d_best_cost = nullptr;
     int* h_best = nullptr;               // pinned: {idx, cost bits}
     float* d_scratch = nullptr;
@@ -146,6 +150,8 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
     ALLOC(c->d_agents_stage, sizeof(float) * 14 * max_agents);
     ALLOC(c->d_xyzr_stage, sizeof(float) * 4 * c->cap_spheres);
     ALLOC(c->d_vel_stage, sizeof(float) * 3 * c->cap_spheres);
+    ALLOC(c->d_snap, sizeof(float) * 14 * max_agents);
+    ALLOC(c->d_prev, sizeof(int));
     ALLOC(c->d_ap_rd, sizeof(float) * max_agents);
     ALLOC(c->d_ap_kf, sizeof(float) * max_agents);
     ALLOC(c->d_ap_idx, sizeof(int) * max_agents);
@@ -198,7 +204,7 @@ extern "C" gmapp_status gmapp_destroy(gmapp_ctx* c) {
     cudaFree(c->d_cost); cudaFree(c->d_minclr); cudaFree(c->d_collided);
     cudaFree(c->d_agents_stage); cudaFree(c->d_xyzr_stage); cudaFree(c->d_vel_stage);
     cudaFree(c->d_best_idx); cudaFree(c->d_best_cost); cudaFree(c->d_scratch);
-    cudaFree(c->d_ap_rd); cudaFree(c->d_ap_kf); cudaFree(c->d_ap_idx);
+    cudaFree(c->d_ap_rd); cudaFree(c->d_ap_kf); cudaFree(c->d_ap_idx); cudaFree(c->d_snap); cudaFree(c->d_prev);
     if (c->h_ap) cudaFreeHost(c->h_ap);
     if (c->h_pinned) cudaFreeHost(c->h_pinned);
     if (c->h_best) cudaFreeHost(c->h_best);
@@ -485,6 +491,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     P.w_goal = g->w_goal; P.w_obs = g->w_obs; P.w_path = g->w_path; P.w_smooth = g->w_smooth; P.a_max = g->a_max;
     P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
     P.agent_idx = c->sub_idx;
+    P.snap_out = c->roll_snap; P.snap_step = c->roll_snap_step;
     P.rd_arr = (c->ap_n > 0 && c->ap_has_rd) ? c->d_ap_rd : nullptr;
     P.kf_arr = (c->ap_n > 0 && c->ap_has_kf) ? c->d_ap_kf : nullptr;
     P.tile_off = tile_off; P.xch_off = xch_off; P.rec_off = rec_off;
@@ -581,7 +588,7 @@ static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_ag
     P.L = cfg.L; P.logL = ilog2(cfg.L);
     P.steps = steps;
     for (int i = 0; i < ng; ++i) P.goal[i] = goal[i];
-    P.dt = dt;
+    P.dt = dt; P.t0 = c->roll_t0;
     P.k_circ = g->k_circ; P.k_att = g->k_att; P.k_damp = g->k_damp;
     P.k_att_rot = g->k_att_rot; P.k_damp_rot = g->k_damp_rot;
     P.c_lin = g->vel_factor * dt * g->inv_mass;
@@ -596,6 +603,7 @@ static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_ag
     P.a_max = g->a_max; P.vel_factor = g->vel_factor;
     P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
     P.agent_idx = c->sub_idx;
+    P.snap_out = c->roll_snap; P.snap_step = c->roll_snap_step;
     P.rd_arr = (c->ap_n > 0 && c->ap_has_rd) ? c->d_ap_rd : nullptr;
     P.kf_arr = (c->ap_n > 0 && c->ap_has_kf) ? c->d_ap_kf : nullptr;
     P.tile_off = cfg.tile_off; P.red_off = cfg.red_off;
@@ -642,7 +650,7 @@ extern "C" gmapp_status gmapp_best_agent_ex(gmapp_ctx* c, float alpha, int prev_
     if (c->last_n_agents < 1) return fail(c, GMAPP_ESTATE, "best_agent: no rollout has run on this context%s");
     if (!isfinite(alpha)) return fail(c, GMAPP_EINVAL, "best_agent: alpha is not finite%s");
     cudaStream_t st = (cudaStream_t)stream;
-    k_best_agent<<<1, 1024, 0, st>>>(c->d_cost, c->d_collided, c->last_n_agents, alpha, prev_best, c->d_best_idx, c->d_best_cost);
+    k_best_agent<<<1, 1024, 0, st>>>(c->d_cost, c->d_collided, c->last_n_agents, alpha, prev_best, nullptr, c->d_best_idx, c->d_best_cost);
     CUDA_TRY(c, cudaGetLastError());
     CUDA_TRY(c, cudaMemcpyAsync(&c->h_best[0], c->d_best_idx, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(c, cudaMemcpyAsync(&c->h_best[2], c->d_best_cost, sizeof(float), cudaMemcpyDeviceToHost, st));
@@ -656,6 +664,41 @@ extern "C" gmapp_status gmapp_best_agent_ex(gmapp_ctx* c, float alpha, int prev_
 extern "C" gmapp_status gmapp_best_agent(gmapp_ctx* c, float alpha, int prev_best, int* out_index, float* out_cost,
                                          void* stream) {
     return gmapp_best_agent_ex(c, alpha, prev_best, out_index, out_cost, nullptr, stream);
+}
+
+// ---------------------------------------------------------------------------------------------
+// closed-loop re-planning (NEXT row N4): n_cycles planning cycles chained on the device
+// ---------------------------------------------------------------------------------------------
+extern "C" gmapp_status gmapp_replan(gmapp_ctx* c, gmapp_kind kind, float* d_agents, int n_agents, const float* goal,
+                                     const gmapp_gains* g, float dt, int steps, int exec_steps, float alpha, int prev_best,
+                                     int n_cycles, float* d_path_out, int32_t* d_best_out, void* stream) {
+    if (!c) return GMAPP_EINVAL;
+    if (!d_agents) return fail(c, GMAPP_EINVAL, "replan: d_agents is NULL%s");
+    if (n_cycles < 1) return fail(c, GMAPP_EINVAL, "replan: n_cycles must be >= 1%s");
+    if (exec_steps < 1 || exec_steps > steps) return fail(c, GMAPP_EINVAL, "replan: need 1 <= exec_steps <= steps%s");
+    if (!isfinite(alpha)) return fail(c, GMAPP_EINVAL, "replan: alpha is not finite%s");
+    if (prev_best >= n_agents) return fail(c, GMAPP_EINVAL, "replan: prev_best out of range%s");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int w = kind == GMAPP_POINT3 ? 6 : 14;
+    const int pb = prev_best < 0 ? -1 : prev_best;
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_prev, &pb, sizeof(int), cudaMemcpyHostToDevice, st));   // pageable 4-byte copy: staged by the runtime
+    gmapp_status s = GMAPP_OK;
+    int launches = 0;
+    for (int cyc = 0; cyc < n_cycles && s == GMAPP_OK; ++cyc) {
+        c->roll_t0 = (float)cyc * (float)exec_steps * dt;      // moving obstacles keep moving between cycles
+        c->roll_snap = c->d_snap; c->roll_snap_step = exec_steps;
+        s = gmapp_rollout(c, kind, d_agents, nullptr, n_agents, goal, g, dt, steps, stream);
+        c->roll_t0 = 0.0f; c->roll_snap = nullptr; c->roll_snap_step = 0;
+        if (s != GMAPP_OK) break;
+        launches += c->info.kernels_launched;
+        k_best_agent<<<1, 1024, 0, st>>>(c->d_cost, c->d_collided, n_agents, alpha, -1, c->d_prev, c->d_best_idx, c->d_best_cost);
+        k_reseed<<<(n_agents * w + 255) / 256, 256, 0, st>>>(c->d_snap, c->d_best_idx, n_agents, w, d_agents, c->d_prev,
+                                                             d_path_out, d_best_out, cyc);
+        CUDA_TRY(c, cudaGetLastError());
+        launches += 2;
+    }
+    c->info.kernels_launched = launches;
+    return s;
 }
 
 extern "C" gmapp_status gmapp_forces(gmapp_ctx* c, gmapp_kind kind, const float* d_agents, int n_agents, const float* goal,

@@ -58,6 +58,10 @@ struct RolloutParams {
     const float* kf_arr;      // per-agent gain k_f
     int rcg_is_rd, rco_is_rd; // Eq. 17 / 18 radii default to the agent's own r_d
     int stage;                // gmapp_rollout_wide.cuh: 1 = pair arrays staged in shared memory (run-time choice)
+    // closed-loop re-planning (gmapp_replan): obstacle time at step 0, and an optional state snapshot
+    float t0;                 // obstacles are evaluated at t0 + k dt
+    float* snap_out;          // [n][6|14] states after snap_step steps (indexed like agents_in), or nullptr
+    int snap_step;            // 1..steps
     int tile_off;             // byte offset of the sphere tile in dynamic shared memory
     int red_off;              // byte offset of the cross-warp exchange scratch
 };
@@ -328,7 +332,7 @@ __device__ __forceinline__ void rollout_point3(const RolloutParams& P, const flo
     }
     StaticAcc<NA> acc;
     for (int k = 0; k < P.steps; ++k) {
-        const float tk = float(k) * P.dt;
+        const float tk = fmaf(float(k), P.dt, P.t0);
         acc.clear();
         if (P.apf) sphere_sweep<NA, MOVING, true, CULL, true>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
         else sphere_sweep<NA, MOVING, true, CULL>(sph, svel, P.n_pad, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
@@ -357,11 +361,16 @@ __device__ __forceinline__ void rollout_point3(const RolloutParams& P, const flo
             p[a][1] = fmaf(P.dt, v[a][1], p[a][1]);
             p[a][2] = fmaf(P.dt, v[a][2], p[a][2]);
             if (cost_warp) ca[a].add_len(norm3f(v[a][0], v[a][1], v[a][2]));   // |p_new - p| = dt |v|
+            if (P.snap_out && k + 1 == P.snap_step && lane_in_group == 0) {
+                float* o = P.snap_out + 6 * size_t(gid[a]);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { o[c] = p[a][c]; o[3 + c] = v[a][c]; }
+            }
         }
     }
     // final pose: distance-only pass
     acc.clear();
-    sphere_sweep<NA, MOVING, false, false>(sph, svel, P.n_pad, lane_in_group, P.L, float(P.steps) * P.dt, p, v,
+    sphere_sweep<NA, MOVING, false, false>(sph, svel, P.n_pad, lane_in_group, P.L, fmaf(float(P.steps), P.dt, P.t0), p, v,
                                            rd, P.eps, mask, acc);
     group_allreduce<NA>(acc, P.L, lane_in_group, group_in_cta, red, P.steps & 1, mask);
     if (lane_in_group == 0) {
@@ -403,6 +412,15 @@ __device__ __forceinline__ Pose6 load_pose6(const float* s) {
     return x;
 }
 
+// [n][14] output layout: motor (r, d = (1/2) (0, p) (x) r) + body twist
+__device__ __forceinline__ void write_pose6(const Pose6& x, float* o) {
+    const Vec3 rv = v3(x.r.x, x.r.y, x.r.z);
+    const Vec3 dv = 0.5f * (fma3(x.r.w, x.p, cross(x.p, rv)));
+    o[0] = x.r.w; o[1] = x.r.x; o[2] = x.r.y; o[3] = x.r.z;
+    o[4] = -0.5f * dot(x.p, rv); o[5] = dv.x; o[6] = dv.y; o[7] = dv.z;
+    o[8] = x.w.x; o[9] = x.w.y; o[10] = x.w.z; o[11] = x.nu.x; o[12] = x.nu.y; o[13] = x.nu.z;
+}
+
 // body wrench (Eq. 6-8): tau = k_ar e_w - k_dr w;  f = k_att e_v - k_damp nu + R^T f_r
 __device__ __forceinline__ void pose6_wrench(const RolloutParams& P, const Pose6& x, Vec3 pos, Quat rg, Vec3 pg,
                                              Vec3 f_r_world, Vec3& tau, Vec3& f) {
@@ -436,7 +454,7 @@ __device__ __forceinline__ void rollout_pose6(const RolloutParams& P, const floa
     StaticAcc<1> acc;
     float p[1][3], v[1][3];
     for (int k = 0; k < P.steps; ++k) {
-        const float tk = float(k) * P.dt;
+        const float tk = fmaf(float(k), P.dt, P.t0);
         pos = x.p;
         Vec3 pdot = qrot(x.r, x.nu);                      // world linear velocity of the body origin
         p[0][0] = pos.x; p[0][1] = pos.y; p[0][2] = pos.z;
@@ -468,12 +486,13 @@ __device__ __forceinline__ void rollout_pose6(const RolloutParams& P, const floa
         x.r = qmul(x.r, rd);
         Quat dz = Quat{0, 0, 0, 0};
         motor_normalise(x.r, dz);
+        if (P.snap_out && k + 1 == P.snap_step && lane_in_group == 0) write_pose6(x, P.snap_out + 14 * size_t(agent));
     }
     pos = x.p;
     p[0][0] = pos.x; p[0][1] = pos.y; p[0][2] = pos.z;
     v[0][0] = v[0][1] = v[0][2] = 0.0f;
     acc.clear();
-    sphere_sweep<1, MOVING, false, false>(sph, svel, P.n_pad, lane_in_group, P.L, float(P.steps) * P.dt, p, v,
+    sphere_sweep<1, MOVING, false, false>(sph, svel, P.n_pad, lane_in_group, P.L, fmaf(float(P.steps), P.dt, P.t0), p, v,
                                           rd, P.eps, mask, acc);
     group_allreduce<1>(acc, P.L, lane_in_group, group_in_cta, red, P.steps & 1, mask);
     if (lane_in_group == 0) {
@@ -481,15 +500,7 @@ __device__ __forceinline__ void rollout_pose6(const RolloutParams& P, const floa
         ca.finish(P, ca.sumV, ca.sumJ, P.cost + 5 * size_t(agent));
         P.minclr[agent] = ca.minclr;
         P.collided[agent] = ca.collided;
-        if (P.agents_out) {
-            float* o = P.agents_out + 14 * size_t(agent);
-            // dual part d = (1/2) (0, p) (x) r
-            Vec3 rv = v3(x.r.x, x.r.y, x.r.z);
-            Vec3 dv = 0.5f * (fma3(x.r.w, x.p, cross(x.p, rv)));
-            o[0] = x.r.w; o[1] = x.r.x; o[2] = x.r.y; o[3] = x.r.z;
-            o[4] = -0.5f * dot(x.p, rv); o[5] = dv.x; o[6] = dv.y; o[7] = dv.z;
-            o[8] = x.w.x; o[9] = x.w.y; o[10] = x.w.z; o[11] = x.nu.x; o[12] = x.nu.y; o[13] = x.nu.z;
-        }
+        if (P.agents_out) write_pose6(x, P.agents_out + 14 * size_t(agent));
     }
 }
 
@@ -628,8 +639,11 @@ __device__ __forceinline__ bool key_less(int ca, float Ca, int ia, int cb, float
     return ia < ib;
 }
 
+// d_prev (nullable): the incumbent is read from device memory (closed-loop re-planning chains cycles without the host)
 __global__ void __launch_bounds__(1024) k_best_agent(const float* __restrict__ cost5, const int* __restrict__ collided,
-                                                     int n, float alpha, int prev_best, int* out_idx, float* out_cost) {
+                                                     int n, float alpha, int prev_best, const int* __restrict__ d_prev,
+                                                     int* out_idx, float* out_cost) {
+    if (d_prev) prev_best = *d_prev;
     // out_idx[0] = winner, out_idx[1] = its collision flag
     __shared__ int s_c[32]; __shared__ float s_C[32]; __shared__ int s_i[32];
     int bc = 2, bi = 0x7fffffff; float bC = __int_as_float(0x7f800000);
@@ -668,6 +682,17 @@ __global__ void __launch_bounds__(1024) k_best_agent(const float* __restrict__ c
             *out_cost = n > 0 ? bC : __int_as_float(0x7fc00000);
         }
     }
+}
+
+// closed-loop re-planning: every agent restarts from the winner's state after exec_steps steps (the snapshot);
+// the winner becomes the incumbent; the robot path and the winners are recorded.  w = 6 or 14 floats per state.
+__global__ void k_reseed(const float* __restrict__ snap, const int* __restrict__ best_idx, int n, int w, float* agents,
+                         int* d_prev, float* path_out, int* best_out, int cycle) {
+    const int best = best_idx[0];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n * w) agents[i] = snap[best * w + (i % w)];
+    if (i < w && path_out) path_out[cycle * w + i] = snap[best * w + i];
+    if (i == 0) { *d_prev = best; if (best_out) best_out[cycle] = best; }
 }
 
 #endif  // GMAPP_MAIN_TU

@@ -162,11 +162,14 @@ struct EpiPoint3 {
         ca.finish(P, P.dt * ca.sumV, cj * cj * ca.sumJ, P.cost + 5 * size_t(i));
         P.minclr[i] = ca.minclr;
         P.collided[i] = ca.collided;
-        if (P.agents_out) {
-            float* o = P.agents_out + 6 * size_t(i);
+        if (P.agents_out) write_state(P.agents_out + 6 * size_t(i));
+    }
+    __device__ __forceinline__ void write_state(float* o) const {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) { o[c] = p[c]; o[3 + c] = v[c]; }
-        }
+        for (int c = 0; c < 3; ++c) { o[c] = p[c]; o[3 + c] = v[c]; }
+    }
+    __device__ __forceinline__ void snapshot(const RolloutParams& P, int k) const {
+        if (P.snap_out && k + 1 == P.snap_step) write_state(P.snap_out + 6 * size_t(gid));
     }
 };
 
@@ -245,14 +248,10 @@ struct EpiPose6 {
         ca.finish(P, ca.sumV, ca.sumJ, P.cost + 5 * size_t(i));
         P.minclr[i] = ca.minclr;
         P.collided[i] = ca.collided;
-        if (P.agents_out) {
-            float* o = P.agents_out + 14 * size_t(i);
-            const Vec3 rv = v3(x.r.x, x.r.y, x.r.z);
-            const Vec3 dv = 0.5f * (fma3(x.r.w, x.p, cross(x.p, rv)));    // dual part d = (1/2) (0, p) (x) r
-            o[0] = x.r.w; o[1] = x.r.x; o[2] = x.r.y; o[3] = x.r.z;
-            o[4] = -0.5f * dot(x.p, rv); o[5] = dv.x; o[6] = dv.y; o[7] = dv.z;
-            o[8] = x.w.x; o[9] = x.w.y; o[10] = x.w.z; o[11] = x.nu.x; o[12] = x.nu.y; o[13] = x.nu.z;
-        }
+        if (P.agents_out) write_pose6(x, P.agents_out + 14 * size_t(i));
+    }
+    __device__ __forceinline__ void snapshot(const RolloutParams& P, int k) const {
+        if (P.snap_out && k + 1 == P.snap_step) write_pose6(x, P.snap_out + 14 * size_t(gid));
     }
 };
 
@@ -285,7 +284,7 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
     X2Acc<NA> acc;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
-        const float tk = float(k) * P.dt;
+        const float tk = fmaf(float(k), P.dt, P.t0);
         acc.clear();
         if (MOVING) {
             if (!last) sweep_x2_moving<NA, true, CULL, APF>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
@@ -349,6 +348,7 @@ __device__ __forceinline__ void wide_epilogue_warp(const RolloutParams& P, int f
         // off the critical path of the sweep warps; the costs of this step and the sum-free part of the next
         // step sit in one block so their independent instruction chains interleave
         me.costs(P, k, t.w);
+        if (writer) me.snapshot(P, k);
         me.pre(P);
     }
 }

@@ -78,6 +78,8 @@ struct RolloutX2Params {
     const float* rd_arr;      // per-agent detection radius r_d, indexed by the caller's agent index
     const float* kf_arr;      // per-agent gain k_f
     int rcg_is_rd, rco_is_rd; // Eq. 17 / 18 radii default to the agent's own r_d
+    float* snap_out;          // closed-loop re-planning: [n][6] states after snap_step steps, or nullptr
+    int snap_step;            // 1..steps
 };
 
 __device__ __forceinline__ int agent_gid(const RolloutX2Params& P, int i) { return P.agent_idx ? P.agent_idx[i] : i; }
@@ -278,6 +280,14 @@ struct AgentX2 {
         ap[0] = fx; ap[1] = fy; ap[2] = fz;
         ca.add_len(norm3f(v[0], v[1], v[2]));                           // |p_new - p| = dt |v_new|
     }
+    // closed-loop re-planning: the state after snap_step steps (call right after post of step k)
+    __device__ __forceinline__ void snapshot(const RolloutX2Params& P, int k) const {
+        if (P.snap_out && k + 1 == P.snap_step) {
+            float* o = P.snap_out + 6 * size_t(gid);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { o[c] = p[c]; o[3 + c] = v[c]; }
+        }
+    }
     __device__ __forceinline__ void finish(const RolloutX2Params& P, float dmin_final) {
         const int i = gid;
         ca.pose(norm3f(P.goal[0] - p[0], P.goal[1] - p[1], P.goal[2] - p[2]), dmin_final, rcg(P), rco(P));
@@ -362,6 +372,7 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
         me.pre(P);
         me.template post<APF>(P, X, Y, Z, fx, fy, fz);
         me.costs(P, k, D, fx, fy, fz);
+        if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.snapshot(P, k);
     }
 }
 
@@ -424,6 +435,7 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     me.pre(P);
     me.template post<APF>(P, X, Y, Z, fx, fy, fz);
     me.costs(P, k, D, fx, fy, fz);
+    if (writer) me.snapshot(P, k);
     __syncwarp();                                         // every lane has read the record before it is rewritten
     if (writer) agent_store(me, rec);
     __syncwarp();
@@ -525,6 +537,7 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
         }
         named_bar_arrive(bar_state, nbar);
         me.costs(P, k, t.w, fx, fy, fz);                   // off the critical path: the sweep warps are already running
+        if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.snapshot(P, k);
     }
 }
 
@@ -567,6 +580,7 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
             ag[a].pre(P);
             ag[a].template post<APF>(P, x[a], y[a], z[a], fx, fy, fz);
             ag[a].costs(P, k, dm[a], fx, fy, fz);
+            if (lane_in_group == 0) ag[a].snapshot(P, k);
         }
     }
 }

@@ -409,6 +409,85 @@ def test_agent_params_errors_and_reset(api, ctx, orc):
     assert np.array_equal(again["final"], base["final"])
 
 
+# ---------------------------------------------------------------------------------- closed-loop re-planning (NEXT row N4)
+@pytest.mark.parametrize("moving", [False, True], ids=["static", "moving"])
+def test_replan_closed_loop_matches_oracle_composition(api, ctx, orc, moving):
+    """gmapp_replan chains cycles on the device; the oracle side composes plain rollouts on the host: roll every
+    class of the ensemble, select with hysteresis, take the winner's state after exec_steps steps, restart."""
+    import copy
+    import torch
+    sc = scenes.fast_clutter(moving=moving, n_agents=24, n_spheres=300, steps=40)
+    n, exec_steps, n_cycles = sc.n_agents, 15, 5
+    classes, which = _ensemble_classes(n)
+    rd = np.array([classes[w]["r_influence"] for w in which], np.float32)
+    kf = np.array([classes[w]["k_circ"] for w in which], np.float32)
+    hh = np.array([classes[w]["heuristic"] for w in which], np.int32)
+    s0 = sc.agents[0].copy()
+    dev = "cuda:0"
+    d_agents = _tensor(np.tile(s0, (n, 1)))
+    d_path = torch.zeros((n_cycles, 6), device=dev); d_best = torch.full((n_cycles,), -7, dtype=torch.int32, device=dev)
+    ctx.set_obstacles(_tensor(sc.xyzr), None if sc.vel is None else _tensor(sc.vel), n=sc.n_spheres)
+    try:
+        ctx.set_agent_params(rd, kf, hh)
+        ctx.replan(api.GMAPP_POINT3, d_agents, sc.goal, sc.gains, sc.dt, sc.steps, exec_steps, n_cycles,
+                   alpha=sc.alpha, prev_best=-1, d_path_out=d_path, d_best_out=d_best)
+        torch.cuda.synchronize()
+    finally:
+        ctx.set_agent_params(n=0)
+    g_path, g_best = d_path.cpu().numpy().astype(np.float64), d_best.cpu().numpy()
+    # oracle composition
+    state, prev = s0.astype(np.float64), -1
+    for c in range(n_cycles):
+        sc_c = copy.copy(sc)
+        sc_c.agents = np.tile(state.astype(np.float32), (n, 1))
+        if moving:                                  # obstacles at time c * exec_steps * dt (FP32 like the device)
+            t0 = np.float32(c) * np.float32(exec_steps) * np.float32(sc.dt)
+            x = sc.xyzr.copy(); x[:, :3] = (sc.xyzr[:, :3].astype(np.float64) + float(t0) * sc.vel.astype(np.float64)).astype(np.float32)
+            sc_c.xyzr = x
+        cost = np.zeros((n, 5)); col = np.zeros(n, np.int32); snap = np.zeros((n, 6))
+        for k, cl in enumerate(classes):
+            idx = np.where(which == k)[0]
+            sc_k = copy.copy(sc_c)
+            sc_k.gains = dict(sc.gains, heuristic=cl["heuristic"], r_influence=float(np.float32(cl["r_influence"])),
+                              k_circ=float(np.float32(cl["k_circ"])))
+            o = orc.rollout_scene(sc_k, threads=4, want_traj=True, agent_slice=idx)
+            cost[idx] = o["cost"]; col[idx] = o["collided"]; snap[idx] = o["traj"][:, exec_steps]
+        want, want_cost = orc.best_agent(cost, col, sc.alpha, prev)
+        got = int(g_best[c])
+        assert got == want or abs(cost[got, 0] - want_cost) <= 1e-6 * abs(want_cost), (c, got, want)
+        # the device restarts from its own FP32 winner state: follow it, and allow the error to build up over cycles
+        assert np.abs(g_path[c, :3] - snap[got, :3]).max() <= POS_TOL * (c + 1), (c, np.abs(g_path[c, :3] - snap[got, :3]).max())
+        assert np.abs(g_path[c, 3:] - snap[got, 3:]).max() <= 1e-3 * (c + 1)
+        state, prev = g_path[c], got                # continue from the device's state so errors do not compound in the check
+    after = d_agents.cpu().numpy()
+    assert np.array_equal(after, np.tile(after[0], (n, 1))) and np.allclose(after[0], g_path[-1])
+    assert len(set(g_best.tolist())) >= 1 and g_best.min() >= 0
+
+
+def test_replan_pose6_runs_and_errors(api, ctx, orc):
+    import torch
+    sc = scenes.config4(n_agents=16, n_spheres=256, steps=30)
+    st14 = api.pose_to_state14(sc.quat, sc.pos, sc.twist)
+    goal8 = api.pose_to_state14(sc.goal_quat, sc.goal, np.zeros(6))[0, :8]
+    ctx.set_obstacles(_tensor(sc.xyzr), _tensor(sc.vel), n=sc.n_spheres)
+    d_agents = _tensor(st14)
+    d_path = torch.zeros((3, 14), device="cuda:0"); d_best = torch.zeros(3, dtype=torch.int32, device="cuda:0")
+    ctx.replan(api.GMAPP_MOTOR6, d_agents, goal8, sc.gains, sc.dt, sc.steps, 10, 3, d_path_out=d_path, d_best_out=d_best)
+    torch.cuda.synchronize()
+    # first cycle against the oracle: winner and its state after 10 steps
+    o = orc.rollout_scene(sc, threads=4, want_traj=True)
+    want, _ = orc.best_agent(o["cost"], o["collided"], sc.alpha, -1)
+    assert int(d_best[0]) == want
+    q, t, tw = api.state14_to_pose(d_path.cpu().numpy()[:1])
+    assert np.abs(t[0] - o["traj"][want, 10, 9:12]).max() <= POS_TOL
+    assert np.all(np.isfinite(d_path.cpu().numpy()))
+    for bad in (dict(exec_steps=0), dict(exec_steps=31), dict(n_cycles=0)):
+        kw = dict(exec_steps=10, n_cycles=2); kw.update(bad)
+        with pytest.raises(api.GmappError) as e:
+            ctx.replan(api.GMAPP_MOTOR6, d_agents, goal8, sc.gains, sc.dt, sc.steps, kw["exec_steps"], kw["n_cycles"])
+        assert e.value.status == api.GMAPP_EINVAL
+
+
 # ---------------------------------------------------------------------------------- launch variants
 @pytest.mark.parametrize("tuning", [
     dict(lanes_per_agent=8, agents_per_thread=1), dict(lanes_per_agent=32, agents_per_thread=1),
