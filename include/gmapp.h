@@ -117,6 +117,23 @@ gmapp_status gmapp_set_obstacles(gmapp_ctx* ctx, const float* d_xyzr, const floa
 /* Same with HOST arrays (copied through the context's pinned staging buffer). */
 gmapp_status gmapp_set_obstacles_host(gmapp_ctx* ctx, const float* h_xyzr, const float* h_vel, int n, void* cuda_stream);
 
+/* Sphere-world builder (perception stage: workspace crop, "voxelise at 2 r_O", the occupied
+ * voxel centres are the spheres of S_W, Eq. 5; S_W stays in GPU memory).  d_points [n][3]
+ * DEVICE point cloud (world frame; NaN / out-of-box points are dropped); lo, hi: HOST float[3] workspace box
+ * (lo <= p < hi); pitch = 2 r_O.  Voxel index floor((p - lo) / pitch) in FP32; the spheres are the occupied voxels in
+ * increasing linear voxel index (z-major, then y, then x) with centre lo + (i + 1/2) pitch and radius pitch / 2.
+ * The context's sphere world becomes `capacity` static slots: the first min(count, capacity) are those spheres, the
+ * rest far-away sentinels that never act -- so no count has to come back to the host; d_count_out (nullable DEVICE
+ * int32) receives the number of occupied voxels (> capacity means the tail was dropped).  Asynchronous.  Errors:
+ * EINVAL for bad arguments, ECAPACITY for capacity > max_spheres, > 4096 voxels per axis or > 2^25 voxels. */
+gmapp_status gmapp_build_sphere_world(gmapp_ctx* ctx, const float* d_points, int n_points, const float* lo,
+                                      const float* hi, float pitch, int capacity, int32_t* d_count_out,
+                                      void* cuda_stream);
+
+/* Copy the first n spheres of the resident sphere world, (x, y, z, r) each, into a caller-owned DEVICE buffer
+ * [n][4] (after gmapp_build_sphere_world: the occupied-voxel spheres, then sentinels at 1e18).  Asynchronous. */
+gmapp_status gmapp_get_obstacles(gmapp_ctx* ctx, float* d_xyzr_out, int n, void* cuda_stream);
+
 /* Optional launch tuning for later gmapp_rollout / gmapp_forces calls; NULL restores automatic choice. */
 gmapp_status gmapp_set_tuning(gmapp_ctx* ctx, const gmapp_tuning* tuning);
 

@@ -44,7 +44,7 @@ class gmapp_launch_info(C.Structure):
 
 
 EXPORTS = ["gmapp_default_gains", "gmapp_create", "gmapp_destroy", "gmapp_set_obstacles",
-           "gmapp_set_obstacles_host", "gmapp_set_tuning", "gmapp_set_agent_params", "gmapp_rollout", "gmapp_replan", "gmapp_best_agent", "gmapp_best_agent_ex",
+           "gmapp_set_obstacles_host", "gmapp_build_sphere_world", "gmapp_get_obstacles", "gmapp_set_tuning", "gmapp_set_agent_params", "gmapp_rollout", "gmapp_replan", "gmapp_best_agent", "gmapp_best_agent_ex",
            "gmapp_forces",
            "gmapp_get_results", "gmapp_plan_cycle_host", "gmapp_get_launch_info", "gmapp_measure_fp32_peak",
            "gmapp_sm_count", "gmapp_last_error"]
@@ -67,6 +67,8 @@ def _load():
     lib.gmapp_destroy.argtypes = [vp]
     lib.gmapp_set_obstacles.argtypes = [vp, vp, vp, C.c_int, vp]
     lib.gmapp_set_obstacles_host.argtypes = [vp, vp, vp, C.c_int, vp]
+    lib.gmapp_build_sphere_world.argtypes = [vp, vp, C.c_int, fp, fp, C.c_float, C.c_int, vp, vp]
+    lib.gmapp_get_obstacles.argtypes = [vp, vp, C.c_int, vp]
     lib.gmapp_set_tuning.argtypes = [vp, C.POINTER(gmapp_tuning)]
     lib.gmapp_set_agent_params.argtypes = [vp, vp, vp, vp, C.c_int, vp]
     lib.gmapp_rollout.argtypes = [vp, C.c_int, vp, vp, C.c_int, fp, C.POINTER(gmapp_gains), C.c_float, C.c_int, vp]
@@ -185,6 +187,17 @@ class Context:
         self._check(_lib.gmapp_set_obstacles_host(self._h, x.ctypes.data_as(C.c_void_p),
                                                   None if v is None else v.ctypes.data_as(C.c_void_p),
                                                   int(x.shape[0]), _stream(stream)))
+
+    def build_sphere_world(self, d_points, lo, hi, pitch, capacity, d_count_out=None, n_points=None, stream=None):
+        n = int(d_points.shape[0]) if n_points is None else n_points
+        lp, k1 = _farr(lo, 3)
+        hp, k2 = _farr(hi, 3)
+        self._check(_lib.gmapp_build_sphere_world(self._h, _ptr(d_points), n, lp, hp, C.c_float(pitch), int(capacity),
+                                                  _ptr(d_count_out), _stream(stream)))
+
+    def get_obstacles(self, d_xyzr_out, n=None, stream=None):
+        n = int(d_xyzr_out.shape[0]) if n is None else n
+        self._check(_lib.gmapp_get_obstacles(self._h, _ptr(d_xyzr_out), n, _stream(stream)))
 
     def set_tuning(self, lanes_per_agent=0, agents_per_thread=0, cull=-1, stage=-1, max_ctas=0, scalar_path=0,
                    reset=False):

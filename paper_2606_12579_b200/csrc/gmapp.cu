@@ -11,6 +11,7 @@
 #include "gmapp_kernels.cuh"
 #include "gmapp_rollout_x2.cuh"
 #include "gmapp_tables.h"
+#include "gmapp_voxel.cuh"
 
 using namespace gmapp;
 
@@ -47,6 +48,8 @@ struct gmapp_ctx {
     int ap_count[2] = {0, 0};            // agents per heuristic; d_ap_idx holds class 0 first, then class 1
     float ap_min_rd = 0.0f;
     const int* sub_idx = nullptr;        // the sub-launch being issued (one per heuristic)
+    // sphere-world builder (gmapp_build_sphere_world): voxel bitmap (2^25 voxels), block sums, occupied-voxel count
+    unsigned* d_vox_bitmap = nullptr; int* d_vox_sums = nullptr; int* d_vox_count = nullptr;
     // closed-loop re-planning (gmapp_replan)
     float* d_snap = nullptr;             // [max_agents][14]
     int* d_prev = nullptr;               // incumbent on the device
@@ -150,6 +153,9 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
     ALLOC(c->d_agents_stage, sizeof(float) * 14 * max_agents);
     ALLOC(c->d_xyzr_stage, sizeof(float) * 4 * c->cap_spheres);
     ALLOC(c->d_vel_stage, sizeof(float) * 3 * c->cap_spheres);
+    ALLOC(c->d_vox_bitmap, sizeof(unsigned) * (1u << 20));
+    ALLOC(c->d_vox_sums, sizeof(int) * 1024);
+    ALLOC(c->d_vox_count, sizeof(int));
     ALLOC(c->d_snap, sizeof(float) * 14 * max_agents);
     ALLOC(c->d_prev, sizeof(int));
     ALLOC(c->d_ap_rd, sizeof(float) * max_agents);
@@ -205,6 +211,7 @@ extern "C" gmapp_status gmapp_destroy(gmapp_ctx* c) {
     cudaFree(c->d_agents_stage); cudaFree(c->d_xyzr_stage); cudaFree(c->d_vel_stage);
     cudaFree(c->d_best_idx); cudaFree(c->d_best_cost); cudaFree(c->d_scratch);
     cudaFree(c->d_ap_rd); cudaFree(c->d_ap_kf); cudaFree(c->d_ap_idx); cudaFree(c->d_snap); cudaFree(c->d_prev);
+    cudaFree(c->d_vox_bitmap); cudaFree(c->d_vox_sums); cudaFree(c->d_vox_count);
     if (c->h_ap) cudaFreeHost(c->h_ap);
     if (c->h_pinned) cudaFreeHost(c->h_pinned);
     if (c->h_best) cudaFreeHost(c->h_best);
@@ -269,6 +276,57 @@ extern "C" gmapp_status gmapp_set_obstacles(gmapp_ctx* c, const float* d_xyzr, c
     c->pair_valid = false;
     // sphere-pair layout of the packed kernels, for r_agent = 0 (repacked lazily if a rollout asks for another r_agent)
     return effective_pairs(c, 0.0f, st, nullptr);
+}
+
+// ---------------------------------------------------------------------------------------------
+// sphere-world builder (NEXT row N3): point cloud -> crop -> voxelise -> occupied-voxel centres as S_W, on the device
+// ---------------------------------------------------------------------------------------------
+extern "C" gmapp_status gmapp_build_sphere_world(gmapp_ctx* c, const float* d_points, int n_points, const float* lo,
+                                                 const float* hi, float pitch, int capacity, int32_t* d_count_out,
+                                                 void* stream) {
+    if (!c) return GMAPP_EINVAL;
+    if (n_points < 0 || (n_points > 0 && !d_points) || !lo || !hi) return fail(c, GMAPP_EINVAL, "build_sphere_world: NULL points / bounds or n_points < 0%s");
+    if (!isfinite(pitch) || !(pitch > 0.0f)) return fail(c, GMAPP_EINVAL, "build_sphere_world: pitch must be finite and > 0%s");
+    if (capacity < 1) return fail(c, GMAPP_EINVAL, "build_sphere_world: capacity must be >= 1%s");
+    if (capacity > c->max_spheres) return fail(c, GMAPP_ECAPACITY, "build_sphere_world: capacity = %s%ld exceeds max_spheres = %ld", "", capacity, c->max_spheres);
+    VoxelGrid G;
+    double nvox = 1.0;
+    for (int a = 0; a < 3; ++a) {
+        if (!isfinite(lo[a]) || !isfinite(hi[a]) || !(hi[a] > lo[a])) return fail(c, GMAPP_EINVAL, "build_sphere_world: need finite lo < hi%s");
+        G.lo[a] = lo[a]; G.hi[a] = hi[a];
+        const double d = ceil(((double)hi[a] - (double)lo[a]) / (double)pitch);
+        if (d > 4096.0) return fail(c, GMAPP_ECAPACITY, "build_sphere_world: more than 4096 voxels along an axis%s");
+        G.dim[a] = d < 1.0 ? 1 : (int)d;
+        nvox *= G.dim[a];
+    }
+    if (nvox > (double)(1u << 25)) return fail(c, GMAPP_ECAPACITY, "build_sphere_world: the voxel grid exceeds 2^25 voxels%s");
+    G.pitch = pitch;
+    G.n_words = ((int)nvox + 31) / 32;
+    const int n_blocks = (G.n_words + 1023) / 1024;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(c, cudaMemsetAsync(c->d_vox_bitmap, 0, sizeof(unsigned) * (size_t)n_blocks * 1024, st));
+    if (n_points > 0) k_vox_mark<<<(n_points + 255) / 256, 256, 0, st>>>(d_points, n_points, G, c->d_vox_bitmap);
+    k_vox_count<<<n_blocks, 1024, 0, st>>>(c->d_vox_bitmap, G.n_words, c->d_vox_sums);
+    k_vox_scan<<<1, 1024, 0, st>>>(c->d_vox_sums, n_blocks, c->d_vox_count);
+    k_vox_emit<<<n_blocks, 1024, 0, st>>>(c->d_vox_bitmap, c->d_vox_sums, G, capacity, c->d_sph_raw);
+    const int nf = fill_count(c, capacity);
+    k_vox_fill<<<(nf + 255) / 256, 256, 0, st>>>(c->d_vox_count, capacity, nf, c->d_sph_raw, c->d_svel);
+    CUDA_TRY(c, cudaGetLastError());
+    if (d_count_out) CUDA_TRY(c, cudaMemcpyAsync(d_count_out, c->d_vox_count, sizeof(int), cudaMemcpyDeviceToDevice, st));
+    // the sphere world now holds `capacity` slots: the occupied voxels first, sentinels behind them
+    c->n_spheres = capacity;
+    c->moving = false;
+    c->eff_valid = false;
+    c->pair_valid = false;
+    return effective_pairs(c, 0.0f, st, nullptr);
+}
+
+extern "C" gmapp_status gmapp_get_obstacles(gmapp_ctx* c, float* d_xyzr_out, int n, void* stream) {
+    if (!c) return GMAPP_EINVAL;
+    if (c->n_spheres < 0) return fail(c, GMAPP_ESTATE, "get_obstacles: no sphere world has been set%s");
+    if (n < 0 || n > c->n_spheres || (n > 0 && !d_xyzr_out)) return fail(c, GMAPP_EINVAL, "get_obstacles: need 0 <= n <= %s%ld spheres and a buffer", "", c->n_spheres);
+    if (n > 0) CUDA_TRY(c, cudaMemcpyAsync(d_xyzr_out, c->d_sph_raw, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return GMAPP_OK;
 }
 
 extern "C" gmapp_status gmapp_set_obstacles_host(gmapp_ctx* c, const float* h_xyzr, const float* h_vel, int n, void* stream) {

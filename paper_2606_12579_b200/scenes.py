@@ -221,3 +221,25 @@ def by_name(name: str, **kw) -> Scene:
     if name.startswith("config5"):
         return config5(**kw)
     return table[name](**kw)
+
+
+def depth_cloud(seed: int = 0, n_points: int = 200_000, n_objects: int = 12):
+    """Synthetic fused depth cloud (stands in for the paper's two 848x480 depth cameras; its frames are
+    not available): points on the camera-facing surfaces of a few objects and a table plane inside the workspace W,
+    sensor noise, a share of far outliers and of NaN dropouts.  Returns (points [n,3] float32, lo [3], hi [3]).
+    No arithmetic of the method: only random draws."""
+    rng = np.random.default_rng(seed)
+    n_obj = int(0.6 * n_points); n_tab = int(0.3 * n_points); n_out = n_points - n_obj - n_tab
+    centres = rng.uniform(_W_LO + 0.15, _W_HI - 0.15, size=(n_objects, 3))
+    radii = rng.uniform(0.04, 0.12, size=n_objects)
+    which = rng.integers(0, n_objects, size=n_obj)
+    dirs = rng.normal(size=(n_obj, 3)); dirs /= np.linalg.norm(dirs, axis=1, keepdims=True)
+    dirs[:, 0] = -np.abs(dirs[:, 0])                                  # the half facing the cameras at -x
+    obj = centres[which] + radii[which, None] * dirs + rng.normal(0.0, 0.002, size=(n_obj, 3))
+    tab = np.c_[rng.uniform(_W_LO[0], _W_HI[0], n_tab), rng.uniform(_W_LO[1], _W_HI[1], n_tab),
+                0.05 + rng.normal(0.0, 0.002, n_tab)]
+    out = rng.uniform(-3.0, 3.0, size=(n_out, 3))
+    pts = np.concatenate([obj, tab, out], axis=0)
+    pts = pts[rng.permutation(pts.shape[0])]
+    pts[rng.random(pts.shape[0]) < 0.02] = np.nan                     # depth dropouts
+    return _f32(pts), _f32(_W_LO), _f32(_W_HI)

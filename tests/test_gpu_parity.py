@@ -488,6 +488,68 @@ def test_replan_pose6_runs_and_errors(api, ctx, orc):
         assert e.value.status == api.GMAPP_EINVAL
 
 
+# ---------------------------------------------------------------------------------- sphere-world builder (NEXT row N3)
+@pytest.mark.parametrize("n_points,pitch", [(200_000, 0.04), (814_080, 0.02), (1000, 0.1), (0, 0.04)])
+def test_sphere_world_builder_bit_exact(api, ctx, n_points, pitch):
+    """Integer / index work: the device's sphere list must equal the oracle's bit for bit (same order)."""
+    import torch
+    from oracle import voxel
+    pts, lo, hi = scenes.depth_cloud(seed=2, n_points=max(n_points, 1))
+    pts = pts[:n_points]
+    want, dims, lin = voxel.sphere_world_from_points(pts, lo, hi, pitch)
+    cap = 32768
+    d_pts = _tensor(pts) if n_points else torch.zeros((1, 3), device="cuda:0")
+    d_cnt = torch.full((1,), -1, dtype=torch.int32, device="cuda:0")
+    ctx.build_sphere_world(d_pts, lo, hi, pitch, cap, d_count_out=d_cnt, n_points=n_points)
+    out = torch.empty((cap, 4), device="cuda:0")
+    ctx.get_obstacles(out)
+    torch.cuda.synchronize()
+    got, cnt = out.cpu().numpy(), int(d_cnt[0])
+    assert cnt == want.shape[0]
+    m = min(cnt, cap)
+    assert np.array_equal(got[:m], want[:m])                       # bit-exact, voxel-index order
+    assert np.all(got[m:, 0] == np.float32(1e18)) and np.all(got[m:, 3] == 0)
+
+
+def test_sphere_world_builder_overflow_and_errors(api, ctx):
+    import torch
+    from oracle import voxel
+    pts, lo, hi = scenes.depth_cloud(seed=4, n_points=50_000)
+    want, _, _ = voxel.sphere_world_from_points(pts, lo, hi, 0.04)
+    cap = 100
+    assert want.shape[0] > cap
+    d_cnt = torch.zeros(1, dtype=torch.int32, device="cuda:0")
+    ctx.build_sphere_world(_tensor(pts), lo, hi, 0.04, cap, d_count_out=d_cnt)
+    out = torch.empty((cap, 4), device="cuda:0"); ctx.get_obstacles(out); torch.cuda.synchronize()
+    assert int(d_cnt[0]) == want.shape[0] and np.array_equal(out.cpu().numpy(), want[:cap])    # the tail is dropped, count says so
+    for kw in (dict(pitch=0.0), dict(capacity=0), dict(hi=lo), dict(pitch=1e-5)):
+        a = dict(lo=lo, hi=hi, pitch=0.04, capacity=cap); a.update(kw)
+        with pytest.raises(api.GmappError):
+            ctx.build_sphere_world(_tensor(pts), a["lo"], a["hi"], a["pitch"], a["capacity"])
+
+
+def test_rollout_over_built_world_equals_rollout_over_uploaded_spheres(api, ctx, orc):
+    """Perception -> planning on the device: a rollout over the built sphere world is bit-identical to a rollout over
+    the oracle's sphere list uploaded with gmapp_set_obstacles, and matches the FP64 oracle on it."""
+    import copy
+    from oracle import voxel
+    pts, lo, hi = scenes.depth_cloud(seed=7, n_points=120_000)
+    want, _, _ = voxel.sphere_world_from_points(pts, lo, hi, 0.04)
+    sc = scenes.config2(n_agents=40, steps=60)
+    sc = copy.copy(sc); sc.xyzr = want; sc.vel = None
+    ref = api.run_scene(ctx, sc)                                     # spheres uploaded
+    cap = int(want.shape[0]) + 123                                   # capacity above the count: sentinels behind
+    import torch
+    ctx.build_sphere_world(_tensor(pts), lo, hi, 0.04, cap)
+    agents = _tensor(sc.agents); out = torch.empty_like(agents)
+    ctx.rollout(api.GMAPP_POINT3, agents, out, sc.goal, sc.gains, sc.dt, sc.steps)
+    cost = torch.empty((sc.n_agents, 5), device="cuda:0"); ctx.get_results(cost)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), ref["final"]) and np.array_equal(cost.cpu().numpy(), ref["cost"])
+    o = orc.rollout_scene(sc, threads=8)
+    assert np.abs(ref["final"][:, :3].astype(np.float64) - o["final"][:, :3]).max() <= POS_TOL
+
+
 # ---------------------------------------------------------------------------------- launch variants
 @pytest.mark.parametrize("tuning", [
     dict(lanes_per_agent=8, agents_per_thread=1), dict(lanes_per_agent=32, agents_per_thread=1),

@@ -564,3 +564,44 @@ def test_P14_apf_rollout_superposition_and_mirror(orc):
     xm = sc.xyzr.astype(np.float64).copy(); xm[:, :3] = xm[:, :3] @ M
     totm = orc.forces_point3(stm, xm.astype(np.float32), None, (sc.goal @ M).astype(np.float32), g)["f_rep"]
     assert np.allclose(totm, tot @ M, rtol=1e-12, atol=1e-12)
+
+
+# ---------------------------------------------------------------------------------- P15: sphere-world builder (N3)
+def test_P15_voxel_oracle_brute_force_and_invariants():
+    from oracle import voxel
+    rng = np.random.default_rng(3)
+    lo, hi, pitch = np.float32([-0.5, -0.5, 0.0]), np.float32([0.5, 0.5, 1.0]), np.float32(0.04)
+    pts = rng.uniform(-0.7, 1.2, size=(400, 3)).astype(np.float32)
+    pts[::37] = np.nan
+    xyzr, dims, lin = voxel.sphere_world_from_points(pts, lo, hi, pitch)
+    # float32(0.04) is a hair below 0.04, so 1 m holds 25 full voxels and a sliver of a 26th
+    assert list(dims) == [26, 26, 26]
+    D = 26
+    # brute force with a Python set, one point at a time
+    want = set()
+    for p in pts:
+        if np.any(np.isnan(p)) or not (np.all(p >= lo) and np.all(p < hi)):
+            continue
+        i = [int(np.floor(np.float32(np.float32(p[a] - lo[a]) / pitch))) for a in range(3)]
+        if all(i[a] < dims[a] for a in range(3)):
+            want.add((i[2] * D + i[1]) * D + i[0])
+    assert sorted(want) == lin.tolist() and 0 < len(want) <= 400
+    assert np.all(np.diff(lin) > 0) and np.all(xyzr[:, 3] == np.float32(0.02))
+    # every kept point lies in the cube of half-width pitch/2 (+ rounding) around one emitted centre
+    inside = ~np.isnan(pts).any(axis=1) & np.all((pts >= lo) & (pts < hi), axis=1)
+    d = np.abs(pts[inside][:, None, :].astype(np.float64) - xyzr[None, :, :3].astype(np.float64)).max(axis=2).min(axis=1)
+    assert d.max() <= 0.02 + 1e-6
+    # hand case: one point in the first voxel, one in the last
+    x2, _, l2 = voxel.sphere_world_from_points(np.float32([[-0.49, -0.49, 0.01], [0.49, 0.49, 0.99]]), lo, hi, pitch)
+    assert l2.tolist() == [0, (24 * D + 24) * D + 24]
+    assert np.allclose(x2[0], [-0.48, -0.48, 0.02, 0.02], atol=1e-7) and np.allclose(x2[1], [0.48, 0.48, 0.98, 0.02], atol=1e-6)
+    # idempotence: voxelising the emitted centres gives the same spheres
+    x3, _, l3 = voxel.sphere_world_from_points(xyzr[:, :3], lo, hi, pitch)
+    assert np.array_equal(l3, lin) and np.array_equal(x3, xyzr)
+
+
+def test_depth_cloud_is_seeded_and_shaped():
+    a, lo, hi = scenes.depth_cloud(seed=1, n_points=5000)
+    b, _, _ = scenes.depth_cloud(seed=1, n_points=5000)
+    assert a.shape == (5000, 3) and a.dtype == np.float32 and np.array_equal(a, b, equal_nan=True)
+    assert 0 < np.isnan(a).any(axis=1).sum() < 500
