@@ -333,6 +333,26 @@ def run_ours(args):
     torch.cuda.synchronize(dev)
     replan_ms = rp0.elapsed_time(rp1) / n_cyc
 
+    # ---- sphere-world builder (gmapp_build_sphere_world) on a separate context: 2 x 848 x 480 points (the paper's two
+    # depth cameras), 4 cm voxels; HBM-bound (12 B read per point)
+    vox = None
+    if world == 1:
+        pts, lo_w, hi_w = scenes.depth_cloud(seed=0, n_points=2 * 848 * 480)
+        d_pts = torch.from_numpy(pts).to(dev)
+        vctx = api.Context(max_agents=1, max_spheres=32768, device=local_rank)
+        for _ in range(3):
+            vctx.build_sphere_world(d_pts, lo_w, hi_w, 0.04, 32768)
+        ve = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(20)]
+        torch.cuda.synchronize(dev)
+        for a, b in ve:
+            flush.zero_()
+            a.record(); vctx.build_sphere_world(d_pts, lo_w, hi_w, 0.04, 32768); b.record()
+        torch.cuda.synchronize(dev)
+        vms = float(np.mean([a.elapsed_time(b) for a, b in ve]))
+        vox = {"points": int(pts.shape[0]), "ms": vms, "GB_per_s": pts.nbytes / (vms * 1e-3) / 1e9,
+               "note": "7 small launches (memset, mark, count, scan, emit, fill, pair pack); launch-latency bound at this size"}
+        vctx.close()
+
     # ---- end to end through the C ABI with HOST buffers (sphere + agent upload, 8-byte result download)
     for _ in range(3):
         ctx.plan_cycle_host(kind, h_agents, goal, gains, scene.dt, scene.steps, h_xyzr=scene.xyzr, h_vel=scene.vel,
@@ -388,6 +408,7 @@ def run_ours(args):
             "replan": {"ms_per_cycle": replan_ms, "cycles_per_s": 1e3 / replan_ms, "cycles": n_cyc, "exec_steps": exec_steps,
                        "note": "gmapp_replan: rollout + selection + restart chained on the device (the paper's control "
                                "loop runs at ~100 Hz, PAPER.md:47)"},
+            "sphere_world_builder": vox,
             "cull_variant": {"kernel_ms": cull_ms, "interactions_per_s": pairs_local / (cull_ms * 1e-3),
                              "note": "same kernel with the warp-vote skip of the force math (tuning cull=1); "
                                      "bit-identical results; not used for the roofline"},

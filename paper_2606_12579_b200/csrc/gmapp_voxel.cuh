@@ -34,7 +34,10 @@ __global__ void k_vox_mark(const float* __restrict__ pts, int n, const __grid_co
     const int iz = int(floorf(__fdiv_rn(z - G.lo[2], G.pitch)));
     if (ix >= G.dim[0] || iy >= G.dim[1] || iz >= G.dim[2]) return;
     const unsigned v = (unsigned(iz) * G.dim[1] + iy) * G.dim[0] + ix;
-    atomicOr(&bitmap[v >> 5], 1u << (v & 31));
+    // most points fall into a voxel that is already marked: test first (a stale 0 only costs a redundant atomic), so
+    // the atomics per word drop from thousands to a handful and the kernel stays bound by reading the points
+    const unsigned bit = 1u << (v & 31);
+    if (!(__ldcg(&bitmap[v >> 5]) & bit)) atomicOr(&bitmap[v >> 5], bit);
 }
 
 // block sums of popcounts: 1024 words per block
