@@ -124,7 +124,8 @@ gmapp_status gmapp_set_obstacles_host(gmapp_ctx* ctx, const float* h_xyzr, const
  * increasing linear voxel index (z-major, then y, then x) with centre lo + (i + 1/2) pitch and radius pitch / 2.
  * The context's sphere world becomes `capacity` static slots: the first min(count, capacity) are those spheres, the
  * rest far-away sentinels that never act -- so no count has to come back to the host; d_count_out (nullable DEVICE
- * int32) receives the number of occupied voxels (> capacity means the tail was dropped).  Asynchronous.  Errors:
+ * int32) receives the number of occupied voxels (> capacity means the tail was dropped).  The packed rollout kernels
+ * read that count on the device and sweep only the real spheres.  Asynchronous.  Errors:
  * EINVAL for bad arguments, ECAPACITY for capacity > max_spheres, > 4096 voxels per axis or > 2^25 voxels. */
 gmapp_status gmapp_build_sphere_world(gmapp_ctx* ctx, const float* d_points, int n_points, const float* lo,
                                       const float* hi, float pitch, int capacity, int32_t* d_count_out,

@@ -54,6 +54,7 @@ struct gmapp_ctx {
     float* d_snap = nullptr;             // [max_agents][14]
     int* d_prev = nullptr;               // incumbent on the device
     float roll_t0 = 0.0f; float* roll_snap = nullptr; int roll_snap_step = 0;
+    bool built_world = false;            // the sphere world came from gmapp_build_sphere_world: its count lives in d_vox_count
     int* d_best_idx = nullptr; float* d_best_cost = nullptr;
     int* h_best = nullptr;               // pinned: {idx, cost bits}
     float* d_scratch = nullptr;
@@ -271,6 +272,7 @@ extern "C" gmapp_status gmapp_set_obstacles(gmapp_ctx* c, const float* d_xyzr, c
     k_pack_spheres<<<(nf + 255) / 256, 256, 0, st>>>(d_xyzr, d_vel, n, nf, 0.0f, c->d_sph_raw, c->d_svel);
     CUDA_TRY(c, cudaGetLastError());
     c->n_spheres = n;
+    c->built_world = false;
     c->moving = (d_vel != nullptr) && n > 0;
     c->eff_valid = false;
     c->pair_valid = false;
@@ -315,6 +317,7 @@ extern "C" gmapp_status gmapp_build_sphere_world(gmapp_ctx* c, const float* d_po
     if (d_count_out) CUDA_TRY(c, cudaMemcpyAsync(d_count_out, c->d_vox_count, sizeof(int), cudaMemcpyDeviceToDevice, st));
     // the sphere world now holds `capacity` slots: the occupied voxels first, sentinels behind them
     c->n_spheres = capacity;
+    c->built_world = true;
     c->moving = false;
     c->eff_valid = false;
     c->pair_valid = false;
@@ -550,6 +553,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
     P.agent_idx = c->sub_idx;
     P.snap_out = c->roll_snap; P.snap_step = c->roll_snap_step;
+    P.count_dev = c->built_world ? c->d_vox_count : nullptr; P.n_cap = c->n_spheres;
     P.rd_arr = (c->ap_n > 0 && c->ap_has_rd) ? c->d_ap_rd : nullptr;
     P.kf_arr = (c->ap_n > 0 && c->ap_has_kf) ? c->d_ap_kf : nullptr;
     P.tile_off = tile_off; P.xch_off = xch_off; P.rec_off = rec_off;
@@ -662,6 +666,7 @@ static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_ag
     P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
     P.agent_idx = c->sub_idx;
     P.snap_out = c->roll_snap; P.snap_step = c->roll_snap_step;
+    P.count_dev = c->built_world ? c->d_vox_count : nullptr; P.n_cap = c->n_spheres;
     P.rd_arr = (c->ap_n > 0 && c->ap_has_rd) ? c->d_ap_rd : nullptr;
     P.kf_arr = (c->ap_n > 0 && c->ap_has_kf) ? c->d_ap_kf : nullptr;
     P.tile_off = cfg.tile_off; P.red_off = cfg.red_off;

@@ -62,6 +62,8 @@ struct RolloutParams {
     float t0;                 // obstacles are evaluated at t0 + k dt
     float* snap_out;          // [n][6|14] states after snap_step steps (indexed like agents_in), or nullptr
     int snap_step;            // 1..steps
+    const int* count_dev;     // nullable: device-resident sphere count of a built sphere world (wide kernel only)
+    int n_cap;
     int tile_off;             // byte offset of the sphere tile in dynamic shared memory
     int red_off;              // byte offset of the cross-warp exchange scratch
 };

@@ -261,7 +261,7 @@ struct EpiPose6 {
 // ---------------------------------------------------------------------------------------------
 // sweep warps: packed f32x2 sweeps over sphere pairs; tile = A, B (, U, V when MOVING) arrays of n2p float4 each
 template <int NA, bool MOVING, bool CULL, bool APF, bool PER>
-__device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const float4* tile, int astride, int first_agent,
+__device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const float4* tile, int astride, int n2p, int first_agent,
                                                  int lane_in_group, int group_in_cta, float4* xch) {
     const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
     const int half = (NA == 2) ? (lane >> 4) : 0;
@@ -287,11 +287,11 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
         const float tk = fmaf(float(k), P.dt, P.t0);
         acc.clear();
         if (MOVING) {
-            if (!last) sweep_x2_moving<NA, true, CULL, APF>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
-            else       sweep_x2_moving<NA, false, false>(tA, tB, tU, tV, P.n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
+            if (!last) sweep_x2_moving<NA, true, CULL, APF>(tA, tB, tU, tV, n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
+            else       sweep_x2_moving<NA, false, false>(tA, tB, tU, tV, n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
         } else {
-            if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
-            else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
+            if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
+            else       sweep_x2<NA, false, false>(tA, tB, n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
         }
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
@@ -363,14 +363,19 @@ __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
     const int tid = threadIdx.x;
     constexpr int NARR = MOVING ? 4 : 2;                    // pair arrays: A, B (, U, V)
+    int n2p = P.n2p;
+    if (P.count_dev) {                                      // built sphere world: sweep only the pairs holding real spheres
+        const int n = min(*P.count_dev, P.n_cap), h = (n + 1) >> 1;
+        n2p = min(P.n2p, ((h + P.L - 1) >> P.logL) << P.logL);
+    }
     const float4* tile = P.pairA;                           // stage 0: read the pair arrays from global memory / L2
     int astride = P.pair_stride;
     if (STAGE == 1) {
         float4* t = reinterpret_cast<float4*>(smem_raw + P.tile_off);
         if (tid == 0) { mbar_init(bar, 1); fence_mbar_init(); }
         __syncthreads();
-        if (tid == 0) {
-            const uint32_t bytes = uint32_t(P.n2p) * 16u;
+        if (tid == 0 && n2p > 0) {
+            const uint32_t bytes = uint32_t(n2p) * 16u;
             mbar_arrive_expect_tx(bar, NARR * bytes);
             const uint32_t chunk = 32768u;
             for (int r = 0; r < NARR; ++r) {
@@ -382,7 +387,7 @@ __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__
             }
         }
         tile = t;
-        astride = P.n2p;
+        astride = n2p;
     }
     const int cta_first = blockIdx.x * P.agents_per_cta;
     int cta_end = cta_first + P.agents_per_cta;
@@ -405,11 +410,11 @@ __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__
         else wide_epilogue_warp<EpiPoint3<(MOVING || APF)>, 1>(P, first, lane, group_in_cta, xch);
         return;
     }
-    if (STAGE == 1) mbar_wait(bar, 0);
+    if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
     if (na <= 0) return;
     const int lane_in_group = tid & (P.L - 1);
-    if (NA2 == 2 && na >= 2) { if (P.rd_arr) wide_sweep_warps<NA2, MOVING, CULL, APF, true>(P, tile, astride, first, lane_in_group, group_in_cta, xch); else wide_sweep_warps<NA2, MOVING, CULL, APF, false>(P, tile, astride, first, lane_in_group, group_in_cta, xch); }
-    else { if (P.rd_arr) wide_sweep_warps<1, MOVING, CULL, APF, true>(P, tile, astride, first, lane_in_group, group_in_cta, xch); else wide_sweep_warps<1, MOVING, CULL, APF, false>(P, tile, astride, first, lane_in_group, group_in_cta, xch); }
+    if (NA2 == 2 && na >= 2) { if (P.rd_arr) wide_sweep_warps<NA2, MOVING, CULL, APF, true>(P, tile, astride, n2p, first, lane_in_group, group_in_cta, xch); else wide_sweep_warps<NA2, MOVING, CULL, APF, false>(P, tile, astride, n2p, first, lane_in_group, group_in_cta, xch); }
+    else { if (P.rd_arr) wide_sweep_warps<1, MOVING, CULL, APF, true>(P, tile, astride, n2p, first, lane_in_group, group_in_cta, xch); else wide_sweep_warps<1, MOVING, CULL, APF, false>(P, tile, astride, n2p, first, lane_in_group, group_in_cta, xch); }
 }
 
 }  // namespace gmapp

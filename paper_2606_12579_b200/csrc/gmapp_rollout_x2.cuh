@@ -80,6 +80,8 @@ struct RolloutX2Params {
     int rcg_is_rd, rco_is_rd; // Eq. 17 / 18 radii default to the agent's own r_d
     float* snap_out;          // closed-loop re-planning: [n][6] states after snap_step steps, or nullptr
     int snap_step;            // 1..steps
+    const int* count_dev;     // nullable: device-resident sphere count of a built sphere world (gmapp_build_sphere_world);
+    int n_cap;                // the kernel then sweeps only the pairs that hold real spheres (the slots behind are sentinels)
 };
 
 __device__ __forceinline__ int agent_gid(const RolloutX2Params& P, int i) { return P.agent_idx ? P.agent_idx[i] : i; }
@@ -336,7 +338,7 @@ __device__ __forceinline__ void warp_combine(const X2Acc<NA>& acc, int lane, flo
 // group body, L == 32: one warp per group does everything; agent a on lanes 0-15, agent b on lanes 16-31
 // ---------------------------------------------------------------------------------------------
 template <int NA, bool CULL, bool APF, bool PER>
-__device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, const float4* tA, const float4* tB,
+__device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                    int first_agent, int lane) {
     const int half = (NA == 2) ? (lane >> 4) : 0;
     const unsigned full = 0xffffffffu;
@@ -360,8 +362,8 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
             for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
         }
         acc.clear();
-        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane, 32, p, v, rd, P.eps, full, acc);
-        else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane, 32, p, v, rd, P.eps, full, acc);
+        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, n2p, lane, 32, p, v, rd, P.eps, full, acc);
+        else       sweep_x2<NA, false, false>(tA, tB, n2p, lane, 32, p, v, rd, P.eps, full, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
         if (last) {
@@ -398,7 +400,7 @@ __device__ __forceinline__ void agent_load(AgentX2& a, const float* r) {
 }
 
 template <int NA, bool CULL, bool APF, bool PER>
-__device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float4* tA, const float4* tB, int agent0,
+__device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p, int agent0,
                                            int lane, int k, float* rec0) {
     const int half = (NA == 2) ? (lane >> 4) : 0;
     const unsigned full = 0xffffffffu;
@@ -422,8 +424,8 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     const bool last = (k == P.steps);
     X2Acc<NA> acc;
     acc.clear();
-    if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane, 32, p, v, rd, P.eps, full, acc);
-    else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane, 32, p, v, rd, P.eps, full, acc);
+    if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, n2p, lane, 32, p, v, rd, P.eps, full, acc);
+    else       sweep_x2<NA, false, false>(tA, tB, n2p, lane, 32, p, v, rd, P.eps, full, acc);
     float X, Y, Z, D;
     warp_combine<NA>(acc, lane, X, Y, Z, D);
     const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
@@ -442,7 +444,7 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
 }
 
 template <bool CULL, bool APF, bool PER>
-__device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, const float4* tA, const float4* tB,
+__device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                     int first_agent, int n_mine, int lane, float* recs) {
     // records of this warp's agents: recs[i * kAgentRecWords], i < n_mine
     for (int i = lane; i < n_mine; i += 32) {
@@ -453,8 +455,8 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
     __syncwarp();
     for (int k = 0; k <= P.steps; ++k) {
         int i = 0;
-        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL, APF, PER>(P, tA, tB, first_agent + i, lane, k, recs + i * kAgentRecWords);
-        if (i < n_mine) chunk_step<1, CULL, APF, PER>(P, tA, tB, first_agent + i, lane, k, recs + i * kAgentRecWords);
+        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL, APF, PER>(P, tA, tB, n2p, first_agent + i, lane, k, recs + i * kAgentRecWords);
+        if (i < n_mine) chunk_step<1, CULL, APF, PER>(P, tA, tB, n2p, first_agent + i, lane, k, recs + i * kAgentRecWords);
     }
 }
 
@@ -466,7 +468,7 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
 //   epilogue warp k: sync(bar_part) -> read part[k&1] -> integrate -> write state[k&1] -> arrive(bar_state) -> costs
 // ---------------------------------------------------------------------------------------------
 template <int NA, bool CULL, bool APF, bool PER>
-__device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, const float4* tA, const float4* tB,
+__device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                   int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
     const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
     const int half = (NA == 2) ? (lane >> 4) : 0;
@@ -488,8 +490,8 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         acc.clear();
-        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
-        else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
+        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
+        else       sweep_x2<NA, false, false>(tA, tB, n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
         const int par = k & 1;
@@ -545,7 +547,7 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
 // group body, L < 32 (several groups per warp): plain butterfly, every lane integrates its group's agents
 // ---------------------------------------------------------------------------------------------
 template <int NA, bool CULL, bool APF, bool PER>
-__device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, const float4* tA, const float4* tB,
+__device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                      int first_agent, int lane_in_group) {
     const unsigned mask = __activemask();
     AgentX2 ag[NA];
@@ -561,8 +563,8 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 #pragma unroll
             for (int i = 0; i < 3; ++i) { p[a][i] = ag[a].p[i]; v[a][i] = ag[a].v[i]; }
         acc.clear();
-        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, P.n2p, lane_in_group, P.L, p, v, rd, P.eps, mask, acc);
-        else       sweep_x2<NA, false, false>(tA, tB, P.n2p, lane_in_group, P.L, p, v, rd, P.eps, mask, acc);
+        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, n2p, lane_in_group, P.L, p, v, rd, P.eps, mask, acc);
+        else       sweep_x2<NA, false, false>(tA, tB, n2p, lane_in_group, P.L, p, v, rd, P.eps, mask, acc);
         float x[NA], y[NA], z[NA], dm[NA];
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
@@ -600,12 +602,17 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
     const float4* tA = P.pairA;
     const float4* tB = P.pairB;
     const int tid = threadIdx.x;
+    int n2p = P.n2p;
+    if (P.count_dev) {                                      // built sphere world: the count never went to the host
+        const int n = min(*P.count_dev, P.n_cap), h = (n + 1) >> 1;
+        n2p = min(P.n2p, ((h + P.L - 1) >> P.logL) << P.logL);
+    }
     if (STAGE == 1) {
         float4* tile = reinterpret_cast<float4*>(smem_raw + P.tile_off);
         if (tid == 0) { mbar_init(bar, 1); fence_mbar_init(); }
         __syncthreads();
-        if (tid == 0) {
-            const uint32_t bytes = uint32_t(P.n2p) * 16u;
+        if (tid == 0 && n2p > 0) {
+            const uint32_t bytes = uint32_t(n2p) * 16u;
             mbar_arrive_expect_tx(bar, 2u * bytes);
             const uint32_t chunk = 32768u;
             for (uint32_t o = 0; o < bytes; o += chunk) {
@@ -615,7 +622,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
             }
         }
         tA = tile;
-        tB = tile + P.n2p;
+        tB = tile + n2p;
     }
     const int cta_first = blockIdx.x * P.agents_per_cta;
     int cta_end = cta_first + P.agents_per_cta;
@@ -636,11 +643,11 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
             else group_epilogue_warp<1, APF>(P, first, tid & 31, group_in_cta, xch);
             return;
         }
-        if (STAGE == 1) mbar_wait(bar, 0);
+        if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
         if (na <= 0) return;
         const int lane_in_group = tid & (P.L - 1);
-        if (AT == 2 && na >= 2) { if (P.rd_arr) group_sweep_warps<NA2, CULL, APF, true>(P, tA, tB, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<NA2, CULL, APF, false>(P, tA, tB, first, lane_in_group, group_in_cta, xch); }
-        else { if (P.rd_arr) group_sweep_warps<1, CULL, APF, true>(P, tA, tB, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<1, CULL, APF, false>(P, tA, tB, first, lane_in_group, group_in_cta, xch); }
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_sweep_warps<NA2, CULL, APF, true>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<NA2, CULL, APF, false>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); }
+        else { if (P.rd_arr) group_sweep_warps<1, CULL, APF, true>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<1, CULL, APF, false>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); }
         return;
     }
     if (MODE == 4) {
@@ -648,24 +655,24 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         const int nw = blockDim.x >> 5, w = tid >> 5, n_cta = cta_end - cta_first;
         const int base = n_cta / nw, rem = n_cta % nw;
         const int start = w * base + (w < rem ? w : rem), n_mine = base + (w < rem ? 1 : 0);
-        if (STAGE == 1) mbar_wait(bar, 0);
+        if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
         if (n_mine <= 0) return;
         float* recs = reinterpret_cast<float*>(smem_raw + P.rec_off) + start * kAgentRecWords;
-        { if (P.rd_arr) warp_rollout_chunks<CULL, APF, true>(P, tA, tB, cta_first + start, n_mine, tid & 31, recs); else warp_rollout_chunks<CULL, APF, false>(P, tA, tB, cta_first + start, n_mine, tid & 31, recs); }
+        { if (P.rd_arr) warp_rollout_chunks<CULL, APF, true>(P, tA, tB, n2p, cta_first + start, n_mine, tid & 31, recs); else warp_rollout_chunks<CULL, APF, false>(P, tA, tB, n2p, cta_first + start, n_mine, tid & 31, recs); }
         return;
     }
     const int group_in_cta = tid >> P.logL;
     const int lane_in_group = tid & (P.L - 1);
     const int first = cta_first + group_in_cta * AT;
     const int na = cta_end - first;
-    if (STAGE == 1) mbar_wait(bar, 0);
+    if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
     if (na <= 0) return;
     if (MODE == 1) {
-        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_warp<NA2, CULL, APF, true>(P, tA, tB, first, lane_in_group); else group_rollout_warp<NA2, CULL, APF, false>(P, tA, tB, first, lane_in_group); }
-        else { if (P.rd_arr) group_rollout_warp<1, CULL, APF, true>(P, tA, tB, first, lane_in_group); else group_rollout_warp<1, CULL, APF, false>(P, tA, tB, first, lane_in_group); }
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_warp<NA2, CULL, APF, true>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_warp<NA2, CULL, APF, false>(P, tA, tB, n2p, first, lane_in_group); }
+        else { if (P.rd_arr) group_rollout_warp<1, CULL, APF, true>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_warp<1, CULL, APF, false>(P, tA, tB, n2p, first, lane_in_group); }
     } else {
-        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_narrow<NA2, CULL, APF, true>(P, tA, tB, first, lane_in_group); else group_rollout_narrow<NA2, CULL, APF, false>(P, tA, tB, first, lane_in_group); }
-        else { if (P.rd_arr) group_rollout_narrow<1, CULL, APF, true>(P, tA, tB, first, lane_in_group); else group_rollout_narrow<1, CULL, APF, false>(P, tA, tB, first, lane_in_group); }
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_narrow<NA2, CULL, APF, true>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_narrow<NA2, CULL, APF, false>(P, tA, tB, n2p, first, lane_in_group); }
+        else { if (P.rd_arr) group_rollout_narrow<1, CULL, APF, true>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_narrow<1, CULL, APF, false>(P, tA, tB, n2p, first, lane_in_group); }
     }
 }
 
