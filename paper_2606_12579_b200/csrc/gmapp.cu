@@ -677,7 +677,8 @@ static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_ag
     if (wide) {
         while (cfg.groups * cfg.L > 512 || cfg.L > pow2_ceil(n2)) cfg.L >>= 1;
         P.L = cfg.L; P.logL = ilog2(cfg.L);
-        cfg.block = cfg.groups * cfg.L + 32 * cfg.groups;
+        P.two_warp_epi = (kind == GMAPP_MOTOR6 && cfg.groups <= 3) ? 1 : 0;
+        cfg.block = cfg.groups * cfg.L + (P.two_warp_epi ? 64 : 32) * cfg.groups;
         s = effective_pairs(c, g->r_agent, st, &launches);
         if (s != GMAPP_OK) return s;
         P.pairA = c->d_pairA; P.pair_stride = c->cap_spheres / 2; P.n2p = round_up(n2, cfg.L);

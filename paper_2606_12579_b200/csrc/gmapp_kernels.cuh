@@ -64,6 +64,7 @@ struct RolloutParams {
     int snap_step;            // 1..steps
     const int* count_dev;     // nullable: device-resident sphere count of a built sphere world (wide kernel only)
     int n_cap;
+    int two_warp_epi;         // wide kernel, 6D agents: a rot warp and a lin warp per group (G <= 3)
     int tile_off;             // byte offset of the sphere tile in dynamic shared memory
     int red_off;              // byte offset of the cross-warp exchange scratch
 };

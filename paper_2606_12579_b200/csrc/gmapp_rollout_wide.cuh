@@ -354,6 +354,104 @@ __device__ __forceinline__ void wide_epilogue_warp(const RolloutParams& P, int f
 }
 
 // ---------------------------------------------------------------------------------------------
+// 6D agents, two epilogue warps per group.  With zero repulsive torque (reading G18) the rotational dynamics
+// (r, w) never sees the sphere sums, so a ROT warp runs it on its own -- log of the relative rotation, torque, new
+// angular velocity, rotor increment, new rotor -- one step ahead, and hands a 5 x float4 record per step to the LIN
+// warp: [r_k] [e_w, c2] [phi, B] [r_{k+1}] [w_{k+1}, C].  The LIN warp does what needs the position and the sums.
+// The single-warp epilogue spent ~520 dependent instructions per step on one warp and was the bottleneck of config 4;
+// split, the chain per step is max(rot, lin).
+// Hand-over by two named barriers per group, strictly alternating so that barrier generations never overlap:
+//   rot step k:  compute record k -> sync(empty) [k >= 1: lin has read record k-1] -> write -> arrive(full)
+//   lin step k:  sync(full) -> read record k -> arrive(empty) -> ... the usual epilogue step
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void wide_rot_warp(const RolloutParams& P, int agent, int lane, int group_in_cta, float4* rec) {
+    const int bar_full = 9 + 2 * group_in_cta, bar_empty = 10 + 2 * group_in_cta;
+    const int gid = agent_gid(P, agent);
+    Pose6 x = load_pose6(P.agents_in + 14 * size_t(gid));
+    Quat rg = Quat{P.goal[0], P.goal[1], P.goal[2], P.goal[3]}, dg = Quat{P.goal[4], P.goal[5], P.goal[6], P.goal[7]};
+    motor_normalise(rg, dg);
+    for (int k = 0; k < P.steps; ++k) {
+        Vec3 ew; float c2;
+        se3_log_rot(qmul(qconj(x.r), rg), ew, c2);
+        const Vec3 tau = fma3(P.k_att_rot, ew, (-P.k_damp_rot) * x.w);
+        const Vec3 w_new = fma3(P.c_rot, tau, x.w);                        // Eq. 9-10, rotational block
+        const Vec3 phi = P.dt * w_new;
+        float ch, sh_over_th, Bc, Cc;
+        se3_exp_coeffs(phi, ch, sh_over_th, Bc, Cc);
+        const Quat rd = Quat{ch, sh_over_th * phi.x, sh_over_th * phi.y, sh_over_th * phi.z};
+        Quat r_new = qmul(x.r, rd);                                        // Eq. 11, rotor part
+        Quat dz = Quat{0, 0, 0, 0};
+        motor_normalise(r_new, dz);
+        if (k >= 1) named_bar_sync(bar_empty, 64);
+        if (lane == 0) {
+            rec[0] = make_float4(x.r.w, x.r.x, x.r.y, x.r.z);
+            rec[1] = make_float4(ew.x, ew.y, ew.z, c2);
+            rec[2] = make_float4(phi.x, phi.y, phi.z, Bc);
+            rec[3] = make_float4(r_new.w, r_new.x, r_new.y, r_new.z);
+            rec[4] = make_float4(w_new.x, w_new.y, w_new.z, Cc);
+        }
+        named_bar_arrive(bar_full, 64);
+        x.r = r_new; x.w = w_new;
+    }
+    if (P.steps >= 1) named_bar_sync(bar_empty, 64);                       // balance the lin warp's last arrive
+}
+
+template <bool DIRECT>
+__device__ __forceinline__ void wide_lin_warp(const RolloutParams& P, int agent, int lane, int group_in_cta,
+                                              float4* xch, const float4* rec) {
+    const int W = P.L >> 5;
+    const float4* part = xch;
+    float4* state = xch + 2 * W;
+    const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
+    const int bar_full = 9 + 2 * group_in_cta, bar_empty = 10 + 2 * group_in_cta;
+    const bool writer = lane == 0;
+    EpiPose6<DIRECT> me;
+    me.init(P, agent);
+    if (writer) {
+        state[(1 * 1 + 0) * 2] = make_float4(me.pub[0], me.pub[1], me.pub[2], 0.0f);
+        state[(1 * 1 + 0) * 2 + 1] = make_float4(me.pub[3], me.pub[4], me.pub[5], 0.0f);
+    }
+    named_bar_arrive(bar_state, nbar);
+    Vec3 ew = v3(0, 0, 0); float c2 = 0.0f;
+    for (int k = 0; k <= P.steps; ++k) {
+        const bool last = (k == P.steps);
+        const int par = k & 1;
+        if (!last) {
+            named_bar_sync(bar_full, 64);
+            const float4 a0 = rec[0], a1 = rec[1], a2 = rec[2], a3 = rec[3], a4 = rec[4];
+            named_bar_arrive(bar_empty, 64);
+            me.x.r = Quat{a0.x, a0.y, a0.z, a0.w};
+            ew = v3(a1.x, a1.y, a1.z); c2 = a1.w;
+            me.phi = v3(a2.x, a2.y, a2.z); me.Bc = a2.w;
+            me.r_new = Quat{a3.x, a3.y, a3.z, a3.w};
+            me.w_new = v3(a4.x, a4.y, a4.z); me.Cc = a4.w;
+            // the part of Eq. 8 / Eq. 7 that needs the position: e_v = V^-1(e_w) R^T (p_g - p), f without f_r
+            me.pos = me.x.p;
+            const Vec3 ev = se3_log_lin(ew, c2, qrot_inv(me.x.r, me.pg - me.pos));
+            me.fpre = fma3(P.k_att, ev, (-P.k_damp) * me.x.nu);
+        }
+        named_bar_sync(bar_part, nbar);
+        float4 t = part[(par * W) * 1];
+        for (int w = 1; w < W; ++w) {
+            const float4 o = part[(par * W + w) * 1];
+            t.x += o.x; t.y += o.y; t.z += o.z; t.w = fminf(t.w, o.w);
+        }
+        if (last) {
+            if (writer) me.finish(P, t.w);
+            return;
+        }
+        me.post(P, t.x, t.y, t.z);
+        if (writer) {
+            state[(par * 1 + 0) * 2] = make_float4(me.pub[0], me.pub[1], me.pub[2], 0.0f);
+            state[(par * 1 + 0) * 2 + 1] = make_float4(me.pub[3], me.pub[4], me.pub[5], 0.0f);
+        }
+        named_bar_arrive(bar_state, nbar);
+        me.costs(P, k, t.w);
+        if (writer) me.snapshot(P, k);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // the kernel: threads [0, G L) sweep, [G L, G L + 32 G) one epilogue warp per group; G <= 4, L >= 64
 // KIND 0 = 3D point agents (AT 1 or 2 per group), KIND 1 = 6D motor agents (one per group)
 // ---------------------------------------------------------------------------------------------
@@ -402,7 +500,20 @@ __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__
     const int first = cta_first + group_in_cta * ATE;
     const int na = cta_end - first;
     float4* xch = reinterpret_cast<float4*>(smem_raw + P.red_off) + group_in_cta * (2 * W * 2 + 2 * 2 * 2);
-    if (is_epi) {
+    if (KIND == 1 && P.two_warp_epi) {
+        // threads [n_sweep, n_sweep + 32 G): lin warps; [n_sweep + 32 G, n_sweep + 64 G): rot warps
+        if (tid >= n_sweep) {
+            const int e = (tid - n_sweep) >> 5, g = e % G;
+            const int ag = cta_first + g;
+            if (ag >= cta_end) return;
+            float4* base = reinterpret_cast<float4*>(smem_raw + P.red_off);
+            float4* xg = base + g * (2 * W * 2 + 2 * 2 * 2);
+            float4* rec = base + 112 + 5 * g;
+            if (e < G) wide_lin_warp<(MOVING || APF)>(P, ag, tid & 31, g, xg, rec);
+            else wide_rot_warp(P, ag, tid & 31, g, rec);
+            return;
+        }
+    } else if (is_epi) {
         if (na <= 0) return;
         const int lane = tid & 31;
         if (KIND == 1) wide_epilogue_warp<EpiPose6<(MOVING || APF)>, 1>(P, first, lane, group_in_cta, xch);
