@@ -490,7 +490,8 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     const gmapp_tuning* t = c->has_tuning ? &c->tuning : nullptr;
     int max_ctas = c->num_sms;
     if (t && t->max_ctas > 0 && t->max_ctas < max_ctas) max_ctas = t->max_ctas;
-    const int A = (n_agents + max_ctas - 1) / max_ctas;           // agents per CTA: one wave of the SMs
+    int A = (n_agents + max_ctas - 1) / max_ctas;                 // agents per CTA: one wave of the SMs
+    if (A > 1024) A = 1024;                                       // beyond 1024 agents per CTA: several waves of CTAs
     const int grid = (n_agents + A - 1) / A;
     int at = A >= 2 ? 2 : 1;
     if (t && t->agents_per_thread) at = t->agents_per_thread;

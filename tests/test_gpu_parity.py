@@ -550,6 +550,23 @@ def test_rollout_over_built_world_equals_rollout_over_uploaded_spheres(api, ctx,
     assert np.abs(ref["final"][:, :3].astype(np.float64) - o["final"][:, :3]).max() <= POS_TOL
 
 
+def test_more_agents_than_one_wave_holds(api, orc):
+    """200 000 agents: more than 148 x 1024, so the chunked kernel runs several waves of CTAs; sampled agents vs oracle."""
+    c = api.Context(max_agents=200_000, max_spheres=256)
+    try:
+        sc = scenes.config5(200_000, 128, steps=8)
+        idx = np.random.default_rng(0).choice(200_000, 48, replace=False)
+        idx.sort()
+        g = api.run_scene(c, sc)
+        assert g["info"]["grid"] > c.sm_count and np.all(np.isfinite(g["cost"]))
+        o = orc.rollout_scene(sc, threads=8, agent_slice=idx)
+        assert np.abs(g["final"][idx, :3].astype(np.float64) - o["final"][:, :3]).max() <= POS_TOL
+        assert np.abs(g["cost"][idx].astype(np.float64) - o["cost"]).max() <= 1e-4
+        assert np.array_equal(g["collided"][idx], o["collided"])
+    finally:
+        c.close()
+
+
 # ---------------------------------------------------------------------------------- launch variants
 @pytest.mark.parametrize("tuning", [
     dict(lanes_per_agent=8, agents_per_thread=1), dict(lanes_per_agent=32, agents_per_thread=1),
