@@ -160,6 +160,12 @@ gmapp_status gmapp_rollout(gmapp_ctx* ctx, gmapp_kind kind, const float* d_agent
                            int n_agents, const float* goal, const gmapp_gains* gains, float dt, int steps,
                            void* cuda_stream);
 
+/* Explored paths (PAPER.md:51 lists them among the planner's outputs; Eq. 15): while d_traj is set,
+ * every gmapp_rollout also writes all steps+1 poses of every agent to the caller-owned DEVICE buffer
+ * d_traj [n_agents][steps+1][6|14] (same state layout as the agents; pose 0 is the start state as given).  The buffer
+ * must hold the largest later rollout.  NULL switches it off (the default).  One 24- or 56-byte store per agent-step. */
+gmapp_status gmapp_set_trajectory_output(gmapp_ctx* ctx, float* d_traj);
+
 /* Closed-loop re-planning (Fig. 2 steps 3-5: the planner re-plans from the robot's state while
  * the control thread follows the best agent).  n_cycles planning cycles are chained ON THE DEVICE, nothing
  * synchronises: cycle c rolls all agents `steps` steps from d_agents (obstacles at time c * exec_steps * dt),

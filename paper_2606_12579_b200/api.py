@@ -44,7 +44,7 @@ class gmapp_launch_info(C.Structure):
 
 
 EXPORTS = ["gmapp_default_gains", "gmapp_create", "gmapp_destroy", "gmapp_set_obstacles",
-           "gmapp_set_obstacles_host", "gmapp_build_sphere_world", "gmapp_get_obstacles", "gmapp_set_tuning", "gmapp_set_agent_params", "gmapp_rollout", "gmapp_replan", "gmapp_best_agent", "gmapp_best_agent_ex",
+           "gmapp_set_obstacles_host", "gmapp_build_sphere_world", "gmapp_get_obstacles", "gmapp_set_tuning", "gmapp_set_agent_params", "gmapp_rollout", "gmapp_set_trajectory_output", "gmapp_replan", "gmapp_best_agent", "gmapp_best_agent_ex",
            "gmapp_forces",
            "gmapp_get_results", "gmapp_plan_cycle_host", "gmapp_get_launch_info", "gmapp_measure_fp32_peak",
            "gmapp_sm_count", "gmapp_last_error"]
@@ -72,6 +72,7 @@ def _load():
     lib.gmapp_set_tuning.argtypes = [vp, C.POINTER(gmapp_tuning)]
     lib.gmapp_set_agent_params.argtypes = [vp, vp, vp, vp, C.c_int, vp]
     lib.gmapp_rollout.argtypes = [vp, C.c_int, vp, vp, C.c_int, fp, C.POINTER(gmapp_gains), C.c_float, C.c_int, vp]
+    lib.gmapp_set_trajectory_output.argtypes = [vp, vp]
     lib.gmapp_replan.argtypes = [vp, C.c_int, vp, C.c_int, fp, C.POINTER(gmapp_gains), C.c_float, C.c_int, C.c_int, C.c_float,
                                  C.c_int, C.c_int, vp, vp, vp]
     lib.gmapp_best_agent.argtypes = [vp, C.c_float, C.c_int, ip, fp, vp]
@@ -224,6 +225,9 @@ class Context:
         g = gains if isinstance(gains, gmapp_gains) else make_gains(gains)
         self._check(_lib.gmapp_rollout(self._h, kind, _ptr(d_agents), _ptr(d_agents_out), n, gp, C.byref(g),
                                        C.c_float(dt), int(steps), _stream(stream)))
+
+    def set_trajectory_output(self, d_traj=None):
+        self._check(_lib.gmapp_set_trajectory_output(self._h, _ptr(d_traj)))
 
     def replan(self, kind, d_agents, goal, gains, dt, steps, exec_steps, n_cycles, alpha=0.9, prev_best=-1,
                d_path_out=None, d_best_out=None, n_agents=None, stream=None):

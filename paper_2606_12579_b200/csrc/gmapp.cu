@@ -54,6 +54,7 @@ struct gmapp_ctx {
     float* d_snap = nullptr;             // [max_agents][14]
     int* d_prev = nullptr;               // incumbent on the device
     float roll_t0 = 0.0f; float* roll_snap = nullptr; int roll_snap_step = 0;
+    float* roll_traj = nullptr;          // trajectory output of the next rollouts (gmapp_set_trajectory_output)
     bool built_world = false;            // the sphere world came from gmapp_build_sphere_world: its count lives in d_vox_count
     int* d_best_idx = nullptr; float* d_best_cost = nullptr;
     int* h_best = nullptr;               // pinned: {idx, cost bits}
@@ -108,7 +109,8 @@ static rollout_fn rollout_kernel(int kind, int at, bool moving, bool cull, int s
 #undef PICK
 }
 static const int kX2SweepThreads = 512;       // sweep threads per CTA; mode 2 adds one epilogue warp per group (<= 672 in all)
-static rollout_x2_fn rollout_x2_kernel(int at, int mode, bool cull, int stage, bool apf) {
+static rollout_x2_fn rollout_x2_kernel(int at, int mode, bool cull, int stage, bool apf, bool extras) {
+    if (extras) return apf ? gmapp::rollout_x2_kernel_apf_x(at, mode, cull, stage) : gmapp::rollout_x2_kernel_cf_x(at, mode, cull, stage);
     return apf ? gmapp::rollout_x2_kernel_apf(at, mode, cull, stage) : gmapp::rollout_x2_kernel_cf(at, mode, cull, stage);
 }
 static rollout_fn rollout_wide_kernel(int kind, int at, bool moving, bool cull, int stage, bool apf) {
@@ -194,8 +196,8 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
     for (int at = 1; at <= 2; ++at)
         for (int md = 0; md < 5; ++md)
             for (int cu = 0; cu < 4; ++cu)
-                for (int hf = 0; hf < 2; ++hf) {
-                    e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, md, cu & 1, cu >> 1, hf != 0),
+                for (int hf = 0; hf < 4; ++hf) {
+                    e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, md, cu & 1, cu >> 1, (hf & 1) != 0, (hf >> 1) != 0),
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
                     if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
                 }
@@ -553,7 +555,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     P.w_goal = g->w_goal; P.w_obs = g->w_obs; P.w_path = g->w_path; P.w_smooth = g->w_smooth; P.a_max = g->a_max;
     P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
     P.agent_idx = c->sub_idx;
-    P.snap_out = c->roll_snap; P.snap_step = c->roll_snap_step;
+    P.snap_out = c->roll_snap; P.snap_step = c->roll_snap_step; P.traj_out = c->roll_traj;
     P.count_dev = c->built_world ? c->d_vox_count : nullptr; P.n_cap = c->n_spheres;
     P.rd_arr = (c->ap_n > 0 && c->ap_has_rd) ? c->d_ap_rd : nullptr;
     P.kf_arr = (c->ap_n > 0 && c->ap_has_kf) ? c->d_ap_kf : nullptr;
@@ -561,7 +563,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     const int block = mode == 4 ? tmax : (mode >= 2 ? G * L + 32 * G : round_up(G * L, 32));
     const int smem = tile_off + (stage == 1 ? (int)tile_bytes : 0);
     P.stage = stage;
-    rollout_x2_fn fn = rollout_x2_kernel(at, mode, cull != 0, stage, g->heuristic == 1);
+    rollout_x2_fn fn = rollout_x2_kernel(at, mode, cull != 0, stage, g->heuristic == 1, P.snap_out != nullptr || P.traj_out != nullptr);
     fn<<<grid, block, smem, st>>>(P);
     CUDA_TRY(c, cudaGetLastError());
     ++launches;
@@ -597,6 +599,11 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
     const int ng = kind == GMAPP_POINT3 ? 3 : 8;
     for (int i = 0; i < ng; ++i) if (!isfinite(goal[i])) return fail(c, GMAPP_EINVAL, "rollout: non-finite goal%s");
     c->sub_idx = nullptr;
+    if (c->roll_traj) {                     // pose 0 of every path = the start state, as given
+        const size_t wb = sizeof(float) * (kind == GMAPP_POINT3 ? 6 : 14);
+        CUDA_TRY(c, cudaMemcpy2DAsync(c->roll_traj, wb * (size_t)(steps + 1), d_agents, wb, wb, (size_t)n_agents,
+                                      cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    }
     if (c->ap_n > 0) {
         // heterogeneous ensemble: one launch per heuristic over that heuristic's agents (the paper runs one
         // specialised kernel per heuristic), per-agent r_d / k_f read inside the kernels
@@ -666,7 +673,7 @@ static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_ag
     P.a_max = g->a_max; P.vel_factor = g->vel_factor;
     P.cost = c->d_cost; P.minclr = c->d_minclr; P.collided = c->d_collided;
     P.agent_idx = c->sub_idx;
-    P.snap_out = c->roll_snap; P.snap_step = c->roll_snap_step;
+    P.snap_out = c->roll_snap; P.snap_step = c->roll_snap_step; P.traj_out = c->roll_traj;
     P.count_dev = c->built_world ? c->d_vox_count : nullptr; P.n_cap = c->n_spheres;
     P.rd_arr = (c->ap_n > 0 && c->ap_has_rd) ? c->d_ap_rd : nullptr;
     P.kf_arr = (c->ap_n > 0 && c->ap_has_kf) ? c->d_ap_kf : nullptr;
@@ -734,6 +741,12 @@ extern "C" gmapp_status gmapp_best_agent(gmapp_ctx* c, float alpha, int prev_bes
 // ---------------------------------------------------------------------------------------------
 // closed-loop re-planning (NEXT row N4): n_cycles planning cycles chained on the device
 // ---------------------------------------------------------------------------------------------
+extern "C" gmapp_status gmapp_set_trajectory_output(gmapp_ctx* c, float* d_traj) {
+    if (!c) return GMAPP_EINVAL;
+    c->roll_traj = d_traj;
+    return GMAPP_OK;
+}
+
 extern "C" gmapp_status gmapp_replan(gmapp_ctx* c, gmapp_kind kind, float* d_agents, int n_agents, const float* goal,
                                      const gmapp_gains* g, float dt, int steps, int exec_steps, float alpha, int prev_best,
                                      int n_cycles, float* d_path_out, int32_t* d_best_out, void* stream) {

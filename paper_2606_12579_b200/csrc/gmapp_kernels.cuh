@@ -62,6 +62,7 @@ struct RolloutParams {
     float t0;                 // obstacles are evaluated at t0 + k dt
     float* snap_out;          // [n][6|14] states after snap_step steps (indexed like agents_in), or nullptr
     int snap_step;            // 1..steps
+    float* traj_out;          // nullable: [n][steps+1][6|14] every pose of every agent (pose 0 = start state, written by the host side)
     const int* count_dev;     // nullable: device-resident sphere count of a built sphere world (wide kernel only)
     int n_cap;
     int two_warp_epi;         // wide kernel, 6D agents: a rot warp and a lin warp per group (G <= 3)
@@ -369,6 +370,11 @@ __device__ __forceinline__ void rollout_point3(const RolloutParams& P, const flo
 #pragma unroll
                 for (int c = 0; c < 3; ++c) { o[c] = p[a][c]; o[3 + c] = v[a][c]; }
             }
+            if (P.traj_out && lane_in_group == 0) {
+                float* o = P.traj_out + 6 * (size_t(gid[a]) * (P.steps + 1) + k + 1);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { o[c] = p[a][c]; o[3 + c] = v[a][c]; }
+            }
         }
     }
     // final pose: distance-only pass
@@ -490,6 +496,7 @@ __device__ __forceinline__ void rollout_pose6(const RolloutParams& P, const floa
         Quat dz = Quat{0, 0, 0, 0};
         motor_normalise(x.r, dz);
         if (P.snap_out && k + 1 == P.snap_step && lane_in_group == 0) write_pose6(x, P.snap_out + 14 * size_t(agent));
+        if (P.traj_out && lane_in_group == 0) write_pose6(x, P.traj_out + 14 * (size_t(agent) * (P.steps + 1) + k + 1));
     }
     pos = x.p;
     p[0][0] = pos.x; p[0][1] = pos.y; p[0][2] = pos.z;

@@ -170,6 +170,7 @@ struct EpiPoint3 {
     }
     __device__ __forceinline__ void snapshot(const RolloutParams& P, int k) const {
         if (P.snap_out && k + 1 == P.snap_step) write_state(P.snap_out + 6 * size_t(gid));
+        if (P.traj_out) write_state(P.traj_out + 6 * (size_t(gid) * (P.steps + 1) + k + 1));
     }
 };
 
@@ -252,6 +253,7 @@ struct EpiPose6 {
     }
     __device__ __forceinline__ void snapshot(const RolloutParams& P, int k) const {
         if (P.snap_out && k + 1 == P.snap_step) write_pose6(x, P.snap_out + 14 * size_t(gid));
+        if (P.traj_out) write_pose6(x, P.traj_out + 14 * (size_t(gid) * (P.steps + 1) + k + 1));
     }
 };
 

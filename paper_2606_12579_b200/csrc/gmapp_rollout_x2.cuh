@@ -80,6 +80,7 @@ struct RolloutX2Params {
     int rcg_is_rd, rco_is_rd; // Eq. 17 / 18 radii default to the agent's own r_d
     float* snap_out;          // closed-loop re-planning: [n][6] states after snap_step steps, or nullptr
     int snap_step;            // 1..steps
+    float* traj_out;          // nullable: [n][steps+1][6] every pose of every agent (pose 0 = start state, written by the host side)
     const int* count_dev;     // nullable: device-resident sphere count of a built sphere world (gmapp_build_sphere_world);
     int n_cap;                // the kernel then sweeps only the pairs that hold real spheres (the slots behind are sentinels)
 };
@@ -289,6 +290,11 @@ struct AgentX2 {
 #pragma unroll
             for (int c = 0; c < 3; ++c) { o[c] = p[c]; o[3 + c] = v[c]; }
         }
+        if (P.traj_out) {                                   // explored paths: every pose of every agent
+            float* o = P.traj_out + 6 * (size_t(gid) * (P.steps + 1) + k + 1);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { o[c] = p[c]; o[3 + c] = v[c]; }
+        }
     }
     __device__ __forceinline__ void finish(const RolloutX2Params& P, float dmin_final) {
         const int i = gid;
@@ -337,7 +343,7 @@ __device__ __forceinline__ void warp_combine(const X2Acc<NA>& acc, int lane, flo
 // ---------------------------------------------------------------------------------------------
 // group body, L == 32: one warp per group does everything; agent a on lanes 0-15, agent b on lanes 16-31
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL, bool APF, bool PER>
+template <int NA, bool CULL, bool APF, bool PER, bool XT>
 __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                    int first_agent, int lane) {
     const int half = (NA == 2) ? (lane >> 4) : 0;
@@ -374,7 +380,7 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
         me.pre(P);
         me.template post<APF>(P, X, Y, Z, fx, fy, fz);
         me.costs(P, k, D, fx, fy, fz);
-        if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.snapshot(P, k);
+        if ((lane & 15) == 0 && (NA == 2 || lane == 0)) { if (XT) me.snapshot(P, k); }
     }
 }
 
@@ -399,7 +405,7 @@ __device__ __forceinline__ void agent_load(AgentX2& a, const float* r) {
     a.gid = __float_as_int(r[20]); a.rd = r[21]; a.kf = r[22];
 }
 
-template <int NA, bool CULL, bool APF, bool PER>
+template <int NA, bool CULL, bool APF, bool PER, bool XT>
 __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p, int agent0,
                                            int lane, int k, float* rec0) {
     const int half = (NA == 2) ? (lane >> 4) : 0;
@@ -437,13 +443,13 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     me.pre(P);
     me.template post<APF>(P, X, Y, Z, fx, fy, fz);
     me.costs(P, k, D, fx, fy, fz);
-    if (writer) me.snapshot(P, k);
+    if (writer) { if (XT) me.snapshot(P, k); }
     __syncwarp();                                         // every lane has read the record before it is rewritten
     if (writer) agent_store(me, rec);
     __syncwarp();
 }
 
-template <bool CULL, bool APF, bool PER>
+template <bool CULL, bool APF, bool PER, bool XT>
 __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                     int first_agent, int n_mine, int lane, float* recs) {
     // records of this warp's agents: recs[i * kAgentRecWords], i < n_mine
@@ -455,8 +461,8 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
     __syncwarp();
     for (int k = 0; k <= P.steps; ++k) {
         int i = 0;
-        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL, APF, PER>(P, tA, tB, n2p, first_agent + i, lane, k, recs + i * kAgentRecWords);
-        if (i < n_mine) chunk_step<1, CULL, APF, PER>(P, tA, tB, n2p, first_agent + i, lane, k, recs + i * kAgentRecWords);
+        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL, APF, PER, XT>(P, tA, tB, n2p, first_agent + i, lane, k, recs + i * kAgentRecWords);
+        if (i < n_mine) chunk_step<1, CULL, APF, PER, XT>(P, tA, tB, n2p, first_agent + i, lane, k, recs + i * kAgentRecWords);
     }
 }
 
@@ -507,7 +513,7 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
     }
 }
 
-template <int NA, bool APF>
+template <int NA, bool APF, bool XT>
 __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, int first_agent, int lane,
                                                     int group_in_cta, float4* xch) {
     const int W = P.L >> 5;
@@ -539,14 +545,14 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
         }
         named_bar_arrive(bar_state, nbar);
         me.costs(P, k, t.w, fx, fy, fz);                   // off the critical path: the sweep warps are already running
-        if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.snapshot(P, k);
+        if ((lane & 15) == 0 && (NA == 2 || lane == 0)) { if (XT) me.snapshot(P, k); }
     }
 }
 
 // ---------------------------------------------------------------------------------------------
 // group body, L < 32 (several groups per warp): plain butterfly, every lane integrates its group's agents
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL, bool APF, bool PER>
+template <int NA, bool CULL, bool APF, bool PER, bool XT>
 __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                      int first_agent, int lane_in_group) {
     const unsigned mask = __activemask();
@@ -582,7 +588,7 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
             ag[a].pre(P);
             ag[a].template post<APF>(P, x[a], y[a], z[a], fx, fy, fz);
             ag[a].costs(P, k, dm[a], fx, fy, fz);
-            if (lane_in_group == 0) ag[a].snapshot(P, k);
+            if (lane_in_group == 0) { if (XT) ag[a].snapshot(P, k); }
         }
     }
 }
@@ -595,7 +601,9 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 // 4: many agents per CTA, each warp walks its block of agents in chunks of two (state records in shared memory);
 // STAGE 1 = sphere pairs staged in shared memory by TMA bulk copies (a template parameter on purpose: as a run-time
 // choice the tile pointers become generic and every LDS turns into a generic LD, measured 10 % slower)
-template <int AT, int MODE, bool CULL, int STAGE, int MAXT, bool APF>
+// XT = extras: the state snapshot of gmapp_replan and the trajectory output (kept out of the plain kernels: the few
+// extra stores in the epilogue perturb the register allocation of the sweep warps by 3 %)
+template <int AT, int MODE, bool CULL, int STAGE, int MAXT, bool APF, bool XT>
 __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ RolloutX2Params P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
@@ -639,8 +647,8 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         float4* xch = reinterpret_cast<float4*>(smem_raw + P.xch_off) + group_in_cta * (2 * W * 2 + 2 * 2 * 2);
         if (is_epi) {                                      // the epilogue warps never touch the sphere tile
             if (na <= 0) return;
-            if (AT == 2 && na >= 2) group_epilogue_warp<NA2, APF>(P, first, tid & 31, group_in_cta, xch);
-            else group_epilogue_warp<1, APF>(P, first, tid & 31, group_in_cta, xch);
+            if (AT == 2 && na >= 2) group_epilogue_warp<NA2, APF, XT>(P, first, tid & 31, group_in_cta, xch);
+            else group_epilogue_warp<1, APF, XT>(P, first, tid & 31, group_in_cta, xch);
             return;
         }
         if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
@@ -658,7 +666,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
         if (n_mine <= 0) return;
         float* recs = reinterpret_cast<float*>(smem_raw + P.rec_off) + start * kAgentRecWords;
-        { if (P.rd_arr) warp_rollout_chunks<CULL, APF, true>(P, tA, tB, n2p, cta_first + start, n_mine, tid & 31, recs); else warp_rollout_chunks<CULL, APF, false>(P, tA, tB, n2p, cta_first + start, n_mine, tid & 31, recs); }
+        { if (P.rd_arr) warp_rollout_chunks<CULL, APF, true, XT>(P, tA, tB, n2p, cta_first + start, n_mine, tid & 31, recs); else warp_rollout_chunks<CULL, APF, false, XT>(P, tA, tB, n2p, cta_first + start, n_mine, tid & 31, recs); }
         return;
     }
     const int group_in_cta = tid >> P.logL;
@@ -668,11 +676,11 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
     if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
     if (na <= 0) return;
     if (MODE == 1) {
-        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_warp<NA2, CULL, APF, true>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_warp<NA2, CULL, APF, false>(P, tA, tB, n2p, first, lane_in_group); }
-        else { if (P.rd_arr) group_rollout_warp<1, CULL, APF, true>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_warp<1, CULL, APF, false>(P, tA, tB, n2p, first, lane_in_group); }
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_warp<NA2, CULL, APF, true, XT>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_warp<NA2, CULL, APF, false, XT>(P, tA, tB, n2p, first, lane_in_group); }
+        else { if (P.rd_arr) group_rollout_warp<1, CULL, APF, true, XT>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_warp<1, CULL, APF, false, XT>(P, tA, tB, n2p, first, lane_in_group); }
     } else {
-        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_narrow<NA2, CULL, APF, true>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_narrow<NA2, CULL, APF, false>(P, tA, tB, n2p, first, lane_in_group); }
-        else { if (P.rd_arr) group_rollout_narrow<1, CULL, APF, true>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_narrow<1, CULL, APF, false>(P, tA, tB, n2p, first, lane_in_group); }
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_narrow<NA2, CULL, APF, true, XT>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_narrow<NA2, CULL, APF, false, XT>(P, tA, tB, n2p, first, lane_in_group); }
+        else { if (P.rd_arr) group_rollout_narrow<1, CULL, APF, true, XT>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_narrow<1, CULL, APF, false, XT>(P, tA, tB, n2p, first, lane_in_group); }
     }
 }
 

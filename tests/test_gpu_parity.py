@@ -567,6 +567,48 @@ def test_more_agents_than_one_wave_holds(api, orc):
         c.close()
 
 
+# ---------------------------------------------------------------------------------- explored paths (every pose)
+@pytest.mark.parametrize("tuning", [None, dict(lanes_per_agent=32), dict(max_ctas=1), dict(lanes_per_agent=8, agents_per_thread=2, max_ctas=5),
+                                    dict(scalar_path=1)], ids=lambda t: "auto" if t is None else "-".join(f"{k[:4]}{v}" for k, v in t.items()))
+def test_trajectory_output_matches_oracle_at_every_step(api, ctx, orc, tuning):
+    """Positions within 1e-4 m at EVERY step (north_star asks for step 100), for every kernel family."""
+    import torch
+    try:
+        for moving in (False, True):
+            sc = scenes.fast_clutter(moving=moving, n_agents=45, n_spheres=333)
+            traj = torch.full((sc.n_agents, sc.steps + 1, 6), float("nan"), device="cuda:0")
+            ctx.set_trajectory_output(traj)
+            g = api.run_scene(ctx, sc, tuning=tuning)
+            ctx.set_trajectory_output(None)
+            o = orc.rollout_scene(sc, threads=8, want_traj=True)
+            t = traj.cpu().numpy().astype(np.float64)
+            assert np.all(np.isfinite(t))
+            assert np.array_equal(t[:, 0].astype(np.float32), sc.agents) and np.array_equal(t[:, -1].astype(np.float32), g["final"])
+            assert np.abs(t[:, :, :3] - o["traj"][:, :, :3]).max() <= POS_TOL
+            assert np.abs(t[:, :, 3:] - o["traj"][:, :, 3:]).max() <= 1e-3
+    finally:
+        ctx.set_trajectory_output(None)
+        ctx.set_tuning(reset=True)
+
+
+def test_trajectory_output_pose6(api, ctx, orc):
+    import torch
+    sc = scenes.config4(n_agents=24, n_spheres=512, steps=120)
+    traj = torch.zeros((sc.n_agents, sc.steps + 1, 14), device="cuda:0")
+    try:
+        ctx.set_trajectory_output(traj)
+        g = api.run_scene(ctx, sc)
+    finally:
+        ctx.set_trajectory_output(None)
+    o = orc.rollout_scene(sc, threads=8, want_traj=True)
+    t = traj.cpu().numpy()
+    for k in (1, 30, 60, 100, 120):
+        q, pos, tw = api.state14_to_pose(t[:, k])
+        assert np.abs(pos - o["traj"][:, k, 9:12]).max() <= POS_TOL
+        assert _rot_angle(o["traj"][:, k, :9].reshape(-1, 3, 3), _quat_to_R(q)).max() <= ANG_TOL
+    assert np.array_equal(t[:, -1], g["final"])
+
+
 # ---------------------------------------------------------------------------------- launch variants
 @pytest.mark.parametrize("tuning", [
     dict(lanes_per_agent=8, agents_per_thread=1), dict(lanes_per_agent=32, agents_per_thread=1),
