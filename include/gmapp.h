@@ -74,16 +74,19 @@ typedef struct {
 
 /* Launch tuning (all 0 / -1 = choose automatically from N_a, N_O and the SM count).               */
 typedef struct {
-    int32_t lanes_per_agent;     /* threads that share one agent's sphere sum; power of two 1..1024 */
+    int32_t lanes_per_agent;     /* threads that share one agent's sphere sum; power of two 1..1024 (packed kernels:
+                                    <= 512; with more than 32 agents per CTA only 32 is accepted there)  */
     int32_t agents_per_thread;   /* 1 or 2: agents evaluated per staged sphere load                  */
     int32_t cull;                /* -1 auto, 0 = branch-free force math for every pair,
                                     1 = warp-vote skip of the force math when no lane's pair is inside r_d
                                     (Alg. 1 line 7 is such a branch); results are identical */
-    int32_t stage;               /* -1 auto, 0 = read spheres from global/L2, 1 = stage the whole sphere set in
-                                    shared memory (TMA bulk copy), 2 = stream tiles through a TMA ring         */
+    int32_t stage;               /* -1 auto (1 when the set fits), 0 = read spheres from global memory / L2,
+                                    1 = stage the whole sphere set in shared memory by TMA bulk copies
+                                    (EINVAL when it does not fit)                                             */
     int32_t max_ctas;            /* 0 = SM count; cap on the grid (for scaling experiments)           */
-    int32_t scalar_path;         /* 0 = packed f32x2 kernel where it applies (POINT3, static spheres);
-                                    1 = force the scalar FP32 kernel (A/B comparison)                     */
+    int32_t scalar_path;         /* 0 = packed f32x2 kernels where they apply (POINT3 over static spheres in every
+                                    shape; moving spheres and MOTOR6 agents when a group spans >= 64 lanes and
+                                    there are <= 4 groups per CTA); 1 = force the scalar FP32 kernel (A/B)    */
     int32_t reserved[2];
 } gmapp_tuning;
 
