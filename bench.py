@@ -332,6 +332,21 @@ def run_ours(args):
     rp1.record()
     torch.cuda.synchronize(dev)
     replan_ms = rp0.elapsed_time(rp1) / n_cyc
+    # the same 50 cycles captured once as a CUDA graph and replayed
+    side = torch.cuda.Stream(device=dev)
+    side.wait_stream(torch.cuda.current_stream(dev))
+    with torch.cuda.stream(side):
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            ctx.replan(kind, d_loop, goal, gains, scene.dt, scene.steps, exec_steps, n_cyc)
+    torch.cuda.synchronize(dev)
+    d_loop.copy_(d_agents)
+    graph.replay(); torch.cuda.synchronize(dev)
+    d_loop.copy_(d_agents)
+    rp0.record(); graph.replay(); rp1.record()
+    torch.cuda.synchronize(dev)
+    replan_graph_ms = rp0.elapsed_time(rp1) / n_cyc
+    del graph
 
     # ---- sphere-world builder (gmapp_build_sphere_world) on a separate context: 2 x 848 x 480 points (the paper's two
     # depth cameras), 4 cm voxels; HBM-bound (12 B read per point)
@@ -405,7 +420,7 @@ def run_ours(args):
                          "peak_measured_ffma_tflops": peak_meas, "peak_measured_ffma2_tflops": peak_meas_x2,
                          "frac_of_measured_ffma": achieved / peak_meas if peak_meas else None,
                          "launch": info_bf},
-            "replan": {"ms_per_cycle": replan_ms, "cycles_per_s": 1e3 / replan_ms, "cycles": n_cyc, "exec_steps": exec_steps,
+            "replan": {"ms_per_cycle": replan_ms, "cycles_per_s": 1e3 / replan_ms, "cuda_graph_ms_per_cycle": replan_graph_ms, "cycles": n_cyc, "exec_steps": exec_steps,
                        "note": "gmapp_replan: rollout + selection + restart chained on the device (the paper's control "
                                "loop runs at ~100 Hz, PAPER.md:47)"},
             "sphere_world_builder": vox,

@@ -249,6 +249,8 @@ extern "C" gmapp_status gmapp_get_launch_info(const gmapp_ctx* c, gmapp_launch_i
 // ---------------------------------------------------------------------------------------------
 // obstacles
 // ---------------------------------------------------------------------------------------------
+__global__ void k_set_int(int* p, int v) { *p = v; }
+
 __global__ void k_add_ragent(const float4* __restrict__ raw, float4* __restrict__ eff, int n, int n_fill, float r_agent) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_fill) return;
@@ -758,8 +760,9 @@ extern "C" gmapp_status gmapp_replan(gmapp_ctx* c, gmapp_kind kind, float* d_age
     if (prev_best >= n_agents) return fail(c, GMAPP_EINVAL, "replan: prev_best out of range%s");
     cudaStream_t st = (cudaStream_t)stream;
     const int w = kind == GMAPP_POINT3 ? 6 : 14;
-    const int pb = prev_best < 0 ? -1 : prev_best;
-    CUDA_TRY(c, cudaMemcpyAsync(c->d_prev, &pb, sizeof(int), cudaMemcpyHostToDevice, st));   // pageable 4-byte copy: staged by the runtime
+    // the incumbent goes to the device by a tiny kernel argument, not a host copy, so the whole call can be captured
+    // in a CUDA graph and replayed
+    k_set_int<<<1, 1, 0, st>>>(c->d_prev, prev_best < 0 ? -1 : prev_best);
     gmapp_status s = GMAPP_OK;
     int launches = 0;
     for (int cyc = 0; cyc < n_cycles && s == GMAPP_OK; ++cyc) {

@@ -464,6 +464,38 @@ def test_replan_closed_loop_matches_oracle_composition(api, ctx, orc, moving):
     assert len(set(g_best.tolist())) >= 1 and g_best.min() >= 0
 
 
+def test_replan_is_capturable_in_a_cuda_graph(api, ctx):
+    """The whole closed loop (n cycles of rollout, selection, restart) as ONE CUDA graph: replays reproduce the
+    directly launched result bit for bit."""
+    import torch
+    sc = scenes.config3(n_agents=300)
+    ctx.set_obstacles(_tensor(sc.xyzr), None, n=sc.n_spheres)
+    start = _tensor(np.tile(sc.agents[0], (sc.n_agents, 1)))
+    rd = np.where(np.arange(sc.n_agents) % 2 == 0, 0.2, 0.1).astype(np.float32)
+    try:
+        ctx.set_agent_params(r_influence=rd)
+        def run(agents, path, best):
+            ctx.replan(api.GMAPP_POINT3, agents, sc.goal, sc.gains, sc.dt, 40, 10, 4, d_path_out=path, d_best_out=best)
+        a0 = start.clone(); p0 = torch.zeros((4, 6), device="cuda:0"); b0 = torch.zeros(4, dtype=torch.int32, device="cuda:0")
+        run(a0, p0, b0); torch.cuda.synchronize()
+        a1 = start.clone(); p1 = torch.zeros_like(p0); b1 = torch.zeros_like(b0)
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            run(a1, p1, b1)                                   # warm-up on the capture stream
+            side.synchronize()
+            a1.copy_(start)
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=side):
+                run(a1, p1, b1)
+        for _ in range(2):
+            a1.copy_(start); p1.zero_(); b1.zero_()
+            graph.replay(); torch.cuda.synchronize()
+            assert torch.equal(p1, p0) and torch.equal(b1, b0) and torch.equal(a1, a0)
+    finally:
+        ctx.set_agent_params(n=0)
+
+
 def test_replan_pose6_runs_and_errors(api, ctx, orc):
     import torch
     sc = scenes.config4(n_agents=16, n_spheres=256, steps=30)
