@@ -516,8 +516,9 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
         if (L > 32 && G > 7) return fail(c, GMAPP_EINVAL, "rollout: lanes_per_agent > 32 allows at most 7 groups per CTA, need %s%ld", "", G);
     } else {
         L = pow2_floor(tmax / G);
-        const int cap = pow2_ceil(n2 > 0 ? n2 : 1);               // no more lanes than sphere pairs
-        if (L > cap) L = cap;
+        int cap = pow2_ceil(n2 > 0 ? n2 : 1);                     // no more lanes than sphere pairs ...
+        if (cap < 32 && n2 > 0) cap = 32;                         // ... but a whole warp per group when it fits: the full-warp
+        if (L > cap) L = cap;                                     // reduction beats the sub-warp one even with idle lanes
         if (L > 32 && G > 7) L = 32;                              // two named barriers per multi-warp group
     }
     const int mode = chunked ? 4 : (L >= 64 ? (G <= 4 ? 2 : 3) : (L == 32 ? 1 : 0));
