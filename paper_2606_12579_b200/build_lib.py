@@ -1,4 +1,4 @@
-"""Build libgmapp.so in-tree for sm_100a: six translation units compiled in parallel, then linked.
+"""Build libgmapp.so in-tree for sm_100a: ten translation units compiled in parallel, then linked.
 
 Stand-alone on purpose (no import of the binding: api.py refuses to import while the library is missing):
     python paper_2606_12579_b200/build_lib.py [--force]
@@ -11,7 +11,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_PKG, "csrc")
 _INCLUDE = os.path.join(os.path.dirname(_PKG), "include")
 SO = os.path.join(_PKG, "libgmapp.so")
-TUS = ["gmapp.cu", "gmapp_x2_cf.cu", "gmapp_x2_cf_x.cu", "gmapp_x2_apf.cu", "gmapp_x2_apf_x.cu", "gmapp_wide.cu"]
+TUS = ["gmapp.cu", "gmapp_wide.cu"] + ["gmapp_x2_%s%s%s.cu" % (h, x, m) for m in ("", "_mv") for h in ("cf", "apf") for x in ("", "_x")]
 NVCC = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
         "-diag-suppress", "128"]          # 128: "loop is not reachable" in the if-constant branches of the templates
 

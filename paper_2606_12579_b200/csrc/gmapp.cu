@@ -109,12 +109,16 @@ static rollout_fn rollout_kernel(int kind, int at, bool moving, bool cull, int s
 #undef PICK
 }
 static const int kX2SweepThreads = 512;       // sweep threads per CTA; mode 2 adds one epilogue warp per group (<= 672 in all)
-static rollout_x2_fn rollout_x2_kernel(int at, int mode, bool cull, int stage, bool apf, bool extras) {
+static rollout_x2_fn rollout_x2_kernel(int at, int mode, bool cull, int stage, bool apf, bool extras, bool moving) {
+    if (moving) {
+        if (extras) return apf ? gmapp::rollout_x2_kernel_apf_x_mv(at, mode, cull, stage) : gmapp::rollout_x2_kernel_cf_x_mv(at, mode, cull, stage);
+        return apf ? gmapp::rollout_x2_kernel_apf_mv(at, mode, cull, stage) : gmapp::rollout_x2_kernel_cf_mv(at, mode, cull, stage);
+    }
     if (extras) return apf ? gmapp::rollout_x2_kernel_apf_x(at, mode, cull, stage) : gmapp::rollout_x2_kernel_cf_x(at, mode, cull, stage);
     return apf ? gmapp::rollout_x2_kernel_apf(at, mode, cull, stage) : gmapp::rollout_x2_kernel_cf(at, mode, cull, stage);
 }
-static rollout_fn rollout_wide_kernel(int kind, int at, bool moving, bool cull, int stage, bool apf) {
-    return gmapp::rollout_wide_kernel_tu(kind, at, moving, cull, stage, apf);
+static rollout_fn rollout_wide_kernel(bool moving, bool cull, int stage, bool apf) {
+    return gmapp::rollout_wide_kernel_tu(moving, cull, stage, apf);
 }
 static int rollout_max_threads(int kind, int at) { return (kind == GMAPP_MOTOR6 || at == 2) ? 512 : 1024; }
 
@@ -185,19 +189,17 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
                                                  cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
                         if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
                     }
-    for (int kind = 0; kind < 2; ++kind)
-        for (int at = 1; at <= (kind == 0 ? 2 : 1); ++at)
-            for (int mv = (kind == 0 ? 1 : 0); mv < 2; ++mv)
-                for (int cu = 0; cu < 8; ++cu) {
-                    e = cudaFuncSetAttribute((const void*)rollout_wide_kernel(kind, at, mv, cu & 1, (cu >> 1) & 1, (cu >> 2) != 0),
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
-                    if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
-                }
+    for (int mv = 0; mv < 2; ++mv)
+        for (int cu = 0; cu < 8; ++cu) {
+            e = cudaFuncSetAttribute((const void*)rollout_wide_kernel(mv, cu & 1, (cu >> 1) & 1, (cu >> 2) != 0),
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
+            if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
+        }
     for (int at = 1; at <= 2; ++at)
         for (int md = 0; md < 5; ++md)
             for (int cu = 0; cu < 4; ++cu)
-                for (int hf = 0; hf < 4; ++hf) {
-                    e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, md, cu & 1, cu >> 1, (hf & 1) != 0, (hf >> 1) != 0),
+                for (int hf = 0; hf < 8; ++hf) {
+                    e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, md, cu & 1, cu >> 1, (hf & 1) != 0, (hf & 2) != 0, (hf & 4) != 0),
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
                     if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
                 }
@@ -487,7 +489,7 @@ static gmapp_status choose_launch(gmapp_ctx* c, int kind, int n_agents, LaunchCf
 
 
 // ---------------------------------------------------------------------------------------------
-// packed f32x2 rollout (POINT3, static spheres): launch selection + launch
+// packed f32x2 rollout (POINT3, static or moving spheres): launch selection + launch
 // ---------------------------------------------------------------------------------------------
 static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float* d_agents_out, int n_agents,
                                       const float* goal, const gmapp_gains* g, float dt, int steps, cudaStream_t st) {
@@ -527,7 +529,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     // dynamic shared memory: [0,64) mbarrier; [64, 64+4 KB) cross-warp exchange; sphere-pair tile at 4224
     const int xch_off = 64, rec_off = 4224;
     const int tile_off = rec_off + (chunked ? round_up(A * 24 * 4, 128) : 0);      // mode 4: 24-word state record per agent
-    const size_t tile_bytes = (size_t)n2p * 32;
+    const size_t tile_bytes = (size_t)n2p * (c->moving ? 64 : 32);       // pair arrays A, B (+ U, V when the spheres move)
     const bool fits = tile_off + tile_bytes <= (size_t)c->smem_optin;
     int stage = fits ? 1 : 0;
     if (t && t->stage >= 0) {
@@ -546,7 +548,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     P.L = L; P.logL = ilog2(L);
     P.steps = steps;
     for (int i = 0; i < 3; ++i) P.goal[i] = goal[i];
-    P.dt = dt;
+    P.dt = dt; P.t0 = c->roll_t0;
     P.k_circ = g->k_circ; P.k_att = g->k_att; P.k_damp = g->k_damp;
     P.c_lin = g->vel_factor * dt * g->inv_mass;
     P.inv_mass = g->inv_mass; P.vel_factor = g->vel_factor;
@@ -566,7 +568,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     const int block = mode == 4 ? tmax : (mode >= 2 ? G * L + 32 * G : round_up(G * L, 32));
     const int smem = tile_off + (stage == 1 ? (int)tile_bytes : 0);
     P.stage = stage;
-    rollout_x2_fn fn = rollout_x2_kernel(at, mode, cull != 0, stage, g->heuristic == 1, P.snap_out != nullptr || P.traj_out != nullptr);
+    rollout_x2_fn fn = rollout_x2_kernel(at, mode, cull != 0, stage, g->heuristic == 1, P.snap_out != nullptr || P.traj_out != nullptr, c->moving);
     fn<<<grid, block, smem, st>>>(P);
     CUDA_TRY(c, cudaGetLastError());
     ++launches;
@@ -643,7 +645,7 @@ static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_ag
                                 const float* goal, const gmapp_gains* g, float dt, int steps, cudaStream_t stream) {
     gmapp_status s;
     const int ng = kind == GMAPP_POINT3 ? 3 : 8;
-    if (kind == GMAPP_POINT3 && !c->moving && !(c->has_tuning && c->tuning.scalar_path))
+    if (kind == GMAPP_POINT3 && !(c->has_tuning && c->tuning.scalar_path))
         return launch_rollout_x2(c, d_agents, d_agents_out, n_agents, goal, g, dt, steps, (cudaStream_t)stream);
     LaunchCfg cfg;
     s = choose_launch(c, kind, n_agents, &cfg);
@@ -684,11 +686,11 @@ static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_ag
     // few agents per CTA and many lanes per agent: sweep warps + one epilogue warp per group (gmapp_rollout_wide.cuh)
     const bool scalar_forced = c->has_tuning && c->tuning.scalar_path;
     const int n2 = (c->n_spheres + 1) / 2;
-    bool wide = !scalar_forced && (kind == GMAPP_MOTOR6 || c->moving) && cfg.groups <= 4 && cfg.L >= 64 && n2 >= 64;
+    bool wide = !scalar_forced && kind == GMAPP_MOTOR6 && cfg.groups <= 4 && cfg.L >= 64 && n2 >= 64;
     if (wide) {
         while (cfg.groups * cfg.L > 512 || cfg.L > pow2_ceil(n2)) cfg.L >>= 1;
         P.L = cfg.L; P.logL = ilog2(cfg.L);
-        P.two_warp_epi = (kind == GMAPP_MOTOR6 && cfg.groups <= 3) ? 1 : 0;
+        P.two_warp_epi = cfg.groups <= 3 ? 1 : 0;
         cfg.block = cfg.groups * cfg.L + (P.two_warp_epi ? 64 : 32) * cfg.groups;
         s = effective_pairs(c, g->r_agent, st, &launches);
         if (s != GMAPP_OK) return s;
@@ -699,7 +701,7 @@ static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_ag
         cfg.smem = cfg.tile_off + (cfg.stage == 1 ? (int)tile_bytes : 0);
     }
     P.stage = cfg.stage;
-    rollout_fn fn = wide ? rollout_wide_kernel(kind, cfg.at, c->moving, cfg.cull != 0, cfg.stage, g->heuristic == 1)
+    rollout_fn fn = wide ? rollout_wide_kernel(c->moving, cfg.cull != 0, cfg.stage, g->heuristic == 1)
                          : rollout_kernel(kind, cfg.at, c->moving, cfg.cull != 0, cfg.stage);
     fn<<<cfg.grid, cfg.block, cfg.smem, st>>>(P);
     CUDA_TRY(c, cudaGetLastError());

@@ -29,81 +29,6 @@ __device__ __forceinline__ void warp_combine(const StaticAcc<NA>& acc, int lane,
 }
 
 // ---------------------------------------------------------------------------------------------
-// packed f32x2 sweep for MOVING spheres.  Sphere pairs: A = (cx0,cx1,cy0,cy1), B = (cz0,cz1,-R0,-R1) at t = 0,
-// U = (ux0,ux1,uy0,uy1), V = (uz0,uz1,0,0).  Per pair (reading G5/G25): c(t) = c + t u, v_rel = v - u,
-// f_j = w [ (s/|v_rel|) v_rel - |v_rel| d ],  w = s / (d_O |d|^2),  s = d.v_rel, accumulated directly
-// (k_f applied after the sum).  The distance half is the static one.
-// ---------------------------------------------------------------------------------------------
-template <int NA, bool FORCE, bool CULL, bool APF = false, class RD = RdSel<NA, false>>
-__device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, const float4* __restrict__ tB,
-                                                const float4* __restrict__ tU, const float4* __restrict__ tV, int n2p,
-                                                int lane, int L, float tk, const float (&p)[NA][3], const float (&v)[NA][3],
-                                                const RD& rd, float eps, unsigned mask, X2Acc<NA>& acc) {
-    const u64 tiny = bc2(kTiny), half = bc2(0.5f), t2 = bc2(tk);
-#pragma unroll 2
-    for (int j = lane; j < n2p; j += L) {
-        const float4 s0 = tA[j], s1 = tB[j], s2 = tU[j], s3 = tV[j];
-        const u64 ux = pk2(s2.x, s2.y), uy = pk2(s2.z, s2.w), uz = pk2(s3.x, s3.y), nR = pk2(s1.z, s1.w);
-        const u64 cx = fma2(ux, t2, pk2(s0.x, s0.y)), cy = fma2(uy, t2, pk2(s0.z, s0.w)), cz = fma2(uz, t2, pk2(s1.x, s1.y));
-        u64 dx[NA], dy[NA], dz[NA], q[NA], yy[NA];
-        float d0[NA], d1[NA];
-        bool any = false;
-#pragma unroll
-        for (int a = 0; a < NA; ++a) {
-            dx[a] = sub2(cx, bc2(p[a][0])); dy[a] = sub2(cy, bc2(p[a][1])); dz[a] = sub2(cz, bc2(p[a][2]));
-            q[a] = fma2(dx[a], dx[a], fma2(dy[a], dy[a], fma2(dz[a], dz[a], tiny)));
-            float q0, q1; upk2(q[a], q0, q1);
-            const u64 y = pk2(rsqrt_approx(q0), rsqrt_approx(q1));
-            yy[a] = y;
-            const u64 t = mul2(q[a], y);
-            const u64 hy = mul2(y, half);
-            float t0, t1; upk2(t, t0, t1);
-            const u64 e = pk2(fmaf(-t0, t0, q0), fmaf(-t1, t1, q1));
-            const u64 ds = fma2(hy, e, add2(t, nR));
-            upk2(ds, d0[a], d1[a]);
-            acc.dmin[a] = min3f(acc.dmin[a], d0[a], d1[a]);
-            if (CULL) any = any || (fminf(d0[a], d1[a]) <= rd.get(a));
-        }
-        if (!FORCE) continue;
-        if (CULL) { if (!__any_sync(mask, any)) continue; }
-        if (APF) {                                          // Eq. 1 depends on positions only
-#pragma unroll
-            for (int a = 0; a < NA; ++a) {
-                float r0 = 0.0f, r1 = 0.0f;
-                if (d0[a] <= rd.get(a)) r0 = rcp_approx(fmaxf(d0[a], eps));
-                if (d1[a] <= rd.get(a)) r1 = rcp_approx(fmaxf(d1[a], eps));
-                const u64 ro = pk2(r0, r1);
-                const u64 m = mul2(mul2(sub2(bc2(rcp_approx(rd.get(a))), ro), mul2(ro, ro)), yy[a]);
-                acc.bx[a] = fma2(m, dx[a], acc.bx[a]);
-                acc.by[a] = fma2(m, dy[a], acc.by[a]);
-                acc.bz[a] = fma2(m, dz[a], acc.bz[a]);
-            }
-            continue;
-        }
-#pragma unroll
-        for (int a = 0; a < NA; ++a) {
-            const u64 vx = sub2(bc2(v[a][0]), ux), vy = sub2(bc2(v[a][1]), uy), vz = sub2(bc2(v[a][2]), uz);
-            const u64 n2 = fma2(vx, vx, fma2(vy, vy, fma2(vz, vz, tiny)));
-            float m0, m1; upk2(n2, m0, m1);
-            const float i0 = rsqrt_approx(m0), i1 = rsqrt_approx(m1);
-            const u64 inv = pk2(i0, i1), ninv = pk2(-i0, -i1);
-            const u64 nvn = mul2(n2, ninv);                                              // -|v_rel|
-            const u64 den = mul2(pk2(fmaxf(d0[a], eps), fmaxf(d1[a], eps)), q[a]);
-            float n0, n1; upk2(den, n0, n1);
-            float r0 = 0.0f, r1 = 0.0f;
-            if (d0[a] <= rd.get(a)) r0 = rcp_approx(n0);
-            if (d1[a] <= rd.get(a)) r1 = rcp_approx(n1);
-            const u64 s = fma2(dx[a], vx, fma2(dy[a], vy, mul2(dz[a], vz)));
-            const u64 w = mul2(s, pk2(r0, r1));
-            const u64 c1 = mul2(mul2(w, s), inv), c2 = mul2(w, nvn);
-            acc.bx[a] = fma2(c1, vx, fma2(c2, dx[a], acc.bx[a]));
-            acc.by[a] = fma2(c1, vy, fma2(c2, dy[a], acc.by[a]));
-            acc.bz[a] = fma2(c1, vz, fma2(c2, dz[a], acc.bz[a]));
-        }
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
 // epilogue-side agent models.  Interface: init, pre (no sums needed), post (sums known -> new state, pub[6] =
 // position and WORLD linear velocity for the sweep warps), costs, finish.
 // ---------------------------------------------------------------------------------------------

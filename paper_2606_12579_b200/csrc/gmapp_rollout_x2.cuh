@@ -78,6 +78,7 @@ struct RolloutX2Params {
     int xch_off;              // byte offset of the cross-warp exchange area
     int rec_off;              // byte offset of the per-agent state records (mode 4)
     int stage;                // 1: sphere pairs staged in shared memory by TMA bulk copies; 0: read through L1/L2
+    float t0;                 // moving spheres: obstacles are evaluated at t0 + k dt (pair arrays U, V behind A, B)
     int apf;                  // 1: APF heuristic (Eq. 1) instead of the circular field (Eq. 2-3)
     // heterogeneous ensemble (gmapp_set_agent_params): all nullable
     const int* agent_idx;     // [n_agents] this launch's agents as indices into the caller's arrays (one launch per heuristic)
@@ -179,6 +180,90 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
             acc.bz[a] = fma2(w, dz[a], acc.bz[a]);
         }
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// packed f32x2 sweep for MOVING spheres.  Sphere pairs: A = (cx0,cx1,cy0,cy1), B = (cz0,cz1,-R0,-R1) at t = 0,
+// U = (ux0,ux1,uy0,uy1), V = (uz0,uz1,0,0).  Per pair (reading G5/G25): c(t) = c + t u, v_rel = v - u,
+// f_j = w [ (s/|v_rel|) v_rel - |v_rel| d ],  w = s / (d_O |d|^2),  s = d.v_rel, accumulated directly
+// (k_f applied after the sum).  The distance half is the static one.
+// ---------------------------------------------------------------------------------------------
+template <int NA, bool FORCE, bool CULL, bool APF = false, class RD = RdSel<NA, false>>
+__device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, const float4* __restrict__ tB,
+                                                const float4* __restrict__ tU, const float4* __restrict__ tV, int n2p,
+                                                int lane, int L, float tk, const float (&p)[NA][3], const float (&v)[NA][3],
+                                                const RD& rd, float eps, unsigned mask, X2Acc<NA>& acc) {
+    const u64 tiny = bc2(kTiny), half = bc2(0.5f), t2 = bc2(tk);
+#pragma unroll 2
+    for (int j = lane; j < n2p; j += L) {
+        const float4 s0 = tA[j], s1 = tB[j], s2 = tU[j], s3 = tV[j];
+        const u64 ux = pk2(s2.x, s2.y), uy = pk2(s2.z, s2.w), uz = pk2(s3.x, s3.y), nR = pk2(s1.z, s1.w);
+        const u64 cx = fma2(ux, t2, pk2(s0.x, s0.y)), cy = fma2(uy, t2, pk2(s0.z, s0.w)), cz = fma2(uz, t2, pk2(s1.x, s1.y));
+        u64 dx[NA], dy[NA], dz[NA], q[NA], yy[NA];
+        float d0[NA], d1[NA];
+        bool any = false;
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            dx[a] = sub2(cx, bc2(p[a][0])); dy[a] = sub2(cy, bc2(p[a][1])); dz[a] = sub2(cz, bc2(p[a][2]));
+            q[a] = fma2(dx[a], dx[a], fma2(dy[a], dy[a], fma2(dz[a], dz[a], tiny)));
+            float q0, q1; upk2(q[a], q0, q1);
+            const u64 y = pk2(rsqrt_approx(q0), rsqrt_approx(q1));
+            yy[a] = y;
+            const u64 t = mul2(q[a], y);
+            const u64 hy = mul2(y, half);
+            float t0, t1; upk2(t, t0, t1);
+            const u64 e = pk2(fmaf(-t0, t0, q0), fmaf(-t1, t1, q1));
+            const u64 ds = fma2(hy, e, add2(t, nR));
+            upk2(ds, d0[a], d1[a]);
+            acc.dmin[a] = min3f(acc.dmin[a], d0[a], d1[a]);
+            if (CULL) any = any || (fminf(d0[a], d1[a]) <= rd.get(a));
+        }
+        if (!FORCE) continue;
+        if (CULL) { if (!__any_sync(mask, any)) continue; }
+        if (APF) {                                          // Eq. 1 depends on positions only
+#pragma unroll
+            for (int a = 0; a < NA; ++a) {
+                float r0 = 0.0f, r1 = 0.0f;
+                if (d0[a] <= rd.get(a)) r0 = rcp_approx(fmaxf(d0[a], eps));
+                if (d1[a] <= rd.get(a)) r1 = rcp_approx(fmaxf(d1[a], eps));
+                const u64 ro = pk2(r0, r1);
+                const u64 m = mul2(mul2(sub2(bc2(rcp_approx(rd.get(a))), ro), mul2(ro, ro)), yy[a]);
+                acc.bx[a] = fma2(m, dx[a], acc.bx[a]);
+                acc.by[a] = fma2(m, dy[a], acc.by[a]);
+                acc.bz[a] = fma2(m, dz[a], acc.bz[a]);
+            }
+            continue;
+        }
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            const u64 vx = sub2(bc2(v[a][0]), ux), vy = sub2(bc2(v[a][1]), uy), vz = sub2(bc2(v[a][2]), uz);
+            const u64 n2 = fma2(vx, vx, fma2(vy, vy, fma2(vz, vz, tiny)));
+            float m0, m1; upk2(n2, m0, m1);
+            const float i0 = rsqrt_approx(m0), i1 = rsqrt_approx(m1);
+            const u64 inv = pk2(i0, i1), ninv = pk2(-i0, -i1);
+            const u64 nvn = mul2(n2, ninv);                                              // -|v_rel|
+            const u64 den = mul2(pk2(fmaxf(d0[a], eps), fmaxf(d1[a], eps)), q[a]);
+            float n0, n1; upk2(den, n0, n1);
+            float r0 = 0.0f, r1 = 0.0f;
+            if (d0[a] <= rd.get(a)) r0 = rcp_approx(n0);
+            if (d1[a] <= rd.get(a)) r1 = rcp_approx(n1);
+            const u64 s = fma2(dx[a], vx, fma2(dy[a], vy, mul2(dz[a], vz)));
+            const u64 w = mul2(s, pk2(r0, r1));
+            const u64 c1 = mul2(mul2(w, s), inv), c2 = mul2(w, nvn);
+            acc.bx[a] = fma2(c1, vx, fma2(c2, dx[a], acc.bx[a]));
+            acc.by[a] = fma2(c1, vy, fma2(c2, dy[a], acc.by[a]));
+            acc.bz[a] = fma2(c1, vz, fma2(c2, dz[a], acc.bz[a]));
+        }
+    }
+}
+
+// One entry point for both sweeps.  The pair arrays sit at equal distances: B = A + d, U = A + 2 d, V = A + 3 d.
+template <int NA, bool FORCE, bool CULL, bool APF, bool MV, class RD>
+__device__ __forceinline__ void sweep_any(const float4* __restrict__ tA, const float4* __restrict__ tB, int n2p, int lane, int L,
+                                          float tk, const float (&p)[NA][3], const float (&v)[NA][3], const RD& rd, float eps,
+                                          unsigned mask, X2Acc<NA>& acc) {
+    if (MV) sweep_x2_moving<NA, FORCE, CULL, APF>(tA, tB, tB + (tB - tA), tB + 2 * (tB - tA), n2p, lane, L, tk, p, v, rd, eps, mask, acc);
+    else    sweep_x2<NA, FORCE, CULL, APF>(tA, tB, n2p, lane, L, p, v, rd, eps, mask, acc);
 }
 
 // Transposed butterfly over a full warp.  In: per-lane partial (x,y,z) of NA agents.  Out: every lane of
@@ -349,7 +434,7 @@ __device__ __forceinline__ void warp_combine(const X2Acc<NA>& acc, int lane, flo
 // ---------------------------------------------------------------------------------------------
 // group body, L == 32: one warp per group does everything; agent a on lanes 0-15, agent b on lanes 16-31
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL, bool APF, bool PER, bool XT>
+template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
 __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                    int first_agent, int lane) {
     const int half = (NA == 2) ? (lane >> 4) : 0;
@@ -363,6 +448,7 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
     X2Acc<NA> acc;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);                  // pose S+1: distance-only pass
+        const float tk = fmaf(float(k), P.dt, P.t0);       // obstacle time (moving spheres)
         if (NA == 2) {
 #pragma unroll
             for (int i = 0; i < 3; ++i) {
@@ -374,8 +460,8 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
             for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
         }
         acc.clear();
-        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, n2p, lane, 32, p, v, rd, P.eps, full, acc);
-        else       sweep_x2<NA, false, false>(tA, tB, n2p, lane, 32, p, v, rd, P.eps, full, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p, lane, 32, tk, p, v, rd, P.eps, full, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p, lane, 32, tk, p, v, rd, P.eps, full, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
         if (last) {
@@ -384,7 +470,7 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
         }
         float fx, fy, fz;
         me.pre(P);
-        me.template post<APF>(P, X, Y, Z, fx, fy, fz);
+        me.template post<(APF || MV)>(P, X, Y, Z, fx, fy, fz);
         me.costs(P, k, D, fx, fy, fz);
         if ((lane & 15) == 0 && (NA == 2 || lane == 0)) { if (XT) me.snapshot(P, k); }
     }
@@ -411,7 +497,7 @@ __device__ __forceinline__ void agent_load(AgentX2& a, const float* r) {
     a.gid = __float_as_int(r[20]); a.rd = r[21]; a.kf = r[22];
 }
 
-template <int NA, bool CULL, bool APF, bool PER, bool XT>
+template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
 __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p, int agent0,
                                            int lane, int k, float* rec0) {
     const int half = (NA == 2) ? (lane >> 4) : 0;
@@ -434,10 +520,11 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
         rd.v[0] = me.rd;
     }
     const bool last = (k == P.steps);
+    const float tk = fmaf(float(k), P.dt, P.t0);
     X2Acc<NA> acc;
     acc.clear();
-    if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, n2p, lane, 32, p, v, rd, P.eps, full, acc);
-    else       sweep_x2<NA, false, false>(tA, tB, n2p, lane, 32, p, v, rd, P.eps, full, acc);
+    if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p, lane, 32, tk, p, v, rd, P.eps, full, acc);
+    else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p, lane, 32, tk, p, v, rd, P.eps, full, acc);
     float X, Y, Z, D;
     warp_combine<NA>(acc, lane, X, Y, Z, D);
     const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
@@ -447,7 +534,7 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     }
     float fx, fy, fz;
     me.pre(P);
-    me.template post<APF>(P, X, Y, Z, fx, fy, fz);
+    me.template post<(APF || MV)>(P, X, Y, Z, fx, fy, fz);
     me.costs(P, k, D, fx, fy, fz);
     if (writer) { if (XT) me.snapshot(P, k); }
     __syncwarp();                                         // every lane has read the record before it is rewritten
@@ -455,7 +542,7 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     __syncwarp();
 }
 
-template <bool CULL, bool APF, bool PER, bool XT>
+template <bool CULL, bool APF, bool PER, bool XT, bool MV>
 __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                     int first_agent, int n_mine, int lane, float* recs) {
     // records of this warp's agents: recs[i * kAgentRecWords], i < n_mine
@@ -467,8 +554,8 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
     __syncwarp();
     for (int k = 0; k <= P.steps; ++k) {
         int i = 0;
-        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL, APF, PER, XT>(P, tA, tB, n2p, first_agent + i, lane, k, recs + i * kAgentRecWords);
-        if (i < n_mine) chunk_step<1, CULL, APF, PER, XT>(P, tA, tB, n2p, first_agent + i, lane, k, recs + i * kAgentRecWords);
+        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL, APF, PER, XT, MV>(P, tA, tB, n2p, first_agent + i, lane, k, recs + i * kAgentRecWords);
+        if (i < n_mine) chunk_step<1, CULL, APF, PER, XT, MV>(P, tA, tB, n2p, first_agent + i, lane, k, recs + i * kAgentRecWords);
     }
 }
 
@@ -479,7 +566,7 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
 //   sweep warp k:    write part[k&1] -> arrive(bar_part) -> sync(bar_state) -> read state[k&1]
 //   epilogue warp k: sync(bar_part) -> read part[k&1] -> integrate -> write state[k&1] -> arrive(bar_state) -> costs
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL, bool APF, bool PER>
+template <int NA, bool CULL, bool APF, bool PER, bool MV>
 __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                   int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
     const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
@@ -501,9 +588,10 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
     X2Acc<NA> acc;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
+        const float tk = fmaf(float(k), P.dt, P.t0);
         acc.clear();
-        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
-        else       sweep_x2<NA, false, false>(tA, tB, n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
         const int par = k & 1;
@@ -519,7 +607,7 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
     }
 }
 
-template <int NA, bool APF, bool XT>
+template <int NA, bool APF, bool XT>   // APF here = "the sums are the force itself" (APF heuristic or moving spheres)
 __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, int first_agent, int lane,
                                                     int group_in_cta, float4* xch) {
     const int W = P.L >> 5;
@@ -558,7 +646,7 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
 // ---------------------------------------------------------------------------------------------
 // group body, L < 32 (several groups per warp): plain butterfly, every lane integrates its group's agents
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL, bool APF, bool PER, bool XT>
+template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
 __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                      int first_agent, int lane_in_group) {
     const unsigned mask = __activemask();
@@ -570,13 +658,14 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
     X2Acc<NA> acc;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
+        const float tk = fmaf(float(k), P.dt, P.t0);
 #pragma unroll
         for (int a = 0; a < NA; ++a)
 #pragma unroll
             for (int i = 0; i < 3; ++i) { p[a][i] = ag[a].p[i]; v[a][i] = ag[a].v[i]; }
         acc.clear();
-        if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, n2p, lane_in_group, P.L, p, v, rd, P.eps, mask, acc);
-        else       sweep_x2<NA, false, false>(tA, tB, n2p, lane_in_group, P.L, p, v, rd, P.eps, mask, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
         float x[NA], y[NA], z[NA], dm[NA];
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
@@ -592,7 +681,7 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
             if (last) { if (lane_in_group == 0) ag[a].finish(P, dm[a]); continue; }
             float fx, fy, fz;
             ag[a].pre(P);
-            ag[a].template post<APF>(P, x[a], y[a], z[a], fx, fy, fz);
+            ag[a].template post<(APF || MV)>(P, x[a], y[a], z[a], fx, fy, fz);
             ag[a].costs(P, k, dm[a], fx, fy, fz);
             if (lane_in_group == 0) { if (XT) ag[a].snapshot(P, k); }
         }
@@ -609,7 +698,7 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 // choice the tile pointers become generic and every LDS turns into a generic LD, measured 10 % slower)
 // XT = extras: the state snapshot of gmapp_replan and the trajectory output (kept out of the plain kernels: the few
 // extra stores in the epilogue perturb the register allocation of the sweep warps by 3 %)
-template <int AT, int MODE, bool CULL, int STAGE, int MAXT, bool APF, bool XT>
+template <int AT, int MODE, bool CULL, int STAGE, int MAXT, bool APF, bool XT, bool MV>
 __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ RolloutX2Params P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
@@ -627,12 +716,15 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         __syncthreads();
         if (tid == 0 && n2p > 0) {
             const uint32_t bytes = uint32_t(n2p) * 16u;
-            mbar_arrive_expect_tx(bar, 2u * bytes);
+            constexpr int NARR = MV ? 4 : 2;                // pair arrays A, B (, U, V), equally spaced in global memory
+            mbar_arrive_expect_tx(bar, NARR * bytes);
             const uint32_t chunk = 32768u;
-            for (uint32_t o = 0; o < bytes; o += chunk) {
-                const uint32_t nb = bytes - o < chunk ? bytes - o : chunk;
-                tma_bulk_g2s(reinterpret_cast<unsigned char*>(tile) + o, reinterpret_cast<const unsigned char*>(P.pairA) + o, nb, bar);
-                tma_bulk_g2s(reinterpret_cast<unsigned char*>(tile) + bytes + o, reinterpret_cast<const unsigned char*>(P.pairB) + o, nb, bar);
+            for (int r = 0; r < NARR; ++r) {
+                const unsigned char* src = reinterpret_cast<const unsigned char*>(P.pairA + size_t(r) * (P.pairB - P.pairA));
+                for (uint32_t o = 0; o < bytes; o += chunk) {
+                    const uint32_t nb = bytes - o < chunk ? bytes - o : chunk;
+                    tma_bulk_g2s(reinterpret_cast<unsigned char*>(tile) + r * bytes + o, src + o, nb, bar);
+                }
             }
         }
         tA = tile;
@@ -653,15 +745,15 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         float4* xch = reinterpret_cast<float4*>(smem_raw + P.xch_off) + group_in_cta * (2 * W * 2 + 2 * 2 * 2);
         if (is_epi) {                                      // the epilogue warps never touch the sphere tile
             if (na <= 0) return;
-            if (AT == 2 && na >= 2) group_epilogue_warp<NA2, APF, XT>(P, first, tid & 31, group_in_cta, xch);
-            else group_epilogue_warp<1, APF, XT>(P, first, tid & 31, group_in_cta, xch);
+            if (AT == 2 && na >= 2) group_epilogue_warp<NA2, (APF || MV), XT>(P, first, tid & 31, group_in_cta, xch);
+            else group_epilogue_warp<1, (APF || MV), XT>(P, first, tid & 31, group_in_cta, xch);
             return;
         }
         if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
         if (na <= 0) return;
         const int lane_in_group = tid & (P.L - 1);
-        if (AT == 2 && na >= 2) { if (P.rd_arr) group_sweep_warps<NA2, CULL, APF, true>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<NA2, CULL, APF, false>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); }
-        else { if (P.rd_arr) group_sweep_warps<1, CULL, APF, true>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<1, CULL, APF, false>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); }
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_sweep_warps<NA2, CULL, APF, true, MV>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<NA2, CULL, APF, false, MV>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); }
+        else { if (P.rd_arr) group_sweep_warps<1, CULL, APF, true, MV>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<1, CULL, APF, false, MV>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); }
         return;
     }
     if (MODE == 4) {
@@ -672,7 +764,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
         if (n_mine <= 0) return;
         float* recs = reinterpret_cast<float*>(smem_raw + P.rec_off) + start * kAgentRecWords;
-        { if (P.rd_arr) warp_rollout_chunks<CULL, APF, true, XT>(P, tA, tB, n2p, cta_first + start, n_mine, tid & 31, recs); else warp_rollout_chunks<CULL, APF, false, XT>(P, tA, tB, n2p, cta_first + start, n_mine, tid & 31, recs); }
+        { if (P.rd_arr) warp_rollout_chunks<CULL, APF, true, XT, MV>(P, tA, tB, n2p, cta_first + start, n_mine, tid & 31, recs); else warp_rollout_chunks<CULL, APF, false, XT, MV>(P, tA, tB, n2p, cta_first + start, n_mine, tid & 31, recs); }
         return;
     }
     const int group_in_cta = tid >> P.logL;
@@ -682,11 +774,11 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
     if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
     if (na <= 0) return;
     if (MODE == 1) {
-        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_warp<NA2, CULL, APF, true, XT>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_warp<NA2, CULL, APF, false, XT>(P, tA, tB, n2p, first, lane_in_group); }
-        else { if (P.rd_arr) group_rollout_warp<1, CULL, APF, true, XT>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_warp<1, CULL, APF, false, XT>(P, tA, tB, n2p, first, lane_in_group); }
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_warp<NA2, CULL, APF, true, XT, MV>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_warp<NA2, CULL, APF, false, XT, MV>(P, tA, tB, n2p, first, lane_in_group); }
+        else { if (P.rd_arr) group_rollout_warp<1, CULL, APF, true, XT, MV>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_warp<1, CULL, APF, false, XT, MV>(P, tA, tB, n2p, first, lane_in_group); }
     } else {
-        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_narrow<NA2, CULL, APF, true, XT>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_narrow<NA2, CULL, APF, false, XT>(P, tA, tB, n2p, first, lane_in_group); }
-        else { if (P.rd_arr) group_rollout_narrow<1, CULL, APF, true, XT>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_narrow<1, CULL, APF, false, XT>(P, tA, tB, n2p, first, lane_in_group); }
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_narrow<NA2, CULL, APF, true, XT, MV>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_narrow<NA2, CULL, APF, false, XT, MV>(P, tA, tB, n2p, first, lane_in_group); }
+        else { if (P.rd_arr) group_rollout_narrow<1, CULL, APF, true, XT, MV>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_narrow<1, CULL, APF, false, XT, MV>(P, tA, tB, n2p, first, lane_in_group); }
     }
 }
 

@@ -295,7 +295,7 @@ def _apf(scene, k=1e-4):
 def test_apf_rollout_point3(api, ctx, orc, moving):
     sc = _apf(scenes.fast_clutter(moving=moving))
     g, o = _check_rollout(api, ctx, orc, sc)
-    assert g["info"]["packed_x2"] == (0 if moving else 1)
+    assert g["info"]["packed_x2"] == 1          # point agents take the packed kernels, moving spheres too
     # the heuristic really changes the motion (guards against a silently ignored flag)
     base = api.run_scene(ctx, scenes.fast_clutter(moving=moving))
     assert np.abs(base["final"] - g["final"]).max() > 1e-3
