@@ -84,9 +84,9 @@ typedef struct {
                                     1 = stage the whole sphere set in shared memory by TMA bulk copies
                                     (EINVAL when it does not fit)                                             */
     int32_t max_ctas;            /* 0 = SM count; cap on the grid (for scaling experiments)           */
-    int32_t scalar_path;         /* 0 = packed f32x2 kernels where they apply (POINT3 over static spheres in every
-                                    shape; moving spheres and MOTOR6 agents when a group spans >= 64 lanes and
-                                    there are <= 4 groups per CTA); 1 = force the scalar FP32 kernel (A/B)    */
+    int32_t scalar_path;         /* 0 = packed f32x2 kernels where they apply (POINT3 in every shape, static and
+                                    moving spheres; MOTOR6 agents when a group spans >= 64 lanes and there
+                                    are <= 4 groups per CTA); 1 = force the scalar FP32 kernel (A/B)    */
     int32_t reserved[2];
 } gmapp_tuning;
 

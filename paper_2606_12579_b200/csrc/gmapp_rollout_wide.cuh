@@ -1,4 +1,4 @@
-// gmapp_rollout_wide.cuh -- rollout kernel for MOVING spheres and 6D motor agents when a group of lanes spans
+// gmapp_rollout_wide.cuh -- rollout kernel for 6D motor agents (static or moving spheres) when a group of lanes spans
 // several warps (L >= 64, <= 4 groups per CTA: the few-agents / many-spheres shape of config 4).
 //
 // Same machine mapping as the multi-warp mode of gmapp_rollout_x2.cuh: W = L/32 sweep warps per group evaluate the

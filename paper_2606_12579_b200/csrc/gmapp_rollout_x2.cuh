@@ -1,5 +1,5 @@
-// gmapp_rollout_x2.cuh -- the packed-FP32 rollout kernel for 3D point agents over static spheres (sm_100a); its sweep,
-// reduction and hand-over pieces are reused by gmapp_rollout_wide.cuh (moving spheres, 6D agents).
+// gmapp_rollout_x2.cuh -- the packed-FP32 rollout kernel for 3D point agents over static or (template flag MV) moving
+// spheres (sm_100a); its sweep, reduction and hand-over pieces are reused by gmapp_rollout_wide.cuh (6D agents).
 //
 // Same method as gmapp_kernels.cuh (Eq. 2-3, 6-11, 16-20 of the paper), different machine mapping:
 //
