@@ -727,10 +727,17 @@ extern "C" gmapp_status gmapp_best_agent_ex(gmapp_ctx* c, float alpha, int prev_
     if (c->last_n_agents < 1) return fail(c, GMAPP_ESTATE, "best_agent: no rollout has run on this context%s");
     if (!isfinite(alpha)) return fail(c, GMAPP_EINVAL, "best_agent: alpha is not finite%s");
     cudaStream_t st = (cudaStream_t)stream;
-    k_best_agent<<<1, 1024, 0, st>>>(c->d_cost, c->d_collided, c->last_n_agents, alpha, prev_best, nullptr, c->d_best_idx, c->d_best_cost);
-    CUDA_TRY(c, cudaGetLastError());
-    CUDA_TRY(c, cudaMemcpyAsync(&c->h_best[0], c->d_best_idx, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(c, cudaMemcpyAsync(&c->h_best[2], c->d_best_cost, sizeof(float), cudaMemcpyDeviceToHost, st));
+    // the kernel writes its 12-byte result straight into pinned host memory (no copy engine round trip) and is
+    // launched with programmatic stream serialisation, so its launch overlaps the tail of the rollout
+    cudaLaunchConfig_t lc;
+    memset(&lc, 0, sizeof lc);
+    lc.gridDim = dim3(1); lc.blockDim = dim3(1024); lc.dynamicSmemBytes = 0; lc.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    lc.attrs = at; lc.numAttrs = 1;
+    CUDA_TRY(c, cudaLaunchKernelEx(&lc, k_best_agent, (const float*)c->d_cost, (const int*)c->d_collided, c->last_n_agents, alpha,
+                                   prev_best, (const int*)nullptr, c->d_best_idx, c->d_best_cost, c->h_best));
     CUDA_TRY(c, cudaStreamSynchronize(st));
     *out_index = c->h_best[0];
     if (out_collided) *out_collided = c->h_best[1];
@@ -775,7 +782,7 @@ extern "C" gmapp_status gmapp_replan(gmapp_ctx* c, gmapp_kind kind, float* d_age
         c->roll_t0 = 0.0f; c->roll_snap = nullptr; c->roll_snap_step = 0;
         if (s != GMAPP_OK) break;
         launches += c->info.kernels_launched;
-        k_best_agent<<<1, 1024, 0, st>>>(c->d_cost, c->d_collided, n_agents, alpha, -1, c->d_prev, c->d_best_idx, c->d_best_cost);
+        k_best_agent<<<1, 1024, 0, st>>>(c->d_cost, c->d_collided, n_agents, alpha, -1, c->d_prev, c->d_best_idx, c->d_best_cost, nullptr);
         k_reseed<<<(n_agents * w + 255) / 256, 256, 0, st>>>(c->d_snap, c->d_best_idx, n_agents, w, d_agents, c->d_prev,
                                                              d_path_out, d_best_out, cyc);
         CUDA_TRY(c, cudaGetLastError());

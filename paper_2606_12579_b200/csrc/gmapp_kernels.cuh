@@ -652,7 +652,10 @@ __device__ __forceinline__ bool key_less(int ca, float Ca, int ia, int cb, float
 // d_prev (nullable): the incumbent is read from device memory (closed-loop re-planning chains cycles without the host)
 __global__ void __launch_bounds__(1024) k_best_agent(const float* __restrict__ cost5, const int* __restrict__ collided,
                                                      int n, float alpha, int prev_best, const int* __restrict__ d_prev,
-                                                     int* out_idx, float* out_cost) {
+                                                     int* out_idx, float* out_cost, int* host_out) {
+    // launched with programmatic stream serialisation behind the rollout (gmapp_best_agent_ex): wait here for its
+    // results; a plain launch returns from this at once
+    cudaGridDependencySynchronize();
     if (d_prev) prev_best = *d_prev;
     // out_idx[0] = winner, out_idx[1] = its collision flag
     __shared__ int s_c[32]; __shared__ float s_C[32]; __shared__ int s_i[32];
@@ -690,6 +693,10 @@ __global__ void __launch_bounds__(1024) k_best_agent(const float* __restrict__ c
             out_idx[0] = n > 0 ? bi : -1;
             out_idx[1] = n > 0 ? bc : 0;
             *out_cost = n > 0 ? bC : __int_as_float(0x7fc00000);
+            if (host_out) {                                  // pinned host memory, read after the stream synchronises
+                host_out[0] = out_idx[0]; host_out[1] = out_idx[1]; host_out[2] = __float_as_int(*out_cost);
+                __threadfence_system();
+            }
         }
     }
 }
