@@ -35,9 +35,6 @@ struct gmapp_ctx {
     float* d_cost = nullptr; float* d_minclr = nullptr; int* d_collided = nullptr;
     int last_n_agents = 0;
     // staging for the *_host entry points
-    float* d_agents_stage = nullptr;     // [max_agents][14]
-    float* d_xyzr_stage = nullptr;       // [max_spheres][4]
-    float* d_vel_stage = nullptr;        // [max_spheres][3]
     float* h_pinned = nullptr;           // spheres*7 + agents*14 floats
     size_t h_pinned_floats = 0;
     // heterogeneous ensemble (gmapp_set_agent_params): per-agent r_d, k_f, and agent indices grouped by heuristic
@@ -157,9 +154,6 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
     ALLOC(c->d_cost, sizeof(float) * 5 * max_agents);
     ALLOC(c->d_minclr, sizeof(float) * max_agents);
     ALLOC(c->d_collided, sizeof(int) * max_agents);
-    ALLOC(c->d_agents_stage, sizeof(float) * 14 * max_agents);
-    ALLOC(c->d_xyzr_stage, sizeof(float) * 4 * c->cap_spheres);
-    ALLOC(c->d_vel_stage, sizeof(float) * 3 * c->cap_spheres);
     ALLOC(c->d_vox_bitmap, sizeof(unsigned) * (1u << 20));
     ALLOC(c->d_vox_sums, sizeof(int) * 1024);
     ALLOC(c->d_vox_count, sizeof(int));
@@ -213,7 +207,6 @@ extern "C" gmapp_status gmapp_destroy(gmapp_ctx* c) {
     cudaDeviceSynchronize();
     cudaFree(c->d_sph_raw); cudaFree(c->d_sph_eff); cudaFree(c->d_svel); cudaFree(c->d_pairA);
     cudaFree(c->d_cost); cudaFree(c->d_minclr); cudaFree(c->d_collided);
-    cudaFree(c->d_agents_stage); cudaFree(c->d_xyzr_stage); cudaFree(c->d_vel_stage);
     cudaFree(c->d_best_idx); cudaFree(c->d_best_cost); cudaFree(c->d_scratch);
     cudaFree(c->d_ap_rd); cudaFree(c->d_ap_kf); cudaFree(c->d_ap_idx); cudaFree(c->d_snap); cudaFree(c->d_prev);
     cudaFree(c->d_vox_bitmap); cudaFree(c->d_vox_sums); cudaFree(c->d_vox_count);
@@ -275,15 +268,16 @@ extern "C" gmapp_status gmapp_set_obstacles(gmapp_ctx* c, const float* d_xyzr, c
     if (n > c->max_spheres) return fail(c, GMAPP_ECAPACITY, "set_obstacles: n = %s%ld exceeds max_spheres = %ld", "", n, c->max_spheres);
     cudaStream_t st = (cudaStream_t)stream;
     const int nf = fill_count(c, n);
-    k_pack_spheres<<<(nf + 255) / 256, 256, 0, st>>>(d_xyzr, d_vel, n, nf, 0.0f, c->d_sph_raw, c->d_svel);
+    // one launch: the float4 sphere array (+ velocities) and the sphere-pair arrays of the packed kernels for
+    // r_agent = 0 (repacked lazily if a rollout asks for another r_agent)
+    k_pack_spheres<<<(nf + 255) / 256, 256, 0, st>>>(d_xyzr, d_vel, n, nf, 0.0f, c->d_sph_raw, c->d_svel, c->d_pairA, c->cap_spheres / 2);
     CUDA_TRY(c, cudaGetLastError());
     c->n_spheres = n;
     c->built_world = false;
     c->moving = (d_vel != nullptr) && n > 0;
     c->eff_valid = false;
-    c->pair_valid = false;
-    // sphere-pair layout of the packed kernels, for r_agent = 0 (repacked lazily if a rollout asks for another r_agent)
-    return effective_pairs(c, 0.0f, st, nullptr);
+    c->pair_valid = true; c->pair_r_agent = 0.0f;
+    return GMAPP_OK;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -348,13 +342,11 @@ extern "C" gmapp_status gmapp_set_obstacles_host(gmapp_ctx* c, const float* h_xy
         // the pinned buffer may still be in flight from an earlier host call on this stream
         CUDA_TRY(c, cudaStreamSynchronize(st));
         memcpy(c->h_pinned, h_xyzr, sizeof(float) * 4 * n);
-        CUDA_TRY(c, cudaMemcpyAsync(c->d_xyzr_stage, c->h_pinned, sizeof(float) * 4 * n, cudaMemcpyHostToDevice, st));
-        if (h_vel) {
-            memcpy(c->h_pinned + 4 * (size_t)n, h_vel, sizeof(float) * 3 * n);
-            CUDA_TRY(c, cudaMemcpyAsync(c->d_vel_stage, c->h_pinned + 4 * (size_t)n, sizeof(float) * 3 * n, cudaMemcpyHostToDevice, st));
-        }
+        if (h_vel) memcpy(c->h_pinned + 4 * (size_t)n, h_vel, sizeof(float) * 3 * n);
     }
-    return gmapp_set_obstacles(c, c->d_xyzr_stage, h_vel ? c->d_vel_stage : nullptr, n, stream);
+    // the packing kernel reads the pinned host buffer itself (unified addressing: one read over the host link instead
+    // of a copy-engine transfer into a staging buffer followed by the same read)
+    return gmapp_set_obstacles(c, c->h_pinned, h_vel ? c->h_pinned + 4 * (size_t)n : nullptr, n, stream);
 }
 
 // sphere array with R = r + r_agent; launches the tiny repack kernel only when r_agent changed
@@ -607,7 +599,7 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
     if (c->roll_traj) {                     // pose 0 of every path = the start state, as given
         const size_t wb = sizeof(float) * (kind == GMAPP_POINT3 ? 6 : 14);
         CUDA_TRY(c, cudaMemcpy2DAsync(c->roll_traj, wb * (size_t)(steps + 1), d_agents, wb, wb, (size_t)n_agents,
-                                      cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+                                      cudaMemcpyDefault, (cudaStream_t)stream));
     }
     if (c->ap_n > 0) {
         // heterogeneous ensemble: one launch per heuristic over that heuristic's agents (the paper runs one
@@ -847,7 +839,6 @@ extern "C" gmapp_status gmapp_plan_cycle_host(gmapp_ctx* c, gmapp_kind kind, con
     if (kind != GMAPP_POINT3 && kind != GMAPP_MOTOR6) return fail(c, GMAPP_EINVAL, "plan_cycle_host: unknown kind%s");
     if (n_agents < 1) return fail(c, GMAPP_EINVAL, "plan_cycle_host: n_agents must be >= 1%s");
     if (n_agents > c->max_agents) return fail(c, GMAPP_ECAPACITY, "plan_cycle_host: n_agents = %s%ld exceeds max_agents = %ld", "", n_agents, c->max_agents);
-    cudaStream_t st = (cudaStream_t)stream;
     gmapp_status s;
     if (h_xyzr || n_spheres == 0) {
         if (h_xyzr || c->n_spheres < 0) {
@@ -859,11 +850,10 @@ extern "C" gmapp_status gmapp_plan_cycle_host(gmapp_ctx* c, gmapp_kind kind, con
     float* hp = c->h_pinned + (size_t)c->cap_spheres * 7;
     // every earlier use of the agent staging area ended with a stream synchronise (this call is synchronous)
     memcpy(hp, h_agents, sizeof(float) * w * (size_t)n_agents);
-    CUDA_TRY(c, cudaMemcpyAsync(c->d_agents_stage, hp, sizeof(float) * w * (size_t)n_agents, cudaMemcpyHostToDevice, st));
-    s = gmapp_rollout(c, kind, c->d_agents_stage, h_agents_out ? c->d_agents_stage : nullptr, n_agents, goal, g, dt, steps, stream);
+    // the rollout reads every start state once and writes every final state once: it does both straight from / to
+    // the pinned host buffer (unified addressing), which saves two copy-engine transfers per cycle
+    s = gmapp_rollout(c, kind, hp, h_agents_out ? hp : nullptr, n_agents, goal, g, dt, steps, stream);
     if (s != GMAPP_OK) return s;
-    if (h_agents_out)
-        CUDA_TRY(c, cudaMemcpyAsync(hp, c->d_agents_stage, sizeof(float) * w * (size_t)n_agents, cudaMemcpyDeviceToHost, st));
     s = gmapp_best_agent(c, alpha, prev_best, out_index, out_cost, stream);     // synchronises
     if (s != GMAPP_OK) return s;
     if (h_agents_out) memcpy(h_agents_out, hp, sizeof(float) * w * (size_t)n_agents);

@@ -626,17 +626,33 @@ __global__ void __launch_bounds__(256) k_forces(const __grid_constant__ ForcePar
 // ---------------------------------------------------------------------------------------------
 // obstacle packing: (xyz, r) [+ vel] -> float4 arrays, R = r + r_a, sentinel padding to n_cap
 // ---------------------------------------------------------------------------------------------
+// When `pairs` is given the same launch also writes the sphere-PAIR arrays of the packed kernels (gmapp_rollout_x2.cuh:
+// A = (cx0,cx1,cy0,cy1), B = (cz0,cz1,-R0,-R1) [, U, V], `stride` float4 apart): even lanes fetch the odd neighbour's
+// sphere by shuffle.  n_cap is even and the block size a multiple of 32, so shuffle partners always exist.
 __global__ void k_pack_spheres(const float* __restrict__ xyzr, const float* __restrict__ vel, int n, int n_cap,
-                               float r_agent, float4* __restrict__ sph, float4* __restrict__ svel) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n_cap) return;
+                               float r_agent, float4* __restrict__ sph, float4* __restrict__ svel,
+                               float4* __restrict__ pairs, int stride) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    // sentinel: far away (|d|^2 ~ 3e36 stays finite in FP32), never gated, never the minimum
+    float4 s = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f), u = make_float4(0, 0, 0, 0);
     if (i < n) {
-        sph[i] = make_float4(xyzr[4 * i], xyzr[4 * i + 1], xyzr[4 * i + 2], xyzr[4 * i + 3] + r_agent);
-        svel[i] = vel ? make_float4(vel[3 * i], vel[3 * i + 1], vel[3 * i + 2], 0.0f) : make_float4(0, 0, 0, 0);
-    } else {
-        // sentinel: far away (|d|^2 ~ 3e36 stays finite in FP32), never gated, never the minimum
-        sph[i] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f);
-        svel[i] = make_float4(0, 0, 0, 0);
+        s = make_float4(xyzr[4 * i], xyzr[4 * i + 1], xyzr[4 * i + 2], xyzr[4 * i + 3] + r_agent);
+        if (vel) u = make_float4(vel[3 * i], vel[3 * i + 1], vel[3 * i + 2], 0.0f);
+    }
+    if (i < n_cap) { sph[i] = s; svel[i] = u; }
+    if (!pairs) return;
+    float4 t, w;
+    t.x = __shfl_down_sync(0xffffffffu, s.x, 1); t.y = __shfl_down_sync(0xffffffffu, s.y, 1);
+    t.z = __shfl_down_sync(0xffffffffu, s.z, 1); t.w = __shfl_down_sync(0xffffffffu, s.w, 1);
+    w.x = __shfl_down_sync(0xffffffffu, u.x, 1); w.y = __shfl_down_sync(0xffffffffu, u.y, 1);
+    w.z = __shfl_down_sync(0xffffffffu, u.z, 1);
+    if ((i & 1) || i >= n_cap) return;
+    const int j = i >> 1;
+    pairs[j] = make_float4(s.x, t.x, s.y, t.y);
+    pairs[stride + j] = make_float4(s.z, t.z, -s.w, -t.w);
+    if (vel) {
+        pairs[2 * stride + j] = make_float4(u.x, w.x, u.y, w.y);
+        pairs[3 * stride + j] = make_float4(u.z, w.z, 0.0f, 0.0f);
     }
 }
 

@@ -733,6 +733,25 @@ def test_r_agent_repack_and_plan_cycle_host(api, ctx, orc):
     assert idx2 == idx
 
 
+def test_plan_cycle_host_moving_and_pose6_equal_the_device_path(api, ctx):
+    """The host entry point lets the kernels read / write the pinned host buffers themselves: results must be
+    bit-identical to the device-buffer path, for moving spheres (odd sphere count: ragged pair) and 6D agents."""
+    sc = scenes.fast_clutter(n_agents=45, n_spheres=333, moving=True)
+    g = api.run_scene(ctx, sc)
+    out = np.empty_like(sc.agents)
+    idx, cost = ctx.plan_cycle_host(api.GMAPP_POINT3, sc.agents, sc.goal, sc.gains, sc.dt, sc.steps,
+                                    h_xyzr=sc.xyzr, h_vel=sc.vel, h_agents_out=out, alpha=sc.alpha, prev_best=sc.prev_best)
+    assert idx == g["best"] and cost == g["best_cost"] and np.array_equal(out, g["final"])
+    sc = scenes.config4(n_agents=24, n_spheres=301, steps=60)
+    g = api.run_scene(ctx, sc)
+    st = api.pose_to_state14(sc.quat, sc.pos, sc.twist)
+    goal = api.pose_to_state14(sc.goal_quat, sc.goal, np.zeros(6))[0, :8]
+    out = np.empty_like(st)
+    idx, cost = ctx.plan_cycle_host(api.GMAPP_MOTOR6, st, goal, sc.gains, sc.dt, sc.steps,
+                                    h_xyzr=sc.xyzr, h_vel=sc.vel, h_agents_out=out, alpha=sc.alpha, prev_best=sc.prev_best)
+    assert idx == g["best"] and cost == g["best_cost"] and np.array_equal(out, g["final"])
+
+
 def test_error_statuses(api):
     import torch
     c = api.Context(max_agents=8, max_spheres=16)
