@@ -34,72 +34,6 @@ __device__ __forceinline__ void warp_combine(const StaticAcc<NA>& acc, int lane,
 // ---------------------------------------------------------------------------------------------
 // DIRECT: the sums are the force itself (moving spheres or APF); else the BAC-CAB assembly of Eq. 2-3
 template <bool DIRECT>
-struct EpiPoint3 {
-    float p[3], v[3], ap[3], pub[6];
-    float ex, ey, ez, inv, nv, fax, fay, faz, fx, fy, fz;
-    int gid; float rd, kf;
-    CostAcc ca;
-    __device__ __forceinline__ float rcg(const RolloutParams& P) const { return P.rcg_is_rd ? rd : P.rcg; }
-    __device__ __forceinline__ float rco(const RolloutParams& P) const { return P.rco_is_rd ? rd : P.rco; }
-    __device__ __forceinline__ void init(const RolloutParams& P, int i) {
-        gid = agent_gid(P, i); rd = agent_rd(P, gid); kf = agent_kf(P, gid);
-        const float* s = P.agents_in + 6 * size_t(gid);
-#pragma unroll
-        for (int c = 0; c < 3; ++c) { p[c] = s[c]; v[c] = s[3 + c]; ap[c] = 0.0f; pub[c] = p[c]; pub[3 + c] = v[c]; }
-        ca.init(norm3f(P.goal[0] - p[0], P.goal[1] - p[1], P.goal[2] - p[2]));
-    }
-    __device__ __forceinline__ void pre(const RolloutParams& P) {
-        ex = P.goal[0] - p[0]; ey = P.goal[1] - p[1]; ez = P.goal[2] - p[2];
-        if (!DIRECT) {
-            const float n2 = fmaf(v[0], v[0], fmaf(v[1], v[1], fmaf(v[2], v[2], kTiny)));
-            inv = rsqrt_approx(n2);
-            inv = inv * fmaf(-0.5f * n2 * inv, inv, 1.5f);
-            nv = n2 * inv;
-        }
-        fax = fmaf(P.k_att, ex, -P.k_damp * v[0]); fay = fmaf(P.k_att, ey, -P.k_damp * v[1]); faz = fmaf(P.k_att, ez, -P.k_damp * v[2]);
-    }
-    __device__ __forceinline__ void post(const RolloutParams& P, float bx, float by, float bz) {
-        if (DIRECT) {                                      // the sweep accumulated the force vector itself
-            fx = fmaf(kf, bx, fax); fy = fmaf(kf, by, fay); fz = fmaf(kf, bz, faz);
-        } else {
-            const float A = fmaf(bx, v[0], fmaf(by, v[1], bz * v[2]));
-            const float c1 = kf * inv * A, c2 = -kf * nv;
-            fx = fmaf(c1, v[0], fmaf(c2, bx, fax)); fy = fmaf(c1, v[1], fmaf(c2, by, fay)); fz = fmaf(c1, v[2], fmaf(c2, bz, faz));
-        }
-        v[0] = fmaf(P.c_lin, fx, v[0]); v[1] = fmaf(P.c_lin, fy, v[1]); v[2] = fmaf(P.c_lin, fz, v[2]);   // Eq. 9-10
-        p[0] = fmaf(P.dt, v[0], p[0]); p[1] = fmaf(P.dt, v[1], p[1]); p[2] = fmaf(P.dt, v[2], p[2]);      // Eq. 11
-#pragma unroll
-        for (int c = 0; c < 3; ++c) { pub[c] = p[c]; pub[3 + c] = v[c]; }
-    }
-    __device__ __forceinline__ void costs(const RolloutParams& P, int k, float dmin) {
-        ca.pose(norm3f(ex, ey, ez), dmin, rcg(P), rco(P));
-        if (k >= 2) {
-            float jx = fx - ap[0], jy = fy - ap[1], jz = fz - ap[2];
-            ca.add_jerk(fmaf(jx, jx, fmaf(jy, jy, jz * jz)));
-        }
-        ap[0] = fx; ap[1] = fy; ap[2] = fz;
-        ca.add_len(norm3f(v[0], v[1], v[2]));
-    }
-    __device__ __forceinline__ void finish(const RolloutParams& P, float dmin) {
-        const int i = gid;
-        ca.pose(norm3f(P.goal[0] - p[0], P.goal[1] - p[1], P.goal[2] - p[2]), dmin, rcg(P), rco(P));
-        const float cj = P.vel_factor * P.dt * P.dt * P.inv_mass;
-        ca.finish(P, P.dt * ca.sumV, cj * cj * ca.sumJ, P.cost + 5 * size_t(i));
-        P.minclr[i] = ca.minclr;
-        P.collided[i] = ca.collided;
-        if (P.agents_out) write_state(P.agents_out + 6 * size_t(i));
-    }
-    __device__ __forceinline__ void write_state(float* o) const {
-#pragma unroll
-        for (int c = 0; c < 3; ++c) { o[c] = p[c]; o[3 + c] = v[c]; }
-    }
-    __device__ __forceinline__ void snapshot(const RolloutParams& P, int k) const {
-        if (P.snap_out && k + 1 == P.snap_step) write_state(P.snap_out + 6 * size_t(gid));
-        if (P.traj_out) write_state(P.traj_out + 6 * (size_t(gid) * (P.steps + 1) + k + 1));
-    }
-};
-
-template <bool DIRECT>
 struct EpiPose6 {
     Pose6 x;
     Quat rg; Vec3 pg;
@@ -380,9 +314,9 @@ __device__ __forceinline__ void wide_lin_warp(const RolloutParams& P, int agent,
 
 // ---------------------------------------------------------------------------------------------
 // the kernel: threads [0, G L) sweep, [G L, G L + 32 G) one epilogue warp per group; G <= 4, L >= 64
-// KIND 0 = 3D point agents (AT 1 or 2 per group), KIND 1 = 6D motor agents (one per group)
+// (or 64 G: a LIN and a ROT warp per group); one 6D motor agent per group
 // ---------------------------------------------------------------------------------------------
-template <int KIND, int AT, bool MOVING, bool CULL, int STAGE, bool APF>
+template <bool MOVING, bool CULL, int STAGE, bool APF>
 __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__ RolloutParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
@@ -417,17 +351,15 @@ __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__
     const int cta_first = blockIdx.x * P.agents_per_cta;
     int cta_end = cta_first + P.agents_per_cta;
     if (cta_end > P.n_agents) cta_end = P.n_agents;
-    constexpr int NA2 = (KIND == 0 && AT == 2) ? 2 : 1;
-    constexpr int ATE = (KIND == 0) ? AT : 1;
-    const int G = (P.agents_per_cta + ATE - 1) / ATE;
+    const int G = P.agents_per_cta;
     const int W = P.L >> 5;
     const int n_sweep = G * P.L;
     const bool is_epi = tid >= n_sweep;
     const int group_in_cta = is_epi ? ((tid - n_sweep) >> 5) : (tid >> P.logL);
-    const int first = cta_first + group_in_cta * ATE;
+    const int first = cta_first + group_in_cta;
     const int na = cta_end - first;
     float4* xch = reinterpret_cast<float4*>(smem_raw + P.red_off) + group_in_cta * (2 * W * 2 + 2 * 2 * 2);
-    if (KIND == 1 && P.two_warp_epi) {
+    if (P.two_warp_epi) {
         // threads [n_sweep, n_sweep + 32 G): lin warps; [n_sweep + 32 G, n_sweep + 64 G): rot warps
         if (tid >= n_sweep) {
             const int e = (tid - n_sweep) >> 5, g = e % G;
@@ -443,16 +375,13 @@ __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__
     } else if (is_epi) {
         if (na <= 0) return;
         const int lane = tid & 31;
-        if (KIND == 1) wide_epilogue_warp<EpiPose6<(MOVING || APF)>, 1>(P, first, lane, group_in_cta, xch);
-        else if (NA2 == 2 && na >= 2) wide_epilogue_warp<EpiPoint3<(MOVING || APF)>, NA2>(P, first, lane, group_in_cta, xch);
-        else wide_epilogue_warp<EpiPoint3<(MOVING || APF)>, 1>(P, first, lane, group_in_cta, xch);
+        wide_epilogue_warp<EpiPose6<(MOVING || APF)>, 1>(P, first, lane, group_in_cta, xch);
         return;
     }
     if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
     if (na <= 0) return;
     const int lane_in_group = tid & (P.L - 1);
-    if (NA2 == 2 && na >= 2) { if (P.rd_arr) wide_sweep_warps<NA2, MOVING, CULL, APF, true>(P, tile, astride, n2p, first, lane_in_group, group_in_cta, xch); else wide_sweep_warps<NA2, MOVING, CULL, APF, false>(P, tile, astride, n2p, first, lane_in_group, group_in_cta, xch); }
-    else { if (P.rd_arr) wide_sweep_warps<1, MOVING, CULL, APF, true>(P, tile, astride, n2p, first, lane_in_group, group_in_cta, xch); else wide_sweep_warps<1, MOVING, CULL, APF, false>(P, tile, astride, n2p, first, lane_in_group, group_in_cta, xch); }
+    { if (P.rd_arr) wide_sweep_warps<1, MOVING, CULL, APF, true>(P, tile, astride, n2p, first, lane_in_group, group_in_cta, xch); else wide_sweep_warps<1, MOVING, CULL, APF, false>(P, tile, astride, n2p, first, lane_in_group, group_in_cta, xch); }
 }
 
 }  // namespace gmapp
