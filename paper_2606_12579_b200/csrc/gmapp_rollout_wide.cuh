@@ -130,6 +130,7 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
     float4* part = xch;
     const float4* state = xch + 2 * W * NA;
     const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
+    const int trips = n2p >> P.logL;                       // n2p is a multiple of L
     const float4* tA = tile; const float4* tB = tile + astride; const float4* tU = tile + 2 * astride; const float4* tV = tile + 3 * astride;
     float p[NA][3], v[NA][3];
     RdSel<NA, PER> rd; rd.u = P.r_d;
@@ -148,11 +149,11 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
         const float tk = fmaf(float(k), P.dt, P.t0);
         acc.clear();
         if (MOVING) {
-            if (!last) sweep_x2_moving<NA, true, CULL, APF>(tA, tB, tU, tV, n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
-            else       sweep_x2_moving<NA, false, false>(tA, tB, tU, tV, n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
+            if (!last) sweep_x2_moving<NA, true, CULL, APF>(tA, tB, tU, tV, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
+            else       sweep_x2_moving<NA, false, false>(tA, tB, tU, tV, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
         } else {
-            if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
-            else       sweep_x2<NA, false, false>(tA, tB, n2p, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
+            if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, trips, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
+            else       sweep_x2<NA, false, false>(tA, tB, trips, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
         }
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
@@ -191,11 +192,7 @@ __device__ __forceinline__ void wide_epilogue_warp(const RolloutParams& P, int f
         const bool last = (k == P.steps);
         const int par = k & 1;
         named_bar_sync(bar_part, nbar);
-        float4 t = part[(par * W) * NA + half];
-        for (int w = 1; w < W; ++w) {
-            const float4 o = part[(par * W + w) * NA + half];
-            t.x += o.x; t.y += o.y; t.z += o.z; t.w = fminf(t.w, o.w);
-        }
+        const float4 t = sum_partials(part + (par * W) * NA + half, W, NA);
         if (last) {
             if (writer) me.finish(P, t.w);
             return;
@@ -292,11 +289,7 @@ __device__ __forceinline__ void wide_lin_warp(const RolloutParams& P, int agent,
             me.fpre = fma3(P.k_att, ev, (-P.k_damp) * me.x.nu);
         }
         named_bar_sync(bar_part, nbar);
-        float4 t = part[(par * W) * 1];
-        for (int w = 1; w < W; ++w) {
-            const float4 o = part[(par * W + w) * 1];
-            t.x += o.x; t.y += o.y; t.z += o.z; t.w = fminf(t.w, o.w);
-        }
+        const float4 t = sum_partials(part + (par * W) * 1, W, 1);
         if (last) {
             if (writer) me.finish(P, t.w);
             return;

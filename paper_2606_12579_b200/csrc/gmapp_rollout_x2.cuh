@@ -120,12 +120,12 @@ struct X2Acc {
 // APF = true: Eq. 1 in the Khatib form on the clamped surface distance (reading N1),
 // f_j = -k_f (1/d_O - 1/r_d) / d_O^2 * d/|d|; the sums then hold the force itself (no velocity factor).
 template <int NA, bool FORCE, bool CULL, bool APF = false, class RD = RdSel<NA, false>>
-__device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const float4* __restrict__ tB, int n2p,
+__device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const float4* __restrict__ tB, int trips,
                                          int lane, int L, const float (&p)[NA][3], const float (&v)[NA][3],
                                          const RD& rd, float eps, unsigned mask, X2Acc<NA>& acc) {
     const u64 tiny = bc2(kTiny), half = bc2(0.5f);
 #pragma unroll kX2Unroll
-    for (int j = lane; j < n2p; j += L) {
+    for (int i = 0, j = lane; i < trips; ++i, j += L) {
         const float4 s0 = tA[j], s1 = tB[j];
         const u64 cx = pk2(s0.x, s0.y), cy = pk2(s0.z, s0.w), cz = pk2(s1.x, s1.y), nR = pk2(s1.z, s1.w);
         u64 dx[NA], dy[NA], dz[NA], q[NA], yy[NA];
@@ -190,12 +190,12 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
 // ---------------------------------------------------------------------------------------------
 template <int NA, bool FORCE, bool CULL, bool APF = false, class RD = RdSel<NA, false>>
 __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, const float4* __restrict__ tB,
-                                                const float4* __restrict__ tU, const float4* __restrict__ tV, int n2p,
+                                                const float4* __restrict__ tU, const float4* __restrict__ tV, int trips,
                                                 int lane, int L, float tk, const float (&p)[NA][3], const float (&v)[NA][3],
                                                 const RD& rd, float eps, unsigned mask, X2Acc<NA>& acc) {
     const u64 tiny = bc2(kTiny), half = bc2(0.5f), t2 = bc2(tk);
 #pragma unroll 2
-    for (int j = lane; j < n2p; j += L) {
+    for (int i = 0, j = lane; i < trips; ++i, j += L) {
         const float4 s0 = tA[j], s1 = tB[j], s2 = tU[j], s3 = tV[j];
         const u64 ux = pk2(s2.x, s2.y), uy = pk2(s2.z, s2.w), uz = pk2(s3.x, s3.y), nR = pk2(s1.z, s1.w);
         const u64 cx = fma2(ux, t2, pk2(s0.x, s0.y)), cy = fma2(uy, t2, pk2(s0.z, s0.w)), cz = fma2(uz, t2, pk2(s1.x, s1.y));
@@ -259,11 +259,11 @@ __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, c
 
 // One entry point for both sweeps.  The pair arrays sit at equal distances: B = A + d, U = A + 2 d, V = A + 3 d.
 template <int NA, bool FORCE, bool CULL, bool APF, bool MV, class RD>
-__device__ __forceinline__ void sweep_any(const float4* __restrict__ tA, const float4* __restrict__ tB, int n2p, int lane, int L,
+__device__ __forceinline__ void sweep_any(const float4* __restrict__ tA, const float4* __restrict__ tB, int trips, int lane, int L,
                                           float tk, const float (&p)[NA][3], const float (&v)[NA][3], const RD& rd, float eps,
                                           unsigned mask, X2Acc<NA>& acc) {
-    if (MV) sweep_x2_moving<NA, FORCE, CULL, APF>(tA, tB, tB + (tB - tA), tB + 2 * (tB - tA), n2p, lane, L, tk, p, v, rd, eps, mask, acc);
-    else    sweep_x2<NA, FORCE, CULL, APF>(tA, tB, n2p, lane, L, p, v, rd, eps, mask, acc);
+    if (MV) sweep_x2_moving<NA, FORCE, CULL, APF>(tA, tB, tB + (tB - tA), tB + 2 * (tB - tA), trips, lane, L, tk, p, v, rd, eps, mask, acc);
+    else    sweep_x2<NA, FORCE, CULL, APF>(tA, tB, trips, lane, L, p, v, rd, eps, mask, acc);
 }
 
 // Transposed butterfly over a full warp.  In: per-lane partial (x,y,z) of NA agents.  Out: every lane of
@@ -432,6 +432,31 @@ __device__ __forceinline__ void warp_combine(const X2Acc<NA>& acc, int lane, flo
 }
 
 // ---------------------------------------------------------------------------------------------
+// epilogue side of the hand-over: add the W per-warp partials (x, y, z summed, w = min).  W is a power of two
+// between 2 and 16; every case issues all its loads before the first add and adds as a tree, so the epilogue
+// warp (the critical path of the latency-bound shapes) waits for one shared-memory round trip, not W.
+// ---------------------------------------------------------------------------------------------
+template <int WC>
+__device__ __forceinline__ float4 sum_partials_n(const float4* q, int stride) {
+    float4 t[WC];
+#pragma unroll
+    for (int w = 0; w < WC; ++w) t[w] = q[w * stride];
+#pragma unroll
+    for (int s = 1; s < WC; s <<= 1)
+#pragma unroll
+        for (int w = 0; w + s < WC; w += 2 * s) {
+            t[w].x += t[w + s].x; t[w].y += t[w + s].y; t[w].z += t[w + s].z; t[w].w = fminf(t[w].w, t[w + s].w);
+        }
+    return t[0];
+}
+__device__ __forceinline__ float4 sum_partials(const float4* q, int W, int stride) {
+    if (W == 4) return sum_partials_n<4>(q, stride);
+    if (W == 2) return sum_partials_n<2>(q, stride);
+    if (W == 8) return sum_partials_n<8>(q, stride);
+    return sum_partials_n<16>(q, stride);
+}
+
+// ---------------------------------------------------------------------------------------------
 // group body, L == 32: one warp per group does everything; agent a on lanes 0-15, agent b on lanes 16-31
 // ---------------------------------------------------------------------------------------------
 template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
@@ -460,8 +485,8 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
             for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
         }
         acc.clear();
-        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p, lane, 32, tk, p, v, rd, P.eps, full, acc);
-        else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p, lane, 32, tk, p, v, rd, P.eps, full, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
         if (last) {
@@ -523,8 +548,8 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     const float tk = fmaf(float(k), P.dt, P.t0);
     X2Acc<NA> acc;
     acc.clear();
-    if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p, lane, 32, tk, p, v, rd, P.eps, full, acc);
-    else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p, lane, 32, tk, p, v, rd, P.eps, full, acc);
+    if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, acc);
+    else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, acc);
     float X, Y, Z, D;
     warp_combine<NA>(acc, lane, X, Y, Z, D);
     const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
@@ -571,6 +596,7 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
                                                   int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
     const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
     const int half = (NA == 2) ? (lane >> 4) : 0;
+    const int trips = n2p >> P.logL;                       // n2p is a multiple of L: the same trip count on every lane
     const unsigned full = 0xffffffffu;
     float4* part = xch;                                    // [2][W][NA]
     const float4* state = xch + 2 * W * NA;                // [2][NA][2]
@@ -590,8 +616,8 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
         const bool last = (k == P.steps);
         const float tk = fmaf(float(k), P.dt, P.t0);
         acc.clear();
-        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
-        else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
         const int par = k & 1;
@@ -622,11 +648,7 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
         const int par = k & 1;
         me.pre(P);                                         // everything that does not need the sphere sums
         named_bar_sync(bar_part, nbar);
-        float4 t = part[(par * W) * NA + half];
-        for (int w = 1; w < W; ++w) {
-            const float4 o = part[(par * W + w) * NA + half];
-            t.x += o.x; t.y += o.y; t.z += o.z; t.w = fminf(t.w, o.w);
-        }
+        const float4 t = sum_partials(part + (par * W) * NA + half, W, NA);
         if (last) {
             if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.finish(P, t.w);
             return;
@@ -650,6 +672,7 @@ template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
 __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                      int first_agent, int lane_in_group) {
     const unsigned mask = __activemask();
+    const int trips = n2p >> P.logL;                       // n2p is a multiple of L
     AgentX2 ag[NA];
     float p[NA][3], v[NA][3];
     RdSel<NA, PER> rd; rd.u = P.r_d;
@@ -664,8 +687,8 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 #pragma unroll
             for (int i = 0; i < 3; ++i) { p[a][i] = ag[a].p[i]; v[a][i] = ag[a].v[i]; }
         acc.clear();
-        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
-        else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
         float x[NA], y[NA], z[NA], dm[NA];
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
