@@ -518,9 +518,11 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     const int mode = chunked ? 4 : (L >= 64 ? (G <= 4 ? 2 : 3) : (L == 32 ? 1 : 0));
     const int n2p = n2 > 0 ? round_up(n2, L) : 0;
     const int cull = (t && t->cull >= 0) ? t->cull : 0;
-    // dynamic shared memory: [0,64) mbarrier; [64, 64+4 KB) cross-warp exchange; sphere-pair tile at 4224
-    const int xch_off = 64, rec_off = 4224;
-    const int tile_off = rec_off + (chunked ? round_up(A * 24 * 4, 128) : 0);      // mode 4: 24-word state record per agent
+    // dynamic shared memory: [0,64) mbarrier; then the exchange area of the multi-warp groups (per group: the
+    // per-lane partials of two agents + the published states = (2 L + 8) float4) or, mode 4, the 24-word state
+    // record of every agent; then the sphere-pair tile
+    const int xch_off = 64, rec_off = 128;
+    const int tile_off = rec_off + (chunked ? round_up(A * 24 * 4, 128) : (mode >= 2 ? round_up(G * (2 * L + 8) * 16, 128) : 0));
     const size_t tile_bytes = (size_t)n2p * (c->moving ? 64 : 32);       // pair arrays A, B (+ U, V when the spheres move)
     const bool fits = tile_off + tile_bytes <= (size_t)c->smem_optin;
     int stage = fits ? 1 : 0;
@@ -687,6 +689,10 @@ static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_ag
         s = effective_pairs(c, g->r_agent, st, &launches);
         if (s != GMAPP_OK) return s;
         P.pairA = c->d_pairA; P.pair_stride = c->cap_spheres / 2; P.n2p = round_up(n2, cfg.L);
+        // exchange area: per group the per-lane partials + the published states ((L + 8) float4), then one 5-float4
+        // record per group for the ROT -> LIN hand-over
+        cfg.tile_off = cfg.red_off + round_up((cfg.groups * (cfg.L + 8) + 5 * cfg.groups) * 16, 128);
+        P.tile_off = cfg.tile_off;
         const size_t tile_bytes = (size_t)P.n2p * 16 * (c->moving ? 4 : 2);
         const bool fits = cfg.tile_off + tile_bytes <= (size_t)c->smem_optin;
         if (cfg.stage == 1 && !fits) cfg.stage = 0;

@@ -16,17 +16,6 @@
 
 namespace gmapp {
 
-template <int NA>
-__device__ __forceinline__ void warp_combine(const StaticAcc<NA>& acc, int lane, float& X, float& Y, float& Z, float& D) {
-    float x[NA], y[NA], z[NA], dm[NA];
-#pragma unroll
-    for (int a = 0; a < NA; ++a) {
-        x[a] = acc.bx[a]; y[a] = acc.by[a]; z[a] = acc.bz[a];
-        dm[a] = fkey_inv(__reduce_min_sync(0xffffffffu, fkey(acc.dmin[a])));
-    }
-    warp_sum3<NA>(x, y, z, lane, X, Y, Z);
-    D = (NA == 2 && (lane & 16)) ? dm[NA - 1] : dm[0];
-}
 
 // ---------------------------------------------------------------------------------------------
 // epilogue-side agent models.  Interface: init, pre (no sums needed), post (sums known -> new state, pub[6] =
@@ -118,17 +107,15 @@ struct EpiPose6 {
 
 // ---------------------------------------------------------------------------------------------
 // group bodies (protocol and hazard argument as in gmapp_rollout_x2.cuh, multi-warp mode)
-// exchange area per group: part[2][W][NA] float4, state[2][NA][2] float4
+// exchange area per group: part[NA][L] float4 (per-lane partials, reduced by the epilogue warp), state[2][NA][2] float4
 // ---------------------------------------------------------------------------------------------
 // sweep warps: packed f32x2 sweeps over sphere pairs; tile = A, B (, U, V when MOVING) arrays of n2p float4 each
 template <int NA, bool MOVING, bool CULL, bool APF, bool PER>
 __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const float4* tile, int astride, int n2p, int first_agent,
                                                  int lane_in_group, int group_in_cta, float4* xch) {
-    const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
-    const int half = (NA == 2) ? (lane >> 4) : 0;
     const unsigned full = 0xffffffffu;
     float4* part = xch;
-    const float4* state = xch + 2 * W * NA;
+    const float4* state = xch + NA * P.L;
     const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
     const int trips = n2p >> P.logL;                       // n2p is a multiple of L
     const float4* tA = tile; const float4* tB = tile + astride; const float4* tU = tile + 2 * astride; const float4* tV = tile + 3 * astride;
@@ -155,10 +142,13 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
             if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, trips, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
             else       sweep_x2<NA, false, false>(tA, tB, trips, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
         }
-        float X, Y, Z, D;
-        warp_combine<NA>(acc, lane, X, Y, Z, D);
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {                     // per-lane partials; the epilogue warp reduces them
+            float x0, x1, y0, y1, z0, z1;
+            upk2(acc.bx[a], x0, x1); upk2(acc.by[a], y0, y1); upk2(acc.bz[a], z0, z1);
+            part[a * P.L + lane_in_group] = make_float4(x0 + x1, y0 + y1, z0 + z1, acc.dmin[a]);
+        }
         const int par = k & 1;
-        if ((lane & 15) == 0 && (NA == 2 || lane == 0)) part[(par * W + wig) * NA + half] = make_float4(X, Y, Z, D);
         named_bar_arrive(bar_part, nbar);
         if (last) return;
         named_bar_sync(bar_state, nbar);
@@ -170,14 +160,13 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
     }
 }
 
-template <class Model, int NA>
+template <class Model, int NA, int NW>
 __device__ __forceinline__ void wide_epilogue_warp(const RolloutParams& P, int first_agent, int lane,
                                                    int group_in_cta, float4* xch) {
-    const int W = P.L >> 5;
     const int half = (NA == 2) ? (lane >> 4) : 0;
     const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
     const float4* part = xch;
-    float4* state = xch + 2 * W * NA;
+    float4* state = xch + NA * P.L;
     const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
     Model me;
     me.init(P, first_agent + half);
@@ -192,7 +181,7 @@ __device__ __forceinline__ void wide_epilogue_warp(const RolloutParams& P, int f
         const bool last = (k == P.steps);
         const int par = k & 1;
         named_bar_sync(bar_part, nbar);
-        const float4 t = sum_partials(part + (par * W) * NA + half, W, NA);
+        const float4 t = group_reduce<NA, NW>(part, P.L, lane);
         if (last) {
             if (writer) me.finish(P, t.w);
             return;
@@ -254,12 +243,11 @@ __device__ __forceinline__ void wide_rot_warp(const RolloutParams& P, int agent,
     if (P.steps >= 1) named_bar_sync(bar_empty, 64);                       // balance the lin warp's last arrive
 }
 
-template <bool DIRECT>
+template <bool DIRECT, int NW>
 __device__ __forceinline__ void wide_lin_warp(const RolloutParams& P, int agent, int lane, int group_in_cta,
                                               float4* xch, const float4* rec) {
-    const int W = P.L >> 5;
     const float4* part = xch;
-    float4* state = xch + 2 * W;
+    float4* state = xch + P.L;
     const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
     const int bar_full = 9 + 2 * group_in_cta, bar_empty = 10 + 2 * group_in_cta;
     const bool writer = lane == 0;
@@ -289,7 +277,7 @@ __device__ __forceinline__ void wide_lin_warp(const RolloutParams& P, int agent,
             me.fpre = fma3(P.k_att, ev, (-P.k_damp) * me.x.nu);
         }
         named_bar_sync(bar_part, nbar);
-        const float4 t = sum_partials(part + (par * W) * 1, W, 1);
+        const float4 t = group_reduce<1, NW>(part, P.L, lane);
         if (last) {
             if (writer) me.finish(P, t.w);
             return;
@@ -345,13 +333,12 @@ __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__
     int cta_end = cta_first + P.agents_per_cta;
     if (cta_end > P.n_agents) cta_end = P.n_agents;
     const int G = P.agents_per_cta;
-    const int W = P.L >> 5;
     const int n_sweep = G * P.L;
     const bool is_epi = tid >= n_sweep;
     const int group_in_cta = is_epi ? ((tid - n_sweep) >> 5) : (tid >> P.logL);
     const int first = cta_first + group_in_cta;
     const int na = cta_end - first;
-    float4* xch = reinterpret_cast<float4*>(smem_raw + P.red_off) + group_in_cta * (2 * W * 2 + 2 * 2 * 2);
+    float4* xch = reinterpret_cast<float4*>(smem_raw + P.red_off) + group_in_cta * (P.L + 8);
     if (P.two_warp_epi) {
         // threads [n_sweep, n_sweep + 32 G): lin warps; [n_sweep + 32 G, n_sweep + 64 G): rot warps
         if (tid >= n_sweep) {
@@ -359,16 +346,21 @@ __global__ void __launch_bounds__(640, 1) k_rollout_wide(const __grid_constant__
             const int ag = cta_first + g;
             if (ag >= cta_end) return;
             float4* base = reinterpret_cast<float4*>(smem_raw + P.red_off);
-            float4* xg = base + g * (2 * W * 2 + 2 * 2 * 2);
-            float4* rec = base + 112 + 5 * g;
-            if (e < G) wide_lin_warp<(MOVING || APF)>(P, ag, tid & 31, g, xg, rec);
-            else wide_rot_warp(P, ag, tid & 31, g, rec);
+            float4* xg = base + g * (P.L + 8);
+            float4* rec = base + G * (P.L + 8) + 5 * g;
+            const int n = P.L >> 5;                        // partials per lane of the reducing warp (NW, 0 = 16)
+            if (e >= G) wide_rot_warp(P, ag, tid & 31, g, rec);
+            else if (n == 8) wide_lin_warp<(MOVING || APF), 8>(P, ag, tid & 31, g, xg, rec);
+            else if (n == 4) wide_lin_warp<(MOVING || APF), 4>(P, ag, tid & 31, g, xg, rec);
+            else if (n == 2) wide_lin_warp<(MOVING || APF), 2>(P, ag, tid & 31, g, xg, rec);
+            else wide_lin_warp<(MOVING || APF), 0>(P, ag, tid & 31, g, xg, rec);
             return;
         }
     } else if (is_epi) {
         if (na <= 0) return;
         const int lane = tid & 31;
-        wide_epilogue_warp<EpiPose6<(MOVING || APF)>, 1>(P, first, lane, group_in_cta, xch);
+        if ((P.L >> 5) == 4) wide_epilogue_warp<EpiPose6<(MOVING || APF)>, 1, 4>(P, first, lane, group_in_cta, xch);   // 4 groups: L = 128
+        else wide_epilogue_warp<EpiPose6<(MOVING || APF)>, 1, 2>(P, first, lane, group_in_cta, xch);                 //           or L = 64
         return;
     }
     if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);

@@ -182,6 +182,24 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
     }
 }
 
+// each 16-lane half of the warp sums its own (x, y, z) over its lanes; every lane of a half gets the three sums.
+// Transposed butterfly: step 8 leaves (x, y) on the lanes with bit 3 clear and z on the others, step 4 one value
+// per lane, steps 2 and 1 finish: 5 shuffles + 3 to hand the sums round.
+__device__ __forceinline__ void half_sum3(float kx, float ky, float kz, int lane, float& X, float& Y, float& Z) {
+    const unsigned full = 0xffffffffu;
+    const bool h8 = lane & 8, h4 = lane & 4;
+    float r1 = __shfl_xor_sync(full, h8 ? kx : kz, 8);
+    float r2 = __shfl_xor_sync(full, ky, 8);
+    if (h8) kz += r1; else { kx += r1; ky += r2; }
+    float send = h8 ? kz : (h4 ? kx : ky);
+    float keep = h8 ? kz : (h4 ? ky : kx);
+    float u = keep + __shfl_xor_sync(full, send, 4);
+    u += __shfl_xor_sync(full, u, 2);
+    u += __shfl_xor_sync(full, u, 1);
+    const int base = lane & 16;
+    X = __shfl_sync(full, u, base); Y = __shfl_sync(full, u, base | 4); Z = __shfl_sync(full, u, base | 8);
+}
+
 // ---------------------------------------------------------------------------------------------
 // packed f32x2 sweep for MOVING spheres.  Sphere pairs: A = (cx0,cx1,cy0,cy1), B = (cz0,cz1,-R0,-R1) at t = 0,
 // U = (ux0,ux1,uy0,uy1), V = (uz0,uz1,0,0).  Per pair (reading G5/G25): c(t) = c + t u, v_rel = v - u,
@@ -273,24 +291,14 @@ __device__ __forceinline__ void warp_sum3(const float (&x)[NA], const float (&y)
                                           int lane, float& X, float& Y, float& Z) {
     const unsigned full = 0xffffffffu;
     float u;
+    (void)u;
     if (NA == 2) {
-        const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4;
+        const bool h16 = lane & 16;
         // step 16: lower half keeps agent 0, upper half keeps agent 1
         float kx = h16 ? x[NA - 1] : x[0], ky = h16 ? y[NA - 1] : y[0], kz = h16 ? z[NA - 1] : z[0];
         float sx = h16 ? x[0] : x[NA - 1], sy = h16 ? y[0] : y[NA - 1], sz = h16 ? z[0] : z[NA - 1];
         kx += __shfl_xor_sync(full, sx, 16); ky += __shfl_xor_sync(full, sy, 16); kz += __shfl_xor_sync(full, sz, 16);
-        // step 8: lanes with bit 3 clear keep (x, y), the others keep z
-        float r1 = __shfl_xor_sync(full, h8 ? kx : kz, 8);
-        float r2 = __shfl_xor_sync(full, ky, 8);
-        if (h8) kz += r1; else { kx += r1; ky += r2; }
-        // step 4: (x, y) lanes split into x and y; z lanes plain
-        float send = h8 ? kz : (h4 ? kx : ky);
-        float keep = h8 ? kz : (h4 ? ky : kx);
-        u = keep + __shfl_xor_sync(full, send, 4);
-        u += __shfl_xor_sync(full, u, 2);
-        u += __shfl_xor_sync(full, u, 1);
-        const int base = lane & 16;
-        X = __shfl_sync(full, u, base); Y = __shfl_sync(full, u, base | 4); Z = __shfl_sync(full, u, base | 8);
+        half_sum3(kx, ky, kz, lane, X, Y, Z);
     } else {
         const bool h16 = lane & 16, h8 = lane & 8;
         float kx = x[0], ky = y[0], kz = z[0];
@@ -449,11 +457,41 @@ __device__ __forceinline__ float4 sum_partials_n(const float4* q, int stride) {
         }
     return t[0];
 }
-__device__ __forceinline__ float4 sum_partials(const float4* q, int W, int stride) {
-    if (W == 4) return sum_partials_n<4>(q, stride);
-    if (W == 2) return sum_partials_n<2>(q, stride);
-    if (W == 8) return sum_partials_n<8>(q, stride);
-    return sum_partials_n<16>(q, stride);
+// NW = 2, 4, 8: exactly that many; NW = 0: n = 16 or 32 in chunks of eight
+template <int NW>
+__device__ __forceinline__ float4 sum_partials(const float4* q, int n, int stride) {
+    if (NW > 0) return sum_partials_n<(NW > 0 ? NW : 2)>(q, stride);
+    float4 t = sum_partials_n<8>(q, stride);
+    for (int m = 8; m < n; m += 8) {
+        const float4 o = sum_partials_n<8>(q + m * stride, stride);
+        t.x += o.x; t.y += o.y; t.z += o.z; t.w = fminf(t.w, o.w);
+    }
+    return t;
+}
+
+// Group reduction done by the epilogue warp (multi-warp groups).  The sweep lanes leave their per-lane partials
+// (x, y, z, dmin) in shared memory as part[NA][L]; lane l of the epilogue warp first adds L/32 of them (NA == 2:
+// lanes 0-15 add L/16 of agent 0, lanes 16-31 of agent 1), then the warp finishes with the transposed butterfly.
+// One butterfly per group and step instead of one per sweep warp.  NW = partials per lane (L/32, NA == 2: L/16) when
+// that is 2, 4 or 8, else 0: a template parameter so that the step loop of the epilogue warp has no dispatch in it.
+template <int NA, int NW>
+__device__ __forceinline__ float4 group_reduce(const float4* part, int L, int lane) {
+    const unsigned full = 0xffffffffu;
+    float X, Y, Z, D;
+    if (NA == 2) {
+        const int half = lane >> 4;
+        const float4 t = sum_partials<NW>(part + half * L + (lane & 15), L >> 4, 16);
+        half_sum3(t.x, t.y, t.z, lane, X, Y, Z);
+        const int key = fkey(t.w);
+        const int k0 = __reduce_min_sync(full, half ? 0x7fffffff : key), k1 = __reduce_min_sync(full, half ? key : 0x7fffffff);
+        D = fkey_inv(half ? k1 : k0);
+    } else {
+        const float4 t = sum_partials<NW>(part + lane, L >> 5, 32);
+        const float x[1] = {t.x}, y[1] = {t.y}, z[1] = {t.z};
+        warp_sum3<1>(x, y, z, lane, X, Y, Z);
+        D = fkey_inv(__reduce_min_sync(full, fkey(t.w)));
+    }
+    return make_float4(X, Y, Z, D);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -586,20 +624,20 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
 
 // ---------------------------------------------------------------------------------------------
 // group bodies, L >= 64: W = L/32 sweep warps + ONE epilogue warp per group.
-// shared exchange area per group: part[2][W][NA] float4 (X, Y, Z, dmin), state[2][NA][2] float4 (p,0), (v,0);
-// both double-buffered by step parity, so one arrive/sync pair per direction and step is race-free:
-//   sweep warp k:    write part[k&1] -> arrive(bar_part) -> sync(bar_state) -> read state[k&1]
-//   epilogue warp k: sync(bar_part) -> read part[k&1] -> integrate -> write state[k&1] -> arrive(bar_state) -> costs
+// shared exchange area per group: part[NA][L] float4 (per-lane x, y, z, dmin), state[2][NA][2] float4 (p,0), (v,0).
+// One arrive/sync pair per direction and step is race-free: the epilogue warp has consumed part (its loads feed the
+// state it publishes) before it arrives at bar_state, and the sweep warps write part again only after that barrier;
+// state is double-buffered by step parity.
+//   sweep warp k:    write part -> arrive(bar_part) -> sync(bar_state) -> read state[k&1]
+//   epilogue warp k: sync(bar_part) -> reduce part -> integrate -> write state[k&1] -> arrive(bar_state) -> costs
 // ---------------------------------------------------------------------------------------------
 template <int NA, bool CULL, bool APF, bool PER, bool MV>
 __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
                                                   int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
-    const int lane = lane_in_group & 31, wig = lane_in_group >> 5, W = P.L >> 5;
-    const int half = (NA == 2) ? (lane >> 4) : 0;
     const int trips = n2p >> P.logL;                       // n2p is a multiple of L: the same trip count on every lane
     const unsigned full = 0xffffffffu;
-    float4* part = xch;                                    // [2][W][NA]
-    const float4* state = xch + 2 * W * NA;                // [2][NA][2]
+    float4* part = xch;                                    // [NA][L]
+    const float4* state = xch + 2 * P.L;                   // [2][NA][2]
     const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
     float p[NA][3], v[NA][3];
     RdSel<NA, PER> rd; rd.u = P.r_d;
@@ -618,10 +656,13 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
         acc.clear();
         if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
         else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
-        float X, Y, Z, D;
-        warp_combine<NA>(acc, lane, X, Y, Z, D);
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {                     // per-lane partials; the epilogue warp reduces them
+            float x0, x1, y0, y1, z0, z1;
+            upk2(acc.bx[a], x0, x1); upk2(acc.by[a], y0, y1); upk2(acc.bz[a], z0, z1);
+            part[a * P.L + lane_in_group] = make_float4(x0 + x1, y0 + y1, z0 + z1, acc.dmin[a]);
+        }
         const int par = k & 1;
-        if ((lane & 15) == 0 && (NA == 2 || lane == 0)) part[(par * W + wig) * NA + half] = make_float4(X, Y, Z, D);
         named_bar_arrive(bar_part, nbar);
         if (last) return;
         named_bar_sync(bar_state, nbar);
@@ -633,13 +674,12 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
     }
 }
 
-template <int NA, bool APF, bool XT>   // APF here = "the sums are the force itself" (APF heuristic or moving spheres)
-__device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, int first_agent, int lane,
+template <int NA, bool APF, bool XT, int NW>   // APF here = "the sums are the force itself" (APF heuristic or moving spheres)
+__device__ __forceinline__ void group_epilogue_warp_n(const RolloutX2Params& P, int first_agent, int lane,
                                                     int group_in_cta, float4* xch) {
-    const int W = P.L >> 5;
     const int half = (NA == 2) ? (lane >> 4) : 0;
     const float4* part = xch;
-    float4* state = xch + 2 * W * NA;
+    float4* state = xch + 2 * P.L;
     const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
     AgentX2 me;
     me.init(P, first_agent + half);
@@ -648,7 +688,7 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
         const int par = k & 1;
         me.pre(P);                                         // everything that does not need the sphere sums
         named_bar_sync(bar_part, nbar);
-        const float4 t = sum_partials(part + (par * W) * NA + half, W, NA);
+        const float4 t = group_reduce<NA, NW>(part, P.L, lane);
         if (last) {
             if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.finish(P, t.w);
             return;
@@ -663,6 +703,16 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
         me.costs(P, k, t.w, fx, fy, fz);                   // off the critical path: the sweep warps are already running
         if ((lane & 15) == 0 && (NA == 2 || lane == 0)) { if (XT) me.snapshot(P, k); }
     }
+}
+
+template <int NA, bool APF, bool XT>
+__device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, int first_agent, int lane,
+                                                    int group_in_cta, float4* xch) {
+    const int n = P.L >> (NA == 2 ? 4 : 5);                // partials per epilogue lane
+    if (n == 4) group_epilogue_warp_n<NA, APF, XT, 4>(P, first_agent, lane, group_in_cta, xch);
+    else if (n == 8) group_epilogue_warp_n<NA, APF, XT, 8>(P, first_agent, lane, group_in_cta, xch);
+    else if (n == 2) group_epilogue_warp_n<NA, APF, XT, 2>(P, first_agent, lane, group_in_cta, xch);
+    else group_epilogue_warp_n<NA, APF, XT, 0>(P, first_agent, lane, group_in_cta, xch);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -759,13 +809,12 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
     constexpr int NA2 = (AT == 2) ? 2 : 1;
     if (MODE == 2) {
         const int G = (P.agents_per_cta + AT - 1) / AT;
-        const int W = P.L >> 5;
         const int n_sweep = G * P.L;
         const bool is_epi = tid >= n_sweep;
         const int group_in_cta = is_epi ? ((tid - n_sweep) >> 5) : (tid >> P.logL);
         const int first = cta_first + group_in_cta * AT;
         const int na = cta_end - first;
-        float4* xch = reinterpret_cast<float4*>(smem_raw + P.xch_off) + group_in_cta * (2 * W * 2 + 2 * 2 * 2);
+        float4* xch = reinterpret_cast<float4*>(smem_raw + P.xch_off) + group_in_cta * (2 * P.L + 8);
         if (is_epi) {                                      // the epilogue warps never touch the sphere tile
             if (na <= 0) return;
             if (AT == 2 && na >= 2) group_epilogue_warp<NA2, (APF || MV), XT>(P, first, tid & 31, group_in_cta, xch);
