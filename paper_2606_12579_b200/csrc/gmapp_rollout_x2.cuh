@@ -471,27 +471,26 @@ __device__ __forceinline__ float4 sum_partials(const float4* q, int n, int strid
 
 // Group reduction done by the epilogue warp (multi-warp groups).  The sweep lanes leave their per-lane partials
 // (x, y, z, dmin) in shared memory as part[NA][L]; lane l of the epilogue warp first adds L/32 of them (NA == 2:
-// lanes 0-15 add L/16 of agent 0, lanes 16-31 of agent 1), then the warp finishes with the transposed butterfly.
+// lanes 0-15 add L/16 of agent 0, lanes 16-31 of agent 1), then the warp finishes with a butterfly.
 // One butterfly per group and step instead of one per sweep warp.  NW = partials per lane (L/32, NA == 2: L/16) when
 // that is 2, 4 or 8, else 0: a template parameter so that the step loop of the epilogue warp has no dispatch in it.
 template <int NA, int NW>
 __device__ __forceinline__ float4 group_reduce(const float4* part, int L, int lane) {
     const unsigned full = 0xffffffffu;
-    float X, Y, Z, D;
-    if (NA == 2) {
-        const int half = lane >> 4;
-        const float4 t = sum_partials<NW>(part + half * L + (lane & 15), L >> 4, 16);
-        half_sum3(t.x, t.y, t.z, lane, X, Y, Z);
-        const int key = fkey(t.w);
-        const int k0 = __reduce_min_sync(full, half ? 0x7fffffff : key), k1 = __reduce_min_sync(full, half ? key : 0x7fffffff);
-        D = fkey_inv(half ? k1 : k0);
-    } else {
-        const float4 t = sum_partials<NW>(part + lane, L >> 5, 32);
-        const float x[1] = {t.x}, y[1] = {t.y}, z[1] = {t.z};
-        warp_sum3<1>(x, y, z, lane, X, Y, Z);
-        D = fkey_inv(__reduce_min_sync(full, fkey(t.w)));
+    float4 t;
+    if (NA == 2) t = sum_partials<NW>(part + (lane >> 4) * L + (lane & 15), L >> 4, 16);
+    else         t = sum_partials<NW>(part + lane, L >> 5, 32);
+    // plain xor butterfly on the four values (over the 16-lane half for two agents): the epilogue warp is the
+    // critical path of the latency-bound shapes, and this form needs no hand-round of the sums at the end
+    // (the transposed butterfly of the sweep-side reductions saves shuffles, which matters there, not here)
+#pragma unroll
+    for (int off = (NA == 2 ? 8 : 16); off > 0; off >>= 1) {
+        t.x += __shfl_xor_sync(full, t.x, off);
+        t.y += __shfl_xor_sync(full, t.y, off);
+        t.z += __shfl_xor_sync(full, t.z, off);
+        t.w = fminf(t.w, __shfl_xor_sync(full, t.w, off));
     }
-    return make_float4(X, Y, Z, D);
+    return t;
 }
 
 // ---------------------------------------------------------------------------------------------
