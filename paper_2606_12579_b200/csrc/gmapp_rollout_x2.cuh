@@ -630,10 +630,12 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
 //   sweep warp k:    write part -> arrive(bar_part) -> sync(bar_state) -> read state[k&1]
 //   epilogue warp k: sync(bar_part) -> reduce part -> integrate -> write state[k&1] -> arrive(bar_state) -> costs
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL, bool APF, bool PER, bool MV>
-__device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
-                                                  int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
-    const int trips = n2p >> P.logL;                       // n2p is a multiple of L: the same trip count on every lane
+template <int NA, bool CULL, bool APF, bool PER, bool MV, bool ONE>
+__device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
+                                                    int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
+    // n2p is a multiple of L: the same trip count on every lane.  ONE: a single trip (as many lanes as sphere pairs,
+    // the latency-bound shapes): known at compile time, so the sweep is straight-line code without loop control
+    const int trips = ONE ? 1 : (n2p >> P.logL);
     const unsigned full = 0xffffffffu;
     float4* part = xch;                                    // [NA][L]
     const float4* state = xch + 2 * P.L;                   // [2][NA][2]
@@ -671,6 +673,13 @@ __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, cons
             p[a][0] = sp.x; p[a][1] = sp.y; p[a][2] = sp.z; v[a][0] = sv.x; v[a][1] = sv.y; v[a][2] = sv.z;
         }
     }
+}
+
+template <int NA, bool CULL, bool APF, bool PER, bool MV>
+__device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
+                                                  int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
+    if ((n2p >> P.logL) == 1) group_sweep_warps_n<NA, CULL, APF, PER, MV, true>(P, tA, tB, n2p, first_agent, lane_in_group, group_in_cta, xch);
+    else group_sweep_warps_n<NA, CULL, APF, PER, MV, false>(P, tA, tB, n2p, first_agent, lane_in_group, group_in_cta, xch);
 }
 
 template <int NA, bool APF, bool XT, int NW>   // APF here = "the sums are the force itself" (APF heuristic or moving spheres)
