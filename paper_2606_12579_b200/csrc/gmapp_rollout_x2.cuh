@@ -496,9 +496,10 @@ __device__ __forceinline__ float4 group_reduce(const float4* part, int L, int la
 // ---------------------------------------------------------------------------------------------
 // group body, L == 32: one warp per group does everything; agent a on lanes 0-15, agent b on lanes 16-31
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
-__device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
-                                                   int first_agent, int lane) {
+template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV, bool ONE>
+__device__ __forceinline__ void group_rollout_warp_n(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
+                                                     int first_agent, int lane) {
+    const int trips = ONE ? 1 : (n2p >> 5);                // ONE: at most 32 sphere pairs, straight-line sweep
     const int half = (NA == 2) ? (lane >> 4) : 0;
     const unsigned full = 0xffffffffu;
     AgentX2 me;
@@ -522,8 +523,8 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
             for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
         }
         acc.clear();
-        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, acc);
-        else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
         if (last) {
@@ -536,6 +537,13 @@ __device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, con
         me.costs(P, k, D, fx, fy, fz);
         if ((lane & 15) == 0 && (NA == 2 || lane == 0)) { if (XT) me.snapshot(P, k); }
     }
+}
+
+template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
+__device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
+                                                   int first_agent, int lane) {
+    if (n2p == 32) group_rollout_warp_n<NA, CULL, APF, PER, XT, MV, true>(P, tA, tB, n2p, first_agent, lane);
+    else group_rollout_warp_n<NA, CULL, APF, PER, XT, MV, false>(P, tA, tB, n2p, first_agent, lane);
 }
 
 // ---------------------------------------------------------------------------------------------
