@@ -117,7 +117,8 @@ gmapp_status gmapp_destroy(gmapp_ctx* ctx);
  * The arrays are read by stream work enqueued in this call (a packing kernel); they may be freed or
  * changed once that work has run.  Radii must be >= 0 and all values finite (not checked on device). */
 gmapp_status gmapp_set_obstacles(gmapp_ctx* ctx, const float* d_xyzr, const float* d_vel, int n, void* cuda_stream);
-/* Same with HOST arrays (copied through the context's pinned staging buffer). */
+/* Same with HOST arrays: copied into the context's pinned buffer, which the packing kernel then reads over the host
+ * link itself (no device staging copy).  Synchronises the stream first if that buffer may still be in use. */
 gmapp_status gmapp_set_obstacles_host(gmapp_ctx* ctx, const float* h_xyzr, const float* h_vel, int n, void* cuda_stream);
 
 /* Sphere-world builder (perception stage: workspace crop, "voxelise at 2 r_O", the occupied
@@ -210,8 +211,8 @@ gmapp_status gmapp_forces(gmapp_ctx* ctx, gmapp_kind kind, const float* d_agents
 gmapp_status gmapp_get_results(gmapp_ctx* ctx, float* d_cost, float* d_min_clearance, int32_t* d_collided,
                                void* cuda_stream);
 
-/* A whole planning cycle from HOST buffers: (optional) sphere upload, agent upload from pinned staging,
- * rollout, selection, 8-byte result download; h_agents_out (may be NULL) receives the final states.
+/* A whole planning cycle from HOST buffers: (optional) sphere upload, agent states read by the rollout kernel straight
+ * from the pinned buffer (and final states written back to it), selection, 12-byte result written to pinned memory; h_agents_out (may be NULL) receives the final states.
  * h_xyzr == NULL keeps the resident sphere world.  Synchronises the stream. */
 gmapp_status gmapp_plan_cycle_host(gmapp_ctx* ctx, gmapp_kind kind, const float* h_agents, float* h_agents_out,
                                    int n_agents, const float* h_xyzr, const float* h_vel, int n_spheres,
