@@ -650,12 +650,30 @@ def test_trajectory_output_pose6(api, ctx, orc):
     dict(max_ctas=5), dict(max_ctas=5, cull=1, agents_per_thread=1),
     dict(scalar_path=1), dict(scalar_path=1, lanes_per_agent=128, agents_per_thread=2, cull=1),
     dict(lanes_per_agent=512, agents_per_thread=1), dict(lanes_per_agent=1, agents_per_thread=2, max_ctas=3),
+    dict(lanes_per_agent=512, agents_per_thread=2), dict(lanes_per_agent=256, agents_per_thread=2),   # 32 / 16 partials per epilogue lane
+    dict(lanes_per_agent=64, agents_per_thread=1, max_ctas=7),                                        # 7 groups of 2 warps
     dict(max_ctas=1), dict(max_ctas=1, cull=1, stage=0),      # > 32 agents per CTA: chunked warps (mode 4)
 ], ids=lambda t: "-".join(f"{k[:4]}{v}" for k, v in t.items()))
 def test_launch_variants_match_oracle(api, ctx, orc, tuning):
     try:
         for moving in (False, True):
             _check_rollout(api, ctx, orc, scenes.fast_clutter(moving=moving, n_agents=45, n_spheres=333), tuning=tuning)
+    finally:
+        ctx.set_tuning(reset=True)
+
+
+@pytest.mark.parametrize("tuning", [None, dict(max_ctas=6), dict(max_ctas=6, lanes_per_agent=64), dict(lanes_per_agent=128),
+                                    dict(lanes_per_agent=64, cull=1), dict(lanes_per_agent=512), dict(scalar_path=1)],
+                         ids=lambda t: "default" if t is None else "-".join(f"{k[:4]}{v}" for k, v in t.items()))
+def test_pose6_launch_variants_match_oracle(api, ctx, orc, tuning):
+    """6D agents across the wide kernel's shapes: LIN + ROT warps (<= 3 groups), one epilogue warp (4 groups),
+    2 / 4 / 8 / 16 partials per reducing lane, static and moving spheres."""
+    try:
+        for moving in (True, False):
+            sc = scenes.config4(n_agents=24, n_spheres=1100, steps=80)
+            if not moving:
+                sc.vel = None
+            _check_rollout(api, ctx, orc, sc, tuning=tuning, smooth_tol=1e-3)
     finally:
         ctx.set_tuning(reset=True)
 
