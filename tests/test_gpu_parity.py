@@ -678,6 +678,17 @@ def test_pose6_launch_variants_match_oracle(api, ctx, orc, tuning):
         ctx.set_tuning(reset=True)
 
 
+def test_moving_sphere_sets_beyond_shared_memory(api, ctx, orc):
+    """9000 moving spheres = 4500 pairs x 64 B = 288 KB: the four pair arrays do not fit shared memory, so the
+    packed kernels (point agents) and the wide kernel (6D) read them through L1 / L2 (stage 0)."""
+    sc = scenes.fast_clutter(n_agents=40, n_spheres=9000, steps=40, moving=True)
+    g, _ = _check_rollout(api, ctx, orc, sc)
+    assert g["info"]["stage"] == 0 and g["info"]["packed_x2"] == 1
+    sc = scenes.config4(n_agents=12, n_spheres=9000, steps=40)
+    g, _ = _check_rollout(api, ctx, orc, sc, smooth_tol=1e-3)
+    assert g["info"]["stage"] == 0
+
+
 def test_cull_is_bitwise_identical_to_branch_free(api, ctx):
     try:
         for sc in (scenes.fast_clutter(), scenes.fast_clutter(moving=True), scenes.config3(n_agents=300)):
