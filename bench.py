@@ -404,7 +404,7 @@ def run_ours(args):
             "wall_ms_per_step_incl_flush": wall_ms / K,
             "e2e": {"value": pairs_global * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                     "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_s / K * 1e3,
-                    "call": "gmapp_plan_cycle_host (host spheres + agents in, best index out)"},
+                    "call": "gmapp_plan_cycle_host (host spheres + agents in, best index out; the packing and rollout kernels read the pinned host buffers over the host link themselves, the selection kernel writes its result to pinned memory)"},
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_TFLOPS, "unit": "TFLOP/s",
                          "frac": achieved / PEAK_TFLOPS, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.config) if world == 1 else None,
