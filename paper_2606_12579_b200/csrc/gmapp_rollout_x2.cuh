@@ -119,7 +119,7 @@ struct X2Acc {
 // One lane's slice of the sphere sum: pairs lane, lane+L, ... ; FORCE=false is the distance-only final pass.
 // APF = true: Eq. 1 in the Khatib form on the clamped surface distance (reading N1),
 // f_j = -k_f (1/d_O - 1/r_d) / d_O^2 * d/|d|; the sums then hold the force itself (no velocity factor).
-template <int NA, bool FORCE, bool CULL, bool APF = false, class RD = RdSel<NA, false>>
+template <int NA, bool FORCE, bool CULL, bool APF = false, class RD = RdSel<NA, false>, bool REFINE = true>
 __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const float4* __restrict__ tB, int trips,
                                          int lane, int L, const float (&p)[NA][3], const float (&v)[NA][3],
                                          const RD& rd, float eps, unsigned mask, X2Acc<NA>& acc) {
@@ -140,12 +140,13 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
             const u64 y = pk2(y0, y1);
             yy[a] = y;
             const u64 t = mul2(q[a], y);
-            // y/2 by an exponent decrement on the integer pipe (exact: y is a normal number for every finite q > 0)
-            const u64 hy = GMAPP_X2_HALF_INT ? pk2(__int_as_float(__float_as_int(y0) - 0x00800000), __int_as_float(__float_as_int(y1) - 0x00800000))
-                                             : mul2(y, half);
-            float t0, t1; upk2(t, t0, t1);
-            const u64 e = pk2(fmaf(-t0, t0, q0), fmaf(-t1, t1, q1));     // Newton residual q - t^2 (exact in the FMA)
-            const u64 ds = fma2(hy, e, add2(t, nR));                     // dist - R, dist to ~1 ulp
+            u64 ds = add2(t, nR);                                        // dist - R from the raw MUFU.RSQ (~1.9e-7 relative in dist)
+            if (REFINE) {
+                const u64 hy = mul2(y, half);
+                float t0, t1; upk2(t, t0, t1);
+                const u64 e = pk2(fmaf(-t0, t0, q0), fmaf(-t1, t1, q1)); // Newton residual q - t^2 (exact in the FMA)
+                ds = fma2(hy, e, ds);                                    // dist - R, dist to ~1 ulp
+            }
             upk2(ds, d0[a], d1[a]);
             acc.dmin[a] = min3f(acc.dmin[a], d0[a], d1[a]);
             if (CULL) any = any || (fminf(d0[a], d1[a]) <= rd.get(a));
@@ -206,7 +207,7 @@ __device__ __forceinline__ void half_sum3(float kx, float ky, float kz, int lane
 // f_j = w [ (s/|v_rel|) v_rel - |v_rel| d ],  w = s / (d_O |d|^2),  s = d.v_rel, accumulated directly
 // (k_f applied after the sum).  The distance half is the static one.
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool FORCE, bool CULL, bool APF = false, class RD = RdSel<NA, false>>
+template <int NA, bool FORCE, bool CULL, bool APF = false, class RD = RdSel<NA, false>, bool REFINE = true>
 __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, const float4* __restrict__ tB,
                                                 const float4* __restrict__ tU, const float4* __restrict__ tV, int trips,
                                                 int lane, int L, float tk, const float (&p)[NA][3], const float (&v)[NA][3],
@@ -228,10 +229,13 @@ __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, c
             const u64 y = pk2(rsqrt_approx(q0), rsqrt_approx(q1));
             yy[a] = y;
             const u64 t = mul2(q[a], y);
-            const u64 hy = mul2(y, half);
-            float t0, t1; upk2(t, t0, t1);
-            const u64 e = pk2(fmaf(-t0, t0, q0), fmaf(-t1, t1, q1));
-            const u64 ds = fma2(hy, e, add2(t, nR));
+            u64 ds = add2(t, nR);
+            if (REFINE) {
+                const u64 hy = mul2(y, half);
+                float t0, t1; upk2(t, t0, t1);
+                const u64 e = pk2(fmaf(-t0, t0, q0), fmaf(-t1, t1, q1));
+                ds = fma2(hy, e, ds);
+            }
             upk2(ds, d0[a], d1[a]);
             acc.dmin[a] = min3f(acc.dmin[a], d0[a], d1[a]);
             if (CULL) any = any || (fminf(d0[a], d1[a]) <= rd.get(a));
@@ -275,13 +279,47 @@ __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, c
     }
 }
 
+// Two-pass distance refinement.  The Newton step on MUFU.RSQ (5 of the ~19 FP32 lane-operations per pair) only matters
+// where an agent is close to a surface: the raw distance is off by <= 1.9e-7 |d|, i.e. the surface distance d_O by a
+// relative 1.9e-7 (1 + R/d_O), which stays below 3.3e-6 (CF; the force is ~ 1/d_O) or 3.4e-6 (APF, ~ 1/d_O^3) while
+// d_O >= R / kNearK.  So a force sweep first runs WITHOUT the refinement and tracks the clearance as always; only if some
+// lane of the warp came closer than thr = (largest R among the lane's own spheres) / kNearK to any of them is the sweep of
+// that warp and step repeated WITH it (rare: an agent within ~1 mm of a 2 cm sphere).  The distance-only final pass and
+// the collision decision it feeds always refine.  Not part of the 35 algorithmic flop per pair either way.
+#ifndef GMAPP_X2_TWO_PASS
+#define GMAPP_X2_TWO_PASS 1
+#endif
+template <bool APF> __device__ __forceinline__ float near_k() { return APF ? 5.0f : 16.0f; }
+
+// thr of this lane: its spheres are the same every step (pairs lane, lane + L, ...), so this runs once per rollout
+template <bool APF>
+__device__ __forceinline__ float lane_near_thr(const float4* __restrict__ tB, int trips, int lane, int L) {
+    float m = 0.0f;                                        // min of -R
+    for (int i = 0, j = lane; i < trips; ++i, j += L) { const float4 s = tB[j]; m = fminf(m, fminf(s.z, s.w)); }
+    return -m / near_k<APF>();
+}
+
 // One entry point for both sweeps.  The pair arrays sit at equal distances: B = A + d, U = A + 2 d, V = A + 3 d.
+template <int NA, bool FORCE, bool CULL, bool APF, bool MV, bool REFINE, class RD>
+__device__ __forceinline__ void sweep_pass(const float4* __restrict__ tA, const float4* __restrict__ tB, int trips, int lane, int L,
+                                           float tk, const float (&p)[NA][3], const float (&v)[NA][3], const RD& rd, float eps,
+                                           unsigned mask, X2Acc<NA>& acc) {
+    if (MV) sweep_x2_moving<NA, FORCE, CULL, APF, RD, REFINE>(tA, tB, tB + (tB - tA), tB + 2 * (tB - tA), trips, lane, L, tk, p, v, rd, eps, mask, acc);
+    else    sweep_x2<NA, FORCE, CULL, APF, RD, REFINE>(tA, tB, trips, lane, L, p, v, rd, eps, mask, acc);
+}
 template <int NA, bool FORCE, bool CULL, bool APF, bool MV, class RD>
 __device__ __forceinline__ void sweep_any(const float4* __restrict__ tA, const float4* __restrict__ tB, int trips, int lane, int L,
                                           float tk, const float (&p)[NA][3], const float (&v)[NA][3], const RD& rd, float eps,
-                                          unsigned mask, X2Acc<NA>& acc) {
-    if (MV) sweep_x2_moving<NA, FORCE, CULL, APF>(tA, tB, tB + (tB - tA), tB + 2 * (tB - tA), trips, lane, L, tk, p, v, rd, eps, mask, acc);
-    else    sweep_x2<NA, FORCE, CULL, APF>(tA, tB, trips, lane, L, p, v, rd, eps, mask, acc);
+                                          unsigned mask, float thr, X2Acc<NA>& acc) {
+    if (FORCE && GMAPP_X2_TWO_PASS) {
+        sweep_pass<NA, FORCE, CULL, APF, MV, false>(tA, tB, trips, lane, L, tk, p, v, rd, eps, mask, acc);
+        bool near = false;
+#pragma unroll
+        for (int a = 0; a < NA; ++a) near = near || (acc.dmin[a] < thr);
+        if (!__any_sync(mask, near)) return;
+        acc.clear();
+    }
+    sweep_pass<NA, FORCE, CULL, APF, MV, true>(tA, tB, trips, lane, L, tk, p, v, rd, eps, mask, acc);
 }
 
 // Transposed butterfly over a full warp.  In: per-lane partial (x,y,z) of NA agents.  Out: every lane of
@@ -509,6 +547,7 @@ __device__ __forceinline__ void group_rollout_warp_n(const RolloutX2Params& P, c
     rd.v[0] = __shfl_sync(full, me.rd, 0);
     if (NA == 2) rd.v[NA - 1] = __shfl_sync(full, me.rd, 16);
     X2Acc<NA> acc;
+    const float thr = lane_near_thr<APF>(tB, trips, lane, 32);
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);                  // pose S+1: distance-only pass
         const float tk = fmaf(float(k), P.dt, P.t0);       // obstacle time (moving spheres)
@@ -523,8 +562,8 @@ __device__ __forceinline__ void group_rollout_warp_n(const RolloutX2Params& P, c
             for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
         }
         acc.clear();
-        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, acc);
-        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, thr, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, thr, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
         if (last) {
@@ -569,7 +608,7 @@ __device__ __forceinline__ void agent_load(AgentX2& a, const float* r) {
 
 template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
 __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p, int agent0,
-                                           int lane, int k, float* rec0) {
+                                           int lane, int k, float thr, float* rec0) {
     const int half = (NA == 2) ? (lane >> 4) : 0;
     const unsigned full = 0xffffffffu;
     float* rec = rec0 + half * kAgentRecWords;
@@ -593,8 +632,8 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     const float tk = fmaf(float(k), P.dt, P.t0);
     X2Acc<NA> acc;
     acc.clear();
-    if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, acc);
-    else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, acc);
+    if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, thr, acc);
+    else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, thr, acc);
     float X, Y, Z, D;
     warp_combine<NA>(acc, lane, X, Y, Z, D);
     const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
@@ -622,10 +661,11 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
         agent_store(a, recs + i * kAgentRecWords);
     }
     __syncwarp();
+    const float thr = lane_near_thr<APF>(tB, n2p >> 5, lane, 32);
     for (int k = 0; k <= P.steps; ++k) {
         int i = 0;
-        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL, APF, PER, XT, MV>(P, tA, tB, n2p, first_agent + i, lane, k, recs + i * kAgentRecWords);
-        if (i < n_mine) chunk_step<1, CULL, APF, PER, XT, MV>(P, tA, tB, n2p, first_agent + i, lane, k, recs + i * kAgentRecWords);
+        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL, APF, PER, XT, MV>(P, tA, tB, n2p, first_agent + i, lane, k, thr, recs + i * kAgentRecWords);
+        if (i < n_mine) chunk_step<1, CULL, APF, PER, XT, MV>(P, tA, tB, n2p, first_agent + i, lane, k, thr, recs + i * kAgentRecWords);
     }
 }
 
@@ -659,12 +699,13 @@ __device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, co
         for (int i = 0; i < 3; ++i) { p[a][i] = s[i]; v[a][i] = s[3 + i]; }
     }
     X2Acc<NA> acc;
+    const float thr = lane_near_thr<APF>(tB, trips, lane_in_group, P.L);
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         const float tk = fmaf(float(k), P.dt, P.t0);
         acc.clear();
-        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
-        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, thr, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, thr, acc);
 #pragma unroll
         for (int a = 0; a < NA; ++a) {                     // per-lane partials; the epilogue warp reduces them
             float x0, x1, y0, y1, z0, z1;
@@ -745,6 +786,7 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 #pragma unroll
     for (int a = 0; a < NA; ++a) { ag[a].init(P, first_agent + a); rd.v[a] = ag[a].rd; }
     X2Acc<NA> acc;
+    const float thr = lane_near_thr<APF>(tB, trips, lane_in_group, P.L);
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         const float tk = fmaf(float(k), P.dt, P.t0);
@@ -753,8 +795,8 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 #pragma unroll
             for (int i = 0; i < 3; ++i) { p[a][i] = ag[a].p[i]; v[a][i] = ag[a].v[i]; }
         acc.clear();
-        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
-        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, thr, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, thr, acc);
         float x[NA], y[NA], z[NA], dm[NA];
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
