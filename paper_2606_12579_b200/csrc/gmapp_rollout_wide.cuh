@@ -118,7 +118,7 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
     const float4* state = xch + NA * P.L;
     const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
     const int trips = n2p >> P.logL;                       // n2p is a multiple of L
-    const float4* tA = tile; const float4* tB = tile + astride; const float4* tU = tile + 2 * astride; const float4* tV = tile + 3 * astride;
+    const float4* tA = tile; const float4* tB = tile + astride;       // (U, V follow at the same spacing)
     float p[NA][3], v[NA][3];
     RdSel<NA, PER> rd; rd.u = P.r_d;
 #pragma unroll
@@ -131,17 +131,14 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
         p[a][0] = sp.x; p[a][1] = sp.y; p[a][2] = sp.z; v[a][0] = sv.x; v[a][1] = sv.y; v[a][2] = sv.z;
     }
     X2Acc<NA> acc;
+    const float thr = lane_near_thr<APF>(tB, trips, lane_in_group, P.L);     // two-pass distance refinement (gmapp_rollout_x2.cuh)
+    bool hot = false;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         const float tk = fmaf(float(k), P.dt, P.t0);
         acc.clear();
-        if (MOVING) {
-            if (!last) sweep_x2_moving<NA, true, CULL, APF>(tA, tB, tU, tV, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
-            else       sweep_x2_moving<NA, false, false>(tA, tB, tU, tV, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, acc);
-        } else {
-            if (!last) sweep_x2<NA, true, CULL, APF>(tA, tB, trips, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
-            else       sweep_x2<NA, false, false>(tA, tB, trips, lane_in_group, P.L, p, v, rd, P.eps, full, acc);
-        }
+        if (!last) sweep_any<NA, true, CULL, APF, MOVING>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, thr, hot, acc);
+        else       sweep_any<NA, false, false, false, MOVING>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, thr, hot, acc);
 #pragma unroll
         for (int a = 0; a < NA; ++a) {                     // per-lane partials; the epilogue warp reduces them
             float x0, x1, y0, y1, z0, z1;

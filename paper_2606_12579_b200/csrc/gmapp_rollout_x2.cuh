@@ -284,8 +284,10 @@ __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, c
 // relative 1.9e-7 (1 + R/d_O), which stays below 3.3e-6 (CF; the force is ~ 1/d_O) or 3.4e-6 (APF, ~ 1/d_O^3) while
 // d_O >= R / kNearK.  So a force sweep first runs WITHOUT the refinement and tracks the clearance as always; only if some
 // lane of the warp came closer than thr = (largest R among the lane's own spheres) / kNearK to any of them is the sweep of
-// that warp and step repeated WITH it (rare: an agent within ~1 mm of a 2 cm sphere).  The distance-only final pass and
-// the collision decision it feeds always refine.  Not part of the 35 algorithmic flop per pair either way.
+// that warp and step repeated WITH it.  Agents of a circular field hug surfaces for many steps, so a warp that had to
+// repeat stays in the refined mode (`hot`, one pass per step, the cost of the always-refined kernel) until its agents
+// are clear again; the decision is a function of the trajectory only, so results stay bit-reproducible.  The
+// distance-only final pass and the collision decision it feeds always refine.  Not part of the 35 algorithmic flop per pair either way.
 #ifndef GMAPP_X2_TWO_PASS
 #define GMAPP_X2_TWO_PASS 1
 #endif
@@ -310,14 +312,22 @@ __device__ __forceinline__ void sweep_pass(const float4* __restrict__ tA, const 
 template <int NA, bool FORCE, bool CULL, bool APF, bool MV, class RD>
 __device__ __forceinline__ void sweep_any(const float4* __restrict__ tA, const float4* __restrict__ tB, int trips, int lane, int L,
                                           float tk, const float (&p)[NA][3], const float (&v)[NA][3], const RD& rd, float eps,
-                                          unsigned mask, float thr, X2Acc<NA>& acc) {
+                                          unsigned mask, float thr, bool& hot, X2Acc<NA>& acc) {
     if (FORCE && GMAPP_X2_TWO_PASS) {
-        sweep_pass<NA, FORCE, CULL, APF, MV, false>(tA, tB, trips, lane, L, tk, p, v, rd, eps, mask, acc);
         bool near = false;
+        if (!hot) {
+            sweep_pass<NA, FORCE, CULL, APF, MV, false>(tA, tB, trips, lane, L, tk, p, v, rd, eps, mask, acc);
+#pragma unroll
+            for (int a = 0; a < NA; ++a) near = near || (acc.dmin[a] < thr);
+            if (!__any_sync(mask, near)) return;
+            acc.clear();                                   // came close: this sweep again, refined, and stay refined
+        }
+        sweep_pass<NA, FORCE, CULL, APF, MV, true>(tA, tB, trips, lane, L, tk, p, v, rd, eps, mask, acc);
+        near = false;
 #pragma unroll
         for (int a = 0; a < NA; ++a) near = near || (acc.dmin[a] < thr);
-        if (!__any_sync(mask, near)) return;
-        acc.clear();
+        hot = __any_sync(mask, near);                      // back to the raw distance once the warp's agents are clear again
+        return;
     }
     sweep_pass<NA, FORCE, CULL, APF, MV, true>(tA, tB, trips, lane, L, tk, p, v, rd, eps, mask, acc);
 }
@@ -548,6 +558,7 @@ __device__ __forceinline__ void group_rollout_warp_n(const RolloutX2Params& P, c
     if (NA == 2) rd.v[NA - 1] = __shfl_sync(full, me.rd, 16);
     X2Acc<NA> acc;
     const float thr = lane_near_thr<APF>(tB, trips, lane, 32);
+    bool hot = false;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);                  // pose S+1: distance-only pass
         const float tk = fmaf(float(k), P.dt, P.t0);       // obstacle time (moving spheres)
@@ -562,8 +573,8 @@ __device__ __forceinline__ void group_rollout_warp_n(const RolloutX2Params& P, c
             for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
         }
         acc.clear();
-        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, thr, acc);
-        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, thr, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, thr, hot, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, thr, hot, acc);
         float X, Y, Z, D;
         warp_combine<NA>(acc, lane, X, Y, Z, D);
         if (last) {
@@ -608,7 +619,7 @@ __device__ __forceinline__ void agent_load(AgentX2& a, const float* r) {
 
 template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
 __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p, int agent0,
-                                           int lane, int k, float thr, float* rec0) {
+                                           int lane, int k, float thr, bool& hot, float* rec0) {
     const int half = (NA == 2) ? (lane >> 4) : 0;
     const unsigned full = 0xffffffffu;
     float* rec = rec0 + half * kAgentRecWords;
@@ -632,8 +643,8 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     const float tk = fmaf(float(k), P.dt, P.t0);
     X2Acc<NA> acc;
     acc.clear();
-    if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, thr, acc);
-    else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, thr, acc);
+    if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, thr, hot, acc);
+    else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, thr, hot, acc);
     float X, Y, Z, D;
     warp_combine<NA>(acc, lane, X, Y, Z, D);
     const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
@@ -662,10 +673,15 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
     }
     __syncwarp();
     const float thr = lane_near_thr<APF>(tB, n2p >> 5, lane, 32);
+    u64 hotbits = 0ull;                                    // refined-mode flag of each chunk (chunks beyond 64 share bits: harmless)
     for (int k = 0; k <= P.steps; ++k) {
-        int i = 0;
-        for (; i + 2 <= n_mine; i += 2) chunk_step<2, CULL, APF, PER, XT, MV>(P, tA, tB, n2p, first_agent + i, lane, k, thr, recs + i * kAgentRecWords);
-        if (i < n_mine) chunk_step<1, CULL, APF, PER, XT, MV>(P, tA, tB, n2p, first_agent + i, lane, k, thr, recs + i * kAgentRecWords);
+        for (int i = 0; i < n_mine; i += 2) {
+            const int c = (i >> 1) & 63;
+            bool hot = (hotbits >> c) & 1ull;
+            if (i + 2 <= n_mine) chunk_step<2, CULL, APF, PER, XT, MV>(P, tA, tB, n2p, first_agent + i, lane, k, thr, hot, recs + i * kAgentRecWords);
+            else                 chunk_step<1, CULL, APF, PER, XT, MV>(P, tA, tB, n2p, first_agent + i, lane, k, thr, hot, recs + i * kAgentRecWords);
+            hotbits = (hotbits & ~(1ull << c)) | (u64(hot) << c);
+        }
     }
 }
 
@@ -700,12 +716,13 @@ __device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, co
     }
     X2Acc<NA> acc;
     const float thr = lane_near_thr<APF>(tB, trips, lane_in_group, P.L);
+    bool hot = false;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         const float tk = fmaf(float(k), P.dt, P.t0);
         acc.clear();
-        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, thr, acc);
-        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, thr, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, thr, hot, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, thr, hot, acc);
 #pragma unroll
         for (int a = 0; a < NA; ++a) {                     // per-lane partials; the epilogue warp reduces them
             float x0, x1, y0, y1, z0, z1;
@@ -787,6 +804,7 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
     for (int a = 0; a < NA; ++a) { ag[a].init(P, first_agent + a); rd.v[a] = ag[a].rd; }
     X2Acc<NA> acc;
     const float thr = lane_near_thr<APF>(tB, trips, lane_in_group, P.L);
+    bool hot = false;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         const float tk = fmaf(float(k), P.dt, P.t0);
@@ -795,8 +813,8 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 #pragma unroll
             for (int i = 0; i < 3; ++i) { p[a][i] = ag[a].p[i]; v[a][i] = ag[a].v[i]; }
         acc.clear();
-        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, thr, acc);
-        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, thr, acc);
+        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, thr, hot, acc);
+        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, mask, thr, hot, acc);
         float x[NA], y[NA], z[NA], dm[NA];
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
