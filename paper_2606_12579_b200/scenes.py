@@ -215,6 +215,34 @@ def fast_clutter(seed: int = 0, n_agents: int = 96, n_spheres: int = 333, steps:
                  agents=_f32(np.c_[p, v]))
 
 
+def grazing(seed: int = 0, n_agents: int = 40, n_extra: int = 70, steps: int = 100, moving: bool = False) -> Scene:
+    """Parity-only scene: agents fly at ~1 m/s tangentially past one large sphere (R = 0.1 m) at surface distances of
+    0.3 - 8 mm, i.e. through and around the band eps <= d_O < R/16 where the force is most sensitive to the distance
+    (exercises the two-pass distance refinement of the packed kernels: raw -> refined -> raw again), with a ragged
+    number of small far-away spheres around."""
+    rng = np.random.default_rng(seed + 2000)
+    R, c0 = 0.1, np.array([0.0, 0.0, 0.5])
+    off = np.linspace(3e-4, 8e-3, n_agents)
+    ang = rng.uniform(0.0, 2.0 * np.pi, size=n_agents)                 # where on the sphere's equator-circle the agent passes
+    up = np.c_[np.zeros(n_agents), np.sin(ang), np.cos(ang)]
+    p = c0 + up * (R + off)[:, None] + np.array([-0.004, 0.0, 0.0])    # 4 mm before the closest point
+    v = np.array([1.0, 0.0, 0.0]) + rng.normal(0.0, 0.02, size=(n_agents, 3))
+    c = rng.uniform([-0.5, -0.5, 0.0], [0.5, 0.5, 1.0], size=(4 * n_extra, 3))
+    c = c[np.linalg.norm(c - c0, axis=1) > 0.32][:n_extra]
+    r = rng.uniform(0.01, 0.03, size=len(c))
+    xyzr = np.r_[np.c_[c0[None], [[R]]], np.c_[c, r]]
+    order = rng.permutation(len(xyzr))                                 # the big sphere lands on an arbitrary lane
+    u = None
+    if moving:
+        u = rng.uniform(-0.3, 0.3, size=(len(xyzr), 3)); u[0] = [0.02, 0.0, 0.0]
+        u = u[order]
+    g = default_gains()
+    g["k_att"] = 1.0
+    g["k_damp"] = 0.1
+    return Scene("grazing" + ("_moving" if moving else ""), KIND_POINT3, _f32(xyzr[order]), None if u is None else _f32(u),
+                 _f32(np.array([0.4, 0.0, 0.6])), g, 1e-3, steps, agents=_f32(np.c_[p, v]))
+
+
 def by_name(name: str, **kw) -> Scene:
     table = {"config1": config1, "config2": config2, "config3": config3, "config4": config4,
              "fast_clutter": fast_clutter}

@@ -623,6 +623,31 @@ def test_trajectory_output_matches_oracle_at_every_step(api, ctx, orc, tuning):
         ctx.set_tuning(reset=True)
 
 
+@pytest.mark.parametrize("tuning", [None, dict(lanes_per_agent=32), dict(lanes_per_agent=8, agents_per_thread=2, max_ctas=5),
+                                    dict(lanes_per_agent=128, agents_per_thread=2), dict(max_ctas=1), dict(stage=0, cull=1)],
+                         ids=lambda t: "auto" if t is None else "-".join(f"{k[:4]}{v}" for k, v in t.items()))
+def test_grazing_band_two_pass_refinement(api, ctx, orc, tuning):
+    """Agents skim a large sphere at 0.3 - 8 mm: surface distances below, inside and above R/16, where the packed
+    kernels switch between the raw MUFU.RSQ distance and the Newton-refined one (and back).  Full parity plus
+    positions / velocities at every step."""
+    import torch
+    try:
+        for moving in (False, True):
+            sc = scenes.grazing(moving=moving)
+            traj = torch.full((sc.n_agents, sc.steps + 1, 6), float("nan"), device="cuda:0")
+            ctx.set_trajectory_output(traj)
+            _, o0 = _check_rollout(api, ctx, orc, sc, tuning=tuning)
+            ctx.set_trajectory_output(None)
+            assert 3e-4 < o0["min_clearance"].min() < 1e-3 and o0["min_clearance"].max() > 6.25e-3   # both sides of the band
+            o = orc.rollout_scene(sc, threads=8, want_traj=True)
+            t = traj.cpu().numpy().astype(np.float64)
+            assert np.abs(t[:, :, :3] - o["traj"][:, :, :3]).max() <= 2e-5       # well inside POS_TOL
+            assert np.abs(t[:, :, 3:] - o["traj"][:, :, 3:]).max() <= 2e-4
+    finally:
+        ctx.set_trajectory_output(None)
+        ctx.set_tuning(reset=True)
+
+
 def test_trajectory_output_pose6(api, ctx, orc):
     import torch
     sc = scenes.config4(n_agents=24, n_spheres=512, steps=120)
