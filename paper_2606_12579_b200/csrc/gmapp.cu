@@ -494,6 +494,9 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     int at = A >= 2 ? 2 : 1;
     if (t && t->agents_per_thread) at = t->agents_per_thread;
     int G = (A + at - 1) / at;                                    // groups per CTA
+    // 9 to 16 one-warp groups: round the warp count up to a multiple of 4 (the kernel then gives the first A - G warps
+    // two agents and the others one), so that the four schedulers of an SM carry the same number of agent-sweeps
+    if (at == 2 && G >= 9 && G <= 16 && !(t && t->lanes_per_agent)) G = (G + 3) & ~3;
     const int tmax = kX2SweepThreads;
     const int ns = c->n_spheres;
     const int n2 = (ns + 1) / 2;

@@ -917,8 +917,17 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
     }
     const int group_in_cta = tid >> P.logL;
     const int lane_in_group = tid & (P.L - 1);
-    const int first = cta_first + group_in_cta * AT;
-    const int na = cta_end - first;
+    int first = cta_first + group_in_cta * AT;
+    int na = cta_end - first;
+    if (MODE == 1 && AT == 2) {
+        // one warp per group, G warps for n <= 2 G agents: the first n - G groups take two agents, the others one, so that
+        // a warp count that is a multiple of 4 loads the four schedulers equally (28 agents on 16 warps = 12 x 2 + 4 x 1,
+        // 7 agent-sweeps per scheduler; 14 warps x 2 would put 8 on two schedulers and 6 on the others)
+        const int G = blockDim.x >> 5, n = cta_end - cta_first;
+        const int g2 = n - G < 0 ? 0 : (n - G > G ? G : n - G);
+        first = cta_first + (group_in_cta < g2 ? 2 * group_in_cta : g2 + group_in_cta);
+        na = group_in_cta < g2 ? 2 : (first < cta_end ? 1 : 0);
+    }
     if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
     if (na <= 0) return;
     if (MODE == 1) {
