@@ -36,9 +36,9 @@ FLOP_PER_PAIR = 35.0
 NOMINAL_SMS, LANES_PER_SM, MAX_GHZ = 148, 128, 1.965
 PEAK_TFLOPS = NOMINAL_SMS * LANES_PER_SM * 2 * MAX_GHZ / 1e3
 # dram__bytes_read.sum + dram__bytes_write.sum of one config-3 rollout launch from the committed ncu capture
-# (profiles/r01_rollout_x2_full.md): 182.3 KB read + 0 B written (algorithmic: 64 KB spheres + 24 KB agents in,
+# (profiles/r01_rollout_x2_full.md, final kernel): 187.6 KB read + 0 B written (algorithmic: 64 KB spheres + 24 KB agents in,
 # 36 KB results out, which stay in L2).  Only valid for the config-3 workload.
-TRAFFIC_BYTES_PER_LAUNCH = {"config3": 182272}
+TRAFFIC_BYTES_PER_LAUNCH = {"config3": 187648}
 
 
 def parse_args():

@@ -600,7 +600,7 @@ def test_more_agents_than_one_wave_holds(api, orc):
 
 
 # ---------------------------------------------------------------------------------- explored paths (every pose)
-@pytest.mark.parametrize("tuning", [None, dict(lanes_per_agent=32), dict(max_ctas=1), dict(lanes_per_agent=8, agents_per_thread=2, max_ctas=5),
+@pytest.mark.parametrize("tuning", [None, dict(lanes_per_agent=32), dict(max_ctas=1), dict(max_ctas=2), dict(lanes_per_agent=8, agents_per_thread=2, max_ctas=5),
                                     dict(scalar_path=1)], ids=lambda t: "auto" if t is None else "-".join(f"{k[:4]}{v}" for k, v in t.items()))
 def test_trajectory_output_matches_oracle_at_every_step(api, ctx, orc, tuning):
     """Positions within 1e-4 m at EVERY step (north_star asks for step 100), for every kernel family."""
@@ -678,6 +678,7 @@ def test_trajectory_output_pose6(api, ctx, orc):
     dict(lanes_per_agent=512, agents_per_thread=2), dict(lanes_per_agent=256, agents_per_thread=2),   # 32 / 16 partials per epilogue lane
     dict(lanes_per_agent=64, agents_per_thread=1, max_ctas=7),                                        # 7 groups of 2 warps
     dict(max_ctas=1), dict(max_ctas=1, cull=1, stage=0),      # > 32 agents per CTA: chunked warps (mode 4)
+    dict(max_ctas=2), dict(max_ctas=2, cull=1, stage=0),      # 23 / 22 agents per CTA on 12 one-warp groups: 11 (10) take two agents, the rest one
 ], ids=lambda t: "-".join(f"{k[:4]}{v}" for k, v in t.items()))
 def test_launch_variants_match_oracle(api, ctx, orc, tuning):
     try:

@@ -605,3 +605,22 @@ def test_depth_cloud_is_seeded_and_shaped():
     b, _, _ = scenes.depth_cloud(seed=1, n_points=5000)
     assert a.shape == (5000, 3) and a.dtype == np.float32 and np.array_equal(a, b, equal_nan=True)
     assert 0 < np.isnan(a).any(axis=1).sum() < 500
+
+
+def test_grazing_scene_is_seeded_and_skims_the_band(orc):
+    """The parity-only `grazing` scene: start surface distances to the 0.1 m sphere span 0.3-8 mm (below, inside and
+    above R/16 = 6.25 mm), nothing else within the influence radius of the start cloud, and the oracle keeps every
+    agent out of collision while the closest ones stay under 1 mm."""
+    a, b = scenes.grazing(), scenes.grazing()
+    assert np.array_equal(a.agents, b.agents) and np.array_equal(a.xyzr, b.xyzr) and a.vel is None
+    big = int(np.argmax(a.xyzr[:, 3]))
+    assert a.xyzr[big, 3] == np.float32(0.1) and (a.xyzr[:, 3] > 0.05).sum() == 1
+    d0 = np.linalg.norm(a.agents[:, :3].astype(np.float64) - a.xyzr[big, :3], axis=1) - 0.1
+    assert 2e-4 < d0.min() < 5e-4 and 7e-3 < d0.max() < 9e-3
+    others = np.delete(np.arange(a.n_spheres), big)
+    dd = np.linalg.norm(a.agents[:, None, :3].astype(np.float64) - a.xyzr[None, others, :3], axis=2) - a.xyzr[None, others, 3]
+    assert dd.min() > a.gains["r_influence"]
+    o = orc.rollout_scene(a)
+    assert not o["collided"].any() and o["min_clearance"].min() < 1e-3 and o["min_clearance"].max() > 6.25e-3
+    m = scenes.grazing(moving=True)
+    assert m.vel is not None and m.vel.shape == (m.n_spheres, 3) and np.array_equal(m.xyzr, a.xyzr)
