@@ -17,6 +17,8 @@
 //    lanes 0-15, agent b on lanes 16-31), publishes the new state and only then accumulates the costs; the
 //    sweep warps pick the state up after a named barrier.  Split arrive / sync barriers and parity double-
 //    buffering: one round trip per step; what does not need the sums is computed before the wait.
+//  * Two-pass distance refinement: force sweeps run on the raw MUFU.RSQ distance; only a warp one of whose lanes came
+//    within R/16 of a surface repeats its sweep with the Newton step (and stays refined while its agents are near).
 //  * With more than 32 agents per CTA every warp owns a block of agents and walks it in chunks of two inside each
 //    step (per-agent state records in shared memory): no cross-warp traffic at all, 0.63 of FP32 peak.
 //  * Template parameters where a run-time choice costs speed: CULL (warp-vote skip of the force half), STAGE (shared
