@@ -648,6 +648,32 @@ def test_grazing_band_two_pass_refinement(api, ctx, orc, tuning):
         ctx.set_tuning(reset=True)
 
 
+@pytest.mark.parametrize("tuning", [None, dict(lanes_per_agent=32), dict(lanes_per_agent=128, agents_per_thread=2), dict(max_ctas=1),
+                                    dict(lanes_per_agent=8, agents_per_thread=2, max_ctas=5)],
+                         ids=lambda t: "auto" if t is None else "-".join(f"{k[:4]}{v}" for k, v in t.items()))
+def test_rollout_kernel_forces_from_one_big_step(api, ctx, orc, tuning):
+    """The force the ROLLOUT kernels themselves sum (raw or refined distance sweep, whichever the warp picks), read
+    back from a one-step rollout with a large step: v1 = v0 + vel_factor dt f (Eq. 9-10), so f = (v1 - v0) / c with
+    c = 0.5 * 0.125 exact.  Within north_star's 1e-5 relative (G29) plus the FP32 rounding of v1 itself, on the grazing
+    scene (surface distances 0.3-8 mm: below, inside and above the R/16 switch) and on fast clutter."""
+    import copy
+    try:
+        for sc0 in (scenes.grazing(), scenes.grazing(moving=True), scenes.fast_clutter(n_agents=45, n_spheres=333),
+                    scenes.fast_clutter(n_agents=45, n_spheres=333, moving=True)):
+            sc = copy.copy(sc0); sc.dt = 0.125; sc.steps = 1
+            g = api.run_scene(ctx, sc, tuning=tuning)
+            c = 0.5 * sc.dt * 1.0                                       # vel_factor * dt * inv_mass (defaults, reading G15/G16)
+            assert sc.gains.get("vel_factor", 0.5) == 0.5 and sc.gains.get("inv_mass", 1.0) == 1.0
+            v0, v1 = sc.agents[:, 3:].astype(np.float64), g["final"][:, 3:].astype(np.float64)
+            ref = orc.forces_point3(sc.agents.astype(np.float64), sc.xyzr, sc.vel, sc.goal, sc.gains, 0.0)
+            err = np.linalg.norm((v1 - v0) / c - ref["f_total"], axis=1)
+            tol = FORCE_RTOL * ref["scale"] + 2.0 ** -23 * np.maximum(np.abs(v1).max(axis=1), 1.0) / c * np.sqrt(3.0)
+            ok = ref["margins"][:, 0] >= 1e-6
+            assert (~ok).sum() <= 1 and np.all(err[ok] <= tol[ok]), (sc.name, (err / tol)[ok].max())
+    finally:
+        ctx.set_tuning(reset=True)
+
+
 def test_trajectory_output_pose6(api, ctx, orc):
     import torch
     sc = scenes.config4(n_agents=24, n_spheres=512, steps=120)
