@@ -409,6 +409,8 @@ def run_ours(args):
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_TFLOPS, "unit": "TFLOP/s",
                          "frac": achieved / PEAK_TFLOPS, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.config) if world == 1 else None,
                          "kernel": "k_rollout (branch-free variant, cull=0)", "kernel_ms": bf_ms,
+                         "distance_refinement": "two-pass: raw MUFU.RSQ sweep, Newton step only for a warp within R/16 of a surface "
+                                                "(neither is part of the 35 flop per pair; DESIGN.md section 6)",
                          "flop_per_pair": FLOP_PER_PAIR, "pairs_per_launch": pairs_local,
                          "peak_how": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (guide unit counts, max clock)",
                          "peak_measured_ffma_tflops": peak_meas, "peak_measured_ffma2_tflops": peak_meas_x2,
