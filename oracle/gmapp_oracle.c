@@ -19,6 +19,10 @@
  * P10 SE(3) exp/log vs scipy expm/logm and 6D == 3D reduction, P11 cost closed forms,
  * P12 agent independence, P13 brute-force numpy restatement, P14 APF (Eq. 1 under reading N1): hand-computed
  * single-sphere cases, F = -grad of the Khatib potential, superposition and mirror symmetry.
+ * P16 (tests/test_oracle_pins_6d.py) the 6D rollout against T <- T expm(dt hat(twist)), e = vee(logm(T^-1 T_g)) on
+ * 4x4 matrices with the closed-form force, random orientations + translation error + repulsion (fixes every
+ * transpose / multiplication order of pose6_wrench and orc_rollout_pose6), P17 rigid-motion equivariance of the 6D
+ * rollout, P18 quat_to_R hand cases + scipy, P19 the diagnostics scale / margins / kappa by hand from P5-A.
  * parity unpinned (fixed by DESIGN.md readings only, the paper gives no value to pin them to):
  * G16 (the 1/2 of Eq. 10 is taken as printed), G18 (frame of the 6D repulsion), G19 (N_k = S+1),
  * G23 (default constants), G24 (collision-first selection key).

@@ -183,6 +183,30 @@ def rollout_pose6(quat, pos, twist, xyzr, vel, goal_quat, goal_pos, gains: dict,
     return out
 
 
+def rollout_pose6_mat(R0, p0, twist0, xyzr, vel, goal_R, goal_p, gains: dict, dt: float, steps: int,
+                      want_traj: bool = False):
+    """6D rollout from rotation MATRICES given in double (no quaternion conversion, no FP32 rounding of the
+    poses): the same C routine as rollout_pose6, for the pins that need exactly rotated / translated inputs."""
+    R0 = _f64c(R0).reshape(-1, 9)
+    p0, tw0 = _f64c(p0), _f64c(twist0)
+    Rg, pg = _f64c(goal_R).reshape(9), _f64c(goal_p)
+    xyzr, vel = _f32c(xyzr), _f32c(vel)
+    n, m = p0.shape[0], xyzr.shape[0]
+    out = dict(R=np.zeros((n, 9)), p=np.zeros((n, 3)), twist=np.zeros((n, 6)), cost=np.zeros((n, 5)),
+               min_clearance=np.zeros(n), collided=np.zeros(n, dtype=np.int32), margins=np.zeros((n, 3)))
+    traj = np.zeros((n, steps + 1, 18)) if want_traj else None
+    g = gains_struct(gains)
+    lib().orc_rollout_pose6(C.c_int(n), _dp(R0), _dp(p0), _dp(tw0), C.c_int(m), _fp(xyzr), _fp(vel),
+                            _dp(Rg), _dp(pg), C.byref(g), C.c_double(float(np.float32(dt))), C.c_int(steps),
+                            C.c_int(1), _dp(out["R"]), _dp(out["p"]), _dp(out["twist"]),
+                            _dp(out["cost"]), _dp(out["min_clearance"]), _ip(out["collided"]),
+                            _dp(out["margins"]), _dp(traj))
+    out["R"] = out["R"].reshape(n, 3, 3)
+    if want_traj:
+        out["traj"] = traj
+    return out
+
+
 def forces_pose6(R, p, twist, xyzr, vel, goal_quat, goal_pos, gains: dict, t_obstacles: float = 0.0):
     R = _f64c(R).reshape(-1, 9)
     p, twist = _f64c(p), _f64c(twist)
