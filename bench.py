@@ -35,10 +35,18 @@ FLOP_PER_PAIR = 35.0
 # FP32 peak from the guide's unit counts and clock: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz
 NOMINAL_SMS, LANES_PER_SM, MAX_GHZ = 148, 128, 1.965
 PEAK_TFLOPS = NOMINAL_SMS * LANES_PER_SM * 2 * MAX_GHZ / 1e3
-# dram__bytes_read.sum + dram__bytes_write.sum of one config-3 rollout launch from the committed ncu capture
-# (profiles/r01_rollout_x2_full.md, final kernel): 187.6 KB read + 0 B written (algorithmic: 64 KB spheres + 24 KB agents in,
-# 36 KB results out, which stay in L2).  Only valid for the config-3 workload.
+# dram__bytes_read.sum + dram__bytes_write.sum of one rollout launch, from committed `ncu --set full` captures (not
+# measurable inside an un-profiled run).  config3: profiles/r01_rollout_x2_full.md, 187.6 KB read + 0 B written
+# (algorithmic: 64 KB sphere pairs + 24 KB agents in; 36 KB results out stay in L2).  Workloads without a capture report
+# null and say why.
 TRAFFIC_BYTES_PER_LAUNCH = {"config3": 187648}
+TRAFFIC_SOURCE = {"config3": "profiles/r01_rollout_x2_full.md (ncu --set full, one launch)"}
+# every BASELINE.json config and the 3 x 3 stress sweep, plus agent counts between the grid points (launch selection)
+ALL_CONFIG_ROWS = (["config1", "config2", "config3", "config4"]
+                   + [f"sweep:{a}x{s}" for s in (4096, 16384, 65536) for a in (1024, 4096, 16384)]
+                   + ["sweep:1500x4096", "sweep:2048x4096", "sweep:3000x4096"])
+# moving spheres (config 4): FP32-pipe lane-operations per pair of the method as SURVEY.md 8(d) counts them (static: 22)
+LANE_OPS_PER_PAIR_MOVING = 36.0
 
 
 def parse_args():
@@ -53,6 +61,8 @@ def parse_args():
     ap.add_argument("--agents-per-thread", type=int, default=0)
     ap.add_argument("--stage", type=int, default=-1)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-all-configs", action="store_true", help="skip the all_configs key (every config + the sweep)")
+    ap.add_argument("--rows", default="", help="comma-separated rows for all_configs (default: all of them)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
@@ -124,28 +134,63 @@ class ClockSampler:
 
 # ------------------------------------------------------------------------------------------ oracle legs
 def oracle_rate(scene, target_seconds: float):
-    """Time the FP64 oracle, as it stands, on the host cores over a bounded sample of `scene`:
-    the first n agents, all spheres, all rollout steps.  Returns (interactions/s, cores, sample text, seconds)."""
+    """Time the FP64 oracle, as it stands, on the host cores over a bounded sample of `scene`: a seeded random sample
+    of n agents, all spheres, all rollout steps.
+    Returns (interactions/s, cores, sample text, seconds)."""
     from oracle import oracle
     cores = oracle.max_threads()
     n_all = scene.n_agents
+    order = np.random.default_rng(12579).permutation(n_all)
     probe = min(n_all, cores)
     t0 = time.perf_counter()
-    oracle.rollout_scene(scene, threads=cores, agent_slice=slice(0, probe))
+    oracle.rollout_scene(scene, threads=cores, agent_slice=np.sort(order[:probe]))
     t_probe = max(time.perf_counter() - t0, 1e-4)
     n = int(min(n_all, max(probe, (target_seconds / t_probe) * probe)))
     n = max(cores, (n // cores) * cores) if n >= cores else n
     # when the whole workload takes less than the target, repeat it so the sample is still ~target seconds of CPU work
     t_est = t_probe * n / probe
     reps = int(max(1, min(50, round(target_seconds / max(t_est, 1e-3))))) if n == n_all else 1
+    idx = np.sort(order[:n])
     t0 = time.perf_counter()
     for _ in range(reps):
-        oracle.rollout_scene(scene, threads=cores, agent_slice=slice(0, n))
+        oracle.rollout_scene(scene, threads=cores, agent_slice=idx)
     dt = time.perf_counter() - t0
     pairs = float(n) * scene.n_spheres * scene.steps * reps
-    sample = (f"first {n} of {n_all} agents x {scene.n_spheres} spheres x {scene.steps} steps, OpenMP over agents"
+    sample = (f"random {n} of {n_all} agents (seeded) x {scene.n_spheres} spheres x {scene.steps} steps, OpenMP over agents"
               + (f", repeated {reps}x" if reps > 1 else ""))
     return pairs / dt, cores, sample, dt
+
+
+def oracle_spot_check(api, scene, g_final, g_collided, n_sample: int = 16):
+    """Ties a timed row to a correct result: the GPU's final states / collision flags of `n_sample` randomly chosen
+    agents (seeded) against the FP64 oracle run on exactly those agents (agent independence, pin P12).  Agents whose
+    ORACLE trajectory moves by more than 1e-5 m under a one-ulp perturbation of the start position are counted as
+    ill-conditioned and excluded from the error maximum (0 on every BASELINE config 1-4)."""
+    from oracle import oracle
+    import copy
+    n = scene.n_agents
+    idx = np.sort(np.random.default_rng(2606).choice(n, min(n_sample, n), replace=False))
+    cores = oracle.max_threads()
+    o = oracle.rollout_scene(scene, threads=cores, agent_slice=idx)
+    s2 = copy.copy(scene)
+    k = np.float32(1.0 + 2.0 ** -23)
+    if scene.kind == 0:
+        s2.agents = scene.agents.copy(); s2.agents[:, :3] *= k
+        o2 = oracle.rollout_scene(s2, threads=cores, agent_slice=idx)
+        po, po2 = o["final"][:, :3], o2["final"][:, :3]
+        pg = g_final[idx, :3].astype(np.float64)
+    else:
+        s2.pos = scene.pos * k
+        o2 = oracle.rollout_scene(s2, threads=cores, agent_slice=idx)
+        po, po2 = o["p"], o2["p"]
+        pg = api.state14_to_pose(g_final[idx])[1]
+    good = np.abs(po2 - po).max(axis=1) <= 1e-5
+    perr = np.abs(pg - po).max(axis=1)
+    waive = (o["margins"][:, 2] < 1e-6 * scene.gains["r_influence"]) | ~good
+    flags_ok = bool(np.array_equal(g_collided[idx][~waive], o["collided"][~waive]))
+    return {"agents": int(idx.size), "max_pos_err_m": float(perr[good].max(initial=0.0)),
+            "pos_tol_m": 1e-4, "collision_flags_equal": flags_ok, "ill_conditioned": int((~good).sum()),
+            "collided_in_sample": int(o["collided"].sum()), "finite": bool(np.all(np.isfinite(g_final)))}
 
 
 def run_reference(args):
@@ -187,6 +232,74 @@ def scaled_scene(name: str, world: int):
     if name == "config1":
         raise SystemExit("config1 is fully specified (16 agents) and is not a multi-GPU workload")
     return getattr(scenes, name)(n_agents=base * world)
+
+
+def measure_row(api, scenes_mod, name, dev, flush, K, check: bool):
+    """One all_configs row: the workload `name` on its own context, default launch selection, branch-free kernel.
+    kernel_ms = mean CUDA-event time of the rollout launch; cycle_ms = rollout + selection + result download."""
+    import torch
+    scene = make_scene(name)
+    kind = scene.kind
+    if kind == scenes_mod.KIND_POINT3:
+        h_agents, goal = np.ascontiguousarray(scene.agents), scene.goal
+    else:
+        h_agents = api.pose_to_state14(scene.quat, scene.pos, scene.twist)
+        goal = api.pose_to_state14(scene.goal_quat, scene.goal, np.zeros(6))[0, :8]
+    ctx = api.Context(max_agents=scene.n_agents, max_spheres=max(scene.n_spheres, 1), device=dev.index or 0)
+    d_xyzr = torch.from_numpy(scene.xyzr).to(dev)
+    d_vel = None if scene.vel is None else torch.from_numpy(scene.vel).to(dev)
+    ctx.set_obstacles(d_xyzr, d_vel, n=scene.n_spheres)
+    d_agents = torch.from_numpy(h_agents).to(dev)
+    d_out = torch.empty_like(d_agents)
+    gains = api.make_gains(scene.gains)
+    for _ in range(3):
+        ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
+        ctx.best_agent_ex(scene.alpha, scene.prev_best)
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+    torch.cuda.synchronize(dev)
+    for i in range(K):
+        flush.zero_()
+        ev[i][0].record()
+        ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
+        ev[i][1].record()
+        best = ctx.best_agent_ex(scene.alpha, scene.prev_best)
+        ev[i][2].record()
+    torch.cuda.synchronize(dev)
+    kernel_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
+    cycle_ms = float(np.mean([e[0].elapsed_time(e[2]) for e in ev]))
+    pairs = float(scene.n_agents) * scene.n_spheres * scene.steps
+    info = ctx.launch_info()
+    row = {"workload": scene.name, "n_agents": scene.n_agents, "n_spheres": scene.n_spheres, "rollout_steps": scene.steps,
+           "kernel_ms": kernel_ms, "cycle_ms": cycle_ms, "interactions_per_s": pairs / (cycle_ms * 1e-3),
+           "kernel_interactions_per_s": pairs / (kernel_ms * 1e-3),
+           "frac": pairs * FLOP_PER_PAIR / (kernel_ms * 1e-3) / 1e12 / PEAK_TFLOPS,
+           "us_per_rollout_step": kernel_ms * 1e3 / scene.steps, "best_index": int(best[0]),
+           "launch": {k: info[k] for k in ("grid", "block", "lanes_per_agent", "agents_per_thread", "agents_per_cta",
+                                           "stage", "tile_spheres", "n_tiles", "smem_bytes", "regs_per_thread", "packed_x2")}}
+    if scene.vel is not None:
+        row["frac_moving_lane_ops"] = (pairs * LANE_OPS_PER_PAIR_MOVING / (kernel_ms * 1e-3)
+                                       / (NOMINAL_SMS * LANES_PER_SM * MAX_GHZ * 1e9))
+        row["frac_note"] = ("moving spheres: `frac` counts the 35 flop of a STATIC pair; frac_moving_lane_ops counts the 36 "
+                            "FP32-pipe lane-operations of a moving pair against 148 x 128 lanes x 1.965 GHz")
+    if check:
+        col = torch.empty(scene.n_agents, dtype=torch.int32, device=dev)
+        ctx.get_results(None, None, col)
+        torch.cuda.synchronize(dev)
+        row["oracle_check"] = oracle_spot_check(api, scene, d_out.cpu().numpy(), col.cpu().numpy())
+    ctx.close()
+    del d_xyzr, d_vel, d_agents, d_out
+    return row
+
+
+def run_all_configs(api, scenes_mod, dev, flush, rows, check: bool):
+    out = {"note": "every BASELINE.json config and the 3 x 3 stress sweep (config 5) plus three agent counts between the grid "
+                   "points; default launch selection, branch-free kernel (cull=0), L2 flushed between timed iterations; "
+                   "frac = 35 flop x pairs / kernel time / 74.45 TFLOP/s; oracle_check = FP64 oracle on 16 seeded random agents",
+           "rows": {}}
+    for name in rows:
+        big = name.startswith("sweep:") and int(name[6:].split("x")[0]) * int(name[6:].split("x")[1]) >= (1 << 28)
+        out["rows"][name] = measure_row(api, scenes_mod, name, dev, flush, 3 if big else 5, check)
+    return out
 
 
 def run_ours(args):
@@ -408,7 +521,11 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_TFLOPS, "unit": "TFLOP/s",
                          "frac": achieved / PEAK_TFLOPS, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.config) if world == 1 else None,
-                         "kernel": "k_rollout (branch-free variant, cull=0)", "kernel_ms": bf_ms,
+                         "traffic_source": TRAFFIC_SOURCE.get(args.config, "null: no committed ncu --set full capture of this workload "
+                                                              "(dram bytes cannot be read outside a profiler)"),
+                         "kernel": ("k_rollout_x2" if info_bf["packed_x2"] else "k_rollout / k_rollout_wide")
+                                   + " (branch-free variant, cull=0; the persistent rollout kernel, one launch per cycle)",
+                         "kernel_ms": bf_ms,
                          "distance_refinement": "two-pass: raw MUFU.RSQ sweep, Newton step only for a warp within R/16 of a surface "
                                                 "(neither is part of the 35 flop per pair; DESIGN.md section 6)",
                          "flop_per_pair": FLOP_PER_PAIR, "pairs_per_launch": pairs_local,
@@ -425,6 +542,9 @@ def run_ours(args):
                                      "bit-identical results; not used for the roofline"},
             "clocks": sampler.summary(),
         }
+        if world == 1 and not args.no_all_configs:
+            rows = [r for r in args.rows.split(",") if r] or ALL_CONFIG_ROWS
+            line["all_configs"] = run_all_configs(api, scenes, dev, flush, rows, check=not args.no_cpu_baseline)
         if world == 1 and not args.no_cpu_baseline:
             r, cores, sample, dt = oracle_rate(scene, args.cpu_seconds)
             line["cpu_baseline"] = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,

@@ -136,7 +136,7 @@ gmapp_status gmapp_build_sphere_world(gmapp_ctx* ctx, const float* d_points, int
                                       void* cuda_stream);
 
 /* Copy the first n spheres of the resident sphere world, (x, y, z, r) each, into a caller-owned DEVICE buffer
- * [n][4] (after gmapp_build_sphere_world: the occupied-voxel spheres, then sentinels at 1e18).  Asynchronous. */
+ * [n][4] (after gmapp_build_sphere_world: the occupied-voxel spheres, then sentinels at (1e6, 1e6, 1e6) with radius 0).  Asynchronous. */
 gmapp_status gmapp_get_obstacles(gmapp_ctx* ctx, float* d_xyzr_out, int n, void* cuda_stream);
 
 /* Optional launch tuning for later gmapp_rollout / gmapp_forces calls; NULL restores automatic choice. */

@@ -27,6 +27,10 @@
 namespace gmapp {
 
 constexpr float kTiny = 1e-30f;          // bias that keeps squared norms > 0 (absorbed exactly otherwise)
+// Sentinel spheres (padding of the sphere arrays) sit at (kFar, kFar, kFar) with radius 0: never gated, never the
+// minimum, and far enough that every quantity derived from them stays FINITE in FP32 (|d|^2 ~ 3e12, d_O |d|^2 ~ 5e18).
+// The sphere world and the agents must stay within |coordinate| <= 1e5 m of the origin.
+constexpr float kFar = 1.0e6f;
 constexpr int kMaxGroupsNamedBar = 15;   // named barriers 1..15
 
 struct RolloutParams {
@@ -633,8 +637,8 @@ __global__ void k_pack_spheres(const float* __restrict__ xyzr, const float* __re
                                float r_agent, float4* __restrict__ sph, float4* __restrict__ svel,
                                float4* __restrict__ pairs, int stride) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    // sentinel: far away (|d|^2 ~ 3e36 stays finite in FP32), never gated, never the minimum
-    float4 s = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f), u = make_float4(0, 0, 0, 0);
+    // sentinel: far away, never gated, never the minimum
+    float4 s = make_float4(kFar, kFar, kFar, 0.0f), u = make_float4(0, 0, 0, 0);
     if (i < n) {
         s = make_float4(xyzr[4 * i], xyzr[4 * i + 1], xyzr[4 * i + 2], xyzr[4 * i + 3] + r_agent);
         if (vel) u = make_float4(vel[3 * i], vel[3 * i + 1], vel[3 * i + 2], 0.0f);

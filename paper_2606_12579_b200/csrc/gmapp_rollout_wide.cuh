@@ -141,9 +141,8 @@ __device__ __forceinline__ void wide_sweep_warps(const RolloutParams& P, const f
         else       sweep_any<NA, false, false, false, MOVING>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, thr, hot, acc);
 #pragma unroll
         for (int a = 0; a < NA; ++a) {                     // per-lane partials; the epilogue warp reduces them
-            float x0, x1, y0, y1, z0, z1;
-            upk2(acc.bx[a], x0, x1); upk2(acc.by[a], y0, y1); upk2(acc.bz[a], z0, z1);
-            part[a * P.L + lane_in_group] = make_float4(x0 + x1, y0 + y1, z0 + z1, acc.dmin[a]);
+            constexpr bool SC = acc_scaled<APF, MOVING>();
+            part[a * P.L + lane_in_group] = make_float4(acc_fold<SC>(acc.bx[a]), acc_fold<SC>(acc.by[a]), acc_fold<SC>(acc.bz[a]), acc.dmin[a]);
         }
         const int par = k & 1;
         named_bar_arrive(bar_part, nbar);

@@ -56,6 +56,21 @@ __device__ __forceinline__ void named_bar_arrive(int id, int count) {
 __device__ __forceinline__ int fkey(float x) { int b = __float_as_int(x); return b ^ ((b >> 31) & 0x7fffffff); }
 __device__ __forceinline__ float fkey_inv(int k) { return __int_as_float(k ^ ((k >> 31) & 0x7fffffff)); }
 
+// One MUFU.RCP per sphere PAIR in the circular-field sweep (static spheres): r = 1 / (K n0 n1) with n = d_O |d|^2,
+// 1/(K n0) = r n1 and 1/n1 = r (K n0).  K = 2^47 centres the product of two denominators (each between ~1e-33, an agent
+// exactly on a sphere centre, and ~1e26, a sphere 1e8 m away) in the FP32 range.  The low half of every accumulator
+// therefore holds its sum divided by K; acc_fold() puts the two halves together.  Sentinel pairs sit at kFar (finite
+// denominators: 0 * inf would poison the real sphere sharing a pair with a sentinel).
+#ifndef GMAPP_X2_PAIR_RCP
+#define GMAPP_X2_PAIR_RCP 0
+#endif
+constexpr float kPairK = 140737488355328.0f;               // 2^47
+template <bool SCALED> __device__ __forceinline__ float acc_fold(u64 v) {
+    float lo, hi; upk2(v, lo, hi);
+    return SCALED ? fmaf(lo, kPairK, hi) : lo + hi;
+}
+template <bool APF, bool MV> __host__ __device__ constexpr bool acc_scaled() { return GMAPP_X2_PAIR_RCP && !APF && !MV; }
+
 struct RolloutX2Params {
     const float4* pairA;      // [n2p] (cx0,cx1,cy0,cy1)
     const float4* pairB;      // [n2p] (cz0,cz1,-R0,-R1)
@@ -141,9 +156,11 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
             const float y0 = rsqrt_approx(q0), y1 = rsqrt_approx(q1);
             const u64 y = pk2(y0, y1);
             yy[a] = y;
-            const u64 t = mul2(q[a], y);
-            u64 ds = add2(t, nR);                                        // dist - R from the raw MUFU.RSQ (~1.9e-7 relative in dist)
+            u64 ds;
+            if (!REFINE) ds = fma2(q[a], y, nR);                         // dist - R from the raw MUFU.RSQ (~1.9e-7 relative in dist), one FFMA2
             if (REFINE) {
+                const u64 t = mul2(q[a], y);
+                ds = add2(t, nR);
                 const u64 hy = mul2(y, half);
                 float t0, t1; upk2(t, t0, t1);
                 const u64 e = pk2(fmaf(-t0, t0, q0), fmaf(-t1, t1, q1)); // Newton residual q - t^2 (exact in the FMA)
@@ -174,8 +191,15 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
             const u64 den = mul2(pk2(fmaxf(d0[a], eps), fmaxf(d1[a], eps)), q[a]);     // d_O * |d|^2
             float n0, n1; upk2(den, n0, n1);
             float r0 = 0.0f, r1 = 0.0f;
+#if GMAPP_X2_PAIR_RCP
+            const float n0k = n0 * kPairK;
+            const float r = rcp_approx(n0k * n1);                            // one MUFU.RCP for the two pairs
+            if (d0[a] <= rd.get(a)) r0 = r * n1;                             // 1 / (K n0); Alg. 1 line 7: outside r_d contributes 0
+            if (d1[a] <= rd.get(a)) r1 = r * n0k;                            // 1 / n1
+#else
             if (d0[a] <= rd.get(a)) r0 = rcp_approx(n0);                     // Alg. 1 line 7: outside r_d contributes 0
             if (d1[a] <= rd.get(a)) r1 = rcp_approx(n1);
+#endif
             const u64 s = fma2(dx[a], bc2(v[a][0]), fma2(dy[a], bc2(v[a][1]), mul2(dz[a], bc2(v[a][2]))));
             const u64 w = mul2(s, pk2(r0, r1));
             acc.bx[a] = fma2(w, dx[a], acc.bx[a]);
@@ -230,9 +254,11 @@ __device__ __forceinline__ void sweep_x2_moving(const float4* __restrict__ tA, c
             float q0, q1; upk2(q[a], q0, q1);
             const u64 y = pk2(rsqrt_approx(q0), rsqrt_approx(q1));
             yy[a] = y;
-            const u64 t = mul2(q[a], y);
-            u64 ds = add2(t, nR);
+            u64 ds;
+            if (!REFINE) ds = fma2(q[a], y, nR);
             if (REFINE) {
+                const u64 t = mul2(q[a], y);
+                ds = add2(t, nR);
                 const u64 hy = mul2(y, half);
                 float t0, t1; upk2(t, t0, t1);
                 const u64 e = pk2(fmaf(-t0, t0, q0), fmaf(-t1, t1, q1));
@@ -474,15 +500,12 @@ struct AgentX2 {
 // warp-level combine shared by the L >= 32 bodies: per-lane partials -> (X, Y, Z, D) of the agent owned by
 // this lane's half (NA == 2: lanes 0-15 agent 0, lanes 16-31 agent 1; NA == 1: the one agent on all lanes)
 // ---------------------------------------------------------------------------------------------
-template <int NA>
+template <int NA, bool SC>
 __device__ __forceinline__ void warp_combine(const X2Acc<NA>& acc, int lane, float& X, float& Y, float& Z, float& D) {
     float x[NA], y[NA], z[NA], dm[NA];
 #pragma unroll
     for (int a = 0; a < NA; ++a) {
-        float lo, hi;
-        upk2(acc.bx[a], lo, hi); x[a] = lo + hi;
-        upk2(acc.by[a], lo, hi); y[a] = lo + hi;
-        upk2(acc.bz[a], lo, hi); z[a] = lo + hi;
+        x[a] = acc_fold<SC>(acc.bx[a]); y[a] = acc_fold<SC>(acc.by[a]); z[a] = acc_fold<SC>(acc.bz[a]);
         dm[a] = fkey_inv(__reduce_min_sync(0xffffffffu, fkey(acc.dmin[a])));
     }
     warp_sum3<NA>(x, y, z, lane, X, Y, Z);
@@ -578,7 +601,7 @@ __device__ __forceinline__ void group_rollout_warp_n(const RolloutX2Params& P, c
         if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, thr, hot, acc);
         else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, thr, hot, acc);
         float X, Y, Z, D;
-        warp_combine<NA>(acc, lane, X, Y, Z, D);
+        warp_combine<NA, acc_scaled<APF, MV>()>(acc, lane, X, Y, Z, D);
         if (last) {
             if ((lane & 15) == 0 && (NA == 2 || lane == 0)) me.finish(P, D);
             return;
@@ -648,7 +671,7 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, thr, hot, acc);
     else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, thr, hot, acc);
     float X, Y, Z, D;
-    warp_combine<NA>(acc, lane, X, Y, Z, D);
+    warp_combine<NA, acc_scaled<APF, MV>()>(acc, lane, X, Y, Z, D);
     const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
     if (last) {
         if (writer) me.finish(P, D);
@@ -727,9 +750,8 @@ __device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, co
         else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, thr, hot, acc);
 #pragma unroll
         for (int a = 0; a < NA; ++a) {                     // per-lane partials; the epilogue warp reduces them
-            float x0, x1, y0, y1, z0, z1;
-            upk2(acc.bx[a], x0, x1); upk2(acc.by[a], y0, y1); upk2(acc.bz[a], z0, z1);
-            part[a * P.L + lane_in_group] = make_float4(x0 + x1, y0 + y1, z0 + z1, acc.dmin[a]);
+            constexpr bool SC = acc_scaled<APF, MV>();
+            part[a * P.L + lane_in_group] = make_float4(acc_fold<SC>(acc.bx[a]), acc_fold<SC>(acc.by[a]), acc_fold<SC>(acc.bz[a]), acc.dmin[a]);
         }
         const int par = k & 1;
         named_bar_arrive(bar_part, nbar);
@@ -820,10 +842,8 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
         float x[NA], y[NA], z[NA], dm[NA];
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
-            float lo, hi;
-            upk2(acc.bx[a], lo, hi); x[a] = lo + hi;
-            upk2(acc.by[a], lo, hi); y[a] = lo + hi;
-            upk2(acc.bz[a], lo, hi); z[a] = lo + hi;
+            constexpr bool SC = acc_scaled<APF, MV>();
+            x[a] = acc_fold<SC>(acc.bx[a]); y[a] = acc_fold<SC>(acc.by[a]); z[a] = acc_fold<SC>(acc.bz[a]);
             dm[a] = acc.dmin[a];
         }
         subwarp_allreduce<NA>(x, y, z, dm, P.L, mask);
@@ -948,7 +968,7 @@ __global__ void k_pack_pairs(const float4* __restrict__ sph_raw, const float4* _
                              float r_agent, float4* __restrict__ pairs, int stride) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n2_fill) return;
-    const float far = 1.0e18f;
+    const float far = kFar;
     float4 s0 = make_float4(far, far, far, 0.0f), s1 = s0, u0 = make_float4(0, 0, 0, 0), u1 = u0;
     if (2 * j < n) { s0 = sph_raw[2 * j]; s0.w += r_agent; if (svel) u0 = svel[2 * j]; }
     if (2 * j + 1 < n) { s1 = sph_raw[2 * j + 1]; s1.w += r_agent; if (svel) u1 = svel[2 * j + 1]; }

@@ -112,7 +112,7 @@ __global__ void k_vox_fill(const int* __restrict__ count, int capacity, int n_fi
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_fill) return;
     const int n = min(*count, capacity);
-    if (i >= n) sph[i] = make_float4(1.0e18f, 1.0e18f, 1.0e18f, 0.0f);
+    if (i >= n) sph[i] = make_float4(kFar, kFar, kFar, 0.0f);
     svel[i] = make_float4(0, 0, 0, 0);
 }
 

@@ -51,9 +51,12 @@ def _rot_angle(Ra, Rb):
     return np.arctan2(np.linalg.norm(vee, axis=-1), c)
 
 
-def _check_best(g, o, orc, scene):
-    """Best index exact unless the oracle's cost gap between the two candidates is below 1e-6 relative."""
+def _check_best(g, o, orc, scene, good=None):
+    """Best index exact unless the oracle's cost gap between the two candidates is below 1e-6 relative.
+    good (optional): mask of well-conditioned agents; the check needs both candidates to be well-conditioned."""
     want, want_cost = orc.best_agent(o["cost"], o["collided"], scene.alpha, scene.prev_best)
+    if good is not None:
+        assert good[want] and good[g["best"]], "the winner itself is an ill-conditioned agent: pick another scene"
     if g["best"] != want:
         cg = o["cost"][g["best"], 0]
         assert o["collided"][g["best"]] == o["collided"][want]
@@ -76,8 +79,12 @@ def _perturbed(scene):
     return s2
 
 
-def _check_rollout(api, ctx, orc, scene, tuning=None, agent_idx=None, smooth_tol=COST_TOL, allow_illcond=0.0):
+def _check_rollout(api, ctx, orc, scene, tuning=None, agent_idx=None, smooth_tol=COST_TOL, allow_illcond=0.0,
+                   cost_slack=True, threads=8, best_among_good=False):
     """Full rollout parity.  agent_idx: compare only these agents (oracle runs on the sample, P12).
+    cost_slack=False: costs within 1e-5 ABSOLUTE, nothing added for the position error (BASELINE configs 1-4).
+    best_among_good: check the best index against the oracle even when some agents are ill-conditioned, as long as
+    both candidates are well-conditioned (full-population tests on the stress scenes).
 
     Conditioning waiver: an agent whose ORACLE trajectory moves by more than
     1e-5 m when its start state is perturbed by one FP32 ulp (it crossed a gate / clamp / cut-locus
@@ -86,8 +93,8 @@ def _check_rollout(api, ctx, orc, scene, tuning=None, agent_idx=None, smooth_tol
     fraction of agents that may be waived (0 for every BASELINE.json config)."""
     g = api.run_scene(ctx, scene, tuning=tuning)
     sl = slice(None) if agent_idx is None else agent_idx
-    o = orc.rollout_scene(scene, threads=8, agent_slice=sl)
-    o2 = orc.rollout_scene(_perturbed(scene), threads=8, agent_slice=sl)
+    o = orc.rollout_scene(scene, threads=threads, agent_slice=sl)
+    o2 = orc.rollout_scene(_perturbed(scene), threads=threads, agent_slice=sl)
     key = "final" if scene.kind == scenes.KIND_POINT3 else "p"
     sens = np.abs(o2[key][:, :3] - o[key][:, :3]).max(axis=1)
     good = sens <= 1e-5
@@ -110,7 +117,7 @@ def _check_rollout(api, ctx, orc, scene, tuning=None, agent_idx=None, smooth_tol
     # costs: 1e-5 absolute plus what the position error itself explains (C_goal, C_obs are means of
     # 1/r_c-Lipschitz functions of position; C_path is 1/d1-Lipschitz in the path length)
     rc = min(scene.gains["r_cost_goal"] or scene.gains["r_influence"], scene.gains["r_cost_obs"] or scene.gains["r_influence"])
-    ctol = COST_TOL + 2.0 * perr / rc
+    ctol = COST_TOL + (2.0 * perr / rc if cost_slack else 0.0 * perr)
     gc = g["cost"][sl].astype(np.float64)
     cerr = np.abs(gc - o["cost"])
     assert np.all(cerr[good, 1:4] <= ctol[good, None]), cerr[good, 1:4].max(axis=0)
@@ -129,6 +136,8 @@ def _check_rollout(api, ctx, orc, scene, tuning=None, agent_idx=None, smooth_tol
         assert g["best"] == want_self
         if good.all():
             _check_best(g, o, orc, scene)
+        elif best_among_good:
+            _check_best(g, o, orc, scene, good)
     return g, o
 
 
@@ -201,18 +210,19 @@ def _R_to_quat(R):
 
 
 # ---------------------------------------------------------------------------------- configs 1-4
+# BASELINE.json configs 1-4 at full size: costs within 1e-5 ABSOLUTE (cost_slack=False), no ill-conditioned agent allowed
 def test_config1_tiny(api, ctx, orc):
-    g, o = _check_rollout(api, ctx, orc, scenes.config1())
+    g, o = _check_rollout(api, ctx, orc, scenes.config1(), cost_slack=False)
     assert g["info"]["kernels_launched"] == 1
 
 
 def test_config2_single_arm(api, ctx, orc):
-    _check_rollout(api, ctx, orc, scenes.config2())
+    _check_rollout(api, ctx, orc, scenes.config2(), cost_slack=False)
 
 
 def test_config2_position_after_100_steps(api, ctx, orc):
     sc = scenes.config2(steps=100)
-    _check_rollout(api, ctx, orc, sc)
+    _check_rollout(api, ctx, orc, sc, cost_slack=False)
 
 
 def test_config2_literal_draw_without_keepout(api, ctx, orc):
@@ -220,24 +230,38 @@ def test_config2_literal_draw_without_keepout(api, ctx, orc):
 
 
 def test_config3_dense_clutter(api, ctx, orc):
-    g, o = _check_rollout(api, ctx, orc, scenes.config3())
+    g, o = _check_rollout(api, ctx, orc, scenes.config3(), cost_slack=False)
     assert g["info"]["stage"] == 1 and g["info"]["grid"] >= 140       # one wave over the SMs, spheres in smem
 
 
 def test_config4_pose6_moving(api, ctx, orc):
-    _check_rollout(api, ctx, orc, scenes.config4(), smooth_tol=1e-3)
+    _check_rollout(api, ctx, orc, scenes.config4(), smooth_tol=1e-3, cost_slack=False)
 
 
 def test_config4_position_after_100_steps(api, ctx, orc):
-    _check_rollout(api, ctx, orc, scenes.config4(steps=100), smooth_tol=1e-3)
+    _check_rollout(api, ctx, orc, scenes.config4(steps=100), smooth_tol=1e-3, cost_slack=False)
 
 
-@pytest.mark.parametrize("na,ns", [(1024, 4096), (4096, 16384), (16384, 65536)])
+# config 5: all nine points of the stress sweep at the config's 200 steps, in the launch configuration bench.py times
+@pytest.mark.parametrize("na", [1024, 4096, 16384])
+@pytest.mark.parametrize("ns", [4096, 16384, 65536])
 def test_config5_sweep_sampled_agents(api, ctx, orc, na, ns):
     # stress sizes: the oracle runs on a random sample of agents over all spheres (independence, P12)
-    sc = scenes.config5(na, ns, steps=100 if ns > 4096 else 200)
+    sc = scenes.config5(na, ns)
+    assert sc.steps == 200
     idx = np.sort(np.random.default_rng(7).choice(na, 24, replace=False))
-    _check_rollout(api, ctx, orc, sc, agent_idx=idx)
+    g, o = _check_rollout(api, ctx, orc, sc, agent_idx=idx, threads=orc.max_threads(), allow_illcond=0.1)
+    # the selection kernel over the full population: exact on the GPU's own costs / flags
+    want_self, _ = orc.best_agent(g["cost"].astype(np.float64), g["collided"], sc.alpha, sc.prev_best)
+    assert g["best"] == want_self
+
+
+# full population where the full oracle is affordable: every collision flag and the best index
+@pytest.mark.parametrize("na,ns", [(1024, 4096), (4096, 4096)])
+def test_config5_full_population_flags_and_best_index(api, ctx, orc, na, ns):
+    sc = scenes.config5(na, ns)
+    g, o = _check_rollout(api, ctx, orc, sc, threads=orc.max_threads(), allow_illcond=0.05, best_among_good=True)
+    assert 0 < o["collided"].sum() < na                                # both flag values occur in the stress scene
 
 
 # ---------------------------------------------------------------------------------- exercised force model
@@ -540,7 +564,7 @@ def test_sphere_world_builder_bit_exact(api, ctx, n_points, pitch):
     assert cnt == want.shape[0]
     m = min(cnt, cap)
     assert np.array_equal(got[:m], want[:m])                       # bit-exact, voxel-index order
-    assert np.all(got[m:, 0] == np.float32(1e18)) and np.all(got[m:, 3] == 0)
+    assert np.all(got[m:, 0] == np.float32(1e6)) and np.all(got[m:, 3] == 0)
 
 
 def test_sphere_world_builder_overflow_and_errors(api, ctx):
