@@ -193,6 +193,15 @@ def oracle_spot_check(api, scene, g_final, g_collided, n_sample: int = 16):
             "collided_in_sample": int(o["collided"].sum()), "finite": bool(np.all(np.isfinite(g_final)))}
 
 
+def measured_hbm_gbs():
+    """HBM copy bandwidth of this pool's B200s: MEASURED_PEAKS.json (driver-written) or the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        return 6650.0, "of fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -255,18 +264,23 @@ def measure_row(api, scenes_mod, name, dev, flush, K, check: bool):
     for _ in range(3):
         ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
         ctx.best_agent_ex(scene.alpha, scene.prev_best)
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(K)]
     torch.cuda.synchronize(dev)
-    for i in range(K):
+    for i in range(K):                                       # the rollout kernel alone
         flush.zero_()
         ev[i][0].record()
         ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
         ev[i][1].record()
-        best = ctx.best_agent_ex(scene.alpha, scene.prev_best)
+    torch.cuda.synchronize(dev)
+    for i in range(K):                                       # the cycle: rollout + selection, nothing recorded in between
+        flush.zero_()
         ev[i][2].record()
+        ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
+        best = ctx.best_agent_ex(scene.alpha, scene.prev_best)
+        ev[i][3].record()
     torch.cuda.synchronize(dev)
     kernel_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
-    cycle_ms = float(np.mean([e[0].elapsed_time(e[2]) for e in ev]))
+    cycle_ms = float(np.mean([e[2].elapsed_time(e[3]) for e in ev]))
     pairs = float(scene.n_agents) * scene.n_spheres * scene.steps
     info = ctx.launch_info()
     row = {"workload": scene.name, "n_agents": scene.n_agents, "n_spheres": scene.n_spheres, "rollout_steps": scene.steps,
@@ -275,7 +289,8 @@ def measure_row(api, scenes_mod, name, dev, flush, K, check: bool):
            "frac": pairs * FLOP_PER_PAIR / (kernel_ms * 1e-3) / 1e12 / PEAK_TFLOPS,
            "us_per_rollout_step": kernel_ms * 1e3 / scene.steps, "best_index": int(best[0]),
            "launch": {k: info[k] for k in ("grid", "block", "lanes_per_agent", "agents_per_thread", "agents_per_cta",
-                                           "stage", "tile_spheres", "n_tiles", "smem_bytes", "regs_per_thread", "packed_x2")}}
+                                           "stage", "tile_spheres", "n_tiles", "smem_bytes", "regs_per_thread", "packed_x2",
+                                           "selection_fused")}}
     if scene.vel is not None:
         row["frac_moving_lane_ops"] = (pairs * LANE_OPS_PER_PAIR_MOVING / (kernel_ms * 1e-3)
                                        / (NOMINAL_SMS * LANES_PER_SM * MAX_GHZ * 1e9))
@@ -339,12 +354,22 @@ def run_ours(args):
     d_out = torch.empty_like(d_agents)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)      # > 126 MB L2
 
+    # the incumbent as a local index on the rank that owns it (-1 elsewhere); the rollout's fused selection tail is armed
+    # with it, and with several ranks the hysteresis rule is applied once, after the all_gather (sharding.py)
+    prev_local = sharding.local_prev(scene.prev_best, lo, hi)
+    ctx.set_selection(scene.alpha, prev_local)
+
+    def select():
+        if world == 1:
+            idx, cost, _ = ctx.best_agent_ex(scene.alpha, prev_local)
+            return idx, cost
+        raw, inc = sharding.selection_keys(ctx.select(scene.alpha, prev_local), lo, prev_local)
+        key = sharding.all_gather_best(raw, inc, scene.alpha)
+        return key[2], key[1]
+
     def cycle():
         ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
-        idx, cost, col = ctx.best_agent_ex(scene.alpha, scene.prev_best)
-        if world > 1:
-            idx = sharding.all_gather_best(sharding.local_key(col, cost, idx, lo))[2]
-        return idx, cost
+        return select()
 
     def barrier():
         if world > 1:
@@ -363,22 +388,18 @@ def run_ours(args):
             flush.zero_()                                    # L2 flush between timed iterations (untimed);
             ev[i][0].record()                                # the cycle is queued behind it: no idle-GPU host gap
             ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
-            ev[i][1].record()
-            idx, cost, col = ctx.best_agent_ex(scene.alpha, scene.prev_best)    # synchronises, 12-byte D2H
-            if world > 1:
-                idx = sharding.all_gather_best(sharding.local_key(col, cost, idx, lo))[2]
+            idx, cost = select()                             # selection (dependent launch or fused tail); the host polls its record
             ev[i][2].record()
         barrier()
     wall_ms = (time.perf_counter() - t_wall0) * 1e3
     step_ms = np.array([e[0].elapsed_time(e[2]) for e in ev])
-    roll_ms = np.array([e[0].elapsed_time(e[1]) for e in ev])
     total_ms = float(step_ms.sum())
     if world > 1:
         t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
     info = ctx.launch_info()
-    launches = K * (info["kernels_launched"] + 1)
+    launches = K * (info["kernels_launched"] + (0 if info["selection_fused"] else 1))
 
     # ---- roofline of the dominant kernel (the rollout), branch-free variant: every pair does the full math
     ctx.set_tuning(**{**tune, "cull": 0})
@@ -423,7 +444,7 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
         ctx.rollout(kind, d_agents, d_out, goal, gains, scene.dt, scene.steps)
-        ctx.best_agent_ex(scene.alpha, scene.prev_best)
+        ctx.best_agent_ex(scene.alpha, prev_local)
         lat.append((time.perf_counter() - t0) * 1e3)
     lat = np.array(lat)
     sampler2.__exit__()
@@ -473,31 +494,35 @@ def run_ours(args):
             a.record(); vctx.build_sphere_world(d_pts, lo_w, hi_w, 0.04, 32768); b.record()
         torch.cuda.synchronize(dev)
         vms = float(np.mean([a.elapsed_time(b) for a, b in ve]))
+        hbm, hbm_how = measured_hbm_gbs()
         vox = {"points": int(pts.shape[0]), "ms": vms, "GB_per_s": pts.nbytes / (vms * 1e-3) / 1e9,
-               "note": "7 small launches (memset, mark, count, scan, emit, fill, pair pack); launch-latency bound at this size"}
+               "frac_of_hbm": pts.nbytes / (vms * 1e-3) / 1e9 / hbm, "hbm_peak_GB_per_s": hbm, "hbm_peak_how": hbm_how,
+               "algorithmic_bytes": int(pts.nbytes),
+               "note": "2 launches: mark the voxel bitmap (12 B read per point), then one kernel that scans, emits the spheres in "
+                       "both layouts, writes the sentinel tail and the count and re-zeroes the bitmap; bit-exact vs oracle/voxel.py"}
         vctx.close()
 
     # ---- end to end through the C ABI with HOST buffers (sphere + agent upload, 8-byte result download)
     for _ in range(3):
         ctx.plan_cycle_host(kind, h_agents, goal, gains, scene.dt, scene.steps, h_xyzr=scene.xyzr, h_vel=scene.vel,
-                            alpha=scene.alpha, prev_best=scene.prev_best)
+                            alpha=scene.alpha, prev_best=prev_local)
     barrier()
     e2e_s = 0.0
     for i in range(K):
         flush.zero_(); torch.cuda.synchronize(dev)
         t0 = time.perf_counter()
         idx_e, cost_e = ctx.plan_cycle_host(kind, h_agents, goal, gains, scene.dt, scene.steps, h_xyzr=scene.xyzr,
-                                            h_vel=scene.vel, alpha=scene.alpha, prev_best=scene.prev_best)
+                                            h_vel=scene.vel, alpha=scene.alpha, prev_best=prev_local)
         if world > 1:
-            col_e = ctx.best_agent_ex(scene.alpha, scene.prev_best)[2]
-            idx_e = sharding.all_gather_best(sharding.local_key(col_e, cost_e, idx_e, lo))[2]
+            raw_e, inc_e = sharding.selection_keys(ctx.select(scene.alpha, prev_local), lo, prev_local)
+            idx_e = sharding.all_gather_best(raw_e, inc_e, scene.alpha)[2]
         e2e_s += time.perf_counter() - t0
     if world > 1:
         t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
     h2d = scene.xyzr.nbytes + (0 if scene.vel is None else scene.vel.nbytes) + h_agents.nbytes
-    d2h = 12
+    d2h = 36
 
     if rank == 0:
         line = {
@@ -507,17 +532,18 @@ def run_ours(args):
             "config": {"workload": scene.name, "n_agents": scene.n_agents, "n_spheres": scene.n_spheres,
                        "rollout_steps": scene.steps, "agents_per_gpu": n_local, "parallelism": f"agents x{world}",
                        "l2": "flushed between timed iterations (256 MB write, untimed)",
-                       "step": "one planning cycle: rollout kernel + selection kernel + 8-byte download",
+                       "step": "one planning cycle: rollout kernel + selection (a dependent launch behind the packed kernels, fused "
+                               "into the tail of the wide 6D kernel) + its 36-byte record polled in pinned memory",
                        "launch": info},
             "planning_cycle_latency_ms": {"device_p50": float(np.percentile(step_ms, 50)),
                                           "device_p99": float(np.percentile(step_ms, 99)),
-                                          "rollout_kernel_mean": float(roll_ms.mean()),
+                                          "rollout_kernel_mean": bf_ms,
                                           "host_200_warm": {"p50": float(np.percentile(lat, 50)), "p99": float(np.percentile(lat, 99)),
                                                             "min": float(lat.min()), "runs": 200}},
             "wall_ms_per_step_incl_flush": wall_ms / K,
             "e2e": {"value": pairs_global * K / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                     "d2h_bytes_per_step": int(d2h), "ms_per_step": e2e_s / K * 1e3,
-                    "call": "gmapp_plan_cycle_host (host spheres + agents in, best index out; the packing and rollout kernels read the pinned host buffers over the host link themselves, the selection kernel writes its result to pinned memory)"},
+                    "call": "gmapp_plan_cycle_host (host spheres + agents in, best index out; the packing and rollout kernels read the pinned host buffers over the host link themselves, the rollout's selection tail writes its record to pinned memory)"},
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": PEAK_TFLOPS, "unit": "TFLOP/s",
                          "frac": achieved / PEAK_TFLOPS, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.config) if world == 1 else None,

@@ -12,14 +12,19 @@
  * kernels; there is no CPU fallback.  Arithmetic is FP32.
  *
  * Conventions
- *  - Every call returns a gmapp_status; nothing throws, aborts or prints.  On error nothing is launched
- *    and gmapp_last_error(ctx) holds a message.
+ *  - Every call returns a gmapp_status; nothing throws, aborts or prints.  Arguments, call order and the launch shape
+ *    are checked BEFORE the first stream operation: on EINVAL / ECAPACITY / ESTATE nothing has been enqueued, and
+ *    gmapp_last_error(ctx) holds a message.  (ECUDA reports a failing CUDA runtime call, wherever it occurs.)
+ *  - Coordinates: the sphere world and the agents must stay within 1e5 m of the origin (padding slots of the sphere
+ *    arrays are sentinel spheres at (1e6, 1e6, 1e6) with radius 0).
  *  - Pointers named d_* are DEVICE pointers, caller-owned (e.g. torch tensors' data_ptr()), 16-byte
  *    alignment is NOT required.  Pointers named h_* and all struct / scalar-array arguments (goal,
  *    gains, tuning) are HOST pointers, read before the call returns.
  *  - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All calls
- *    are asynchronous on that stream except gmapp_best_agent, gmapp_plan_cycle_host,
- *    gmapp_measure_fp32_peak and gmapp_destroy, which synchronise it.
+ *    are asynchronous on that stream except gmapp_best_agent[_ex], gmapp_select, gmapp_plan_cycle_host,
+ *    gmapp_measure_fp32_peak and gmapp_destroy, which synchronise it.  The calls of one planning cycle (rollout,
+ *    selection, results) belong on ONE stream; the *_host entry points may be used from different streams (the pinned
+ *    staging buffer is guarded by an event).
  *  - The context owns only its packed sphere copy, per-agent result scratch and small pinned staging
  *    buffers, all allocated in gmapp_create (no allocation on the hot path).  One context is not
  *    thread-safe; separate contexts are independent.
@@ -80,9 +85,11 @@ typedef struct {
     int32_t cull;                /* -1 auto, 0 = branch-free force math for every pair,
                                     1 = warp-vote skip of the force math when no lane's pair is inside r_d
                                     (Alg. 1 line 7 is such a branch); results are identical */
-    int32_t stage;               /* -1 auto (1 when the set fits), 0 = read spheres from global memory / L2,
-                                    1 = stage the whole sphere set in shared memory by TMA bulk copies
-                                    (EINVAL when it does not fit)                                             */
+    int32_t stage;               /* -1 auto (1 when the set fits; else 2 where the tile ring measures faster than L2 reads:
+                                    >= 8 tiles and whole-warp groups; else 0), 0 = read spheres from global memory / L2,
+                                    1 = stage the whole sphere set in shared memory by TMA bulk copies (EINVAL when it does
+                                    not fit), 2 = stream tiles through a shared-memory ring by TMA bulk copies (packed kernels,
+                                    branch-free, groups of >= 32 lanes; EINVAL otherwise)                                   */
     int32_t max_ctas;            /* 0 = SM count; cap on the grid (for scaling experiments)           */
     int32_t scalar_path;         /* 0 = packed f32x2 kernels where they apply (POINT3 in every shape, static and
                                     moving spheres; MOTOR6 agents when a group spans >= 64 lanes and there
@@ -98,6 +105,8 @@ typedef struct {
     int32_t smem_bytes, regs_per_thread;
     int32_t kernels_launched;    /* kernels this call enqueued */
     int32_t packed_x2;           /* 1 = the packed f32x2 kernel ran, 0 = the scalar kernel */
+    int32_t selection_fused;     /* 1 = the selection ran in the tail of the rollout kernel (wide 6D kernel), 0 = gmapp_best_agent
+                                    launches the selection kernel behind the rollout (programmatic stream serialisation) */
 } gmapp_launch_info;
 
 /* Fill *g with the defaults listed above (k_circ 1, k_att 2, k_damp 0.5, rot 2 / 0.5, inv 1, 1/2,
@@ -118,7 +127,8 @@ gmapp_status gmapp_destroy(gmapp_ctx* ctx);
  * changed once that work has run.  Radii must be >= 0 and all values finite (not checked on device). */
 gmapp_status gmapp_set_obstacles(gmapp_ctx* ctx, const float* d_xyzr, const float* d_vel, int n, void* cuda_stream);
 /* Same with HOST arrays: copied into the context's pinned buffer, which the packing kernel then reads over the host
- * link itself (no device staging copy).  Synchronises the stream first if that buffer may still be in use. */
+ * link itself (no device staging copy).  Waits first (on an event, whatever stream it was) for the packing kernel of an
+ * earlier host call that may still be reading that buffer. */
 gmapp_status gmapp_set_obstacles_host(gmapp_ctx* ctx, const float* h_xyzr, const float* h_vel, int n, void* cuda_stream);
 
 /* Sphere-world builder (perception stage: workspace crop, "voxelise at 2 r_O", the occupied
@@ -139,7 +149,8 @@ gmapp_status gmapp_build_sphere_world(gmapp_ctx* ctx, const float* d_points, int
  * [n][4] (after gmapp_build_sphere_world: the occupied-voxel spheres, then sentinels at (1e6, 1e6, 1e6) with radius 0).  Asynchronous. */
 gmapp_status gmapp_get_obstacles(gmapp_ctx* ctx, float* d_xyzr_out, int n, void* cuda_stream);
 
-/* Optional launch tuning for later gmapp_rollout / gmapp_forces calls; NULL restores automatic choice. */
+/* Optional launch tuning for later gmapp_rollout calls (gmapp_forces has one launch shape and ignores it); NULL restores
+ * the automatic choice. */
 gmapp_status gmapp_set_tuning(gmapp_ctx* ctx, const gmapp_tuning* tuning);
 
 /* Heterogeneous ensemble ("two agents per heuristic type, each with either a large or small
@@ -149,7 +160,7 @@ gmapp_status gmapp_set_tuning(gmapp_ctx* ctx, const gmapp_tuning* tuning);
  * MFI (Eq. 2-3), 1 = APF (Eq. 1)}.  The arrays are copied before the call returns (it synchronises the stream).
  * Later gmapp_rollout calls must pass n_agents == n (else EINVAL); they issue one launch per heuristic present,
  * and the Eq. 17 / 18 radii default to each agent's own r_d.  n = 0 (or all three NULL) restores uniform agents.
- * gmapp_forces keeps using `gains` alone. */
+ * gmapp_forces keeps using `gains` alone (it ignores these arrays). */
 gmapp_status gmapp_set_agent_params(gmapp_ctx* ctx, const float* h_r_influence, const float* h_k_circ,
                                     const int32_t* h_heuristic, int n, void* cuda_stream);
 
@@ -188,7 +199,13 @@ gmapp_status gmapp_replan(gmapp_ctx* ctx, gmapp_kind kind, float* d_agents, int 
 /* Agent selection: lexicographic argmin of (collided, C_i, i) over the last rollout;
  * with prev_best >= 0 the incumbent keeps its place unless the challenger is collision-free while the
  * incumbent collided, or the flags are equal and C_best < alpha * C_prev.  A NaN cost ranks last.
- * Synchronises the stream and returns index and cost to host memory. */
+ * Synchronises the stream and returns index and cost to host memory.
+ * The reduction itself runs in the TAIL of the rollout kernel (the warp that finishes the last agent reduces all
+ * agents' keys and writes the record to pinned host memory): with prev_best < 0, or with the (alpha, prev_best) the
+ * rollout was armed with by gmapp_set_selection, this call only synchronises and reads that record -- no second launch
+ * in the planning cycle.  With other arguments (and after the scalar kernels, which have no such tail) a small
+ * selection kernel is launched.  prev_best >= n_agents of the last rollout counts as "no incumbent".  Errors: ESTATE
+ * before any rollout, EINVAL for non-finite alpha. */
 gmapp_status gmapp_best_agent(gmapp_ctx* ctx, float alpha, int prev_best, int* out_index, float* out_cost,
                               void* cuda_stream);
 
@@ -196,6 +213,21 @@ gmapp_status gmapp_best_agent(gmapp_ctx* ctx, float alpha, int prev_best, int* o
  * of which rolled its own block of agents). */
 gmapp_status gmapp_best_agent_ex(gmapp_ctx* ctx, float alpha, int prev_best, int* out_index, float* out_cost,
                                  int* out_collided, void* cuda_stream);
+
+/* The full selection record of the last rollout for (alpha, prev_best): the selected agent, the plain argmin without
+ * incumbent, and the incumbent's own key this cycle (what several GPUs exchange to apply the hysteresis rule once,
+ * globally).  Same cost and synchronisation as gmapp_best_agent. */
+typedef struct {
+    int32_t index, collided; float cost;              /* selected agent (hysteresis applied)                      */
+    int32_t raw_index, raw_collided; float raw_cost;  /* lexicographic argmin of (collided, C, index), no incumbent */
+    int32_t prev_collided; float prev_cost;           /* the incumbent's key (valid when prev_best >= 0)          */
+} gmapp_selection;
+gmapp_status gmapp_select(gmapp_ctx* ctx, float alpha, int prev_best, gmapp_selection* out, void* cuda_stream);
+
+/* Arm the selection that later gmapp_rollout calls fuse into their tail: hysteresis factor alpha and incumbent prev_best
+ * (< 0 = none, the default; an index beyond a later rollout's agents counts as none).  gmapp_plan_cycle_host and
+ * gmapp_replan arm it themselves.  EINVAL for non-finite alpha or prev_best >= max_agents. */
+gmapp_status gmapp_set_selection(gmapp_ctx* ctx, float alpha, int prev_best);
 
 /* Force query without integration (the control thread's query, Fig. 2 step 5):
  * for each state, d_f_rep [n][3] = sum_j f_j (world frame, Eq. 2-3 / Alg. 1) with obstacles at time
@@ -212,8 +244,10 @@ gmapp_status gmapp_get_results(gmapp_ctx* ctx, float* d_cost, float* d_min_clear
                                void* cuda_stream);
 
 /* A whole planning cycle from HOST buffers: (optional) sphere upload, agent states read by the rollout kernel straight
- * from the pinned buffer (and final states written back to it), selection, 12-byte result written to pinned memory; h_agents_out (may be NULL) receives the final states.
- * h_xyzr == NULL keeps the resident sphere world.  Synchronises the stream. */
+ * from the pinned buffer (and final states written back to it), selection in the rollout's tail, its record written to
+ * pinned memory; h_agents_out (may be NULL) receives the final states.
+ * n_spheres < 0 keeps the resident sphere world (ESTATE if there is none); n_spheres == 0 sets an EMPTY world (no
+ * obstacles); n_spheres > 0 uploads h_xyzr [n][4] (+ h_vel [n][3] or NULL).  Synchronises the stream. */
 gmapp_status gmapp_plan_cycle_host(gmapp_ctx* ctx, gmapp_kind kind, const float* h_agents, float* h_agents_out,
                                    int n_agents, const float* h_xyzr, const float* h_vel, int n_spheres,
                                    const float* goal, const gmapp_gains* gains, float dt, int steps,

@@ -34,17 +34,26 @@ class gmapp_tuning(C.Structure):
                 ("stage", C.c_int32), ("max_ctas", C.c_int32), ("scalar_path", C.c_int32), ("reserved", C.c_int32 * 2)]
 
 
+class gmapp_selection(C.Structure):
+    _fields_ = [("index", C.c_int32), ("collided", C.c_int32), ("cost", C.c_float),
+                ("raw_index", C.c_int32), ("raw_collided", C.c_int32), ("raw_cost", C.c_float),
+                ("prev_collided", C.c_int32), ("prev_cost", C.c_float)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
 class gmapp_launch_info(C.Structure):
     _fields_ = [(k, C.c_int32) for k in
                 ("grid", "block", "lanes_per_agent", "agents_per_thread", "agents_per_cta", "cull", "stage",
-                 "tile_spheres", "n_tiles", "smem_bytes", "regs_per_thread", "kernels_launched", "packed_x2")]
+                 "tile_spheres", "n_tiles", "smem_bytes", "regs_per_thread", "kernels_launched", "packed_x2", "selection_fused")]
 
     def as_dict(self):
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
 
 
 EXPORTS = ["gmapp_default_gains", "gmapp_create", "gmapp_destroy", "gmapp_set_obstacles",
-           "gmapp_set_obstacles_host", "gmapp_build_sphere_world", "gmapp_get_obstacles", "gmapp_set_tuning", "gmapp_set_agent_params", "gmapp_rollout", "gmapp_set_trajectory_output", "gmapp_replan", "gmapp_best_agent", "gmapp_best_agent_ex",
+           "gmapp_set_obstacles_host", "gmapp_build_sphere_world", "gmapp_get_obstacles", "gmapp_set_tuning", "gmapp_set_agent_params", "gmapp_rollout", "gmapp_set_trajectory_output", "gmapp_replan", "gmapp_best_agent", "gmapp_best_agent_ex", "gmapp_select", "gmapp_set_selection",
            "gmapp_forces",
            "gmapp_get_results", "gmapp_plan_cycle_host", "gmapp_get_launch_info", "gmapp_measure_fp32_peak",
            "gmapp_sm_count", "gmapp_last_error"]
@@ -77,6 +86,8 @@ def _load():
                                  C.c_int, C.c_int, vp, vp, vp]
     lib.gmapp_best_agent.argtypes = [vp, C.c_float, C.c_int, ip, fp, vp]
     lib.gmapp_best_agent_ex.argtypes = [vp, C.c_float, C.c_int, ip, fp, ip, vp]
+    lib.gmapp_select.argtypes = [vp, C.c_float, C.c_int, C.POINTER(gmapp_selection), vp]
+    lib.gmapp_set_selection.argtypes = [vp, C.c_float, C.c_int]
     lib.gmapp_forces.argtypes = [vp, C.c_int, vp, C.c_int, fp, C.POINTER(gmapp_gains), C.c_float, vp, vp, vp]
     lib.gmapp_get_results.argtypes = [vp, vp, vp, vp, vp]
     lib.gmapp_plan_cycle_host.argtypes = [vp, C.c_int, vp, vp, C.c_int, vp, vp, C.c_int, fp, C.POINTER(gmapp_gains),
@@ -249,6 +260,14 @@ class Context:
         self._check(_lib.gmapp_best_agent_ex(self._h, C.c_float(alpha), int(prev_best), C.byref(idx), C.byref(cost),
                                              C.byref(col), _stream(stream)))
         return idx.value, cost.value, col.value
+
+    def select(self, alpha=0.9, prev_best=-1, stream=None) -> dict:
+        rec = gmapp_selection()
+        self._check(_lib.gmapp_select(self._h, C.c_float(alpha), int(prev_best), C.byref(rec), _stream(stream)))
+        return rec.as_dict()
+
+    def set_selection(self, alpha=0.9, prev_best=-1):
+        self._check(_lib.gmapp_set_selection(self._h, C.c_float(alpha), int(prev_best)))
 
     def forces(self, kind, d_agents, goal, gains, t_obstacles, d_f_rep, d_f_total, n_agents=None, stream=None):
         n = int(d_agents.shape[0]) if n_agents is None else n_agents

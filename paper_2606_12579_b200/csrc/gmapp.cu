@@ -27,6 +27,8 @@ struct gmapp_ctx {
     float4* d_pairB = nullptr;
     float pair_r_agent = 0.0f;
     bool pair_valid = false;
+    float* d_sph_stats = nullptr;        // {largest R = r_j + r_agent, largest sphere speed} of the pair arrays (tile ring)
+    bool stats_valid = false;
     float eff_r_agent = 0.0f;
     bool eff_valid = false;
     int n_spheres = -1;            // -1: set_obstacles not called yet
@@ -46,15 +48,27 @@ struct gmapp_ctx {
     float ap_min_rd = 0.0f;
     const int* sub_idx = nullptr;        // the sub-launch being issued (one per heuristic)
     // sphere-world builder (gmapp_build_sphere_world): voxel bitmap (2^25 voxels), block sums, occupied-voxel count
-    unsigned* d_vox_bitmap = nullptr; int* d_vox_sums = nullptr; int* d_vox_count = nullptr;
+    unsigned* d_vox_bitmap = nullptr; int* d_vox_count = nullptr;
+    unsigned long long* d_vox_state = nullptr; int* d_vox_sync = nullptr;      // scan state of k_vox_compact (zero between builds)
     // closed-loop re-planning (gmapp_replan)
     float* d_snap = nullptr;             // [max_agents][14]
     int* d_prev = nullptr;               // incumbent on the device
     float roll_t0 = 0.0f; float* roll_snap = nullptr; int roll_snap_step = 0;
     float* roll_traj = nullptr;          // trajectory output of the next rollouts (gmapp_set_trajectory_output)
     bool built_world = false;            // the sphere world came from gmapp_build_sphere_world: its count lives in d_vox_count
-    int* d_best_idx = nullptr; float* d_best_cost = nullptr;
-    int* h_best = nullptr;               // pinned: {idx, cost bits}
+    // selection (S8): the 8-word record {index, collided, cost | raw index, raw collided, raw cost | incumbent collided,
+    // cost} on the device and in pinned host memory, and the ticket counter of the rollout kernels' fused tail
+    int* d_sel_rec = nullptr; int* d_sel_ticket = nullptr;
+    int* h_best = nullptr;               // pinned: the record
+    float sel_alpha = 0.9f; int sel_prev = -1;      // what later rollouts' tails are armed with (gmapp_set_selection)
+    const int* sel_prev_dev = nullptr;   // gmapp_replan: the incumbent lives on the device
+    bool sel_want = false;               // the rollout being issued may fuse the selection into its launches
+    bool sel_fused = false;              // the last rollout did: the record holds (fused_alpha, fused_prev)'s selection
+    float fused_alpha = 0.0f; int fused_prev = -1; bool fused_prev_dev = false;
+    int sel_total = 0;
+    int sel_seq = 0;                     // sequence number of the last rollout's selection record (the host polls pinned memory for it)
+    cudaEvent_t ev_pinned = nullptr;     // after the last kernel that reads the pinned sphere staging buffer
+    bool pinned_busy = false;
     float* d_scratch = nullptr;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     gmapp_tuning tuning;
@@ -155,19 +169,26 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
     ALLOC(c->d_minclr, sizeof(float) * max_agents);
     ALLOC(c->d_collided, sizeof(int) * max_agents);
     ALLOC(c->d_vox_bitmap, sizeof(unsigned) * (1u << 20));
-    ALLOC(c->d_vox_sums, sizeof(int) * 1024);
+    ALLOC(c->d_vox_state, sizeof(unsigned long long) * 1024);
+    ALLOC(c->d_vox_sync, sizeof(int) * 2);
     ALLOC(c->d_vox_count, sizeof(int));
     ALLOC(c->d_snap, sizeof(float) * 14 * max_agents);
     ALLOC(c->d_prev, sizeof(int));
     ALLOC(c->d_ap_rd, sizeof(float) * max_agents);
     ALLOC(c->d_ap_kf, sizeof(float) * max_agents);
     ALLOC(c->d_ap_idx, sizeof(int) * max_agents);
-    ALLOC(c->d_best_idx, sizeof(int) * 2);
-    ALLOC(c->d_best_cost, sizeof(float));
+    ALLOC(c->d_sel_rec, sizeof(int) * 8);
+    ALLOC(c->d_sel_ticket, sizeof(int));
     ALLOC(c->d_scratch, sizeof(float) * 64);
+    ALLOC(c->d_sph_stats, sizeof(float) * 2);
 #undef ALLOC
     if ((e = cudaMallocHost((void**)&c->h_pinned, sizeof(float) * hp)) != cudaSuccess ||
-        (e = cudaMallocHost((void**)&c->h_best, sizeof(int) * 4)) != cudaSuccess ||
+        (e = cudaMallocHost((void**)&c->h_best, sizeof(int) * 16)) != cudaSuccess ||
+        (e = cudaMemset(c->d_sel_ticket, 0, sizeof(int))) != cudaSuccess ||
+        (e = cudaMemset(c->d_vox_bitmap, 0, sizeof(unsigned) * (1u << 20))) != cudaSuccess ||
+        (e = cudaMemset(c->d_vox_state, 0, sizeof(unsigned long long) * 1024)) != cudaSuccess ||
+        (e = cudaMemset(c->d_vox_sync, 0, sizeof(int) * 2)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&c->ev_pinned, cudaEventDisableTiming)) != cudaSuccess ||
         (e = cudaMallocHost((void**)&c->h_ap, sizeof(float) * 3 * (size_t)max_agents)) != cudaSuccess ||
         (e = cudaEventCreate(&c->ev0)) != cudaSuccess || (e = cudaEventCreate(&c->ev1)) != cudaSuccess) {
         gmapp_destroy(c);
@@ -191,10 +212,11 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
         }
     for (int at = 1; at <= 2; ++at)
         for (int md = 0; md < 5; ++md)
-            for (int cu = 0; cu < 4; ++cu)
+            for (int cu = 0; cu < 6; ++cu)
                 for (int hf = 0; hf < 8; ++hf) {
-                    e = cudaFuncSetAttribute((const void*)rollout_x2_kernel(at, md, cu & 1, cu >> 1, (hf & 1) != 0, (hf & 2) != 0, (hf & 4) != 0),
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
+                    const void* fn = (const void*)rollout_x2_kernel(at, md, cu & 1, cu >> 1, (hf & 1) != 0, (hf & 2) != 0, (hf & 4) != 0);
+                    if (!fn) continue;                     // no such variant (tile ring with cull / sub-warp groups)
+                    e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
                     if (e != cudaSuccess) { gmapp_destroy(c); return fail(nullptr, GMAPP_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e)); }
                 }
     *out = c;
@@ -207,14 +229,15 @@ extern "C" gmapp_status gmapp_destroy(gmapp_ctx* c) {
     cudaDeviceSynchronize();
     cudaFree(c->d_sph_raw); cudaFree(c->d_sph_eff); cudaFree(c->d_svel); cudaFree(c->d_pairA);
     cudaFree(c->d_cost); cudaFree(c->d_minclr); cudaFree(c->d_collided);
-    cudaFree(c->d_best_idx); cudaFree(c->d_best_cost); cudaFree(c->d_scratch);
+    cudaFree(c->d_sel_rec); cudaFree(c->d_sel_ticket); cudaFree(c->d_scratch); cudaFree(c->d_sph_stats);
     cudaFree(c->d_ap_rd); cudaFree(c->d_ap_kf); cudaFree(c->d_ap_idx); cudaFree(c->d_snap); cudaFree(c->d_prev);
-    cudaFree(c->d_vox_bitmap); cudaFree(c->d_vox_sums); cudaFree(c->d_vox_count);
+    cudaFree(c->d_vox_bitmap); cudaFree(c->d_vox_state); cudaFree(c->d_vox_sync); cudaFree(c->d_vox_count);
     if (c->h_ap) cudaFreeHost(c->h_ap);
     if (c->h_pinned) cudaFreeHost(c->h_pinned);
     if (c->h_best) cudaFreeHost(c->h_best);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->ev_pinned) cudaEventDestroy(c->ev_pinned);
     delete c;
     return GMAPP_OK;
 }
@@ -229,8 +252,8 @@ extern "C" gmapp_status gmapp_set_tuning(gmapp_ctx* c, const gmapp_tuning* t) {
         (t->lanes_per_agent && (t->lanes_per_agent & (t->lanes_per_agent - 1))))
         return fail(c, GMAPP_EINVAL, "set_tuning: lanes_per_agent must be 0 or a power of two <= 1024%s");
     if (t->agents_per_thread < 0 || t->agents_per_thread > 2) return fail(c, GMAPP_EINVAL, "set_tuning: agents_per_thread must be 0, 1 or 2%s");
-    if (t->cull < -1 || t->cull > 1 || t->stage < -1 || t->stage > 1 || t->max_ctas < 0 || t->scalar_path < 0 || t->scalar_path > 1)
-        return fail(c, GMAPP_EINVAL, "set_tuning: cull in {-1,0,1}, stage in {-1,0,1}, max_ctas >= 0, scalar_path in {0,1}%s");
+    if (t->cull < -1 || t->cull > 1 || t->stage < -1 || t->stage > 2 || t->max_ctas < 0 || t->scalar_path < 0 || t->scalar_path > 1)
+        return fail(c, GMAPP_EINVAL, "set_tuning: cull in {-1,0,1}, stage in {-1,0,1,2}, max_ctas >= 0, scalar_path in {0,1}%s");
     c->tuning = *t; c->has_tuning = true;
     return GMAPP_OK;
 }
@@ -277,6 +300,7 @@ extern "C" gmapp_status gmapp_set_obstacles(gmapp_ctx* c, const float* d_xyzr, c
     c->moving = (d_vel != nullptr) && n > 0;
     c->eff_valid = false;
     c->pair_valid = true; c->pair_r_agent = 0.0f;
+    c->stats_valid = false;
     return GMAPP_OK;
 }
 
@@ -306,22 +330,38 @@ extern "C" gmapp_status gmapp_build_sphere_world(gmapp_ctx* c, const float* d_po
     G.n_words = ((int)nvox + 31) / 32;
     const int n_blocks = (G.n_words + 1023) / 1024;
     cudaStream_t st = (cudaStream_t)stream;
-    CUDA_TRY(c, cudaMemsetAsync(c->d_vox_bitmap, 0, sizeof(unsigned) * (size_t)n_blocks * 1024, st));
-    if (n_points > 0) k_vox_mark<<<(n_points + 255) / 256, 256, 0, st>>>(d_points, n_points, G, c->d_vox_bitmap);
-    k_vox_count<<<n_blocks, 1024, 0, st>>>(c->d_vox_bitmap, G.n_words, c->d_vox_sums);
-    k_vox_scan<<<1, 1024, 0, st>>>(c->d_vox_sums, n_blocks, c->d_vox_count);
-    k_vox_emit<<<n_blocks, 1024, 0, st>>>(c->d_vox_bitmap, c->d_vox_sums, G, capacity, c->d_sph_raw);
     const int nf = fill_count(c, capacity);
-    k_vox_fill<<<(nf + 255) / 256, 256, 0, st>>>(c->d_vox_count, capacity, nf, c->d_sph_raw, c->d_svel);
+    if (G.n_words <= kVoxSmallWords) {
+        // small grids (the paper's workspace): ONE launch -- per-block bitmaps in shared memory, merged, and the block that
+        // finishes last scans and emits (gmapp_voxel.cuh)
+        int grid = (n_points + 2047) / 2048;                // two points per thread
+        if (grid < 1) grid = 1;
+        if (grid > 2 * c->num_sms) grid = 2 * c->num_sms;
+        k_vox_build_small<<<grid, 1024, sizeof(unsigned) * G.n_words, st>>>(d_points, n_points, G, c->d_vox_bitmap, c->d_vox_sync, capacity, nf,
+                                                                       c->d_sph_raw, c->d_svel, c->d_pairA, c->cap_spheres / 2,
+                                                                       c->d_vox_count, d_count_out);
+        CUDA_TRY(c, cudaGetLastError());
+        c->n_spheres = capacity; c->built_world = true; c->moving = false; c->eff_valid = false;
+        c->pair_valid = true; c->pair_r_agent = 0.0f; c->stats_valid = false;
+        return GMAPP_OK;
+    }
+    // large grids, two launches: mark the global bitmap (it is zero: every build leaves it so), then ONE kernel that scans,
+    // emits the spheres into the float4 array and the sphere-pair arrays (r_agent = 0), writes the sentinel tail and the
+    // count, and zeroes the bitmap and its own scan state again
+    if (n_points > 0) k_vox_mark<<<(n_points + 255) / 256, 256, 0, st>>>(d_points, n_points, G, c->d_vox_bitmap);
+    int n_help = (nf + 1023) / 1024;                       // fill helpers: the sentinel tail in parallel
+    if (n_help > 64) n_help = 64;
+    k_vox_compact<<<n_blocks + n_help, 1024, 0, st>>>(c->d_vox_bitmap, c->d_vox_state, c->d_vox_sync, G, capacity, nf, n_blocks,
+                                                      c->d_sph_raw, c->d_svel, c->d_pairA, c->cap_spheres / 2, c->d_vox_count, d_count_out);
     CUDA_TRY(c, cudaGetLastError());
-    if (d_count_out) CUDA_TRY(c, cudaMemcpyAsync(d_count_out, c->d_vox_count, sizeof(int), cudaMemcpyDeviceToDevice, st));
     // the sphere world now holds `capacity` slots: the occupied voxels first, sentinels behind them
     c->n_spheres = capacity;
     c->built_world = true;
     c->moving = false;
     c->eff_valid = false;
-    c->pair_valid = false;
-    return effective_pairs(c, 0.0f, st, nullptr);
+    c->pair_valid = true; c->pair_r_agent = 0.0f;
+    c->stats_valid = false;
+    return GMAPP_OK;
 }
 
 extern "C" gmapp_status gmapp_get_obstacles(gmapp_ctx* c, float* d_xyzr_out, int n, void* stream) {
@@ -339,14 +379,17 @@ extern "C" gmapp_status gmapp_set_obstacles_host(gmapp_ctx* c, const float* h_xy
     if (n > c->max_spheres) return fail(c, GMAPP_ECAPACITY, "set_obstacles_host: n = %s%ld exceeds max_spheres = %ld", "", n, c->max_spheres);
     cudaStream_t st = (cudaStream_t)stream;
     if (n > 0) {
-        // the pinned buffer may still be in flight from an earlier host call on this stream
-        CUDA_TRY(c, cudaStreamSynchronize(st));
+        // the pinned buffer may still be read by the packing kernel of an earlier host call -- on ANY stream: wait for
+        // the event recorded behind that kernel
+        if (c->pinned_busy) { CUDA_TRY(c, cudaEventSynchronize(c->ev_pinned)); c->pinned_busy = false; }
         memcpy(c->h_pinned, h_xyzr, sizeof(float) * 4 * n);
         if (h_vel) memcpy(c->h_pinned + 4 * (size_t)n, h_vel, sizeof(float) * 3 * n);
     }
     // the packing kernel reads the pinned host buffer itself (unified addressing: one read over the host link instead
     // of a copy-engine transfer into a staging buffer followed by the same read)
-    return gmapp_set_obstacles(c, c->h_pinned, h_vel ? c->h_pinned + 4 * (size_t)n : nullptr, n, stream);
+    gmapp_status s = gmapp_set_obstacles(c, c->h_pinned, h_vel ? c->h_pinned + 4 * (size_t)n : nullptr, n, stream);
+    if (s == GMAPP_OK && n > 0) { CUDA_TRY(c, cudaEventRecord(c->ev_pinned, st)); c->pinned_busy = true; }
+    return s;
 }
 
 // sphere array with R = r + r_agent; launches the tiny repack kernel only when r_agent changed
@@ -371,6 +414,44 @@ static gmapp_status effective_pairs(gmapp_ctx* c, float r_agent, cudaStream_t st
                                                     c->d_pairA, c->cap_spheres / 2);
     CUDA_TRY(c, cudaGetLastError());
     c->pair_valid = true; c->pair_r_agent = r_agent;
+    c->stats_valid = false;
+    if (launches) ++*launches;
+    return GMAPP_OK;
+}
+
+// {largest R, largest sphere speed} of the current pair arrays, for the tile ring's refinement prediction; one small
+// launch per sphere world (only when a rollout takes the ring)
+__global__ void __launch_bounds__(1024) k_sphere_stats(const float4* __restrict__ pairs, int stride, int n2, int moving, float* out) {
+    float rmax = 0.0f, u2max = 0.0f;
+    for (int j = threadIdx.x; j < n2; j += blockDim.x) {
+        const float4 b = pairs[stride + j];
+        rmax = fmaxf(rmax, fmaxf(-b.z, -b.w));
+        if (moving) {
+            const float4 u = pairs[2 * stride + j], w = pairs[3 * stride + j];
+            u2max = fmaxf(u2max, fmaxf(fmaf(u.x, u.x, fmaf(u.z, u.z, w.x * w.x)), fmaf(u.y, u.y, fmaf(u.w, u.w, w.y * w.y))));
+        }
+    }
+    __shared__ float sr[32], su[32];
+    for (int off = 16; off > 0; off >>= 1) {
+        rmax = fmaxf(rmax, __shfl_xor_sync(0xffffffffu, rmax, off));
+        u2max = fmaxf(u2max, __shfl_xor_sync(0xffffffffu, u2max, off));
+    }
+    if ((threadIdx.x & 31) == 0) { sr[threadIdx.x >> 5] = rmax; su[threadIdx.x >> 5] = u2max; }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        rmax = sr[threadIdx.x]; u2max = su[threadIdx.x];
+        for (int off = 16; off > 0; off >>= 1) {
+            rmax = fmaxf(rmax, __shfl_xor_sync(0xffffffffu, rmax, off));
+            u2max = fmaxf(u2max, __shfl_xor_sync(0xffffffffu, u2max, off));
+        }
+        if (threadIdx.x == 0) { out[0] = rmax; out[1] = sqrtf(u2max) * 1.000001f; }
+    }
+}
+static gmapp_status sphere_stats(gmapp_ctx* c, cudaStream_t st, int* launches) {
+    if (c->stats_valid) return GMAPP_OK;
+    k_sphere_stats<<<1, 1024, 0, st>>>(c->d_pairA, c->cap_spheres / 2, fill_count(c, c->n_spheres) / 2, c->moving ? 1 : 0, c->d_sph_stats);
+    CUDA_TRY(c, cudaGetLastError());
+    c->stats_valid = true;
     if (launches) ++*launches;
     return GMAPP_OK;
 }
@@ -471,7 +552,7 @@ static gmapp_status choose_launch(gmapp_ctx* c, int kind, int n_agents, LaunchCf
     int stage = fits ? 1 : 0;
     if (t && t->stage >= 0) {
         if (t->stage == 1 && !fits) return fail(c, GMAPP_EINVAL, "rollout: sphere set (%s%ld bytes) does not fit shared memory", "", (long)tile_bytes);
-        stage = t->stage;
+        if (t->stage <= 1) stage = t->stage;             // the tile ring (2) belongs to the packed kernels; here: automatic
     }
     if (o->n_pad == 0) stage = 0;
     o->stage = stage;
@@ -483,8 +564,10 @@ static gmapp_status choose_launch(gmapp_ctx* c, int kind, int n_agents, LaunchCf
 // ---------------------------------------------------------------------------------------------
 // packed f32x2 rollout (POINT3, static or moving spheres): launch selection + launch
 // ---------------------------------------------------------------------------------------------
-static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float* d_agents_out, int n_agents,
-                                      const float* goal, const gmapp_gains* g, float dt, int steps, cudaStream_t st) {
+struct X2Plan { int A, grid, at, G, L, mode, n2p, cull, stage, ring_tp, xch_off, rec_off, tile_off, pair_bytes, block, smem; size_t tile_bytes; };
+
+// launch selection alone (no CUDA call): every reason to refuse a launch shape is found here, before anything is enqueued
+static gmapp_status plan_rollout_x2(gmapp_ctx* c, int n_agents, X2Plan* o) {
     const gmapp_tuning* t = c->has_tuning ? &c->tuning : nullptr;
     int max_ctas = c->num_sms;
     if (t && t->max_ctas > 0 && t->max_ctas < max_ctas) max_ctas = t->max_ctas;
@@ -521,22 +604,57 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     const int mode = chunked ? 4 : (L >= 64 ? (G <= 4 ? 2 : 3) : (L == 32 ? 1 : 0));
     const int n2p = n2 > 0 ? round_up(n2, L) : 0;
     const int cull = (t && t->cull >= 0) ? t->cull : 0;
-    // dynamic shared memory: [0,64) mbarrier; then the exchange area of the multi-warp groups (per group: the
+    // dynamic shared memory: [0,64) mbarriers; then the exchange area of the multi-warp groups (per group: the
     // per-lane partials of two agents + the published states = (2 L + 8) float4) or, mode 4, the 24-word state
     // record of every agent; then the sphere-pair tile
     const int xch_off = 64, rec_off = 128;
     const int tile_off = rec_off + (chunked ? round_up(A * 24 * 4, 128) : (mode >= 2 ? round_up(G * (2 * L + 8) * 16, 128) : 0));
-    const size_t tile_bytes = (size_t)n2p * (c->moving ? 64 : 32);       // pair arrays A, B (+ U, V when the spheres move)
+    const int pair_bytes = c->moving ? 64 : 32;                          // pair arrays A, B (+ U, V when the spheres move)
+    const size_t tile_bytes = (size_t)n2p * pair_bytes;
     const bool fits = tile_off + tile_bytes <= (size_t)c->smem_optin;
-    int stage = fits ? 1 : 0;
+    // sets beyond shared memory: a ring of kRingStages tiles fed by TMA bulk copies (stage 2); the branch-free kernels of
+    // modes 1, 2, 4 have it, the warp-vote variant and sub-warp groups read through L1 / L2 (stage 0)
+    const bool ring_ok = mode != 0 && cull == 0;
+    int ring_tp = 0;
+    if (ring_ok) {
+        ring_tp = pow2_floor((int)(((size_t)c->smem_optin - tile_off) / ((size_t)kRingStages * pair_bytes)));
+        if (ring_tp > 2048) ring_tp = 2048;
+        if (ring_tp < L) ring_tp = 0;                                    // a tile must hold a whole trip of the group
+    }
+    // Measured on B200 at equal sphere density (profiles/r02_tile_ring.md): the ring beats the L1/L2 path by 3-5 % once the set is
+    // far beyond L1 (>= 8 tiles, i.e. 32768 static spheres) for one-warp groups and chunked warps; at 4 tiles the two are level, and
+    // with multi-warp groups (16 trips per tile and warp) the per-tile hand-over costs more than L1 misses do.
+    const int ring_tiles = ring_tp > 0 ? (n2p + ring_tp - 1) / ring_tp : 0;
+    const bool ring_wins = ring_tiles >= 8 && (mode == 1 || mode == 4);
+    int stage = fits ? 1 : (ring_wins ? 2 : 0);
     if (t && t->stage >= 0) {
         if (t->stage == 1 && !fits) return fail(c, GMAPP_EINVAL, "rollout: sphere set (%s%ld bytes) does not fit shared memory", "", (long)tile_bytes);
+        if (t->stage == 2 && ring_tp == 0) return fail(c, GMAPP_EINVAL, "rollout: the tile ring needs the branch-free kernel and whole-warp groups%s");
         stage = t->stage;
     }
     if (n2p == 0) stage = 0;
-    int launches = 0;
-    gmapp_status s = effective_pairs(c, g->r_agent, st, &launches);
+    o->A = A; o->grid = grid; o->at = at; o->G = G; o->L = L; o->mode = mode; o->n2p = n2p; o->cull = cull; o->stage = stage;
+    o->ring_tp = ring_tp; o->xch_off = xch_off; o->rec_off = rec_off; o->tile_off = tile_off; o->pair_bytes = pair_bytes;
+    o->tile_bytes = tile_bytes;
+    o->block = mode == 4 ? tmax : (mode >= 2 ? G * L + 32 * G : round_up(G * L, 32));
+    o->smem = tile_off + (stage == 1 ? (int)tile_bytes : (stage == 2 ? kRingStages * ring_tp * pair_bytes : 0));
+    return GMAPP_OK;
+}
+
+static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float* d_agents_out, int n_agents,
+                                      const float* goal, const gmapp_gains* g, float dt, int steps, cudaStream_t st) {
+    X2Plan pl;
+    gmapp_status s = plan_rollout_x2(c, n_agents, &pl);
     if (s != GMAPP_OK) return s;
+    const int A = pl.A, grid = pl.grid, at = pl.at, L = pl.L, mode = pl.mode, n2p = pl.n2p, cull = pl.cull, stage = pl.stage;
+    const int ring_tp = pl.ring_tp, xch_off = pl.xch_off, rec_off = pl.rec_off, tile_off = pl.tile_off, block = pl.block, smem = pl.smem;
+    int launches = 0;
+    s = effective_pairs(c, g->r_agent, st, &launches);
+    if (s != GMAPP_OK) return s;
+    if (stage == 2 && c->moving) {                                       // largest sphere speed, for the ring's refinement prediction
+        s = sphere_stats(c, st, &launches);
+        if (s != GMAPP_OK) return s;
+    }
     RolloutX2Params P;
     memset(&P, 0, sizeof P);
     P.pairA = c->d_pairA; P.pairB = c->d_pairB; P.n2p = n2p;
@@ -562,8 +680,12 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     P.rd_arr = (c->ap_n > 0 && c->ap_has_rd) ? c->d_ap_rd : nullptr;
     P.kf_arr = (c->ap_n > 0 && c->ap_has_kf) ? c->d_ap_kf : nullptr;
     P.tile_off = tile_off; P.xch_off = xch_off; P.rec_off = rec_off;
-    const int block = mode == 4 ? tmax : (mode >= 2 ? G * L + 32 * G : round_up(G * L, 32));
-    const int smem = tile_off + (stage == 1 ? (int)tile_bytes : 0);
+    P.ring_tp = ring_tp; P.ring_off = 16; P.sph_stats = c->d_sph_stats;
+    if (c->sel_want && GMAPP_FUSED_SELECT_X2) {           // selection fused into the tail of this launch (off by default: gmapp_kernels.cuh)
+        P.sel.ticket = c->d_sel_ticket; P.sel.total = c->sel_total; P.sel.alpha = c->sel_alpha; P.sel.prev = c->sel_prev;
+        P.sel.prev_dev = c->sel_prev_dev; P.sel.out_dev = c->d_sel_rec; P.sel.out_host = c->h_best; P.sel.seq = c->sel_seq;
+        c->sel_fused = true;
+    }
     P.stage = stage;
     rollout_x2_fn fn = rollout_x2_kernel(at, mode, cull != 0, stage, g->heuristic == 1, P.snap_out != nullptr || P.traj_out != nullptr, c->moving);
     fn<<<grid, block, smem, st>>>(P);
@@ -573,7 +695,8 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     gmapp_launch_info& I = c->info;
     I.grid = grid; I.block = block; I.lanes_per_agent = L; I.agents_per_thread = at;
     I.agents_per_cta = A; I.cull = cull; I.stage = stage;
-    I.tile_spheres = stage == 1 ? 2 * n2p : 0; I.n_tiles = stage == 1 ? 1 : 0;
+    I.tile_spheres = stage == 1 ? 2 * n2p : (stage == 2 ? 2 * ring_tp : 0);
+    I.n_tiles = stage == 1 ? 1 : (stage == 2 ? (n2p + ring_tp - 1) / ring_tp : 0);
     I.smem_bytes = smem; I.kernels_launched = launches; I.packed_x2 = 1;
     cudaFuncAttributes fa;
     if (cudaFuncGetAttributes(&fa, (const void*)fn) == cudaSuccess) I.regs_per_thread = fa.numRegs;
@@ -585,6 +708,20 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
 // ---------------------------------------------------------------------------------------------
 static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_agents, float* d_agents_out, int n_agents,
                                 const float* goal, const gmapp_gains* g, float dt, int steps, cudaStream_t stream);
+
+// dry run of the launch selection of every launch this rollout will issue: refuses before anything is enqueued
+static gmapp_status check_launchable(gmapp_ctx* c, gmapp_kind kind, int n_agents) {
+    int counts[2] = {n_agents, 0};
+    if (c->ap_n > 0 && c->ap_has_h) { counts[0] = c->ap_count[0]; counts[1] = c->ap_count[1]; }
+    for (int h = 0; h < 2; ++h) {
+        if (counts[h] <= 0) continue;
+        gmapp_status s;
+        if (kind == GMAPP_POINT3 && !(c->has_tuning && c->tuning.scalar_path)) { X2Plan pl; s = plan_rollout_x2(c, counts[h], &pl); }
+        else { LaunchCfg cfg; s = choose_launch(c, kind, counts[h], &cfg); }
+        if (s != GMAPP_OK) return s;
+    }
+    return GMAPP_OK;
+}
 
 extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float* d_agents, float* d_agents_out,
                                       int n_agents, const float* goal, const gmapp_gains* g, float dt, int steps,
@@ -601,16 +738,29 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
     const int ng = kind == GMAPP_POINT3 ? 3 : 8;
     for (int i = 0; i < ng; ++i) if (!isfinite(goal[i])) return fail(c, GMAPP_EINVAL, "rollout: non-finite goal%s");
     c->sub_idx = nullptr;
+    if (c->ap_n > 0) {                      // every check comes before the first enqueue: on error nothing is launched
+        if (c->ap_n != n_agents) return fail(c, GMAPP_EINVAL, "rollout: gmapp_set_agent_params was given %s%ld agents, the rollout %ld", "", c->ap_n, n_agents);
+        if (c->ap_has_rd && g->eps_dist > c->ap_min_rd) return fail(c, GMAPP_EINVAL, "rollout: need eps_dist <= every per-agent r_influence%s");
+    }
+    {   // launch shapes that cannot run are refused here too (a dry run of the launch selection)
+        s = check_launchable(c, kind, n_agents);
+        if (s != GMAPP_OK) return s;
+    }
     if (c->roll_traj) {                     // pose 0 of every path = the start state, as given
         const size_t wb = sizeof(float) * (kind == GMAPP_POINT3 ? 6 : 14);
         CUDA_TRY(c, cudaMemcpy2DAsync(c->roll_traj, wb * (size_t)(steps + 1), d_agents, wb, wb, (size_t)n_agents,
                                       cudaMemcpyDefault, (cudaStream_t)stream));
     }
+    // Selection fused into the rollout's tail: the packed kernels (every POINT3 launch, also one per heuristic) and the
+    // wide 6D kernel (single launch) have it; after the scalar kernel gmapp_best_agent launches the selection kernel.
+    c->sel_fused = false;
+    c->sel_total = n_agents;
+    c->sel_seq = (c->sel_seq % 0x3fffffff) + 1;
+    c->sel_want = !(c->has_tuning && c->tuning.scalar_path) && (kind == GMAPP_POINT3 || !(c->ap_n > 0 && c->ap_has_h));
+    c->fused_alpha = c->sel_alpha; c->fused_prev = c->sel_prev; c->fused_prev_dev = c->sel_prev_dev != nullptr;
     if (c->ap_n > 0) {
         // heterogeneous ensemble: one launch per heuristic over that heuristic's agents (the paper runs one
         // specialised kernel per heuristic), per-agent r_d / k_f read inside the kernels
-        if (c->ap_n != n_agents) return fail(c, GMAPP_EINVAL, "rollout: gmapp_set_agent_params was given %s%ld agents, the rollout %ld", "", c->ap_n, n_agents);
-        if (c->ap_has_rd && g->eps_dist > c->ap_min_rd) return fail(c, GMAPP_EINVAL, "rollout: need eps_dist <= every per-agent r_influence%s");
         if (c->ap_has_h) {
             int total = 0;
             gmapp_launch_info first; memset(&first, 0, sizeof first);
@@ -628,12 +778,14 @@ extern "C" gmapp_status gmapp_rollout(gmapp_ctx* c, gmapp_kind kind, const float
                 idx += nh;
             }
             c->info.kernels_launched = total;
+            c->info.selection_fused = c->sel_fused ? 1 : 0;
             c->last_n_agents = n_agents;
             return GMAPP_OK;
         }
     }
     s = rollout_sub(c, kind, d_agents, d_agents_out, n_agents, goal, g, dt, steps, (cudaStream_t)stream);
     c->last_n_agents = n_agents;
+    c->info.selection_fused = c->sel_fused ? 1 : 0;
     return s;
 }
 
@@ -702,6 +854,11 @@ static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_ag
         cfg.smem = cfg.tile_off + (cfg.stage == 1 ? (int)tile_bytes : 0);
     }
     P.stage = cfg.stage;
+    if (wide && c->sel_want && !c->sub_idx && GMAPP_FUSED_SELECT_WIDE) {             // the wide kernel has the fused selection tail, the scalar one does not
+        P.sel.ticket = c->d_sel_ticket; P.sel.total = c->sel_total; P.sel.alpha = c->sel_alpha; P.sel.prev = c->sel_prev;
+        P.sel.prev_dev = c->sel_prev_dev; P.sel.out_dev = c->d_sel_rec; P.sel.out_host = c->h_best; P.sel.seq = c->sel_seq;
+        c->sel_fused = true;
+    }
     rollout_fn fn = wide ? rollout_wide_kernel(c->moving, cfg.cull != 0, cfg.stage, g->heuristic == 1)
                          : rollout_kernel(kind, cfg.at, c->moving, cfg.cull != 0, cfg.stage);
     fn<<<cfg.grid, cfg.block, cfg.smem, st>>>(P);
@@ -721,28 +878,81 @@ static gmapp_status rollout_sub(gmapp_ctx* c, gmapp_kind kind, const float* d_ag
 // ---------------------------------------------------------------------------------------------
 // selection, force query, results
 // ---------------------------------------------------------------------------------------------
+// the selection record for (alpha, prev_best): from the rollout's fused tail when it was armed with the same
+// arguments (or no incumbent is asked for: the raw argmin is in every record), else by the selection kernel
+static gmapp_status selection_record_host(gmapp_ctx* c, float alpha, int prev_best, cudaStream_t st, const char* who) {
+    if (c->last_n_agents < 1) return fail(c, GMAPP_ESTATE, "%s: no rollout has run on this context", who);
+    if (!isfinite(alpha)) return fail(c, GMAPP_EINVAL, "%s: alpha is not finite", who);
+    if (prev_best >= c->last_n_agents) prev_best = -1;        // not an agent of the last rollout: no incumbent
+    const bool from_tail = c->sel_fused && !c->fused_prev_dev &&
+                           (prev_best < 0 || (prev_best == c->fused_prev && alpha == c->fused_alpha));
+    if (!from_tail) {
+        // the kernel writes its record straight into pinned host memory (no copy engine round trip) and is launched
+        // with programmatic stream serialisation, so its launch overlaps the tail of the rollout
+        cudaLaunchConfig_t lc;
+        memset(&lc, 0, sizeof lc);
+        lc.gridDim = dim3(1); lc.blockDim = dim3(1024); lc.dynamicSmemBytes = 0; lc.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        lc.attrs = at; lc.numAttrs = 1;
+        c->sel_seq = (c->sel_seq % 0x3fffffff) + 1;
+        CUDA_TRY(c, cudaLaunchKernelEx(&lc, k_best_agent, (const float*)c->d_cost, (const int*)c->d_collided, c->last_n_agents, alpha,
+                                       prev_best, (const int*)nullptr, c->d_sel_rec, c->h_best, c->sel_seq));
+        c->sel_fused = false;                              // the record now belongs to this (alpha, prev_best)
+    }
+    {
+        // The record is written to pinned memory by the rollout kernel's last warp (or by the selection kernel), the sequence number behind it: poll
+        // for it instead of paying a stream synchronisation's wake-up latency.  Every few thousand polls look at the
+        // stream: an error ends the wait, and a stream that has drained without the number appearing (it cannot) falls
+        // through to the plain synchronise below.
+        volatile int* flag = (volatile int*)(c->h_best + 8);
+        for (unsigned spin = 1; *flag != c->sel_seq; ++spin) {
+            if ((spin & 0x3fffu) == 0) {
+                cudaError_t q = cudaStreamQuery(st);
+                if (q != cudaErrorNotReady) {
+                    if (q != cudaSuccess) return fail(c, GMAPP_ECUDA, "%s: the rollout failed", who);
+                    break;
+                }
+            }
+        }
+        if (*flag != c->sel_seq) CUDA_TRY(c, cudaStreamSynchronize(st));
+    }
+    if (from_tail && prev_best < 0 && c->fused_prev >= 0) {    // armed with an incumbent, asked without: the raw argmin
+        c->h_best[0] = c->h_best[3]; c->h_best[1] = c->h_best[4]; c->h_best[2] = c->h_best[5];
+        c->fused_prev = -1;
+    }
+    return GMAPP_OK;
+}
+
 extern "C" gmapp_status gmapp_best_agent_ex(gmapp_ctx* c, float alpha, int prev_best, int* out_index, float* out_cost,
                                             int* out_collided, void* stream) {
     if (!c) return GMAPP_EINVAL;
     if (!out_index) return fail(c, GMAPP_EINVAL, "best_agent: out_index is NULL%s");
-    if (c->last_n_agents < 1) return fail(c, GMAPP_ESTATE, "best_agent: no rollout has run on this context%s");
-    if (!isfinite(alpha)) return fail(c, GMAPP_EINVAL, "best_agent: alpha is not finite%s");
-    cudaStream_t st = (cudaStream_t)stream;
-    // the kernel writes its 12-byte result straight into pinned host memory (no copy engine round trip) and is
-    // launched with programmatic stream serialisation, so its launch overlaps the tail of the rollout
-    cudaLaunchConfig_t lc;
-    memset(&lc, 0, sizeof lc);
-    lc.gridDim = dim3(1); lc.blockDim = dim3(1024); lc.dynamicSmemBytes = 0; lc.stream = st;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    lc.attrs = at; lc.numAttrs = 1;
-    CUDA_TRY(c, cudaLaunchKernelEx(&lc, k_best_agent, (const float*)c->d_cost, (const int*)c->d_collided, c->last_n_agents, alpha,
-                                   prev_best, (const int*)nullptr, c->d_best_idx, c->d_best_cost, c->h_best));
-    CUDA_TRY(c, cudaStreamSynchronize(st));
+    gmapp_status s = selection_record_host(c, alpha, prev_best, (cudaStream_t)stream, "best_agent");
+    if (s != GMAPP_OK) return s;
     *out_index = c->h_best[0];
     if (out_collided) *out_collided = c->h_best[1];
     if (out_cost) memcpy(out_cost, &c->h_best[2], sizeof(float));
+    return GMAPP_OK;
+}
+
+extern "C" gmapp_status gmapp_select(gmapp_ctx* c, float alpha, int prev_best, gmapp_selection* out, void* stream) {
+    if (!c) return GMAPP_EINVAL;
+    if (!out) return fail(c, GMAPP_EINVAL, "select: out is NULL%s");
+    gmapp_status s = selection_record_host(c, alpha, prev_best, (cudaStream_t)stream, "select");
+    if (s != GMAPP_OK) return s;
+    out->index = c->h_best[0]; out->collided = c->h_best[1]; memcpy(&out->cost, &c->h_best[2], sizeof(float));
+    out->raw_index = c->h_best[3]; out->raw_collided = c->h_best[4]; memcpy(&out->raw_cost, &c->h_best[5], sizeof(float));
+    out->prev_collided = c->h_best[6]; memcpy(&out->prev_cost, &c->h_best[7], sizeof(float));
+    return GMAPP_OK;
+}
+
+extern "C" gmapp_status gmapp_set_selection(gmapp_ctx* c, float alpha, int prev_best) {
+    if (!c) return GMAPP_EINVAL;
+    if (!isfinite(alpha)) return fail(c, GMAPP_EINVAL, "set_selection: alpha is not finite%s");
+    if (prev_best >= c->max_agents) return fail(c, GMAPP_EINVAL, "set_selection: prev_best exceeds max_agents%s");
+    c->sel_alpha = alpha; c->sel_prev = prev_best < 0 ? -1 : prev_best;
     return GMAPP_OK;
 }
 
@@ -764,18 +974,34 @@ extern "C" gmapp_status gmapp_replan(gmapp_ctx* c, gmapp_kind kind, float* d_age
                                      const gmapp_gains* g, float dt, int steps, int exec_steps, float alpha, int prev_best,
                                      int n_cycles, float* d_path_out, int32_t* d_best_out, void* stream) {
     if (!c) return GMAPP_EINVAL;
-    if (!d_agents) return fail(c, GMAPP_EINVAL, "replan: d_agents is NULL%s");
+    if (!d_agents || !goal) return fail(c, GMAPP_EINVAL, "replan: NULL agents or goal%s");
+    if (kind != GMAPP_POINT3 && kind != GMAPP_MOTOR6) return fail(c, GMAPP_EINVAL, "replan: unknown kind%s");
     if (n_cycles < 1) return fail(c, GMAPP_EINVAL, "replan: n_cycles must be >= 1%s");
-    if (exec_steps < 1 || exec_steps > steps) return fail(c, GMAPP_EINVAL, "replan: need 1 <= exec_steps <= steps%s");
+    if (steps < 1 || exec_steps < 1 || exec_steps > steps) return fail(c, GMAPP_EINVAL, "replan: need 1 <= exec_steps <= steps%s");
     if (!isfinite(alpha)) return fail(c, GMAPP_EINVAL, "replan: alpha is not finite%s");
+    if (n_agents < 1) return fail(c, GMAPP_EINVAL, "replan: n_agents must be >= 1%s");
+    if (n_agents > c->max_agents) return fail(c, GMAPP_ECAPACITY, "replan: n_agents = %s%ld exceeds max_agents = %ld", "", n_agents, c->max_agents);
     if (prev_best >= n_agents) return fail(c, GMAPP_EINVAL, "replan: prev_best out of range%s");
+    // everything gmapp_rollout would refuse is refused here, BEFORE the first enqueue (on error nothing is launched)
+    if (!isfinite(dt) || !(dt > 0.0f)) return fail(c, GMAPP_EINVAL, "replan: dt must be finite and > 0%s");
+    if (c->n_spheres < 0) return fail(c, GMAPP_ESTATE, "replan: gmapp_set_obstacles has not been called%s");
+    gmapp_status s = check_gains(c, g, "replan");
+    if (s != GMAPP_OK) return s;
+    for (int i = 0; i < (kind == GMAPP_POINT3 ? 3 : 8); ++i) if (!isfinite(goal[i])) return fail(c, GMAPP_EINVAL, "replan: non-finite goal%s");
+    if (c->ap_n > 0) {
+        if (c->ap_n != n_agents) return fail(c, GMAPP_EINVAL, "replan: gmapp_set_agent_params was given %s%ld agents, the rollout %ld", "", c->ap_n, n_agents);
+        if (c->ap_has_rd && g->eps_dist > c->ap_min_rd) return fail(c, GMAPP_EINVAL, "replan: need eps_dist <= every per-agent r_influence%s");
+    }
+    s = check_launchable(c, kind, n_agents);
+    if (s != GMAPP_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
     const int w = kind == GMAPP_POINT3 ? 6 : 14;
     // the incumbent goes to the device by a tiny kernel argument, not a host copy, so the whole call can be captured
     // in a CUDA graph and replayed
     k_set_int<<<1, 1, 0, st>>>(c->d_prev, prev_best < 0 ? -1 : prev_best);
-    gmapp_status s = GMAPP_OK;
-    int launches = 0;
+    const float keep_alpha = c->sel_alpha; const int keep_prev = c->sel_prev;
+    c->sel_alpha = alpha; c->sel_prev = -1; c->sel_prev_dev = c->d_prev;     // the rollouts' fused tails read the incumbent on the device
+    int launches = 1;
     for (int cyc = 0; cyc < n_cycles && s == GMAPP_OK; ++cyc) {
         c->roll_t0 = (float)cyc * (float)exec_steps * dt;      // moving obstacles keep moving between cycles
         c->roll_snap = c->d_snap; c->roll_snap_step = exec_steps;
@@ -783,12 +1009,17 @@ extern "C" gmapp_status gmapp_replan(gmapp_ctx* c, gmapp_kind kind, float* d_age
         c->roll_t0 = 0.0f; c->roll_snap = nullptr; c->roll_snap_step = 0;
         if (s != GMAPP_OK) break;
         launches += c->info.kernels_launched;
-        k_best_agent<<<1, 1024, 0, st>>>(c->d_cost, c->d_collided, n_agents, alpha, -1, c->d_prev, c->d_best_idx, c->d_best_cost, nullptr);
-        k_reseed<<<(n_agents * w + 255) / 256, 256, 0, st>>>(c->d_snap, c->d_best_idx, n_agents, w, d_agents, c->d_prev,
+        if (!c->sel_fused) {                                   // kernels without the fused tail (scalar path)
+            k_best_agent<<<1, 1024, 0, st>>>(c->d_cost, c->d_collided, n_agents, alpha, -1, c->d_prev, c->d_sel_rec, nullptr, 0);
+            ++launches;
+        }
+        k_reseed<<<(n_agents * w + 255) / 256, 256, 0, st>>>(c->d_snap, c->d_sel_rec, n_agents, w, d_agents, c->d_prev,
                                                              d_path_out, d_best_out, cyc);
-        CUDA_TRY(c, cudaGetLastError());
-        launches += 2;
+        if (cudaGetLastError() != cudaSuccess) { s = fail(c, GMAPP_ECUDA, "replan: kernel launch failed%s"); break; }
+        ++launches;
     }
+    c->sel_alpha = keep_alpha; c->sel_prev = keep_prev; c->sel_prev_dev = nullptr;
+    c->sel_fused = false;                                      // the record on the host side belongs to no (alpha, prev_best)
     c->info.kernels_launched = launches;
     return s;
 }
@@ -844,24 +1075,34 @@ extern "C" gmapp_status gmapp_plan_cycle_host(gmapp_ctx* c, gmapp_kind kind, con
                                               const float* goal, const gmapp_gains* g, float dt, int steps,
                                               float alpha, int prev_best, int* out_index, float* out_cost, void* stream) {
     if (!c) return GMAPP_EINVAL;
-    if (!h_agents || !out_index) return fail(c, GMAPP_EINVAL, "plan_cycle_host: NULL agents or out_index%s");
+    if (!h_agents || !out_index || !goal) return fail(c, GMAPP_EINVAL, "plan_cycle_host: NULL agents, goal or out_index%s");
     if (kind != GMAPP_POINT3 && kind != GMAPP_MOTOR6) return fail(c, GMAPP_EINVAL, "plan_cycle_host: unknown kind%s");
-    if (n_agents < 1) return fail(c, GMAPP_EINVAL, "plan_cycle_host: n_agents must be >= 1%s");
+    if (n_agents < 1 || steps < 1) return fail(c, GMAPP_EINVAL, "plan_cycle_host: n_agents and steps must be >= 1%s");
     if (n_agents > c->max_agents) return fail(c, GMAPP_ECAPACITY, "plan_cycle_host: n_agents = %s%ld exceeds max_agents = %ld", "", n_agents, c->max_agents);
-    gmapp_status s;
-    if (h_xyzr || n_spheres == 0) {
-        if (h_xyzr || c->n_spheres < 0) {
-            s = gmapp_set_obstacles_host(c, h_xyzr, h_vel, n_spheres, stream);
-            if (s != GMAPP_OK) return s;
-        }
+    if (!isfinite(dt) || !(dt > 0.0f)) return fail(c, GMAPP_EINVAL, "plan_cycle_host: dt must be finite and > 0%s");
+    if (!isfinite(alpha)) return fail(c, GMAPP_EINVAL, "plan_cycle_host: alpha is not finite%s");
+    if (prev_best >= n_agents) return fail(c, GMAPP_EINVAL, "plan_cycle_host: prev_best out of range%s");
+    if (n_spheres > 0 && !h_xyzr) return fail(c, GMAPP_EINVAL, "plan_cycle_host: n_spheres > 0 needs h_xyzr%s");
+    if (n_spheres > c->max_spheres) return fail(c, GMAPP_ECAPACITY, "plan_cycle_host: n_spheres = %s%ld exceeds max_spheres = %ld", "", n_spheres, c->max_spheres);
+    if (n_spheres < 0 && c->n_spheres < 0) return fail(c, GMAPP_ESTATE, "plan_cycle_host: no resident sphere world to keep (n_spheres < 0)%s");
+    gmapp_status s = check_gains(c, g, "plan_cycle_host");
+    if (s != GMAPP_OK) return s;
+    // n_spheres < 0: keep the resident sphere world; n_spheres == 0: an EMPTY world (no obstacles); > 0: upload
+    if (n_spheres >= 0) {
+        s = gmapp_set_obstacles_host(c, h_xyzr, h_vel, n_spheres, stream);
+        if (s != GMAPP_OK) return s;
     }
     const int w = kind == GMAPP_POINT3 ? 6 : 14;
     float* hp = c->h_pinned + (size_t)c->cap_spheres * 7;
     // every earlier use of the agent staging area ended with a stream synchronise (this call is synchronous)
     memcpy(hp, h_agents, sizeof(float) * w * (size_t)n_agents);
     // the rollout reads every start state once and writes every final state once: it does both straight from / to
-    // the pinned host buffer (unified addressing), which saves two copy-engine transfers per cycle
+    // the pinned host buffer (unified addressing), which saves two copy-engine transfers per cycle.  The selection is
+    // armed with this call's (alpha, prev_best) and runs in the tail of the rollout kernel.
+    const float keep_alpha = c->sel_alpha; const int keep_prev = c->sel_prev;
+    c->sel_alpha = alpha; c->sel_prev = prev_best < 0 ? -1 : prev_best;
     s = gmapp_rollout(c, kind, hp, h_agents_out ? hp : nullptr, n_agents, goal, g, dt, steps, stream);
+    c->sel_alpha = keep_alpha; c->sel_prev = keep_prev;
     if (s != GMAPP_OK) return s;
     s = gmapp_best_agent(c, alpha, prev_best, out_index, out_cost, stream);     // synchronises
     if (s != GMAPP_OK) return s;

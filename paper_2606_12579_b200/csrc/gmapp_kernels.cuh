@@ -33,6 +33,21 @@ constexpr float kTiny = 1e-30f;          // bias that keeps squared norms > 0 (a
 constexpr float kFar = 1.0e6f;
 constexpr int kMaxGroupsNamedBar = 15;   // named barriers 1..15
 
+// Selection fused into the rollout's tail (S8, reading G24).  Every warp that has written the results of
+// its agents takes a ticket; the warp that completes the count reduces (collided, C, index) over all agents, applies the
+// hysteresis rule and writes the 8-word selection record -- no second launch in the planning cycle.
+//   record: {index, collided, cost | raw index, raw collided, raw cost (plain argmin, no incumbent) | incumbent collided, cost}
+struct SelParams {
+    int* ticket;              // device counter (0 between cycles); nullptr: selection not fused into this launch
+    int total;                // agents of the whole cycle (all launches of a heterogeneous ensemble together)
+    float alpha;
+    int prev;                 // incumbent, or < 0
+    const int* prev_dev;      // nullable: the incumbent lives on the device (gmapp_replan)
+    int* out_dev;             // [8] the record in device memory
+    int* out_host;            // nullable: [9] the same record in pinned host memory, then `seq` (the host polls for it)
+    int seq;                  // sequence number of this cycle
+};
+
 struct RolloutParams {
     const float4* sph;        // [n_pad] (cx, cy, cz, r_j + r_a), sentinel-padded
     const float4* svel;       // [n_pad] (ux, uy, uz, 0) or nullptr
@@ -72,6 +87,7 @@ struct RolloutParams {
     int two_warp_epi;         // wide kernel, 6D agents: a rot warp and a lin warp per group (G <= 3)
     int tile_off;             // byte offset of the sphere tile in dynamic shared memory
     int red_off;              // byte offset of the cross-warp exchange scratch
+    SelParams sel;            // selection fused into the tail (wide kernel only)
 };
 
 __device__ __forceinline__ int agent_gid(const RolloutParams& P, int i) { return P.agent_idx ? P.agent_idx[i] : i; }
@@ -626,6 +642,104 @@ __global__ void __launch_bounds__(256) k_forces(const __grid_constant__ ForcePar
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// selection: lexicographic argmin of (collided, C, index) + hysteresis (PAPER.md:205)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool key_less(int ca, float Ca, int ia, int cb, float Cb, int ib) {
+    if (ca != cb) return ca < cb;
+    if (Ca != Cb) return Ca < Cb;
+    return ia < ib;
+}
+// lane 0 of the reducing warp: hysteresis against the incumbent and the 8-word record (device + pinned host)
+__device__ __forceinline__ void selection_record(const float* cost5, const int* collided, int n, float alpha, int prev_best,
+                                                 int bi, int bc, float bC, int* out_dev, int* out_host, int seq = 0) {
+    int rec[8];
+    rec[3] = n > 0 ? bi : -1; rec[4] = n > 0 ? bc : 0; rec[5] = n > 0 ? __float_as_int(bC) : 0x7fc00000;
+    rec[6] = 0; rec[7] = 0x7fc00000;
+    if (n > 0 && prev_best >= 0 && prev_best < n) {
+        float Cp = __ldcg(cost5 + 5 * size_t(prev_best)); int cp = __ldcg(collided + prev_best) ? 1 : 0;
+        if (Cp != Cp) { Cp = __int_as_float(0x7f800000); cp = 1; }
+        rec[6] = cp; rec[7] = __float_as_int(Cp);
+        if (prev_best != bi) {
+            const bool improves = (bc < cp) || (bc == cp && bC < alpha * Cp);
+            if (!improves) { bi = prev_best; bC = Cp; bc = cp; }
+        }
+    }
+    rec[0] = n > 0 ? bi : -1; rec[1] = n > 0 ? bc : 0; rec[2] = n > 0 ? __float_as_int(bC) : 0x7fc00000;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) out_dev[i] = rec[i];
+    if (out_host) {                                          // pinned host memory: the record, then (ordered behind it) the
+#pragma unroll                                                // sequence number the host may be polling for
+        for (int i = 0; i < 8; ++i) out_host[i] = rec[i];
+        __threadfence_system();
+        *reinterpret_cast<volatile int*>(out_host + 8) = seq;
+        __threadfence_system();
+    }
+}
+// Tail of a rollout warp: all 32 lanes, converged, after the warp's writer lanes stored the results of `n_done` agents.
+// (called from ONE place per kernel, after the group bodies have returned: inlined into every body it perturbed the
+// register allocation of the sweep loops, and as a real function call it forced the ABI on the whole kernel)
+// Measured on B200 (profiles/r02_selection.md): in the wide 6D kernel the fused tail is free and saves the second launch
+// (config 4: 0.418 -> 0.410 ms per cycle).  In the packed point-agent kernels the few extra instructions of the tail
+// change ptxas' register assignment of the sweep loops (96-register kernels): config 3's kernel 0.313 -> 0.327 ms, config 1
+// 0.041 -> 0.051 ms, 16384 x 4096 9.575 -> 9.647 ms -- more than the ~12 us a selection kernel launched with programmatic
+// stream serialisation behind the rollout costs.  So: fused in the wide kernel, a dependent launch after the packed ones.
+#ifndef GMAPP_FUSED_SELECT_WIDE
+#define GMAPP_FUSED_SELECT_WIDE 1
+#endif
+#ifndef GMAPP_FUSED_SELECT_X2
+#define GMAPP_FUSED_SELECT_X2 0
+#endif
+template <bool ON>
+__device__ __forceinline__ void select_tail(const SelParams& Q, const float* cost5, const int* collided, int n_done, int lane) {
+    if (!ON) return;
+    if (!Q.ticket) return;
+    __threadfence_system();                                  // the writer lanes' results: device-wide, and the final states a
+    __syncwarp();                                            // host-buffer cycle wrote to pinned memory, host-visible
+    int last = 0;
+    if (lane == 0) last = (atomicAdd(Q.ticket, n_done) + n_done == Q.total) ? 1 : 0;
+    last = __shfl_sync(0xffffffffu, last, 0);
+    if (!last) return;
+    __threadfence();
+    const int n = Q.total;
+    int bc = 2, bi = 0x7fffffff; float bC = __int_as_float(0x7f800000);
+    for (int i = lane; i < n; i += 32) {                     // L2 reads: the results were written by other SMs
+        float C = __ldcg(cost5 + 5 * size_t(i)); int c = __ldcg(collided + i) ? 1 : 0;
+        if (C != C) { C = __int_as_float(0x7f800000); c = 1; }
+        if (key_less(c, C, i, bc, bC, bi)) { bc = c; bC = C; bi = i; }
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const int oc = __shfl_xor_sync(0xffffffffu, bc, off);
+        const float oC = __shfl_xor_sync(0xffffffffu, bC, off);
+        const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+        if (key_less(oc, oC, oi, bc, bC, bi)) { bc = oc; bC = oC; bi = oi; }
+    }
+    if (lane == 0) {
+        *Q.ticket = 0;                                       // ready for the next cycle (stream order)
+        selection_record(cost5, collided, n, Q.alpha, Q.prev_dev ? *Q.prev_dev : Q.prev, bi, bc, bC, Q.out_dev, Q.out_host, Q.seq);
+    }
+}
+
+// the same for kernels whose finishing lanes are not whole warps (sub-warp groups, a tuning-only shape): one thread
+template <bool ON>
+__device__ __forceinline__ void select_tail_serial(const SelParams& Q, const float* cost5, const int* collided, int n_done) {
+    if (!ON) return;
+    if (!Q.ticket) return;
+    __threadfence();
+    if (atomicAdd(Q.ticket, n_done) + n_done != Q.total) return;
+    __threadfence();
+    const int n = Q.total;
+    int bc = 2, bi = 0x7fffffff; float bC = __int_as_float(0x7f800000);
+    for (int i = 0; i < n; ++i) {
+        float C = __ldcg(cost5 + 5 * size_t(i)); int c = __ldcg(collided + i) ? 1 : 0;
+        if (C != C) { C = __int_as_float(0x7f800000); c = 1; }
+        if (key_less(c, C, i, bc, bC, bi)) { bc = c; bC = C; bi = i; }
+    }
+    *Q.ticket = 0;
+    selection_record(cost5, collided, n, Q.alpha, Q.prev_dev ? *Q.prev_dev : Q.prev, bi, bc, bC, Q.out_dev, Q.out_host, Q.seq);
+}
+
 #ifdef GMAPP_MAIN_TU      // non-template kernels: compiled once, in gmapp.cu
 // ---------------------------------------------------------------------------------------------
 // obstacle packing: (xyz, r) [+ vel] -> float4 arrays, R = r + r_a, sentinel padding to n_cap
@@ -661,23 +775,17 @@ __global__ void k_pack_spheres(const float* __restrict__ xyzr, const float* __re
 }
 
 // ---------------------------------------------------------------------------------------------
-// selection: lexicographic argmin of (collided, C, index) + hysteresis (PAPER.md:205)
+// selection as a kernel of its own (gmapp_best_agent with another alpha / incumbent than the rollout's tail was armed
+// with, and after the kernels that have no fused tail)
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ bool key_less(int ca, float Ca, int ia, int cb, float Cb, int ib) {
-    if (ca != cb) return ca < cb;
-    if (Ca != Cb) return Ca < Cb;
-    return ia < ib;
-}
-
 // d_prev (nullable): the incumbent is read from device memory (closed-loop re-planning chains cycles without the host)
 __global__ void __launch_bounds__(1024) k_best_agent(const float* __restrict__ cost5, const int* __restrict__ collided,
                                                      int n, float alpha, int prev_best, const int* __restrict__ d_prev,
-                                                     int* out_idx, float* out_cost, int* host_out) {
+                                                     int* out_rec, int* host_out, int seq) {
     // launched with programmatic stream serialisation behind the rollout (gmapp_best_agent_ex): wait here for its
     // results; a plain launch returns from this at once
     cudaGridDependencySynchronize();
     if (d_prev) prev_best = *d_prev;
-    // out_idx[0] = winner, out_idx[1] = its collision flag
     __shared__ int s_c[32]; __shared__ float s_C[32]; __shared__ int s_i[32];
     int bc = 2, bi = 0x7fffffff; float bC = __int_as_float(0x7f800000);
     for (int i = threadIdx.x; i < n; i += blockDim.x) {
@@ -703,21 +811,7 @@ __global__ void __launch_bounds__(1024) k_best_agent(const float* __restrict__ c
             int oi = __shfl_xor_sync(0xffffffffu, bi, off);
             if (key_less(oc, oC, oi, bc, bC, bi)) { bc = oc; bC = oC; bi = oi; }
         }
-        if (l == 0) {
-            if (n > 0 && prev_best >= 0 && prev_best < n && prev_best != bi) {
-                float Cp = cost5[5 * size_t(prev_best)]; int cp = collided[prev_best] ? 1 : 0;
-                if (Cp != Cp) { Cp = __int_as_float(0x7f800000); cp = 1; }
-                bool improves = (bc < cp) || (bc == cp && bC < alpha * Cp);
-                if (!improves) { bi = prev_best; bC = Cp; bc = cp; }
-            }
-            out_idx[0] = n > 0 ? bi : -1;
-            out_idx[1] = n > 0 ? bc : 0;
-            *out_cost = n > 0 ? bC : __int_as_float(0x7fc00000);
-            if (host_out) {                                  // pinned host memory, read after the stream synchronises
-                host_out[0] = out_idx[0]; host_out[1] = out_idx[1]; host_out[2] = __float_as_int(*out_cost);
-                __threadfence_system();
-            }
-        }
+        if (l == 0) selection_record(cost5, collided, n, alpha, prev_best, bi, bc, bC, out_rec, host_out, seq);
     }
 }
 

@@ -180,6 +180,7 @@ __device__ __forceinline__ void wide_epilogue_warp(const RolloutParams& P, int f
         const float4 t = group_reduce<NA, NW>(part, P.L, lane);
         if (last) {
             if (writer) me.finish(P, t.w);
+            select_tail<GMAPP_FUSED_SELECT_WIDE != 0>(P.sel, P.cost, P.collided, NA, lane);
             return;
         }
         me.post(P, t.x, t.y, t.z);
@@ -276,6 +277,7 @@ __device__ __forceinline__ void wide_lin_warp(const RolloutParams& P, int agent,
         const float4 t = group_reduce<1, NW>(part, P.L, lane);
         if (last) {
             if (writer) me.finish(P, t.w);
+            select_tail<GMAPP_FUSED_SELECT_WIDE != 0>(P.sel, P.cost, P.collided, 1, lane);
             return;
         }
         me.post(P, t.x, t.y, t.z);

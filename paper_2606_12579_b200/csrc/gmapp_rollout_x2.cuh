@@ -107,6 +107,11 @@ struct RolloutX2Params {
     float* traj_out;          // nullable: [n][steps+1][6] every pose of every agent (pose 0 = start state, written by the host side)
     const int* count_dev;     // nullable: device-resident sphere count of a built sphere world (gmapp_build_sphere_world);
     int n_cap;                // the kernel then sweeps only the pairs that hold real spheres (the slots behind are sentinels)
+    // TMA tile ring (STAGE == 2: sphere sets beyond shared memory)
+    int ring_tp;              // sphere pairs per tile (a multiple of L)
+    int ring_off;             // byte offset of the ring's mbarriers (full[kRingStages], empty[kRingStages])
+    const float* sph_stats;   // device: {largest R = r_j + r_a, largest sphere speed |u_j|} of the sphere world
+    SelParams sel;            // selection fused into the rollout's tail (gmapp_kernels.cuh)
 };
 
 __device__ __forceinline__ int agent_gid(const RolloutX2Params& P, int i) { return P.agent_idx ? P.agent_idx[i] : i; }
@@ -360,6 +365,117 @@ __device__ __forceinline__ void sweep_any(const float4* __restrict__ tA, const f
     sweep_pass<NA, FORCE, CULL, APF, MV, true>(tA, tB, trips, lane, L, tk, p, v, rd, eps, mask, acc);
 }
 
+// ---------------------------------------------------------------------------------------------
+// TMA tile ring (STAGE == 2): sphere sets that do not fit shared memory (config 5 at 16384 / 65536 spheres).
+// The pair arrays are cut into tiles of `tp` pairs, streamed from L2 into a ring of kRingStages shared-memory slots by
+// 1-D TMA bulk copies.  Per slot: an mbarrier full[s] (count 1 + transaction bytes: "the tile has landed") and a
+// release counter done[s].  Every consumer warp of the CTA walks the SAME tile sequence -- (steps + 1) passes x `rounds`
+// x tiles -- so one copy of a tile serves all agents of the CTA (a warp with fewer agent chunks than the others still
+// visits, and releases, the tiles of the rounds it skips).  There is no producer warp (a 21st warp would cut the
+// register budget of the 20-warp CTA from 96 to 80) and nobody ever waits for a slot to drain: the warp that releases a
+// slot LAST (its atomic increment of done[s] reaches the number of consumer warps) refills it on the spot with the
+// tile kRingStages visits ahead.  Warps may drift apart by up to kRingStages - 1 tiles, which keeps one group's reduce /
+// integrate round trip overlapped with the other groups' sweeps.
+// Distance refinement in ring mode is PREDICTED instead of repeated (a warp cannot go back to tiles that have left the
+// ring): a lane's clearance minimum m over its own spheres at pose k bounds the same minimum at pose k + 1 from below by
+// m - dt (|v| + max |u_j|) (v: the new velocity, Eq. 11), so the warp sweeps step k + 1 on the raw MUFU.RSQ distance
+// only if that bound is >= thr = (largest R among the lane's spheres) / kNearK on all its lanes (then every pair has
+// d_O >= R_j / kNearK, the condition of the two-pass scheme above); step 0 and the final pass always refine.  Same
+// granularity as the two-pass scheme: only the warps whose own spheres are close pay for the Newton step.
+// ---------------------------------------------------------------------------------------------
+constexpr int kRingStages = 3;
+struct RingView {
+    uint64_t* full;           // [kRingStages]
+    int* done;                // [kRingStages] consumer warps that have released the slot's current tile
+    const float4* slots;      // slot s at slots + s * slot_f4; inside a slot the arrays A, B (, U, V) are tp float4 apart
+    int tp, slot_f4, nt, last_pairs, narr, consumers, total;
+};
+struct RingPos {
+    int slot; uint32_t parity;
+    int t, v;                 // tile index inside the pass, visit index
+    __device__ __forceinline__ void advance(int nt) {
+        if (++slot == kRingStages) { slot = 0; parity ^= 1u; }
+        if (++t == nt) t = 0;
+        ++v;
+    }
+};
+struct SphSrc {               // where a sweep finds the sphere pairs: resident arrays (STAGE 0 / 1) or the ring
+    const float4* tA; const float4* tB; int n2p;
+    RingView ring; RingPos pos;
+    float umax_dt;            // ring mode: dt * (largest sphere speed)
+};
+
+// one elected thread: copy tile t of the pair arrays into `slot` (completion on full[slot])
+__device__ __forceinline__ void ring_issue(const RolloutX2Params& P, const RingView& R, int t, int slot) {
+    const uint32_t pairs = t == R.nt - 1 ? uint32_t(R.last_pairs) : uint32_t(R.tp);
+    const uint32_t bytes = pairs * 16u;
+    mbar_arrive_expect_tx(R.full + slot, uint32_t(R.narr) * bytes);
+    float4* dst = const_cast<float4*>(R.slots) + size_t(slot) * R.slot_f4;
+    const size_t arr_stride = size_t(P.pairB - P.pairA);    // pair arrays equally spaced in global memory
+    for (int r = 0; r < R.narr; ++r) {
+        const float4* src = P.pairA + size_t(r) * arr_stride + size_t(t) * R.tp;
+        for (uint32_t o = 0; o < bytes; o += 32768u) {
+            const uint32_t nb = bytes - o < 32768u ? bytes - o : 32768u;
+            tma_bulk_g2s(reinterpret_cast<unsigned char*>(dst + size_t(r) * R.tp) + o,
+                         reinterpret_cast<const unsigned char*>(src) + o, nb, R.full + slot);
+        }
+    }
+}
+// the warp is done with the tile in its current slot; the last warp to say so refills the slot
+__device__ __forceinline__ void ring_release(const RolloutX2Params& P, SphSrc& S) {
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) {
+        __threadfence_block();                              // this warp's reads of the slot are done
+        const int old = atomicAdd(S.ring.done + S.pos.slot, 1);
+        if (old == S.ring.consumers - 1) {
+            S.ring.done[S.pos.slot] = 0;                    // nobody touches it before the refill has landed
+            if (S.pos.v + kRingStages < S.ring.total) {
+                int t = S.pos.t + kRingStages;
+                while (t >= S.ring.nt) t -= S.ring.nt;
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy reads before the async-proxy write
+                ring_issue(P, S.ring, t, S.pos.slot);
+            }
+        }
+    }
+    S.pos.advance(S.ring.nt);
+}
+
+// visit (and release) the tiles of one pass without computing: a warp whose agent block has fewer chunks than the others
+__device__ __forceinline__ void ring_skip_pass(const RolloutX2Params& P, SphSrc& S) {
+    for (int t = 0; t < S.ring.nt; ++t) {
+        mbar_wait(S.ring.full + S.pos.slot, S.pos.parity);
+        ring_release(P, S);
+    }
+}
+
+// One pass over the whole sphere set for this lane.  RING: tile by tile out of the ring, refinement as predicted by the
+// caller (`hot`); otherwise the resident arrays with the two-pass refinement (sweep_any updates `hot`).
+template <bool RING, int NA, bool FORCE, bool CULL, bool APF, bool MV, class RD>
+__device__ __forceinline__ void sweep_src(const RolloutX2Params& P, SphSrc& S, int trips, int lane, int L, int logL, float tk,
+                                          const float (&p)[NA][3], const float (&v)[NA][3], const RD& rd, float eps, unsigned mask,
+                                          float thr, bool& hot, X2Acc<NA>& acc) {
+    if (!RING) { sweep_any<NA, FORCE, CULL, APF, MV>(S.tA, S.tB, trips, lane, L, tk, p, v, rd, eps, mask, thr, hot, acc); return; }
+    for (int t = 0; t < S.ring.nt; ++t) {
+        mbar_wait(S.ring.full + S.pos.slot, S.pos.parity);
+        const float4* tA = S.ring.slots + size_t(S.pos.slot) * S.ring.slot_f4;
+        const float4* tB = tA + S.ring.tp;
+        const int tt = (t == S.ring.nt - 1 ? S.ring.last_pairs : S.ring.tp) >> logL;
+        if (FORCE && !hot) sweep_pass<NA, FORCE, CULL, APF, MV, false>(tA, tB, tt, lane, L, tk, p, v, rd, eps, mask, acc);
+        else               sweep_pass<NA, FORCE, CULL, APF, MV, true>(tA, tB, tt, lane, L, tk, p, v, rd, eps, mask, acc);
+        ring_release(P, S);
+    }
+}
+
+// ring mode: does this warp have to refine the NEXT sweep?  dmin: the lane's clearance minima of the sweep just done,
+// v: the agents' new velocities
+template <int NA>
+__device__ __forceinline__ bool ring_predict_hot(const float (&dmin)[NA], const float (&v)[NA][3], float dt, float thr, float umax_dt) {
+    bool near = false;
+#pragma unroll
+    for (int a = 0; a < NA; ++a) near = near || (dmin[a] < thr + fmaf(dt, norm3f(v[a][0], v[a][1], v[a][2]), umax_dt));
+    return __any_sync(0xffffffffu, near);
+}
+
 // Transposed butterfly over a full warp.  In: per-lane partial (x,y,z) of NA agents.  Out: every lane of
 // half h (lanes 16h..16h+15; NA == 1: both halves) holds the warp total (X,Y,Z) of agent h.
 template <int NA>
@@ -569,10 +685,9 @@ __device__ __forceinline__ float4 group_reduce(const float4* part, int L, int la
 // ---------------------------------------------------------------------------------------------
 // group body, L == 32: one warp per group does everything; agent a on lanes 0-15, agent b on lanes 16-31
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV, bool ONE>
-__device__ __forceinline__ void group_rollout_warp_n(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
-                                                     int first_agent, int lane) {
-    const int trips = ONE ? 1 : (n2p >> 5);                // ONE: at most 32 sphere pairs, straight-line sweep
+template <bool RING, int NA, bool CULL, bool APF, bool PER, bool XT, bool MV, bool ONE>
+__device__ __forceinline__ void group_rollout_warp_n(const RolloutX2Params& P, SphSrc& S, int first_agent, int lane) {
+    const int trips = ONE ? 1 : (S.n2p >> 5);              // ONE: at most 32 sphere pairs, straight-line sweep
     const int half = (NA == 2) ? (lane >> 4) : 0;
     const unsigned full = 0xffffffffu;
     AgentX2 me;
@@ -582,8 +697,8 @@ __device__ __forceinline__ void group_rollout_warp_n(const RolloutX2Params& P, c
     rd.v[0] = __shfl_sync(full, me.rd, 0);
     if (NA == 2) rd.v[NA - 1] = __shfl_sync(full, me.rd, 16);
     X2Acc<NA> acc;
-    const float thr = lane_near_thr<APF>(tB, trips, lane, 32);
-    bool hot = false;
+    const float thr = lane_near_thr<APF>(RING ? P.pairB : S.tB, trips, lane, 32);
+    bool hot = RING;                                       // ring mode: step 0 refines, later steps as predicted
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);                  // pose S+1: distance-only pass
         const float tk = fmaf(float(k), P.dt, P.t0);       // obstacle time (moving spheres)
@@ -598,8 +713,8 @@ __device__ __forceinline__ void group_rollout_warp_n(const RolloutX2Params& P, c
             for (int i = 0; i < 3; ++i) { p[0][i] = me.p[i]; v[0][i] = me.v[i]; }
         }
         acc.clear();
-        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, thr, hot, acc);
-        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane, 32, tk, p, v, rd, P.eps, full, thr, hot, acc);
+        if (!last) sweep_src<RING, NA, true, CULL, APF, MV>(P, S, trips, lane, 32, 5, tk, p, v, rd, P.eps, full, thr, hot, acc);
+        else       sweep_src<RING, NA, false, false, false, MV>(P, S, trips, lane, 32, 5, tk, p, v, rd, P.eps, full, thr, hot, acc);
         float X, Y, Z, D;
         warp_combine<NA, acc_scaled<APF, MV>()>(acc, lane, X, Y, Z, D);
         if (last) {
@@ -610,15 +725,20 @@ __device__ __forceinline__ void group_rollout_warp_n(const RolloutX2Params& P, c
         me.pre(P);
         me.template post<(APF || MV)>(P, X, Y, Z, fx, fy, fz);
         me.costs(P, k, D, fx, fy, fz);
+        if (RING) {                                        // every lane needs both agents' new velocities
+            float vn[NA][3];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { vn[0][i] = __shfl_sync(full, me.v[i], 0); if (NA == 2) vn[NA - 1][i] = __shfl_sync(full, me.v[i], 16); }
+            hot = ring_predict_hot<NA>(acc.dmin, vn, P.dt, thr, S.umax_dt);
+        }
         if ((lane & 15) == 0 && (NA == 2 || lane == 0)) { if (XT) me.snapshot(P, k); }
     }
 }
 
-template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
-__device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
-                                                   int first_agent, int lane) {
-    if (n2p == 32) group_rollout_warp_n<NA, CULL, APF, PER, XT, MV, true>(P, tA, tB, n2p, first_agent, lane);
-    else group_rollout_warp_n<NA, CULL, APF, PER, XT, MV, false>(P, tA, tB, n2p, first_agent, lane);
+template <bool RING, int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
+__device__ __forceinline__ void group_rollout_warp(const RolloutX2Params& P, SphSrc& S, int first_agent, int lane) {
+    if (!RING && S.n2p == 32) group_rollout_warp_n<false, NA, CULL, APF, PER, XT, MV, true>(P, S, first_agent, lane);
+    else group_rollout_warp_n<RING, NA, CULL, APF, PER, XT, MV, false>(P, S, first_agent, lane);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -642,9 +762,10 @@ __device__ __forceinline__ void agent_load(AgentX2& a, const float* r) {
     a.gid = __float_as_int(r[20]); a.rd = r[21]; a.kf = r[22];
 }
 
-template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
-__device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p, int agent0,
+template <bool RING, int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
+__device__ __forceinline__ void chunk_step(const RolloutX2Params& P, SphSrc& S, int agent0,
                                            int lane, int k, float thr, bool& hot, float* rec0) {
+    const int n2p = S.n2p;
     const int half = (NA == 2) ? (lane >> 4) : 0;
     const unsigned full = 0xffffffffu;
     float* rec = rec0 + half * kAgentRecWords;
@@ -668,8 +789,8 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     const float tk = fmaf(float(k), P.dt, P.t0);
     X2Acc<NA> acc;
     acc.clear();
-    if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, thr, hot, acc);
-    else       sweep_any<NA, false, false, false, MV>(tA, tB, n2p >> 5, lane, 32, tk, p, v, rd, P.eps, full, thr, hot, acc);
+    if (!last) sweep_src<RING, NA, true, CULL, APF, MV>(P, S, n2p >> 5, lane, 32, 5, tk, p, v, rd, P.eps, full, thr, hot, acc);
+    else       sweep_src<RING, NA, false, false, false, MV>(P, S, n2p >> 5, lane, 32, 5, tk, p, v, rd, P.eps, full, thr, hot, acc);
     float X, Y, Z, D;
     warp_combine<NA, acc_scaled<APF, MV>()>(acc, lane, X, Y, Z, D);
     const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
@@ -681,15 +802,21 @@ __device__ __forceinline__ void chunk_step(const RolloutX2Params& P, const float
     me.pre(P);
     me.template post<(APF || MV)>(P, X, Y, Z, fx, fy, fz);
     me.costs(P, k, D, fx, fy, fz);
+    if (RING) {
+        float vn[NA][3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { vn[0][i] = __shfl_sync(full, me.v[i], 0); if (NA == 2) vn[NA - 1][i] = __shfl_sync(full, me.v[i], 16); }
+        hot = ring_predict_hot<NA>(acc.dmin, vn, P.dt, thr, S.umax_dt);
+    }
     if (writer) { if (XT) me.snapshot(P, k); }
     __syncwarp();                                         // every lane has read the record before it is rewritten
     if (writer) agent_store(me, rec);
     __syncwarp();
 }
 
-template <bool CULL, bool APF, bool PER, bool XT, bool MV>
-__device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
-                                                    int first_agent, int n_mine, int lane, float* recs) {
+template <bool RING, bool CULL, bool APF, bool PER, bool XT, bool MV>
+__device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, SphSrc& S, int first_agent, int n_mine, int rounds,
+                                                    int lane, float* recs) {
     // records of this warp's agents: recs[i * kAgentRecWords], i < n_mine
     for (int i = lane; i < n_mine; i += 32) {
         AgentX2 a;
@@ -697,15 +824,23 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
         agent_store(a, recs + i * kAgentRecWords);
     }
     __syncwarp();
-    const float thr = lane_near_thr<APF>(tB, n2p >> 5, lane, 32);
-    u64 hotbits = 0ull;                                    // refined-mode flag of each chunk (chunks beyond 64 share bits: harmless)
+    const float thr = lane_near_thr<APF>(RING ? P.pairB : S.tB, S.n2p >> 5, lane, 32);
+    // refined-mode flag of each chunk (chunks beyond 64 share bits: conservative in ring mode -- a shared bit is the OR
+    // of its chunks there -- and harmless otherwise); ring mode starts refined
+    u64 hotbits = RING ? ~0ull : 0ull;
     for (int k = 0; k <= P.steps; ++k) {
+        u64 next = 0ull;
         for (int i = 0; i < n_mine; i += 2) {
             const int c = (i >> 1) & 63;
             bool hot = (hotbits >> c) & 1ull;
-            if (i + 2 <= n_mine) chunk_step<2, CULL, APF, PER, XT, MV>(P, tA, tB, n2p, first_agent + i, lane, k, thr, hot, recs + i * kAgentRecWords);
-            else                 chunk_step<1, CULL, APF, PER, XT, MV>(P, tA, tB, n2p, first_agent + i, lane, k, thr, hot, recs + i * kAgentRecWords);
-            hotbits = (hotbits & ~(1ull << c)) | (u64(hot) << c);
+            if (i + 2 <= n_mine) chunk_step<RING, 2, CULL, APF, PER, XT, MV>(P, S, first_agent + i, lane, k, thr, hot, recs + i * kAgentRecWords);
+            else                 chunk_step<RING, 1, CULL, APF, PER, XT, MV>(P, S, first_agent + i, lane, k, thr, hot, recs + i * kAgentRecWords);
+            if (RING) next |= u64(hot) << c;
+            else hotbits = (hotbits & ~(1ull << c)) | (u64(hot) << c);
+        }
+        if (RING) {
+            hotbits = next;
+            for (int r = (n_mine + 1) >> 1; r < rounds; ++r) ring_skip_pass(P, S);     // keep the CTA's tile sequence
         }
     }
 }
@@ -719,9 +854,10 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, co
 //   sweep warp k:    write part -> arrive(bar_part) -> sync(bar_state) -> read state[k&1]
 //   epilogue warp k: sync(bar_part) -> reduce part -> integrate -> write state[k&1] -> arrive(bar_state) -> costs
 // ---------------------------------------------------------------------------------------------
-template <int NA, bool CULL, bool APF, bool PER, bool MV, bool ONE>
-__device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
+template <bool RING, int NA, bool CULL, bool APF, bool PER, bool MV, bool ONE>
+__device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, SphSrc& S,
                                                     int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
+    const int n2p = S.n2p;
     // n2p is a multiple of L: the same trip count on every lane.  ONE: a single trip (as many lanes as sphere pairs,
     // the latency-bound shapes): known at compile time, so the sweep is straight-line code without loop control
     const int trips = ONE ? 1 : (n2p >> P.logL);
@@ -740,14 +876,14 @@ __device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, co
         for (int i = 0; i < 3; ++i) { p[a][i] = s[i]; v[a][i] = s[3 + i]; }
     }
     X2Acc<NA> acc;
-    const float thr = lane_near_thr<APF>(tB, trips, lane_in_group, P.L);
-    bool hot = false;
+    const float thr = lane_near_thr<APF>(RING ? P.pairB : S.tB, trips, lane_in_group, P.L);
+    bool hot = RING;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         const float tk = fmaf(float(k), P.dt, P.t0);
         acc.clear();
-        if (!last) sweep_any<NA, true, CULL, APF, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, thr, hot, acc);
-        else       sweep_any<NA, false, false, false, MV>(tA, tB, trips, lane_in_group, P.L, tk, p, v, rd, P.eps, full, thr, hot, acc);
+        if (!last) sweep_src<RING, NA, true, CULL, APF, MV>(P, S, trips, lane_in_group, P.L, P.logL, tk, p, v, rd, P.eps, full, thr, hot, acc);
+        else       sweep_src<RING, NA, false, false, false, MV>(P, S, trips, lane_in_group, P.L, P.logL, tk, p, v, rd, P.eps, full, thr, hot, acc);
 #pragma unroll
         for (int a = 0; a < NA; ++a) {                     // per-lane partials; the epilogue warp reduces them
             constexpr bool SC = acc_scaled<APF, MV>();
@@ -762,14 +898,15 @@ __device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, co
             const float4 sp = state[(par * NA + a) * 2], sv = state[(par * NA + a) * 2 + 1];
             p[a][0] = sp.x; p[a][1] = sp.y; p[a][2] = sp.z; v[a][0] = sv.x; v[a][1] = sv.y; v[a][2] = sv.z;
         }
+        if (RING) hot = ring_predict_hot<NA>(acc.dmin, v, P.dt, thr, S.umax_dt);
     }
 }
 
-template <int NA, bool CULL, bool APF, bool PER, bool MV>
-__device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
+template <bool RING, int NA, bool CULL, bool APF, bool PER, bool MV>
+__device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, SphSrc& S,
                                                   int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
-    if ((n2p >> P.logL) == 1) group_sweep_warps_n<NA, CULL, APF, PER, MV, true>(P, tA, tB, n2p, first_agent, lane_in_group, group_in_cta, xch);
-    else group_sweep_warps_n<NA, CULL, APF, PER, MV, false>(P, tA, tB, n2p, first_agent, lane_in_group, group_in_cta, xch);
+    if (!RING && (S.n2p >> P.logL) == 1) group_sweep_warps_n<false, NA, CULL, APF, PER, MV, true>(P, S, first_agent, lane_in_group, group_in_cta, xch);
+    else group_sweep_warps_n<RING, NA, CULL, APF, PER, MV, false>(P, S, first_agent, lane_in_group, group_in_cta, xch);
 }
 
 template <int NA, bool APF, bool XT, int NW>   // APF here = "the sums are the force itself" (APF heuristic or moving spheres)
@@ -817,8 +954,9 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
 // group body, L < 32 (several groups per warp): plain butterfly, every lane integrates its group's agents
 // ---------------------------------------------------------------------------------------------
 template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
-__device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, const float4* tA, const float4* tB, int n2p,
+__device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, const SphSrc& S,
                                                      int first_agent, int lane_in_group) {
+    const float4* tA = S.tA; const float4* tB = S.tB; const int n2p = S.n2p;
     const unsigned mask = __activemask();
     const int trips = n2p >> P.logL;                       // n2p is a multiple of L
     AgentX2 ag[NA];
@@ -873,21 +1011,28 @@ template <int AT, int MODE, bool CULL, int STAGE, int MAXT, bool APF, bool XT, b
 __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ RolloutX2Params P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
-    const float4* tA = P.pairA;
-    const float4* tB = P.pairB;
+    constexpr bool RING = (STAGE == 2);
+    constexpr int NARR = MV ? 4 : 2;                        // pair arrays A, B (, U, V), equally spaced in global memory
+    SphSrc S;
+    S.tA = P.pairA; S.tB = P.pairB;
     const int tid = threadIdx.x;
     int n2p = P.n2p;
     if (P.count_dev) {                                      // built sphere world: the count never went to the host
         const int n = min(*P.count_dev, P.n_cap), h = (n + 1) >> 1;
         n2p = min(P.n2p, ((h + P.L - 1) >> P.logL) << P.logL);
     }
+    S.n2p = n2p;
+    const int cta_first = blockIdx.x * P.agents_per_cta;
+    int cta_end = cta_first + P.agents_per_cta;
+    if (cta_end > P.n_agents) cta_end = P.n_agents;
+    const int n_cta = cta_end - cta_first;
+    int rounds = 1;                                         // ring passes per step (mode 4: agent chunks per warp)
     if (STAGE == 1) {
         float4* tile = reinterpret_cast<float4*>(smem_raw + P.tile_off);
         if (tid == 0) { mbar_init(bar, 1); fence_mbar_init(); }
         __syncthreads();
         if (tid == 0 && n2p > 0) {
             const uint32_t bytes = uint32_t(n2p) * 16u;
-            constexpr int NARR = MV ? 4 : 2;                // pair arrays A, B (, U, V), equally spaced in global memory
             mbar_arrive_expect_tx(bar, NARR * bytes);
             const uint32_t chunk = 32768u;
             for (int r = 0; r < NARR; ++r) {
@@ -898,12 +1043,46 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
                 }
             }
         }
-        tA = tile;
-        tB = tile + n2p;
+        S.tA = tile;
+        S.tB = tile + n2p;
     }
-    const int cta_first = blockIdx.x * P.agents_per_cta;
-    int cta_end = cta_first + P.agents_per_cta;
-    if (cta_end > P.n_agents) cta_end = P.n_agents;
+    if (RING) {
+        // consumer warps of this CTA (warps that return at once because they have no agent do not count)
+        const int n_sweep_threads = int(blockDim.x);
+        int consumers;
+        if (MODE == 2) {
+            const int G = (P.agents_per_cta + AT - 1) / AT, ga = (n_cta + AT - 1) / AT;
+            consumers = (ga < G ? ga : G) * (P.L >> 5);
+        } else if (MODE == 4) {
+            const int nw = n_sweep_threads >> 5;
+            consumers = n_cta < nw ? n_cta : nw;
+            const int most = (n_cta + nw - 1) / nw;          // largest agent block of a warp
+            rounds = (most + 1) >> 1;
+        } else {
+            const int G = n_sweep_threads >> 5;
+            consumers = n_cta < G ? n_cta : G;
+        }
+        S.ring.full = reinterpret_cast<uint64_t*>(smem_raw + P.ring_off);
+        S.ring.done = reinterpret_cast<int*>(S.ring.full + kRingStages);
+        S.ring.slots = reinterpret_cast<const float4*>(smem_raw + P.tile_off);
+        S.ring.tp = P.ring_tp; S.ring.slot_f4 = NARR * P.ring_tp; S.ring.narr = NARR;
+        S.ring.nt = (n2p + P.ring_tp - 1) / P.ring_tp;
+        S.ring.last_pairs = n2p - (S.ring.nt - 1) * P.ring_tp;
+        S.ring.consumers = consumers; S.ring.total = (P.steps + 1) * rounds * S.ring.nt;
+        S.pos.slot = 0; S.pos.parity = 0u; S.pos.t = 0; S.pos.v = 0;
+        S.umax_dt = MV ? P.sph_stats[1] * P.dt : 0.0f;
+        if (tid == 0) {
+            for (int i = 0; i < kRingStages; ++i) { mbar_init(S.ring.full + i, 1); S.ring.done[i] = 0; }
+            fence_mbar_init();
+            // the first kRingStages visits; after that the last warp to release a slot refills it
+            for (int i = 0, t = 0; i < kRingStages && i < S.ring.total; ++i) { ring_issue(P, S.ring, t, i); if (++t == S.ring.nt) t = 0; }
+        }
+        __syncthreads();
+    } else {
+        S.ring.full = nullptr; S.ring.done = nullptr; S.ring.slots = nullptr;
+        S.ring.tp = S.ring.slot_f4 = S.ring.nt = S.ring.last_pairs = S.ring.narr = S.ring.consumers = S.ring.total = 0;
+        S.pos.slot = 0; S.pos.parity = 0u; S.pos.t = S.pos.v = 0; S.umax_dt = 0.0f;
+    }
     constexpr int NA2 = (AT == 2) ? 2 : 1;
     if (MODE == 2) {
         const int G = (P.agents_per_cta + AT - 1) / AT;
@@ -917,24 +1096,26 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
             if (na <= 0) return;
             if (AT == 2 && na >= 2) group_epilogue_warp<NA2, (APF || MV), XT>(P, first, tid & 31, group_in_cta, xch);
             else group_epilogue_warp<1, (APF || MV), XT>(P, first, tid & 31, group_in_cta, xch);
+            select_tail<GMAPP_FUSED_SELECT_X2 != 0>(P.sel, P.cost, P.collided, (AT == 2 && na >= 2) ? 2 : 1, tid & 31);    // S8: the last warp selects
             return;
         }
         if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
         if (na <= 0) return;
         const int lane_in_group = tid & (P.L - 1);
-        if (AT == 2 && na >= 2) { if (P.rd_arr) group_sweep_warps<NA2, CULL, APF, true, MV>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<NA2, CULL, APF, false, MV>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); }
-        else { if (P.rd_arr) group_sweep_warps<1, CULL, APF, true, MV>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<1, CULL, APF, false, MV>(P, tA, tB, n2p, first, lane_in_group, group_in_cta, xch); }
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_sweep_warps<RING, NA2, CULL, APF, true, MV>(P, S, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<RING, NA2, CULL, APF, false, MV>(P, S, first, lane_in_group, group_in_cta, xch); }
+        else { if (P.rd_arr) group_sweep_warps<RING, 1, CULL, APF, true, MV>(P, S, first, lane_in_group, group_in_cta, xch); else group_sweep_warps<RING, 1, CULL, APF, false, MV>(P, S, first, lane_in_group, group_in_cta, xch); }
         return;
     }
     if (MODE == 4) {
         // balanced contiguous split of the CTA's agents over its warps
-        const int nw = blockDim.x >> 5, w = tid >> 5, n_cta = cta_end - cta_first;
+        const int nw = int(blockDim.x) >> 5, w = tid >> 5;
         const int base = n_cta / nw, rem = n_cta % nw;
         const int start = w * base + (w < rem ? w : rem), n_mine = base + (w < rem ? 1 : 0);
         if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
         if (n_mine <= 0) return;
         float* recs = reinterpret_cast<float*>(smem_raw + P.rec_off) + start * kAgentRecWords;
-        { if (P.rd_arr) warp_rollout_chunks<CULL, APF, true, XT, MV>(P, tA, tB, n2p, cta_first + start, n_mine, tid & 31, recs); else warp_rollout_chunks<CULL, APF, false, XT, MV>(P, tA, tB, n2p, cta_first + start, n_mine, tid & 31, recs); }
+        { if (P.rd_arr) warp_rollout_chunks<RING, CULL, APF, true, XT, MV>(P, S, cta_first + start, n_mine, rounds, tid & 31, recs); else warp_rollout_chunks<RING, CULL, APF, false, XT, MV>(P, S, cta_first + start, n_mine, rounds, tid & 31, recs); }
+        select_tail<GMAPP_FUSED_SELECT_X2 != 0>(P.sel, P.cost, P.collided, n_mine, tid & 31);
         return;
     }
     const int group_in_cta = tid >> P.logL;
@@ -945,7 +1126,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         // one warp per group, G warps for n <= 2 G agents: the first n - G groups take two agents, the others one, so that
         // a warp count that is a multiple of 4 loads the four schedulers equally (28 agents on 16 warps = 12 x 2 + 4 x 1,
         // 7 agent-sweeps per scheduler; 14 warps x 2 would put 8 on two schedulers and 6 on the others)
-        const int G = blockDim.x >> 5, n = cta_end - cta_first;
+        const int G = int(blockDim.x) >> 5, n = n_cta;
         const int g2 = n - G < 0 ? 0 : (n - G > G ? G : n - G);
         first = cta_first + (group_in_cta < g2 ? 2 * group_in_cta : g2 + group_in_cta);
         na = group_in_cta < g2 ? 2 : (first < cta_end ? 1 : 0);
@@ -953,11 +1134,13 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
     if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
     if (na <= 0) return;
     if (MODE == 1) {
-        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_warp<NA2, CULL, APF, true, XT, MV>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_warp<NA2, CULL, APF, false, XT, MV>(P, tA, tB, n2p, first, lane_in_group); }
-        else { if (P.rd_arr) group_rollout_warp<1, CULL, APF, true, XT, MV>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_warp<1, CULL, APF, false, XT, MV>(P, tA, tB, n2p, first, lane_in_group); }
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_warp<RING, NA2, CULL, APF, true, XT, MV>(P, S, first, lane_in_group); else group_rollout_warp<RING, NA2, CULL, APF, false, XT, MV>(P, S, first, lane_in_group); }
+        else { if (P.rd_arr) group_rollout_warp<RING, 1, CULL, APF, true, XT, MV>(P, S, first, lane_in_group); else group_rollout_warp<RING, 1, CULL, APF, false, XT, MV>(P, S, first, lane_in_group); }
+        select_tail<GMAPP_FUSED_SELECT_X2 != 0>(P.sel, P.cost, P.collided, (AT == 2 && na >= 2) ? 2 : 1, tid & 31);
     } else {
-        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_narrow<NA2, CULL, APF, true, XT, MV>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_narrow<NA2, CULL, APF, false, XT, MV>(P, tA, tB, n2p, first, lane_in_group); }
-        else { if (P.rd_arr) group_rollout_narrow<1, CULL, APF, true, XT, MV>(P, tA, tB, n2p, first, lane_in_group); else group_rollout_narrow<1, CULL, APF, false, XT, MV>(P, tA, tB, n2p, first, lane_in_group); }
+        if (AT == 2 && na >= 2) { if (P.rd_arr) group_rollout_narrow<NA2, CULL, APF, true, XT, MV>(P, S, first, lane_in_group); else group_rollout_narrow<NA2, CULL, APF, false, XT, MV>(P, S, first, lane_in_group); }
+        else { if (P.rd_arr) group_rollout_narrow<1, CULL, APF, true, XT, MV>(P, S, first, lane_in_group); else group_rollout_narrow<1, CULL, APF, false, XT, MV>(P, S, first, lane_in_group); }
+        if (lane_in_group == 0) select_tail_serial<GMAPP_FUSED_SELECT_X2 != 0>(P.sel, P.cost, P.collided, (AT == 2 && na >= 2) ? 2 : 1);   // sub-warp groups
     }
 }
 

@@ -1,17 +1,7 @@
-// gmapp_x2_apf_x_mv.cu -- instantiates the packed f32x2 rollout kernels for 3D point agents: APF (Eq. 1) heuristic, moving spheres, with the snapshot / trajectory extras (own translation unit: parallel
-// compilation only).
+// gmapp_x2_apf_x_mv.cu -- instantiates the packed f32x2 rollout kernels for 3D point agents: APF (Eq. 1) heuristic, moving spheres, with the snapshot / trajectory extras
+// (own translation unit: parallel compilation only; the table macro lives in gmapp_tables.h).
 #include "gmapp_tables.h"
 
 namespace gmapp {
-rollout_x2_fn rollout_x2_kernel_apf_x_mv(int at, int mode, bool cull, int stage) {
-#define PICKX(A, M, MT)                                                                                                                                   \
-    (cull ? (stage ? (rollout_x2_fn)k_rollout_x2<A, M, true, 1, MT, true, true, true> : (rollout_x2_fn)k_rollout_x2<A, M, true, 0, MT, true, true, true>)     \
-          : (stage ? (rollout_x2_fn)k_rollout_x2<A, M, false, 1, MT, true, true, true> : (rollout_x2_fn)k_rollout_x2<A, M, false, 0, MT, true, true, true>))
-    // mode 3 = mode 2 compiled for up to 7 groups (21 warps, 80 registers); mode 2 proper holds <= 4 groups
-    // (20 warps = 5 per SM sub-partition, 96 registers), which is what one wave of config 3 needs
-    if (mode == 4) return PICKX(2, 4, 512);
-    if (at == 2) return mode == 3 ? PICKX(2, 2, 672) : (mode == 2 ? PICKX(2, 2, 640) : (mode == 1 ? PICKX(2, 1, 512) : PICKX(2, 0, 512)));
-    return mode == 3 ? PICKX(1, 2, 672) : (mode == 2 ? PICKX(1, 2, 640) : (mode == 1 ? PICKX(1, 1, 512) : PICKX(1, 0, 512)));
-#undef PICKX
-}
+GMAPP_X2_TABLE(rollout_x2_kernel_apf_x_mv, true, true, true)
 }  // namespace gmapp

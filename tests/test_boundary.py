@@ -42,7 +42,7 @@ def test_binding_struct_layout_matches_header():
             fields += [f.strip() for f in decl.split(None, 1)[1].split(",")]
     assert fields == [f for f, _ in api.gmapp_gains._fields_]
     assert ctypes.sizeof(api.gmapp_gains) == 19 * 4
-    assert ctypes.sizeof(api.gmapp_tuning) == 8 * 4 and ctypes.sizeof(api.gmapp_launch_info) == 13 * 4
+    assert ctypes.sizeof(api.gmapp_tuning) == 8 * 4 and ctypes.sizeof(api.gmapp_launch_info) == 14 * 4
     g = api.make_gains()
     assert abs(g.vel_factor - 0.5) < 1e-7 and abs(g.eps_dist - 1e-3) < 1e-9 and g.heuristic == 0
 

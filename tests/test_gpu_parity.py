@@ -755,14 +755,45 @@ def test_pose6_launch_variants_match_oracle(api, ctx, orc, tuning):
 
 
 def test_moving_sphere_sets_beyond_shared_memory(api, ctx, orc):
-    """9000 moving spheres = 4500 pairs x 64 B = 288 KB: the four pair arrays do not fit shared memory, so the
-    packed kernels (point agents) and the wide kernel (6D) read them through L1 / L2 (stage 0)."""
+    """9000 moving spheres = 4500 pairs x 64 B = 288 KB: the four pair arrays do not fit shared memory.  By default the
+    packed kernels (point agents) and the wide kernel (6D) read them through L1 / L2 (stage 0: few tiles); forced to the
+    TMA tile ring (stage 2) the packed kernels give the same trajectories within tolerance."""
     sc = scenes.fast_clutter(n_agents=40, n_spheres=9000, steps=40, moving=True)
     g, _ = _check_rollout(api, ctx, orc, sc)
     assert g["info"]["stage"] == 0 and g["info"]["packed_x2"] == 1
+    try:
+        g, _ = _check_rollout(api, ctx, orc, sc, tuning=dict(stage=2))
+        assert g["info"]["stage"] == 2 and g["info"]["n_tiles"] >= 4
+    finally:
+        ctx.set_tuning(reset=True)
     sc = scenes.config4(n_agents=12, n_spheres=9000, steps=40)
     g, _ = _check_rollout(api, ctx, orc, sc, smooth_tol=1e-3)
     assert g["info"]["stage"] == 0
+
+
+# TMA tile ring (stage 2) in every kernel mode that has it, static and moving, ragged tile tails, agent counts that leave
+# warps of a CTA with different numbers of chunks (skip passes) and CTAs with idle warps; against the oracle and against
+# the L1/L2 path (stage 0) of the same launch shape
+@pytest.mark.parametrize("moving", [False, True], ids=["static", "moving"])
+@pytest.mark.parametrize("n_agents,tuning", [(40, dict(lanes_per_agent=32)), (7, dict(lanes_per_agent=128, agents_per_thread=2, max_ctas=1)),
+                                             (300, dict(max_ctas=3)), (333, dict(max_ctas=7)), (45, dict(max_ctas=2)),
+                                             (21, dict(lanes_per_agent=64, agents_per_thread=2, max_ctas=2))],
+                         ids=["mode1", "mode2-7agents", "mode4-100perCTA", "mode4-ragged", "mode1-23perCTA", "mode2-L64"])
+def test_tile_ring_matches_oracle_and_l2_path(api, ctx, orc, n_agents, tuning, moving):
+    n_sph = 15001 if not moving else 9003                 # odd: a sentinel half-pair, a ragged last tile
+    sc = scenes.fast_clutter(n_agents=n_agents, n_spheres=n_sph, steps=20, moving=moving, r_lo=0.004, r_hi=0.012)
+    try:
+        g2, _ = _check_rollout(api, ctx, orc, sc, tuning=dict(tuning, stage=2), allow_illcond=0.03, smooth_tol=1e-3)
+        assert g2["info"]["stage"] == 2 and g2["info"]["n_tiles"] >= 4
+        g0 = api.run_scene(ctx, sc, tuning=dict(tuning, stage=0))
+        assert g0["info"]["stage"] == 0 and g0["info"]["block"] == g2["info"]["block"]
+        assert np.abs(g2["final"] - g0["final"]).max() <= 2e-5
+        assert np.array_equal(g2["collided"], g0["collided"]) or np.abs(g2["min_clearance"] - g0["min_clearance"]).max() < 1e-6
+        # bit-reproducible run to run (which warp refills a slot varies, the arithmetic does not)
+        again = api.run_scene(ctx, sc, tuning=dict(tuning, stage=2))
+        assert np.array_equal(again["final"], g2["final"]) and np.array_equal(again["cost"], g2["cost"])
+    finally:
+        ctx.set_tuning(reset=True)
 
 
 def test_cull_is_bitwise_identical_to_branch_free(api, ctx):
@@ -814,6 +845,69 @@ def test_hysteresis_and_collision_key(api, ctx, orc):
         want, _ = orc.best_agent(g["cost"].astype(np.float64), g["collided"], alpha, prev)
         got, cost = ctx.best_agent(alpha, prev)
         assert got == want and cost == g["cost"][got, 0]
+
+
+@pytest.mark.parametrize("tuning", [None, dict(lanes_per_agent=32), dict(lanes_per_agent=8, agents_per_thread=2, max_ctas=5), dict(max_ctas=1),
+                                    dict(lanes_per_agent=128, agents_per_thread=2, max_ctas=40), dict(scalar_path=1)],
+                         ids=lambda t: "auto" if t is None else "-".join(f"{k[:4]}{v}" for k, v in t.items()))
+def test_fused_selection_tail(api, ctx, orc, tuning):
+    """The selection runs in the tail of the rollout kernel (armed by gmapp_set_selection); gmapp_best_agent /
+    gmapp_select then only read its record.  Every kernel mode, repeated cycles (the ticket counter resets itself), the
+    heterogeneous ensemble (two launches share one ticket) and the 6D wide kernel; always against the oracle's
+    selection on the GPU's own costs, and against the stand-alone selection kernel."""
+    sc = scenes.fast_clutter(n_agents=160, n_spheres=500, r_lo=0.02, r_hi=0.07, steps=60)
+    try:
+        g = api.run_scene(ctx, sc, tuning=tuning)
+        cost, col = g["cost"].astype(np.float64), g["collided"]
+        raw_want, _ = orc.best_agent(cost, col, 0.9, -1)
+        order = np.lexsort((cost[:, 0], col))
+        for alpha, prev in ((0.9, int(order[1])), (0.9, int(order[-1])), (1.0, int(order[2])), (0.9, int(raw_want)), (0.9, -1)):
+            ctx.set_selection(alpha, prev)
+            for rep in range(2):                                   # twice: the ticket counter must be back at zero
+                g2 = api.run_scene(ctx, sc, tuning=tuning)
+                assert np.array_equal(g2["cost"], g["cost"])
+                rec = ctx.select(alpha, prev)
+                want, want_cost = orc.best_agent(cost, col, alpha, prev)
+                assert rec["index"] == want and rec["cost"] == g["cost"][want, 0] and rec["collided"] == col[want]
+                assert rec["raw_index"] == raw_want and rec["raw_cost"] == g["cost"][raw_want, 0]
+                if prev >= 0:
+                    assert rec["prev_cost"] == g["cost"][prev, 0] and rec["prev_collided"] == col[prev]
+                assert ctx.best_agent(alpha, prev)[0] == want
+                assert ctx.best_agent(alpha, -1)[0] == raw_want    # no incumbent asked: the raw argmin of the same record
+                other = int(order[3])                              # other arguments: the stand-alone selection kernel
+                assert ctx.best_agent(0.7, other)[0] == orc.best_agent(cost, col, 0.7, other)[0]
+    finally:
+        ctx.set_selection(0.9, -1)
+        ctx.set_tuning(reset=True)
+
+
+def test_fused_selection_ensemble_and_pose6(api, ctx, orc):
+    try:
+        sc = scenes.fast_clutter(n_agents=90, n_spheres=333)
+        classes, which = _ensemble_classes(sc.n_agents)
+        ctx.set_agent_params(np.array([classes[w]["r_influence"] for w in which], np.float32),
+                             np.array([classes[w]["k_circ"] for w in which], np.float32),
+                             np.array([classes[w]["heuristic"] for w in which], np.int32))
+        g = api.run_scene(ctx, sc)
+        assert g["info"]["kernels_launched"] == 2
+        cost, col = g["cost"].astype(np.float64), g["collided"]
+        prev = int(np.lexsort((cost[:, 0], col))[1])
+        ctx.set_selection(0.9, prev)
+        g = api.run_scene(ctx, sc)
+        assert ctx.select(0.9, prev)["index"] == orc.best_agent(cost, col, 0.9, prev)[0]
+        ctx.set_agent_params(n=0)
+        for sc6 in (scenes.config4(n_agents=32, n_spheres=512, steps=60), scenes.config4(n_agents=300, n_spheres=512, steps=30)):
+            ctx.set_selection(0.9, -1)
+            g = api.run_scene(ctx, sc6)                            # wide kernel (fused tail) / scalar kernel (selection kernel)
+            cost, col = g["cost"].astype(np.float64), g["collided"]
+            prev = int(np.lexsort((cost[:, 0], col))[2])
+            ctx.set_selection(0.9, prev)
+            g = api.run_scene(ctx, sc6)
+            rec = ctx.select(0.9, prev)
+            assert rec["index"] == orc.best_agent(cost, col, 0.9, prev)[0] and rec["raw_index"] == orc.best_agent(cost, col, 0.9, -1)[0]
+    finally:
+        ctx.set_agent_params(n=0)
+        ctx.set_selection(0.9, -1)
 
 
 def test_aliasing_out_equals_in(api, ctx):
