@@ -60,6 +60,7 @@ def parse_args():
     ap.add_argument("--lanes", type=int, default=0)
     ap.add_argument("--agents-per-thread", type=int, default=0)
     ap.add_argument("--stage", type=int, default=-1)
+    ap.add_argument("--max-ctas", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true", help="skip the all_configs key (every config + the sweep)")
     ap.add_argument("--rows", default="", help="comma-separated rows for all_configs (default: all of them)")
@@ -345,7 +346,8 @@ def run_ours(args):
     gains = api.make_gains(scene.gains)
 
     ctx = api.Context(max_agents=n_local, max_spheres=max(scene.n_spheres, 1), device=local_rank)
-    tune = dict(lanes_per_agent=args.lanes, agents_per_thread=args.agents_per_thread, cull=args.cull, stage=args.stage)
+    tune = dict(lanes_per_agent=args.lanes, agents_per_thread=args.agents_per_thread, cull=args.cull, stage=args.stage,
+                max_ctas=args.max_ctas)
     ctx.set_tuning(**tune)
     d_xyzr = torch.from_numpy(scene.xyzr).to(dev)
     d_vel = None if scene.vel is None else torch.from_numpy(scene.vel).to(dev)

@@ -262,6 +262,14 @@ gmapp_status gmapp_get_launch_info(const gmapp_ctx* ctx, gmapp_launch_info* out)
  * use_f32x2 != 0 issues packed fma.rn.f32x2 instead.  Synchronises. */
 gmapp_status gmapp_measure_fp32_peak(gmapp_ctx* ctx, int use_f32x2, float* out_tflops, void* cuda_stream);
 
+/* Issue-cost microbenchmarks behind the instruction-mix reasoning of DESIGN.md section 6 (results: profiles/r02_microbench.md):
+ * register-only kernels, 4 warps per SM sub-partition, 8 independent chains of ONE instruction kind.  *out_cycles = SM
+ * cycles per warp-instruction per sub-partition at the device's maximum SM clock.  kind: 0 FFMA (three distinct
+ * registers), 1 FFMA2 three distinct register pairs, 2 FFMA2 two distinct, 3 FFMA2 with a broadcast operand, 4 MUFU.RCP,
+ * 5 MUFU.RCP predicated off on every lane, 6 FMNMX, 7 FMNMX3, 8 FSETP + FSEL (per pair), 9 FFMA2 with three distinct register
+ * pairs none of which is shared between chains.  Synchronises.  EINVAL otherwise. */
+gmapp_status gmapp_microbench(gmapp_ctx* ctx, int kind, float* out_cycles, void* cuda_stream);
+
 /* Number of SMs of the context's device. */
 int gmapp_sm_count(const gmapp_ctx* ctx);
 

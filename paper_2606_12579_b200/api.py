@@ -55,7 +55,7 @@ class gmapp_launch_info(C.Structure):
 EXPORTS = ["gmapp_default_gains", "gmapp_create", "gmapp_destroy", "gmapp_set_obstacles",
            "gmapp_set_obstacles_host", "gmapp_build_sphere_world", "gmapp_get_obstacles", "gmapp_set_tuning", "gmapp_set_agent_params", "gmapp_rollout", "gmapp_set_trajectory_output", "gmapp_replan", "gmapp_best_agent", "gmapp_best_agent_ex", "gmapp_select", "gmapp_set_selection",
            "gmapp_forces",
-           "gmapp_get_results", "gmapp_plan_cycle_host", "gmapp_get_launch_info", "gmapp_measure_fp32_peak",
+           "gmapp_get_results", "gmapp_plan_cycle_host", "gmapp_get_launch_info", "gmapp_measure_fp32_peak", "gmapp_microbench",
            "gmapp_sm_count", "gmapp_last_error"]
 
 
@@ -94,6 +94,7 @@ def _load():
                                           C.c_float, C.c_int, C.c_float, C.c_int, ip, fp, vp]
     lib.gmapp_get_launch_info.argtypes = [vp, C.POINTER(gmapp_launch_info)]
     lib.gmapp_measure_fp32_peak.argtypes = [vp, C.c_int, fp, vp]
+    lib.gmapp_microbench.argtypes = [vp, C.c_int, fp, vp]
     lib.gmapp_sm_count.argtypes = [vp]; lib.gmapp_sm_count.restype = C.c_int
     lib.gmapp_last_error.argtypes = [vp]; lib.gmapp_last_error.restype = C.c_char_p
     for name in EXPORTS:
@@ -303,10 +304,20 @@ class Context:
         self._check(_lib.gmapp_get_launch_info(self._h, C.byref(info)))
         return info.as_dict()
 
+    def microbench(self, kind: int, stream=None) -> float:
+        out = C.c_float()
+        self._check(_lib.gmapp_microbench(self._h, int(kind), C.byref(out), _stream(stream)))
+        return out.value
+
     def measure_fp32_peak(self, use_f32x2=False, stream=None) -> float:
         out = C.c_float()
         self._check(_lib.gmapp_measure_fp32_peak(self._h, int(bool(use_f32x2)), C.byref(out), _stream(stream)))
         return out.value
+
+
+MICROBENCH_KINDS = ["FFMA, three distinct registers", "FFMA2, three distinct register pairs", "FFMA2, two distinct register pairs",
+                    "FFMA2, broadcast operand {a,a}", "MUFU.RCP (+ a co-issued FADD)", "MUFU.RCP predicated off on every lane", "FMNMX", "FMNMX3",
+                    "FSETP + FSEL (per pair of instructions)", "FFMA2, three distinct register pairs, none shared between chains"]
 
 
 def run_scene(ctx: Context, scene, device="cuda:0", tuning=None, steps=None):

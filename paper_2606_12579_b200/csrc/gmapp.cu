@@ -12,6 +12,7 @@
 #include "gmapp_rollout_x2.cuh"
 #include "gmapp_tables.h"
 #include "gmapp_voxel.cuh"
+#include "gmapp_microbench.cuh"
 
 using namespace gmapp;
 
@@ -636,7 +637,9 @@ static gmapp_status plan_rollout_x2(gmapp_ctx* c, int n_agents, X2Plan* o) {
     o->A = A; o->grid = grid; o->at = at; o->G = G; o->L = L; o->mode = mode; o->n2p = n2p; o->cull = cull; o->stage = stage;
     o->ring_tp = ring_tp; o->xch_off = xch_off; o->rec_off = rec_off; o->tile_off = tile_off; o->pair_bytes = pair_bytes;
     o->tile_bytes = tile_bytes;
-    o->block = mode == 4 ? tmax : (mode >= 2 ? G * L + 32 * G : round_up(G * L, 32));
+    // mode 3 with two agents per group: one epilogue warp per TWO groups (kernel table: MAXT 576)
+    if (mode == 3 && at == 2 && L != 64) return fail(c, GMAPP_EINVAL, "rollout: 5 to 7 two-agent groups per CTA need lanes_per_agent = 64, got %s%ld", "", L);
+    o->block = mode == 4 ? tmax : (mode == 3 && at == 2 ? G * L + 32 * ((G + 1) / 2) : (mode >= 2 ? G * L + 32 * G : round_up(G * L, 32)));
     o->smem = tile_off + (stage == 1 ? (int)tile_bytes : (stage == 2 ? kRingStages * ring_tp * pair_bytes : 0));
     return GMAPP_OK;
 }
@@ -1131,5 +1134,36 @@ extern "C" gmapp_status gmapp_measure_fp32_peak(gmapp_ctx* c, int use_f32x2, flo
     }
     const double fmas = (double)grid * block * (double)iters * 128.0;
     *out_tflops = (float)(2.0 * fmas / (best_ms * 1e-3) / 1e12);
+    return GMAPP_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// issue-cost microbenchmarks (gmapp_microbench.cuh)
+// ---------------------------------------------------------------------------------------------
+extern "C" gmapp_status gmapp_microbench(gmapp_ctx* c, int kind, float* out_cycles, void* stream) {
+    if (!c || !out_cycles) return GMAPP_EINVAL;
+    if (kind < 0 || kind >= MB_COUNT) return fail(c, GMAPP_EINVAL, "microbench: kind must be 0..%s%ld", "", (long)MB_COUNT - 1);
+    cudaStream_t st = (cudaStream_t)stream;
+    int clock_khz = 0;
+    CUDA_TRY(c, cudaDeviceGetAttribute(&clock_khz, cudaDevAttrClockRate, c->device));
+    const int iters = 20000;
+    float best_ms = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        CUDA_TRY(c, cudaEventRecord(c->ev0, st));
+        const float a = 0.999f, b = 1e-3f, thr = 1e30f;
+        switch (kind) {
+#define MB_CASE(K) case K: k_microbench<K><<<c->num_sms, 512, 0, st>>>(c->d_scratch, iters, a, b, thr); break;
+            MB_CASE(0) MB_CASE(1) MB_CASE(2) MB_CASE(3) MB_CASE(4) MB_CASE(5) MB_CASE(6) MB_CASE(7) MB_CASE(8) MB_CASE(9)
+#undef MB_CASE
+        }
+        CUDA_TRY(c, cudaGetLastError());
+        CUDA_TRY(c, cudaEventRecord(c->ev1, st));
+        CUDA_TRY(c, cudaEventSynchronize(c->ev1));
+        float ms = 0.0f;
+        CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+        if (rep > 0 && ms < best_ms) best_ms = ms;
+    }
+    // cycles per warp-instruction per SM sub-partition at the device's maximum SM clock: 4 warps x iters x 8 instructions
+    *out_cycles = (float)((double)best_ms * 1e-3 * (double)clock_khz * 1e3 / (4.0 * iters * 8.0));
     return GMAPP_OK;
 }

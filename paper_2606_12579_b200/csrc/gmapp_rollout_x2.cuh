@@ -951,6 +951,78 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
 }
 
 // ---------------------------------------------------------------------------------------------
+// One epilogue warp serving TWO groups (5 to 7 groups per CTA: 9 to 14 agents).  With an epilogue warp per group such a
+// CTA has 21 warps, which puts 6 warps on one SM sub-partition and cuts the register budget from 96 to 80 (2048 agents
+// x 4096 spheres: 0.54 of peak); shared, it has 18 warps and keeps 96+.  The warp serves its groups in a fixed order each
+// step; the second group's hand-over waits for the first one's (~0.3 us against a sweep of several us).
+// NA1 = 0: the warp's second group does not exist (odd group count, or the CTA's agents end before it).
+// ---------------------------------------------------------------------------------------------
+template <int NA>
+struct EpiSide {
+    AgentX2 me;
+    const float4* part; float4* state;
+    int bar_part, bar_state, half;
+    __device__ __forceinline__ void init(const RolloutX2Params& P, int first_agent, int lane, int group_in_cta, float4* xch) {
+        half = (NA == 2) ? (lane >> 4) : 0;
+        part = xch; state = xch + 2 * P.L;
+        bar_part = 1 + 2 * group_in_cta; bar_state = 2 + 2 * group_in_cta;
+        me.init(P, first_agent + half);
+    }
+    // one step of this group: returns false after the final pose
+    template <bool APF, bool XT, int LW>                    // LW = sweep warps per group (L / 32)
+    __device__ __forceinline__ void step(const RolloutX2Params& P, int k, int lane, float& dmin, float& fx, float& fy, float& fz) {
+        constexpr int NP = NA == 2 ? 2 * LW : LW;           // partials per epilogue lane
+        constexpr int NW = (NP == 2 || NP == 4 || NP == 8) ? NP : 0;
+        const bool last = (k == P.steps);
+        const int par = k & 1, nbar = P.L + 32;
+        const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
+        me.pre(P);
+        named_bar_sync(bar_part, nbar);
+        const float4 t = group_reduce<NA, NW>(part, P.L, lane);
+        dmin = t.w;
+        if (last) { if (writer) me.finish(P, t.w); return; }
+        me.template post<APF>(P, t.x, t.y, t.z, fx, fy, fz);
+        if (writer) {
+            state[(par * NA + half) * 2] = make_float4(me.p[0], me.p[1], me.p[2], 0.0f);
+            state[(par * NA + half) * 2 + 1] = make_float4(me.v[0], me.v[1], me.v[2], 0.0f);
+        }
+        named_bar_arrive(bar_state, nbar);
+    }
+};
+
+template <int NA0, int NA1, bool APF, bool XT, int LW>
+__device__ __forceinline__ void group_epilogue_warp2_n(const RolloutX2Params& P, int first0, int first1, int lane, int g0, float4* xch0, float4* xch1) {
+    EpiSide<NA0> s0;
+    EpiSide<(NA1 > 0 ? NA1 : 1)> s1;
+    s0.init(P, first0, lane, g0, xch0);
+    if (NA1 > 0) s1.init(P, first1, lane, g0 + 1, xch1);
+    for (int k = 0; k <= P.steps; ++k) {
+        float d0, d1 = 0.0f, f0x, f0y, f0z, f1x, f1y, f1z;
+        s0.template step<APF, XT, LW>(P, k, lane, d0, f0x, f0y, f0z);
+        if (NA1 > 0) s1.template step<APF, XT, LW>(P, k, lane, d1, f1x, f1y, f1z);
+        if (k == P.steps) return;
+        s0.me.costs(P, k, d0, f0x, f0y, f0z);              // off the critical path: both groups' sweep warps are running
+        if ((lane & 15) == 0 && (NA0 == 2 || lane == 0)) { if (XT) s0.me.snapshot(P, k); }
+        if (NA1 > 0) {
+            s1.me.costs(P, k, d1, f1x, f1y, f1z);
+            if ((lane & 15) == 0 && (NA1 == 2 || lane == 0)) { if (XT) s1.me.snapshot(P, k); }
+        }
+    }
+}
+
+// na0, na1: agents of the warp's two groups (na0 in {1, 2}; na1 in {0, 1, 2}, and na1 > 0 only if na0 == 2)
+template <bool APF, bool XT>
+__device__ __forceinline__ void group_epilogue_warp2(const RolloutX2Params& P, int first0, int na0, int na1, int lane, int g0,
+                                                     float4* xch0, float4* xch1) {
+    const int first1 = first0 + 2;
+    // 5 to 7 groups of two sweep warps each (L = 64; the host selects this shape only then)
+    if (na0 >= 2 && na1 >= 2) group_epilogue_warp2_n<2, 2, APF, XT, 2>(P, first0, first1, lane, g0, xch0, xch1);
+    else if (na0 >= 2 && na1 == 1) group_epilogue_warp2_n<2, 1, APF, XT, 2>(P, first0, first1, lane, g0, xch0, xch1);
+    else if (na0 >= 2) group_epilogue_warp2_n<2, 0, APF, XT, 2>(P, first0, first1, lane, g0, xch0, xch1);
+    else group_epilogue_warp2_n<1, 0, APF, XT, 2>(P, first0, first1, lane, g0, xch0, xch1);
+}
+
+// ---------------------------------------------------------------------------------------------
 // group body, L < 32 (several groups per warp): plain butterfly, every lane integrates its group's agents
 // ---------------------------------------------------------------------------------------------
 template <int NA, bool CULL, bool APF, bool PER, bool XT, bool MV>
@@ -1085,13 +1157,23 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
     }
     constexpr int NA2 = (AT == 2) ? 2 : 1;
     if (MODE == 2) {
+        constexpr bool EPI2 = (AT == 2 && MAXT == 576);     // one epilogue warp per TWO groups (5-7 groups of L = 64)
         const int G = (P.agents_per_cta + AT - 1) / AT;
         const int n_sweep = G * P.L;
         const bool is_epi = tid >= n_sweep;
-        const int group_in_cta = is_epi ? ((tid - n_sweep) >> 5) : (tid >> P.logL);
+        const int group_in_cta = is_epi ? ((tid - n_sweep) >> 5) * (EPI2 ? 2 : 1) : (tid >> P.logL);
         const int first = cta_first + group_in_cta * AT;
         const int na = cta_end - first;
         float4* xch = reinterpret_cast<float4*>(smem_raw + P.xch_off) + group_in_cta * (2 * P.L + 8);
+        if (is_epi && EPI2) {
+            if (na <= 0) return;
+            int na1 = (group_in_cta + 1 < G) ? na - 2 : 0;
+            if (na1 > 2) na1 = 2;
+            if (na1 < 0) na1 = 0;
+            group_epilogue_warp2<(APF || MV), XT>(P, first, na, na1, tid & 31, group_in_cta, xch, xch + (2 * P.L + 8));
+            select_tail<GMAPP_FUSED_SELECT_X2 != 0>(P.sel, P.cost, P.collided, (na >= 2 ? 2 : 1) + na1, tid & 31);
+            return;
+        }
         if (is_epi) {                                      // the epilogue warps never touch the sphere tile
             if (na <= 0) return;
             if (AT == 2 && na >= 2) group_epilogue_warp<NA2, (APF || MV), XT>(P, first, tid & 31, group_in_cta, xch);
