@@ -984,6 +984,42 @@ def test_error_statuses(api):
         api.Context(max_agents=0, max_spheres=4)
 
 
+def test_errors_enqueue_nothing_and_plan_cycle_sphere_count(api, ctx, orc):
+    """(1) A refused rollout has enqueued nothing: the trajectory buffer (whose pose-0 copy used to be enqueued before the
+    per-agent-parameter check) is untouched.  (2) gmapp_plan_cycle_host: n_spheres < 0 keeps the resident sphere world,
+    n_spheres == 0 sets an EMPTY one (include/gmapp.h)."""
+    import torch
+    sc = scenes.fast_clutter(n_agents=20, n_spheres=50, steps=10)
+    ctx.set_obstacles(_tensor(sc.xyzr), None, n=sc.n_spheres)
+    traj = torch.full((20, 11, 6), -7.0, device="cuda:0")
+    try:
+        ctx.set_trajectory_output(traj)
+        ctx.set_agent_params(r_influence=np.full(19, 0.1, np.float32))
+        with pytest.raises(api.GmappError) as e:
+            ctx.rollout(api.GMAPP_POINT3, _tensor(sc.agents), None, sc.goal, sc.gains, sc.dt, sc.steps)
+        assert e.value.status == api.GMAPP_EINVAL
+        torch.cuda.synchronize()
+        assert bool((traj == -7.0).all())
+        ctx.set_agent_params(n=0)
+        with pytest.raises(api.GmappError):                      # replan: bad gains are refused before the first launch
+            ctx.replan(api.GMAPP_POINT3, _tensor(sc.agents), sc.goal, dict(sc.gains, eps_dist=0.0), sc.dt, sc.steps, 5, 2)
+        torch.cuda.synchronize()
+        assert bool((traj == -7.0).all())
+    finally:
+        ctx.set_agent_params(n=0)
+        ctx.set_trajectory_output(None)
+    sc = scenes.fast_clutter(n_agents=30, n_spheres=120, steps=60)
+    out_a = np.zeros_like(sc.agents); out_b = np.zeros_like(sc.agents); out_c = np.zeros_like(sc.agents)
+    ctx.plan_cycle_host(api.GMAPP_POINT3, sc.agents, sc.goal, sc.gains, sc.dt, sc.steps, h_xyzr=sc.xyzr, h_agents_out=out_a)
+    ctx.plan_cycle_host(api.GMAPP_POINT3, sc.agents, sc.goal, sc.gains, sc.dt, sc.steps, h_xyzr=None, h_agents_out=out_b)
+    assert np.array_equal(out_a, out_b)                          # kept
+    ctx.plan_cycle_host(api.GMAPP_POINT3, sc.agents, sc.goal, sc.gains, sc.dt, sc.steps,
+                        h_xyzr=np.zeros((0, 4), np.float32), h_agents_out=out_c)
+    free = orc.rollout_point3(sc.agents, np.zeros((0, 4), np.float32), None, sc.goal, sc.gains, sc.dt, sc.steps)
+    assert np.abs(out_c[:, :3] - free["final"][:, :3]).max() <= 1e-6          # emptied: the no-obstacle rollout
+    assert np.abs(out_c - out_a).max() > 1e-4
+
+
 def test_fp32_peak_microbenchmark(api, ctx):
     t = ctx.measure_fp32_peak()
     assert 30.0 < t < 90.0, t          # 148 SMs x 128 lanes x 2 x ~1.9 GHz ~ 72 TFLOP/s
