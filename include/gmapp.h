@@ -145,6 +145,24 @@ gmapp_status gmapp_build_sphere_world(gmapp_ctx* ctx, const float* d_points, int
                                       const float* hi, float pitch, int capacity, int32_t* d_count_out,
                                       void* cuda_stream);
 
+/* ALLOCATION-FREE variant of the sphere-world builder, for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it).  No context: the scratch memory (voxel bitmap + block
+ * counter) is a file-scope static device array of the library -- 33 024 bytes that every GPU that loads the library
+ * holds until the process exits -- and the call performs no cudaMalloc / cudaFree / allocating library routine.
+ * Same computation and conventions as gmapp_build_sphere_world (Eq. 5); the result
+ * goes to the CALLER's DEVICE buffer d_xyzr_out [capacity][4] (16-byte aligned): the min(count, capacity) occupied-voxel
+ * spheres (x, y, z, r) in increasing linear voxel index, then sentinels (1e6, 1e6, 1e6, 0) -- i.e. what
+ * gmapp_build_sphere_world + gmapp_get_obstacles return, bit for bit; d_count_out (nullable DEVICE int32) = occupied voxels.
+ * Feed it to gmapp_set_obstacles.  LIMIT: the voxel grid may hold at most 262 144 voxels (e.g. 64^3; the paper's 1 m^3
+ * workspace at pitch 4 cm has 15 625) and 4096 per axis; larger grids return GMAPP_ECAPACITY with nothing launched
+ * (use gmapp_build_sphere_world).  `device` = CUDA device index 0..63, made current by the call.  Asynchronous on
+ * cuda_stream (a memset of the scratch, then one kernel).  All calls on a device SHARE the one scratch array (it is cleared
+ * at the start of every call): calls whose stream work overlaps on the same GPU race -- keep them on one stream or order them.
+ * Errors: EINVAL / ECAPACITY / ECUDA; the message is in gmapp_last_error(NULL). */
+gmapp_status gmapp_build_sphere_world_static(int device, const float* d_points, int n_points, const float* lo,
+                                             const float* hi, float pitch, int capacity, float* d_xyzr_out,
+                                             int32_t* d_count_out, void* cuda_stream);
+
 /* Copy the first n spheres of the resident sphere world, (x, y, z, r) each, into a caller-owned DEVICE buffer
  * [n][4] (after gmapp_build_sphere_world: the occupied-voxel spheres, then sentinels at (1e6, 1e6, 1e6) with radius 0).  Asynchronous. */
 gmapp_status gmapp_get_obstacles(gmapp_ctx* ctx, float* d_xyzr_out, int n, void* cuda_stream);

@@ -53,7 +53,7 @@ class gmapp_launch_info(C.Structure):
 
 
 EXPORTS = ["gmapp_default_gains", "gmapp_create", "gmapp_destroy", "gmapp_set_obstacles",
-           "gmapp_set_obstacles_host", "gmapp_build_sphere_world", "gmapp_get_obstacles", "gmapp_set_tuning", "gmapp_set_agent_params", "gmapp_rollout", "gmapp_set_trajectory_output", "gmapp_replan", "gmapp_best_agent", "gmapp_best_agent_ex", "gmapp_select", "gmapp_set_selection",
+           "gmapp_set_obstacles_host", "gmapp_build_sphere_world", "gmapp_build_sphere_world_static", "gmapp_get_obstacles", "gmapp_set_tuning", "gmapp_set_agent_params", "gmapp_rollout", "gmapp_set_trajectory_output", "gmapp_replan", "gmapp_best_agent", "gmapp_best_agent_ex", "gmapp_select", "gmapp_set_selection",
            "gmapp_forces",
            "gmapp_get_results", "gmapp_plan_cycle_host", "gmapp_get_launch_info", "gmapp_measure_fp32_peak", "gmapp_microbench",
            "gmapp_sm_count", "gmapp_last_error"]
@@ -77,6 +77,7 @@ def _load():
     lib.gmapp_set_obstacles.argtypes = [vp, vp, vp, C.c_int, vp]
     lib.gmapp_set_obstacles_host.argtypes = [vp, vp, vp, C.c_int, vp]
     lib.gmapp_build_sphere_world.argtypes = [vp, vp, C.c_int, fp, fp, C.c_float, C.c_int, vp, vp]
+    lib.gmapp_build_sphere_world_static.argtypes = [C.c_int, vp, C.c_int, fp, fp, C.c_float, C.c_int, vp, vp, vp]
     lib.gmapp_get_obstacles.argtypes = [vp, vp, C.c_int, vp]
     lib.gmapp_set_tuning.argtypes = [vp, C.POINTER(gmapp_tuning)]
     lib.gmapp_set_agent_params.argtypes = [vp, vp, vp, vp, C.c_int, vp]
@@ -159,6 +160,19 @@ def state14_to_pose(state14):
     rw, rv, dw, dv = r[:, 0], r[:, 1:], d[:, 0], d[:, 1:]
     t = 2.0 * (rw[:, None] * dv - dw[:, None] * rv + np.cross(rv, dv))
     return r.copy(), t, s[:, 8:].copy()
+
+
+def build_sphere_world_static(d_points, lo, hi, pitch, capacity, d_xyzr_out, d_count_out=None, n_points=None, device=0,
+                              stream=None):
+    """gmapp_build_sphere_world_static: the allocation-free sphere-world builder (no context; scratch in a static device
+    array of the library, at most 262 144 voxels).  d_xyzr_out: caller-owned device tensor [capacity][4]."""
+    n = int(d_points.shape[0]) if n_points is None else n_points
+    lp, k1 = _farr(lo, 3)
+    hp, k2 = _farr(hi, 3)
+    st = _lib.gmapp_build_sphere_world_static(int(device), _ptr(d_points), n, lp, hp, C.c_float(pitch), int(capacity),
+                                              _ptr(d_xyzr_out), _ptr(d_count_out), _stream(stream))
+    if st != GMAPP_OK:
+        raise GmappError(st, _lib.gmapp_last_error(None).decode())
 
 
 class Context:

@@ -1167,3 +1167,149 @@ extern "C" gmapp_status gmapp_microbench(gmapp_ctx* c, int kind, float* out_cycl
     *out_cycles = (float)((double)best_ms * 1e-3 * (double)clock_khz * 1e3 / (4.0 * iters * 8.0));
     return GMAPP_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// Allocation-free entry point: the sphere-world builder with its scratch in a file-scope static device array.
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+// no context, no cudaMalloc / cudaFree / allocating library routine anywhere on this path.
+//
+// The scratch -- the voxel bitmap of the largest grid this entry point accepts, kStaticMaxVoxels = 262 144 voxels = 8192
+// words, plus the finished-block counter -- is g_static_scratch below: 33 024 bytes that EVERY GPU that loads the library
+// holds until the process exits.  In host code the array's NAME is a host-side stand-in, not a device address: the
+// address is fetched once per device, with that device current, by cudaGetSymbolAddress, and that pointer is what the
+// kernel gets.  All calls (of every thread, on every stream) share the one array of a device: it is cleared at the start
+// of every call (stream-ordered memset; it also keeps the previous call's contents otherwise), and two calls whose
+// stream work OVERLAPS on the same GPU race on it -- keep calls on one stream, or order them yourself.
+// ---------------------------------------------------------------------------------------------
+constexpr int kStaticMaxVoxels = kVoxSmallWords * 32;
+constexpr int kStaticScratchWords = kVoxSmallWords + 64;     // bitmap words, then the counter (padded to 256 bytes)
+static __device__ __align__(256) unsigned g_static_scratch[kStaticScratchWords];
+
+// the small-grid build of gmapp_voxel.cuh writing only a caller-owned (x, y, z, r) array: per-block bitmaps in shared
+// memory, merged into the scratch bitmap; the block that finishes last scans it and emits the spheres over the sentinels
+__global__ void __launch_bounds__(1024) k_vox_build_static(const float* __restrict__ pts, int n_points, const __grid_constant__ VoxelGrid G,
+                                                           unsigned* scratch, int capacity, float4* xyzr_out, int* count_out) {
+    extern __shared__ unsigned sbits[];                      // [n_words] this block's bitmap; the last block: the merged one
+    __shared__ int s[32];
+    __shared__ int s_last;
+    unsigned* bitmap = scratch;
+    int* done = reinterpret_cast<int*>(scratch + kVoxSmallWords);
+    const int t = threadIdx.x, lane = t & 31, wid = t >> 5, nw = G.n_words;
+    for (int w = t; w < nw; w += 1024) sbits[w] = 0u;
+    __syncthreads();
+    for (int i = blockIdx.x * 1024 + t; i < n_points; i += gridDim.x * 1024) {
+        const int v = vox_of_point(pts, i, G);
+        if (v >= 0) {
+            const unsigned bit = 1u << (v & 31);
+            if (!(sbits[v >> 5] & bit)) atomicOr(&sbits[v >> 5], bit);
+        }
+    }
+    for (int i = blockIdx.x * 1024 + t; i < capacity; i += gridDim.x * 1024) xyzr_out[i] = make_float4(kFar, kFar, kFar, 0.0f);
+    __syncthreads();
+    for (int w = t; w < nw; w += 1024) {
+        const unsigned m = sbits[w];
+        if (m && (m & ~__ldcg(&bitmap[w]))) atomicOr(&bitmap[w], m);
+    }
+    __threadfence();
+    __syncthreads();
+    if (t == 0) s_last = (atomicAdd(done, 1) == int(gridDim.x) - 1) ? 1 : 0;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    const int per = (nw + 1023) / 1024;                      // thread t owns the contiguous words [t per, t per + per)
+    int mine = 0;
+    for (int k = 0; k < per; ++k) {
+        const int w = t * per + k;
+        if (w < nw) { const unsigned m = __ldcg(&bitmap[w]); sbits[w] = m; mine += __popc(m); }
+    }
+    int inc = mine;
+    for (int off = 1; off < 32; off <<= 1) { int o = __shfl_up_sync(0xffffffffu, inc, off); if (lane >= off) inc += o; }
+    if (lane == 31) s[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        int ws = s[lane], wi = ws;
+        for (int off = 1; off < 32; off <<= 1) { int o = __shfl_up_sync(0xffffffffu, wi, off); if (lane >= off) wi += o; }
+        s[lane] = wi - ws;
+        if (lane == 31 && count_out) *count_out = wi;
+    }
+    __syncthreads();
+    int rank = s[wid] + inc - mine;
+    for (int k = 0; k < per; ++k) {
+        const int w = t * per + k;
+        if (w >= nw) break;
+        unsigned bits = sbits[w];
+        while (bits) {
+            const int bpos = __ffs(bits) - 1;
+            bits &= bits - 1;
+            if (rank < capacity) xyzr_out[rank] = vox_sphere((unsigned(w) << 5) + bpos, G);
+            ++rank;
+        }
+    }
+}
+
+#include <mutex>
+namespace {
+struct StaticDev { bool ready; unsigned* scratch; int sms; };
+StaticDev g_static_dev[64];                                  // zero-initialised: not ready
+std::mutex g_static_mutex;
+}  // namespace
+
+// once per device, with that device current: the DEVICE address of g_static_scratch and the SM count
+static gmapp_status static_setup(int device, StaticDev* out) {
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDev& d = g_static_dev[device];
+    if (!d.ready) {
+        void* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess || !p) return fail(nullptr, GMAPP_ECUDA, "build_sphere_world_static: cudaGetSymbolAddress failed: %s", cudaGetErrorString(e));
+        int sms = 0;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+        if (e != cudaSuccess || sms < 1) return fail(nullptr, GMAPP_ECUDA, "build_sphere_world_static: cudaDeviceGetAttribute failed: %s", cudaGetErrorString(e));
+        d.scratch = (unsigned*)p; d.sms = sms; d.ready = true;
+    }
+    *out = d;
+    return GMAPP_OK;
+}
+
+extern "C" gmapp_status gmapp_build_sphere_world_static(int device, const float* d_points, int n_points, const float* lo,
+                                                        const float* hi, float pitch, int capacity, float* d_xyzr_out,
+                                                        int32_t* d_count_out, void* stream) {
+    if (device < 0 || device >= 64) return fail(nullptr, GMAPP_EINVAL, "build_sphere_world_static: device must be 0..63%s");
+    if (n_points < 0 || (n_points > 0 && !d_points) || !lo || !hi || !d_xyzr_out)
+        return fail(nullptr, GMAPP_EINVAL, "build_sphere_world_static: NULL points / bounds / output or n_points < 0%s");
+    if (((uintptr_t)d_xyzr_out & 15u) != 0) return fail(nullptr, GMAPP_EINVAL, "build_sphere_world_static: d_xyzr_out must be 16-byte aligned%s");
+    if (!isfinite(pitch) || !(pitch > 0.0f)) return fail(nullptr, GMAPP_EINVAL, "build_sphere_world_static: pitch must be finite and > 0%s");
+    if (capacity < 1 || capacity > (1 << 24)) return fail(nullptr, GMAPP_EINVAL, "build_sphere_world_static: capacity must be 1..2^24%s");
+    VoxelGrid G;
+    double nvox = 1.0;
+    for (int a = 0; a < 3; ++a) {
+        if (!isfinite(lo[a]) || !isfinite(hi[a]) || !(hi[a] > lo[a])) return fail(nullptr, GMAPP_EINVAL, "build_sphere_world_static: need finite lo < hi%s");
+        G.lo[a] = lo[a]; G.hi[a] = hi[a];
+        const double d = ceil(((double)hi[a] - (double)lo[a]) / (double)pitch);
+        if (d > 4096.0) return fail(nullptr, GMAPP_ECAPACITY, "build_sphere_world_static: more than 4096 voxels along an axis (static scratch: %s%ld voxels in all)", "", (long)kStaticMaxVoxels);
+        G.dim[a] = d < 1.0 ? 1 : (int)d;
+        nvox *= G.dim[a];
+    }
+    if (nvox > (double)kStaticMaxVoxels)
+        return fail(nullptr, GMAPP_ECAPACITY, "build_sphere_world_static: the voxel grid (%s%ld voxels) exceeds the static scratch of %ld voxels; "
+                    "use gmapp_build_sphere_world", "", (long)nvox, (long)kStaticMaxVoxels);
+    G.pitch = pitch;
+    G.n_words = ((int)nvox + 31) / 32;
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) return fail(nullptr, GMAPP_ECUDA, "build_sphere_world_static: cudaSetDevice: %s", cudaGetErrorString(e));
+    StaticDev dev;
+    gmapp_status s = static_setup(device, &dev);
+    if (s != GMAPP_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    // the array keeps the last call's contents: the bitmap words and the counter must start at zero
+    e = cudaMemsetAsync(dev.scratch, 0, sizeof(unsigned) * kStaticScratchWords, st);
+    if (e != cudaSuccess) return fail(nullptr, GMAPP_ECUDA, "build_sphere_world_static: cudaMemsetAsync: %s", cudaGetErrorString(e));
+    int grid = (n_points + 2047) / 2048;                    // two points per thread
+    if (grid < 1) grid = 1;
+    if (grid > 2 * dev.sms) grid = 2 * dev.sms;
+    k_vox_build_static<<<grid, 1024, sizeof(unsigned) * G.n_words, st>>>(d_points, n_points, G, dev.scratch, capacity,
+                                                                        reinterpret_cast<float4*>(d_xyzr_out), d_count_out);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(nullptr, GMAPP_ECUDA, "build_sphere_world_static: kernel launch: %s", cudaGetErrorString(e));
+    return GMAPP_OK;
+}
