@@ -331,7 +331,10 @@ class Context:
 
 MICROBENCH_KINDS = ["FFMA, three distinct registers", "FFMA2, three distinct register pairs", "FFMA2, two distinct register pairs",
                     "FFMA2, broadcast operand {a,a}", "MUFU.RCP (+ a co-issued FADD)", "MUFU.RCP predicated off on every lane", "FMNMX", "FMNMX3",
-                    "FSETP + FSEL (per pair of instructions)", "FFMA2, three distinct register pairs, none shared between chains"]
+                    "FSETP + FSEL (per pair of instructions)", "FFMA2, three distinct register pairs, none shared between chains",
+                    "FFMA2 + FMNMX on separate chains (per pair of instructions)", "FFMA2 + 2 FMNMX (per triple)",
+                    "FFMA + FMNMX (per pair)",
+                    "sweep mix: 16 FFMA2 + 4 MUFU + 5 FMNMX/FMNMX3 + 2 FSETP + 2 FSEL (per group of 29; reported per 8 'instructions' = x 0.5 groups)"]
 
 
 def run_scene(ctx: Context, scene, device="cuda:0", tuning=None, steps=None):

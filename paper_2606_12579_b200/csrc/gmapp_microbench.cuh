@@ -19,7 +19,11 @@ enum MicroKind {
     MB_FMNMX3 = 7,           // min.f32 (3 inputs)
     MB_FSETP_FSEL = 8,       // setp.gt.f32 + selp.f32 (two instructions per chain step: the reported cost is per PAIR)
     MB_FFMA2_3OP_NOREUSE = 9,// fma.rn.f32x2 X_i, X_i, Y_i, Z_i  three distinct register pairs, none shared between chains
-    MB_COUNT = 10
+    MB_FFMA2_FMNMX = 10,     // one FFMA2 + one FMNMX on separate chains (cost per PAIR): 2.03 if the ALU op co-issues, 3.06 if not
+    MB_FFMA2_2FMNMX = 11,    // one FFMA2 + two FMNMX (per triple)
+    MB_FFMA_FMNMX = 12,      // one scalar FFMA + one FMNMX (per pair)
+    MB_SWEEP_MIX = 13,       // the raw sweep's mix per agent-trip: 16 FFMA2, 4 MUFU, 5 FMNMX, 2 FSETP+FSEL (cost per group of 29)
+    MB_COUNT = 14
 };
 
 template <int KIND>
@@ -47,13 +51,51 @@ __global__ void __launch_bounds__(512) k_microbench(float* out, int iters, float
             if (KIND == MB_MUFU_RCP_PRED_OFF) asm volatile("{ .reg .pred p; setp.gt.f32 p, %0, %1; @p rcp.approx.ftz.f32 %0, %0; }" : "+f"(x[i]) : "f"(thr));
             if (KIND == MB_FMNMX) asm volatile("max.f32 %0, %0, %1;" : "+f"(x[i]) : "f"(a));
             if (KIND == MB_FMNMX3) asm volatile("min.f32 %0, %0, %1, %2;" : "+f"(x[i]) : "f"(a), "f"(b));
+            if (KIND == MB_FFMA2_FMNMX) {
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(X[i]) : "l"(A), "l"(B));
+                asm volatile("max.f32 %0, %0, %1;" : "+f"(x[i]) : "f"(a));
+            }
+            if (KIND == MB_FFMA2_2FMNMX) {
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(X[i]) : "l"(A), "l"(B));
+                asm volatile("max.f32 %0, %0, %1;" : "+f"(x[i]) : "f"(a));
+                asm volatile("min.f32 %0, %0, %1;" : "+f"(x[i]) : "f"(b));
+            }
+            if (KIND == MB_FFMA_FMNMX) {
+                float lo, hi;
+                asm volatile("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(X[i]));
+                asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(lo) : "f"(a), "f"(b));
+                asm volatile("mov.b64 %0, {%1, %2};" : "=l"(X[i]) : "f"(lo), "f"(hi));
+                asm volatile("max.f32 %0, %0, %1;" : "+f"(x[i]) : "f"(a));
+            }
+            if (KIND == MB_SWEEP_MIX && (i & 1) == 0) {      // 4 groups per round; chains: X[i], X[i+1] packed; x[i], x[i+1] scalar
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(X[i]) : "l"(A), "l"(B));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(X[i + 1]) : "l"(A), "l"(B));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(Y[i]) : "l"(A), "l"(B));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(Y[i + 1]) : "l"(A), "l"(B));
+                asm volatile("{ .reg .f32 t; rsqrt.approx.ftz.f32 t, %0; max.f32 %0, t, %1; }" : "+f"(x[i]) : "f"(a));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(Z[i]) : "l"(A), "l"(B));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(Z[i + 1]) : "l"(A), "l"(B));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(X[i]) : "l"(A), "l"(B));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(X[i + 1]) : "l"(A), "l"(B));
+                asm volatile("{ .reg .f32 t; rsqrt.approx.ftz.f32 t, %0; max.f32 %0, t, %1; }" : "+f"(x[i + 1]) : "f"(a));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(Y[i]) : "l"(A), "l"(B));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(Y[i + 1]) : "l"(A), "l"(B));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(Z[i]) : "l"(A), "l"(B));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(Z[i + 1]) : "l"(A), "l"(B));
+                asm volatile("{ .reg .f32 t; .reg .pred p; rcp.approx.ftz.f32 t, %0; min.f32 t, t, %1, %2; setp.gt.f32 p, t, %3; selp.f32 %0, %1, t, p; }" : "+f"(x[i]) : "f"(a), "f"(b), "f"(thr));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(X[i]) : "l"(A), "l"(B));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(X[i + 1]) : "l"(A), "l"(B));
+                asm volatile("{ .reg .f32 t; .reg .pred p; rcp.approx.ftz.f32 t, %0; max.f32 t, t, %1; setp.gt.f32 p, t, %3; selp.f32 %0, %2, t, p; }" : "+f"(x[i + 1]) : "f"(a), "f"(b), "f"(thr));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(Y[i]) : "l"(A), "l"(B));
+                asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(Y[i + 1]) : "l"(A), "l"(B));
+            }
             if (KIND == MB_FSETP_FSEL) asm volatile("{ .reg .pred p; setp.gt.f32 p, %0, %1; selp.f32 %0, %2, %0, p; }" : "+f"(x[i]) : "f"(thr), "f"(a));
         }
     }
     float s = 0.0f;
 #pragma unroll
     for (int i = 0; i < 8; ++i) { float lo, hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(X[i])); s += x[i] + lo + hi; }
-    if (KIND == MB_FFMA2_3OP_NOREUSE) {
+    if (KIND == MB_FFMA2_3OP_NOREUSE || KIND == MB_SWEEP_MIX) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) { float lo, hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(Y[i] ^ Z[i])); s += lo + hi; }
     }

@@ -138,6 +138,84 @@ struct X2Acc {
     }
 };
 
+// Stage-major sweep over U trips at once (circular field, static spheres, branch-free).  ptxas keeps unrolled trips
+// strictly one after another (it only interleaves what the SOURCE writes stage by stage, as the NA agents of a trip), and
+// a warp issues in order: with one trip at a time a warp has NA packed chains in flight and exposes the MUFU.RSQ -> FMA ->
+// MUFU.RCP -> FMA latency of every trip.  Written stage by stage over K = NA x U (agent, trip) slots, two trips' chains
+// overlap inside the warp.  Same arithmetic per pair, same order of accumulation per lane (trip u before trip u + 1).
+#ifndef GMAPP_X2_U
+#define GMAPP_X2_U 1
+#endif
+#ifndef GMAPP_X2_U_UNROLL
+#define GMAPP_X2_U_UNROLL 2
+#endif
+constexpr int kX2UUnroll = GMAPP_X2_U_UNROLL;
+template <int NA, int U, class RD, bool REFINE>
+__device__ __forceinline__ void sweep_x2_cf_u(const float4* __restrict__ tA, const float4* __restrict__ tB, int iters,
+                                              int j0, int L, const float (&p)[NA][3], const float (&v)[NA][3],
+                                              const RD& rd, float eps, X2Acc<NA>& acc) {
+    constexpr int K = NA * U;
+    const u64 tiny = bc2(kTiny), half = bc2(0.5f);
+#pragma unroll kX2UUnroll
+    for (int i = 0, j = j0; i < iters; ++i, j += U * L) {
+        u64 cx[U], cy[U], cz[U], nR[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const float4 s0 = tA[j + u * L], s1 = tB[j + u * L];
+            cx[u] = pk2(s0.x, s0.y); cy[u] = pk2(s0.z, s0.w); cz[u] = pk2(s1.x, s1.y); nR[u] = pk2(s1.z, s1.w);
+        }
+        u64 dx[K], dy[K], dz[K], q[K], y[K];
+        float d0[K], d1[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k) {                          // stage 1: d, |d|^2
+            const int a = k % NA, u = k / NA;
+            dx[k] = sub2(cx[u], bc2(p[a][0])); dy[k] = sub2(cy[u], bc2(p[a][1])); dz[k] = sub2(cz[u], bc2(p[a][2]));
+            q[k] = fma2(dx[k], dx[k], fma2(dy[k], dy[k], fma2(dz[k], dz[k], tiny)));
+        }
+#pragma unroll
+        for (int k = 0; k < K; ++k) {                          // stage 2: MUFU.RSQ
+            float q0, q1; upk2(q[k], q0, q1);
+            y[k] = pk2(rsqrt_approx(q0), rsqrt_approx(q1));
+        }
+#pragma unroll
+        for (int k = 0; k < K; ++k) {                          // stage 3: surface distance, clearance minimum
+            const int a = k % NA, u = k / NA;
+            u64 ds;
+            if (!REFINE) ds = fma2(q[k], y[k], nR[u]);
+            if (REFINE) {
+                const u64 t = mul2(q[k], y[k]);
+                ds = add2(t, nR[u]);
+                const u64 hy = mul2(y[k], half);
+                float t0, t1, q0, q1; upk2(t, t0, t1); upk2(q[k], q0, q1);
+                const u64 e = pk2(fmaf(-t0, t0, q0), fmaf(-t1, t1, q1));
+                ds = fma2(hy, e, ds);
+            }
+            upk2(ds, d0[k], d1[k]);
+            acc.dmin[a] = min3f(acc.dmin[a], d0[k], d1[k]);
+        }
+        u64 rr[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k) {                          // stage 4: gate, clamp, MUFU.RCP
+            const int a = k % NA;
+            const u64 den = mul2(pk2(fmaxf(d0[k], eps), fmaxf(d1[k], eps)), q[k]);
+            float n0, n1; upk2(den, n0, n1);
+            float r0 = 0.0f, r1 = 0.0f;
+            if (d0[k] <= rd.get(a)) r0 = rcp_approx(n0);
+            if (d1[k] <= rd.get(a)) r1 = rcp_approx(n1);
+            rr[k] = pk2(r0, r1);
+        }
+#pragma unroll
+        for (int k = 0; k < K; ++k) {                          // stage 5: s = d.v, w, accumulate
+            const int a = k % NA;
+            const u64 s = fma2(dx[k], bc2(v[a][0]), fma2(dy[k], bc2(v[a][1]), mul2(dz[k], bc2(v[a][2]))));
+            const u64 w = mul2(s, rr[k]);
+            acc.bx[a] = fma2(w, dx[k], acc.bx[a]);
+            acc.by[a] = fma2(w, dy[k], acc.by[a]);
+            acc.bz[a] = fma2(w, dz[k], acc.bz[a]);
+        }
+    }
+}
+
 // One lane's slice of the sphere sum: pairs lane, lane+L, ... ; FORCE=false is the distance-only final pass.
 // APF = true: Eq. 1 in the Khatib form on the clamped surface distance (reading N1),
 // f_j = -k_f (1/d_O - 1/r_d) / d_O^2 * d/|d|; the sums then hold the force itself (no velocity factor).
@@ -146,8 +224,14 @@ __device__ __forceinline__ void sweep_x2(const float4* __restrict__ tA, const fl
                                          int lane, int L, const float (&p)[NA][3], const float (&v)[NA][3],
                                          const RD& rd, float eps, unsigned mask, X2Acc<NA>& acc) {
     const u64 tiny = bc2(kTiny), half = bc2(0.5f);
+    int i_first = 0;
+    if (GMAPP_X2_U > 1 && FORCE && !CULL && !APF && !GMAPP_X2_PAIR_RCP) {     // U trips at once, stage by stage; the tail below
+        const int iters = trips / GMAPP_X2_U;
+        sweep_x2_cf_u<NA, GMAPP_X2_U, RD, REFINE>(tA, tB, iters, lane, L, p, v, rd, eps, acc);
+        i_first = iters * GMAPP_X2_U;
+    }
 #pragma unroll kX2Unroll
-    for (int i = 0, j = lane; i < trips; ++i, j += L) {
+    for (int i = i_first, j = lane + i_first * L; i < trips; ++i, j += L) {
         const float4 s0 = tA[j], s1 = tB[j];
         const u64 cx = pk2(s0.x, s0.y), cy = pk2(s0.z, s0.w), cz = pk2(s1.x, s1.y), nR = pk2(s1.z, s1.w);
         u64 dx[NA], dy[NA], dz[NA], q[NA], yy[NA];
