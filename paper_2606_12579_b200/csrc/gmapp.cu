@@ -565,7 +565,7 @@ static gmapp_status choose_launch(gmapp_ctx* c, int kind, int n_agents, LaunchCf
 // ---------------------------------------------------------------------------------------------
 // packed f32x2 rollout (POINT3, static or moving spheres): launch selection + launch
 // ---------------------------------------------------------------------------------------------
-struct X2Plan { int A, grid, at, G, L, mode, n2p, cull, stage, ring_tp, xch_off, rec_off, tile_off, pair_bytes, block, smem; size_t tile_bytes; };
+struct X2Plan { int Lk, A, grid, at, G, L, mode, n2p, cull, stage, ring_tp, xch_off, rec_off, tile_off, pair_bytes, block, smem; size_t tile_bytes; };
 
 // launch selection alone (no CUDA call): every reason to refuse a launch shape is found here, before anything is enqueued
 static gmapp_status plan_rollout_x2(gmapp_ctx* c, int n_agents, X2Plan* o) {
@@ -602,14 +602,22 @@ static gmapp_status plan_rollout_x2(gmapp_ctx* c, int n_agents, X2Plan* o) {
         if (L > cap) L = cap;                                     // reduction beats the sub-warp one even with idle lanes
         if (L > 32 && G > 7) L = 32;                              // two named barriers per multi-warp group
     }
+    // 5 to 7 two-agent groups per CTA: mixed group widths -- 16 sweep warps, the first 2 G - 8 groups 64 lanes wide, the others
+    // 128, one epilogue warp per two groups (gmapp_rollout_x2.cuh, group_epilogue_warp2); needs at least 128 sphere pairs
+    if (!chunked && at == 2 && L >= 64 && G >= 5 && G <= 7 && pow2_ceil(n2 > 0 ? n2 : 1) < 128) L = 32;
     const int mode = chunked ? 4 : (L >= 64 ? (G <= 4 ? 2 : 3) : (L == 32 ? 1 : 0));
-    const int n2p = n2 > 0 ? round_up(n2, L) : 0;
+    const bool mixed = mode == 3 && at == 2;
+    if (mixed && L != 64) return fail(c, GMAPP_EINVAL, "rollout: 5 to 7 two-agent groups per CTA take lanes_per_agent = 64 (mixed 64 / 128), got %s%ld", "", L);
+    const int Lk = mixed ? 128 : L;                               // what the kernel pads the pair arrays to (P.L)
+    const int n2p = n2 > 0 ? round_up(n2, Lk) : 0;
     const int cull = (t && t->cull >= 0) ? t->cull : 0;
     // dynamic shared memory: [0,64) mbarriers; then the exchange area of the multi-warp groups (per group: the
     // per-lane partials of two agents + the published states = (2 L + 8) float4) or, mode 4, the 24-word state
     // record of every agent; then the sphere-pair tile
     const int xch_off = 64, rec_off = 128;
-    const int tile_off = rec_off + (chunked ? round_up(A * 24 * 4, 128) : (mode >= 2 ? round_up(G * (2 * L + 8) * 16, 128) : 0));
+    const int tile_off = rec_off + (chunked ? round_up(A * 24 * 4, 128)
+                                            : mixed ? round_up(((2 * G - 8) * 136 + (8 - G) * 264) * 16, 128)
+                                            : (mode >= 2 ? round_up(G * (2 * L + 8) * 16, 128) : 0));
     const int pair_bytes = c->moving ? 64 : 32;                          // pair arrays A, B (+ U, V when the spheres move)
     const size_t tile_bytes = (size_t)n2p * pair_bytes;
     const bool fits = tile_off + tile_bytes <= (size_t)c->smem_optin;
@@ -620,7 +628,7 @@ static gmapp_status plan_rollout_x2(gmapp_ctx* c, int n_agents, X2Plan* o) {
     if (ring_ok) {
         ring_tp = pow2_floor((int)(((size_t)c->smem_optin - tile_off) / ((size_t)kRingStages * pair_bytes)));
         if (ring_tp > 2048) ring_tp = 2048;
-        if (ring_tp < L) ring_tp = 0;                                    // a tile must hold a whole trip of the group
+        if (ring_tp < Lk) ring_tp = 0;                                   // a tile must hold a whole trip of the group
     }
     // Measured on B200 at equal sphere density (profiles/r02_tile_ring.md): the ring beats the L1/L2 path by 3-5 % once the set is
     // far beyond L1 (>= 8 tiles, i.e. 32768 static spheres) for one-warp groups and chunked warps; at 4 tiles the two are level, and
@@ -637,9 +645,9 @@ static gmapp_status plan_rollout_x2(gmapp_ctx* c, int n_agents, X2Plan* o) {
     o->A = A; o->grid = grid; o->at = at; o->G = G; o->L = L; o->mode = mode; o->n2p = n2p; o->cull = cull; o->stage = stage;
     o->ring_tp = ring_tp; o->xch_off = xch_off; o->rec_off = rec_off; o->tile_off = tile_off; o->pair_bytes = pair_bytes;
     o->tile_bytes = tile_bytes;
-    // mode 3 with two agents per group: one epilogue warp per TWO groups (kernel table: MAXT 576)
-    if (mode == 3 && at == 2 && L != 64) return fail(c, GMAPP_EINVAL, "rollout: 5 to 7 two-agent groups per CTA need lanes_per_agent = 64, got %s%ld", "", L);
-    o->block = mode == 4 ? tmax : (mode == 3 && at == 2 ? G * L + 32 * ((G + 1) / 2) : (mode >= 2 ? G * L + 32 * G : round_up(G * L, 32)));
+    // mixed widths: 16 sweep warps + one epilogue warp per TWO groups (kernel table: MAXT 576 is the tag of that variant)
+    o->block = mode == 4 ? tmax : (mixed ? 32 * (16 + (G + 1) / 2) : (mode >= 2 ? G * L + 32 * G : round_up(G * L, 32)));
+    o->Lk = Lk;
     o->smem = tile_off + (stage == 1 ? (int)tile_bytes : (stage == 2 ? kRingStages * ring_tp * pair_bytes : 0));
     return GMAPP_OK;
 }
@@ -663,7 +671,7 @@ static gmapp_status launch_rollout_x2(gmapp_ctx* c, const float* d_agents, float
     P.pairA = c->d_pairA; P.pairB = c->d_pairB; P.n2p = n2p;
     P.agents_in = d_agents; P.agents_out = d_agents_out;
     P.n_agents = n_agents; P.agents_per_cta = A;
-    P.L = L; P.logL = ilog2(L);
+    P.L = pl.Lk; P.logL = ilog2(pl.Lk);
     P.steps = steps;
     for (int i = 0; i < 3; ++i) P.goal[i] = goal[i];
     P.dt = dt; P.t0 = c->roll_t0;

@@ -940,15 +940,17 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, Sp
 // ---------------------------------------------------------------------------------------------
 template <bool RING, int NA, bool CULL, bool APF, bool PER, bool MV, bool ONE>
 __device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, SphSrc& S,
-                                                    int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
+                                                    int first_agent, int lane_in_group, int group_in_cta, float4* xch,
+                                                    int gL = 0, int glogL = 0) {
+    const int L = gL ? gL : P.L, logL = gL ? glogL : P.logL;      // gL > 0: the group's own width (mixed widths in one CTA)
     const int n2p = S.n2p;
     // n2p is a multiple of L: the same trip count on every lane.  ONE: a single trip (as many lanes as sphere pairs,
     // the latency-bound shapes): known at compile time, so the sweep is straight-line code without loop control
-    const int trips = ONE ? 1 : (n2p >> P.logL);
+    const int trips = ONE ? 1 : (n2p >> logL);
     const unsigned full = 0xffffffffu;
     float4* part = xch;                                    // [NA][L]
-    const float4* state = xch + 2 * P.L;                   // [2][NA][2]
-    const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = P.L + 32;
+    const float4* state = xch + 2 * L;                   // [2][NA][2]
+    const int bar_part = 1 + 2 * group_in_cta, bar_state = 2 + 2 * group_in_cta, nbar = L + 32;
     float p[NA][3], v[NA][3];
     RdSel<NA, PER> rd; rd.u = P.r_d;
 #pragma unroll
@@ -960,18 +962,18 @@ __device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, Sp
         for (int i = 0; i < 3; ++i) { p[a][i] = s[i]; v[a][i] = s[3 + i]; }
     }
     X2Acc<NA> acc;
-    const float thr = lane_near_thr<APF>(RING ? P.pairB : S.tB, trips, lane_in_group, P.L);
+    const float thr = lane_near_thr<APF>(RING ? P.pairB : S.tB, trips, lane_in_group, L);
     bool hot = RING;
     for (int k = 0; k <= P.steps; ++k) {
         const bool last = (k == P.steps);
         const float tk = fmaf(float(k), P.dt, P.t0);
         acc.clear();
-        if (!last) sweep_src<RING, NA, true, CULL, APF, MV>(P, S, trips, lane_in_group, P.L, P.logL, tk, p, v, rd, P.eps, full, thr, hot, acc);
-        else       sweep_src<RING, NA, false, false, false, MV>(P, S, trips, lane_in_group, P.L, P.logL, tk, p, v, rd, P.eps, full, thr, hot, acc);
+        if (!last) sweep_src<RING, NA, true, CULL, APF, MV>(P, S, trips, lane_in_group, L, logL, tk, p, v, rd, P.eps, full, thr, hot, acc);
+        else       sweep_src<RING, NA, false, false, false, MV>(P, S, trips, lane_in_group, L, logL, tk, p, v, rd, P.eps, full, thr, hot, acc);
 #pragma unroll
         for (int a = 0; a < NA; ++a) {                     // per-lane partials; the epilogue warp reduces them
             constexpr bool SC = acc_scaled<APF, MV>();
-            part[a * P.L + lane_in_group] = make_float4(acc_fold<SC>(acc.bx[a]), acc_fold<SC>(acc.by[a]), acc_fold<SC>(acc.bz[a]), acc.dmin[a]);
+            part[a * L + lane_in_group] = make_float4(acc_fold<SC>(acc.bx[a]), acc_fold<SC>(acc.by[a]), acc_fold<SC>(acc.bz[a]), acc.dmin[a]);
         }
         const int par = k & 1;
         named_bar_arrive(bar_part, nbar);
@@ -988,9 +990,10 @@ __device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, Sp
 
 template <bool RING, int NA, bool CULL, bool APF, bool PER, bool MV>
 __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, SphSrc& S,
-                                                  int first_agent, int lane_in_group, int group_in_cta, float4* xch) {
-    if (!RING && (S.n2p >> P.logL) == 1) group_sweep_warps_n<false, NA, CULL, APF, PER, MV, true>(P, S, first_agent, lane_in_group, group_in_cta, xch);
-    else group_sweep_warps_n<RING, NA, CULL, APF, PER, MV, false>(P, S, first_agent, lane_in_group, group_in_cta, xch);
+                                                  int first_agent, int lane_in_group, int group_in_cta, float4* xch,
+                                                  int gL = 0, int glogL = 0) {
+    if (!RING && (S.n2p >> (gL ? glogL : P.logL)) == 1) group_sweep_warps_n<false, NA, CULL, APF, PER, MV, true>(P, S, first_agent, lane_in_group, group_in_cta, xch, gL, glogL);
+    else group_sweep_warps_n<RING, NA, CULL, APF, PER, MV, false>(P, S, first_agent, lane_in_group, group_in_cta, xch, gL, glogL);
 }
 
 template <int NA, bool APF, bool XT, int NW>   // APF here = "the sums are the force itself" (APF heuristic or moving spheres)
@@ -1035,34 +1038,41 @@ __device__ __forceinline__ void group_epilogue_warp(const RolloutX2Params& P, in
 }
 
 // ---------------------------------------------------------------------------------------------
-// One epilogue warp serving TWO groups (5 to 7 groups per CTA: 9 to 14 agents).  With an epilogue warp per group such a
-// CTA has 21 warps, which puts 6 warps on one SM sub-partition and cuts the register budget from 96 to 80 (2048 agents
-// x 4096 spheres: 0.54 of peak); shared, it has 18 warps and keeps 96+.  The warp serves its groups in a fixed order each
-// step; the second group's hand-over waits for the first one's (~0.3 us against a sweep of several us).
+// 5 to 7 groups per CTA (9 to 14 agents): MIXED GROUP WIDTHS and one epilogue warp serving TWO groups.
+// With G groups of two sweep warps each the four schedulers of the SM carry unequal numbers of sweep warps (2048 agents: 14
+// warps, 4 : 4 : 3 : 3) and an epilogue warp per group makes 21 warps, which cuts the register budget from 96 to 80.  Instead
+// the CTA always has 16 sweep warps: the first y = 2 G - 8 groups are 2 warps wide (L = 64), the other 8 - G groups 4 warps
+// (L = 128).  y is even and the 2-wide groups come first, so every run of four consecutive warps holds two 2-wide groups or
+// one 4-wide group and every scheduler carries the same number of agent-sweeps per step; a one-agent group (odd agent
+// count) is the last group and therefore 4 wide.  ceil(G / 2) shared epilogue warps: 19 or 20 warps, 96 registers.  An
+// epilogue warp serves its groups in a fixed order each step; the second group's hand-over waits for the first one's
+// (~0.3 us against a sweep of several us).
 // NA1 = 0: the warp's second group does not exist (odd group count, or the CTA's agents end before it).
 // ---------------------------------------------------------------------------------------------
 template <int NA>
 struct EpiSide {
     AgentX2 me;
     const float4* part; float4* state;
-    int bar_part, bar_state, half;
-    __device__ __forceinline__ void init(const RolloutX2Params& P, int first_agent, int lane, int group_in_cta, float4* xch) {
+    int bar_part, bar_state, half, L;
+    __device__ __forceinline__ void init(const RolloutX2Params& P, int first_agent, int lane, int group_in_cta, float4* xch, int L_) {
         half = (NA == 2) ? (lane >> 4) : 0;
-        part = xch; state = xch + 2 * P.L;
+        L = L_;                                             // this group's width: 64 or 128 lanes
+        part = xch; state = xch + 2 * L;
         bar_part = 1 + 2 * group_in_cta; bar_state = 2 + 2 * group_in_cta;
         me.init(P, first_agent + half);
     }
     // one step of this group: returns false after the final pose
-    template <bool APF, bool XT, int LW>                    // LW = sweep warps per group (L / 32)
+    template <bool APF, bool XT>
     __device__ __forceinline__ void step(const RolloutX2Params& P, int k, int lane, float& dmin, float& fx, float& fy, float& fz) {
-        constexpr int NP = NA == 2 ? 2 * LW : LW;           // partials per epilogue lane
-        constexpr int NW = (NP == 2 || NP == 4 || NP == 8) ? NP : 0;
         const bool last = (k == P.steps);
-        const int par = k & 1, nbar = P.L + 32;
+        const int par = k & 1, nbar = L + 32;
         const bool writer = (lane & 15) == 0 && (NA == 2 || lane == 0);
         me.pre(P);
         named_bar_sync(bar_part, nbar);
-        const float4 t = group_reduce<NA, NW>(part, P.L, lane);
+        // partials per epilogue lane: L / 16 (two agents) or L / 32; the group is 2 or 4 sweep warps wide (a uniform branch)
+        float4 t;
+        if (L == 64) t = group_reduce<NA, (NA == 2 ? 4 : 2)>(part, 64, lane);
+        else         t = group_reduce<NA, (NA == 2 ? 8 : 4)>(part, 128, lane);
         dmin = t.w;
         if (last) { if (writer) me.finish(P, t.w); return; }
         me.template post<APF>(P, t.x, t.y, t.z, fx, fy, fz);
@@ -1074,16 +1084,17 @@ struct EpiSide {
     }
 };
 
-template <int NA0, int NA1, bool APF, bool XT, int LW>
-__device__ __forceinline__ void group_epilogue_warp2_n(const RolloutX2Params& P, int first0, int first1, int lane, int g0, float4* xch0, float4* xch1) {
+template <int NA0, int NA1, bool APF, bool XT>
+__device__ __forceinline__ void group_epilogue_warp2_n(const RolloutX2Params& P, int first0, int first1, int lane, int g0,
+                                                       float4* xch0, float4* xch1, int L0, int L1) {
     EpiSide<NA0> s0;
     EpiSide<(NA1 > 0 ? NA1 : 1)> s1;
-    s0.init(P, first0, lane, g0, xch0);
-    if (NA1 > 0) s1.init(P, first1, lane, g0 + 1, xch1);
+    s0.init(P, first0, lane, g0, xch0, L0);
+    if (NA1 > 0) s1.init(P, first1, lane, g0 + 1, xch1, L1);
     for (int k = 0; k <= P.steps; ++k) {
         float d0, d1 = 0.0f, f0x, f0y, f0z, f1x, f1y, f1z;
-        s0.template step<APF, XT, LW>(P, k, lane, d0, f0x, f0y, f0z);
-        if (NA1 > 0) s1.template step<APF, XT, LW>(P, k, lane, d1, f1x, f1y, f1z);
+        s0.template step<APF, XT>(P, k, lane, d0, f0x, f0y, f0z);
+        if (NA1 > 0) s1.template step<APF, XT>(P, k, lane, d1, f1x, f1y, f1z);
         if (k == P.steps) return;
         s0.me.costs(P, k, d0, f0x, f0y, f0z);              // off the critical path: both groups' sweep warps are running
         if ((lane & 15) == 0 && (NA0 == 2 || lane == 0)) { if (XT) s0.me.snapshot(P, k); }
@@ -1097,13 +1108,12 @@ __device__ __forceinline__ void group_epilogue_warp2_n(const RolloutX2Params& P,
 // na0, na1: agents of the warp's two groups (na0 in {1, 2}; na1 in {0, 1, 2}, and na1 > 0 only if na0 == 2)
 template <bool APF, bool XT>
 __device__ __forceinline__ void group_epilogue_warp2(const RolloutX2Params& P, int first0, int na0, int na1, int lane, int g0,
-                                                     float4* xch0, float4* xch1) {
+                                                     float4* xch0, float4* xch1, int L0, int L1) {
     const int first1 = first0 + 2;
-    // 5 to 7 groups of two sweep warps each (L = 64; the host selects this shape only then)
-    if (na0 >= 2 && na1 >= 2) group_epilogue_warp2_n<2, 2, APF, XT, 2>(P, first0, first1, lane, g0, xch0, xch1);
-    else if (na0 >= 2 && na1 == 1) group_epilogue_warp2_n<2, 1, APF, XT, 2>(P, first0, first1, lane, g0, xch0, xch1);
-    else if (na0 >= 2) group_epilogue_warp2_n<2, 0, APF, XT, 2>(P, first0, first1, lane, g0, xch0, xch1);
-    else group_epilogue_warp2_n<1, 0, APF, XT, 2>(P, first0, first1, lane, g0, xch0, xch1);
+    if (na0 >= 2 && na1 >= 2) group_epilogue_warp2_n<2, 2, APF, XT>(P, first0, first1, lane, g0, xch0, xch1, L0, L1);
+    else if (na0 >= 2 && na1 == 1) group_epilogue_warp2_n<2, 1, APF, XT>(P, first0, first1, lane, g0, xch0, xch1, L0, L1);
+    else if (na0 >= 2) group_epilogue_warp2_n<2, 0, APF, XT>(P, first0, first1, lane, g0, xch0, xch1, L0, L1);
+    else group_epilogue_warp2_n<1, 0, APF, XT>(P, first0, first1, lane, g0, xch0, xch1, L0, L1);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1164,7 +1174,7 @@ __device__ __forceinline__ void group_rollout_narrow(const RolloutX2Params& P, c
 // XT = extras: the state snapshot of gmapp_replan and the trajectory output (kept out of the plain kernels: the few
 // extra stores in the epilogue perturb the register allocation of the sweep warps by 3 %)
 template <int AT, int MODE, bool CULL, int STAGE, int MAXT, bool APF, bool XT, bool MV>
-__global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ RolloutX2Params P) {
+__global__ void __launch_bounds__(MAXT == 576 ? 640 : MAXT, 1) k_rollout_x2(const __grid_constant__ RolloutX2Params P) {   // (MAXT 576 = tag of the mixed-width variant: 19 or 20 warps)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw);
     constexpr bool RING = (STAGE == 2);
@@ -1206,7 +1216,11 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         // consumer warps of this CTA (warps that return at once because they have no agent do not count)
         const int n_sweep_threads = int(blockDim.x);
         int consumers;
-        if (MODE == 2) {
+        if (MODE == 2 && AT == 2 && MAXT == 576) {          // mixed group widths: the sweep warps of the groups that have agents
+            const int G = (P.agents_per_cta + 1) / 2, y = 2 * G - 8, ga = (n_cta + 1) / 2;
+            consumers = 0;
+            for (int g = 0; g < G && g < ga; ++g) consumers += g < y ? 2 : 4;
+        } else if (MODE == 2) {
             const int G = (P.agents_per_cta + AT - 1) / AT, ga = (n_cta + AT - 1) / AT;
             consumers = (ga < G ? ga : G) * (P.L >> 5);
         } else if (MODE == 4) {
@@ -1240,24 +1254,47 @@ __global__ void __launch_bounds__(MAXT, 1) k_rollout_x2(const __grid_constant__ 
         S.pos.slot = 0; S.pos.parity = 0u; S.pos.t = S.pos.v = 0; S.umax_dt = 0.0f;
     }
     constexpr int NA2 = (AT == 2) ? 2 : 1;
-    if (MODE == 2) {
-        constexpr bool EPI2 = (AT == 2 && MAXT == 576);     // one epilogue warp per TWO groups (5-7 groups of L = 64)
-        const int G = (P.agents_per_cta + AT - 1) / AT;
-        const int n_sweep = G * P.L;
-        const bool is_epi = tid >= n_sweep;
-        const int group_in_cta = is_epi ? ((tid - n_sweep) >> 5) * (EPI2 ? 2 : 1) : (tid >> P.logL);
-        const int first = cta_first + group_in_cta * AT;
-        const int na = cta_end - first;
-        float4* xch = reinterpret_cast<float4*>(smem_raw + P.xch_off) + group_in_cta * (2 * P.L + 8);
-        if (is_epi && EPI2) {
-            if (na <= 0) return;
-            int na1 = (group_in_cta + 1 < G) ? na - 2 : 0;
+    if (MODE == 2 && AT == 2 && MAXT == 576) {
+        // mixed group widths (see group_epilogue_warp2): 16 sweep warps, groups [0, y) 2 warps wide, [y, G) 4 warps wide
+        const int G = (P.agents_per_cta + 1) / 2, y = 2 * G - 8, w = tid >> 5;
+        const bool is_epi = w >= 16;
+        float4* xbase = reinterpret_cast<float4*>(smem_raw + P.xch_off);
+        // group g: lanes, first sweep warp, exchange area (2 L + 8 float4 per group)
+        #define GMAPP_MIX_L(g) ((g) < y ? 64 : 128)
+        #define GMAPP_MIX_W0(g) ((g) < y ? 2 * (g) : 2 * y + 4 * ((g) - y))
+        #define GMAPP_MIX_X(g) (xbase + ((g) < y ? (g) * 136 : y * 136 + ((g) - y) * 264))
+        if (is_epi) {
+            const int g0 = 2 * (w - 16), first = cta_first + 2 * g0, na = cta_end - first;
+            if (g0 >= G || na <= 0) return;
+            int na1 = (g0 + 1 < G) ? na - 2 : 0;
             if (na1 > 2) na1 = 2;
             if (na1 < 0) na1 = 0;
-            group_epilogue_warp2<(APF || MV), XT>(P, first, na, na1, tid & 31, group_in_cta, xch, xch + (2 * P.L + 8));
+            group_epilogue_warp2<(APF || MV), XT>(P, first, na, na1, tid & 31, g0, GMAPP_MIX_X(g0), GMAPP_MIX_X(g0 + 1),
+                                                  GMAPP_MIX_L(g0), GMAPP_MIX_L(g0 + 1));
             select_tail<GMAPP_FUSED_SELECT_X2 != 0>(P.sel, P.cost, P.collided, (na >= 2 ? 2 : 1) + na1, tid & 31);
             return;
         }
+        const int g = w < 2 * y ? (w >> 1) : y + ((w - 2 * y) >> 2);
+        const int first = cta_first + 2 * g, na = cta_end - first;
+        if (STAGE == 1 && n2p > 0) mbar_wait(bar, 0);
+        if (g >= G || na <= 0) return;
+        const int gL = GMAPP_MIX_L(g), glogL = g < y ? 6 : 7, lane_in_group = tid - 32 * GMAPP_MIX_W0(g);
+        float4* xch = GMAPP_MIX_X(g);
+        if (na >= 2) { if (P.rd_arr) group_sweep_warps<RING, 2, CULL, APF, true, MV>(P, S, first, lane_in_group, g, xch, gL, glogL); else group_sweep_warps<RING, 2, CULL, APF, false, MV>(P, S, first, lane_in_group, g, xch, gL, glogL); }
+        else { if (P.rd_arr) group_sweep_warps<RING, 1, CULL, APF, true, MV>(P, S, first, lane_in_group, g, xch, gL, glogL); else group_sweep_warps<RING, 1, CULL, APF, false, MV>(P, S, first, lane_in_group, g, xch, gL, glogL); }
+        return;
+        #undef GMAPP_MIX_L
+        #undef GMAPP_MIX_W0
+        #undef GMAPP_MIX_X
+    }
+    if (MODE == 2) {
+        const int G = (P.agents_per_cta + AT - 1) / AT;
+        const int n_sweep = G * P.L;
+        const bool is_epi = tid >= n_sweep;
+        const int group_in_cta = is_epi ? ((tid - n_sweep) >> 5) : (tid >> P.logL);
+        const int first = cta_first + group_in_cta * AT;
+        const int na = cta_end - first;
+        float4* xch = reinterpret_cast<float4*>(smem_raw + P.xch_off) + group_in_cta * (2 * P.L + 8);
         if (is_epi) {                                      // the epilogue warps never touch the sphere tile
             if (na <= 0) return;
             if (AT == 2 && na >= 2) group_epilogue_warp<NA2, (APF || MV), XT>(P, first, tid & 31, group_in_cta, xch);

@@ -20,7 +20,8 @@ rollout_x2_fn rollout_x2_kernel_apf_x_mv(int at, int mode, bool cull, int stage)
 // One table per translation unit: (agents per group, mode, cull, stage) -> kernel.  stage 2 (TMA tile ring) exists in the
 // branch-free form only (cull is an explicit tuning knob; with it, sets beyond shared memory are read through L2).
 // mode 2 proper holds <= 4 groups (20 warps = 5 per SM sub-partition, 96 registers), which is what one wave of config 3 needs.
-// mode 3 = 5 to 7 groups: with two agents per group (MAXT 576) one epilogue warp serves two groups (18 warps, 96+ registers);
+// mode 3 = 5 to 7 groups: with two agents per group (tag MAXT 576) mixed group widths, 16 sweep warps and one epilogue warp per two
+// groups (19 or 20 warps, 96 registers);
 // with one agent per group (a tuning-only shape) the mode-2 code compiled for 21 warps (80 registers).
 #define GMAPP_X2_PICK(A, M, MT, F, X, V)                                                                                     \
     (stage == 2 ? (rollout_x2_fn)k_rollout_x2<A, M, false, 2, MT, F, X, V>                                                  \
