@@ -511,8 +511,9 @@ def run_ours(args):
         vox = {"points": int(pts.shape[0]), "ms": vms, "GB_per_s": pts.nbytes / (vms * 1e-3) / 1e9,
                "frac_of_hbm": pts.nbytes / (vms * 1e-3) / 1e9 / hbm, "hbm_peak_GB_per_s": hbm, "hbm_peak_how": hbm_how,
                "algorithmic_bytes": int(pts.nbytes),
-               "note": "2 launches: mark the voxel bitmap (12 B read per point), then one kernel that scans, emits the spheres in "
-                       "both layouts, writes the sentinel tail and the count and re-zeroes the bitmap; bit-exact vs oracle/voxel.py"}
+               "note": "ONE launch (k_vox_build_small: per-block voxel bitmaps in shared memory, 12 B read per point; the block that "
+                       "finishes last scans the merged bitmap and emits the spheres in both layouts, the sentinel tail and the count); "
+                       "grids beyond 262144 voxels: mark + compact, 2 launches; bit-exact vs oracle/voxel.py"}
         vctx.close()
 
     # ---- end to end through the C ABI with HOST buffers (sphere + agent upload, 8-byte result download)
