@@ -754,6 +754,32 @@ def test_pose6_launch_variants_match_oracle(api, ctx, orc, tuning):
         ctx.set_tuning(reset=True)
 
 
+# mixed group widths (9 to 14 agents per CTA: 16 sweep warps, 2 G - 8 groups of 64 lanes and 8 - G of 128, an epilogue warp per two
+# groups): every group count, odd agent counts (a one-agent last group), a ragged last CTA, static / moving spheres, APF
+@pytest.mark.parametrize("n_agents,max_ctas", [(9, 1), (10, 1), (11, 1), (12, 1), (13, 1), (14, 1), (25, 2), (23, 2), (40, 3)])
+def test_mixed_group_widths_match_oracle(api, ctx, orc, n_agents, max_ctas):
+    A = -(-n_agents // max_ctas); G = (A + 1) // 2
+    assert 5 <= G <= 7
+    try:
+        for moving, apf in ((False, False), (True, False), (False, True)):
+            sc = scenes.fast_clutter(n_agents=n_agents, n_spheres=333, moving=moving, steps=60)
+            if apf:
+                sc = _apf(sc)
+            g, _ = _check_rollout(api, ctx, orc, sc, tuning=dict(max_ctas=max_ctas))
+            assert g["info"]["block"] == 32 * (16 + (G + 1) // 2) and g["info"]["lanes_per_agent"] == 64 and g["info"]["packed_x2"] == 1
+        # positions at every step (the hand-over of every group and step), against the oracle's trajectory
+        import torch
+        sc = scenes.fast_clutter(n_agents=n_agents, n_spheres=333, steps=40)
+        traj = torch.zeros((n_agents, sc.steps + 1, 6), device="cuda:0")
+        ctx.set_trajectory_output(traj)
+        api.run_scene(ctx, sc, tuning=dict(max_ctas=max_ctas))
+        o = orc.rollout_scene(sc, threads=4, want_traj=True)
+        assert np.abs(traj.cpu().numpy()[:, :, :3].astype(np.float64) - o["traj"][:, :, :3]).max() <= 2e-5
+    finally:
+        ctx.set_trajectory_output(None)
+        ctx.set_tuning(reset=True)
+
+
 def test_moving_sphere_sets_beyond_shared_memory(api, ctx, orc):
     """9000 moving spheres = 4500 pairs x 64 B = 288 KB: the four pair arrays do not fit shared memory.  By default the
     packed kernels (point agents) and the wide kernel (6D) read them through L1 / L2 (stage 0: few tiles); forced to the
