@@ -146,6 +146,12 @@ struct X2Acc {
 #ifndef GMAPP_X2_U
 #define GMAPP_X2_U 1
 #endif
+// Group widths as compile-time constants where the common shapes have them (128 lanes: config 3 and the 1024-agent sweep rows;
+// 64 / 128 in the mixed-width mode): the unrolled trips then address the tile with immediate offsets instead of one LEA per
+// array and trip -- 0.75 issue cycles of 44 per agent-trip (config 3: 0.3130 -> 0.3060 ms).
+#ifndef GMAPP_X2_L128
+#define GMAPP_X2_L128 1
+#endif
 #ifndef GMAPP_X2_U_UNROLL
 #define GMAPP_X2_U_UNROLL 2
 #endif
@@ -938,11 +944,13 @@ __device__ __forceinline__ void warp_rollout_chunks(const RolloutX2Params& P, Sp
 //   sweep warp k:    write part -> arrive(bar_part) -> sync(bar_state) -> read state[k&1]
 //   epilogue warp k: sync(bar_part) -> reduce part -> integrate -> write state[k&1] -> arrive(bar_state) -> costs
 // ---------------------------------------------------------------------------------------------
-template <bool RING, int NA, bool CULL, bool APF, bool PER, bool MV, bool ONE>
+template <bool RING, int NA, bool CULL, bool APF, bool PER, bool MV, bool ONE, int LC = 0>
 __device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, SphSrc& S,
                                                     int first_agent, int lane_in_group, int group_in_cta, float4* xch,
                                                     int gL = 0, int glogL = 0) {
-    const int L = gL ? gL : P.L, logL = gL ? glogL : P.logL;      // gL > 0: the group's own width (mixed widths in one CTA)
+    // LC > 0: the width as a compile-time constant (the unrolled trips then address the tile with immediate offsets);
+    // gL > 0: the group's own width (mixed widths in one CTA); else the launch's uniform P.L
+    const int L = LC ? LC : (gL ? gL : P.L), logL = LC ? (LC == 128 ? 7 : 6) : (gL ? glogL : P.logL);
     const int n2p = S.n2p;
     // n2p is a multiple of L: the same trip count on every lane.  ONE: a single trip (as many lanes as sphere pairs,
     // the latency-bound shapes): known at compile time, so the sweep is straight-line code without loop control
@@ -988,11 +996,16 @@ __device__ __forceinline__ void group_sweep_warps_n(const RolloutX2Params& P, Sp
     }
 }
 
-template <bool RING, int NA, bool CULL, bool APF, bool PER, bool MV>
+template <bool RING, int NA, bool CULL, bool APF, bool PER, bool MV, int LC = 0>
 __device__ __forceinline__ void group_sweep_warps(const RolloutX2Params& P, SphSrc& S,
                                                   int first_agent, int lane_in_group, int group_in_cta, float4* xch,
                                                   int gL = 0, int glogL = 0) {
+    if (GMAPP_X2_L128 && LC > 0 && !RING) {                 // mixed-width mode: the group's width is known at compile time
+        group_sweep_warps_n<false, NA, CULL, APF, PER, MV, false, LC>(P, S, first_agent, lane_in_group, group_in_cta, xch);
+        return;
+    }
     if (!RING && (S.n2p >> (gL ? glogL : P.logL)) == 1) group_sweep_warps_n<false, NA, CULL, APF, PER, MV, true>(P, S, first_agent, lane_in_group, group_in_cta, xch, gL, glogL);
+    else if (GMAPP_X2_L128 && !RING && !gL && P.L == 128) group_sweep_warps_n<false, NA, CULL, APF, PER, MV, false, 128>(P, S, first_agent, lane_in_group, group_in_cta, xch);
     else group_sweep_warps_n<RING, NA, CULL, APF, PER, MV, false>(P, S, first_agent, lane_in_group, group_in_cta, xch, gL, glogL);
 }
 
@@ -1280,7 +1293,17 @@ __global__ void __launch_bounds__(MAXT == 576 ? 640 : MAXT, 1) k_rollout_x2(cons
         if (g >= G || na <= 0) return;
         const int gL = GMAPP_MIX_L(g), glogL = g < y ? 6 : 7, lane_in_group = tid - 32 * GMAPP_MIX_W0(g);
         float4* xch = GMAPP_MIX_X(g);
-        if (na >= 2) { if (P.rd_arr) group_sweep_warps<RING, 2, CULL, APF, true, MV>(P, S, first, lane_in_group, g, xch, gL, glogL); else group_sweep_warps<RING, 2, CULL, APF, false, MV>(P, S, first, lane_in_group, g, xch, gL, glogL); }
+        // Compile-time widths (64 / 128) for the two-agent groups -- unless this CTA also has a one-agent group next to 128-wide
+        // two-agent groups: three different sweep bodies running on one SM measured 10 % slower than two (1500 agents, 11 per
+        // CTA: 1.146 -> 1.270 ms), so such a CTA keeps the run-time width for all its groups.  (The per-agent-radius variant and
+        // the one-agent group always use the run-time width: fewer instantiations.)
+        const int ga = (n_cta + 1) >> 1;
+        const bool lc_ok = !((n_cta & 1) && ga - 1 > y);
+        if (na >= 2) {
+            if (P.rd_arr || !lc_ok) { if (P.rd_arr) group_sweep_warps<RING, 2, CULL, APF, true, MV>(P, S, first, lane_in_group, g, xch, gL, glogL); else group_sweep_warps<RING, 2, CULL, APF, false, MV>(P, S, first, lane_in_group, g, xch, gL, glogL); }
+            else if (g < y) group_sweep_warps<RING, 2, CULL, APF, false, MV, 64>(P, S, first, lane_in_group, g, xch, gL, glogL);
+            else group_sweep_warps<RING, 2, CULL, APF, false, MV, 128>(P, S, first, lane_in_group, g, xch, gL, glogL);
+        }
         else { if (P.rd_arr) group_sweep_warps<RING, 1, CULL, APF, true, MV>(P, S, first, lane_in_group, g, xch, gL, glogL); else group_sweep_warps<RING, 1, CULL, APF, false, MV>(P, S, first, lane_in_group, g, xch, gL, glogL); }
         return;
         #undef GMAPP_MIX_L
