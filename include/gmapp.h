@@ -175,7 +175,8 @@ gmapp_status gmapp_set_tuning(gmapp_ctx* ctx, const gmapp_tuning* tuning);
  * detection radius"; Alg. 1 takes r_d per agent; one specialised kernel per heuristic,
  * PAPER.md:262-266).  HOST arrays of n values, any of them NULL (= take the value from `gains`):
  * h_r_influence[i] = r_d of agent i (> 0), h_k_circ[i] = k_f of agent i, h_heuristic[i] in {0 = circular field /
- * MFI (Eq. 2-3), 1 = APF (Eq. 1)}.  The arrays are copied before the call returns (it synchronises the stream).
+ * MFI (Eq. 2-3), 1 = APF (Eq. 1)}.  The arrays are copied into the context's pinned staging buffer before the call returns and go
+ * to the device by asynchronous copies on cuda_stream (an earlier call's copies, on whatever stream, are waited for first).
  * Later gmapp_rollout calls must pass n_agents == n (else EINVAL); they issue one launch per heuristic present,
  * and the Eq. 17 / 18 radii default to each agent's own r_d.  n = 0 (or all three NULL) restores uniform agents.
  * gmapp_forces keeps using `gains` alone (it ignores these arrays). */

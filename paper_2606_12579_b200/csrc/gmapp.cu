@@ -70,6 +70,8 @@ struct gmapp_ctx {
     int sel_seq = 0;                     // sequence number of the last rollout's selection record (the host polls pinned memory for it)
     cudaEvent_t ev_pinned = nullptr;     // after the last kernel that reads the pinned sphere staging buffer
     bool pinned_busy = false;
+    cudaEvent_t ev_ap = nullptr;         // after the last copy out of the pinned per-agent-parameter staging buffer h_ap
+    bool ap_busy = false;
     float* d_scratch = nullptr;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
     gmapp_tuning tuning;
@@ -190,6 +192,7 @@ extern "C" gmapp_status gmapp_create(gmapp_ctx** out, int device, int max_agents
         (e = cudaMemset(c->d_vox_state, 0, sizeof(unsigned long long) * 1024)) != cudaSuccess ||
         (e = cudaMemset(c->d_vox_sync, 0, sizeof(int) * 2)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&c->ev_pinned, cudaEventDisableTiming)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&c->ev_ap, cudaEventDisableTiming)) != cudaSuccess ||
         (e = cudaMallocHost((void**)&c->h_ap, sizeof(float) * 3 * (size_t)max_agents)) != cudaSuccess ||
         (e = cudaEventCreate(&c->ev0)) != cudaSuccess || (e = cudaEventCreate(&c->ev1)) != cudaSuccess) {
         gmapp_destroy(c);
@@ -239,6 +242,7 @@ extern "C" gmapp_status gmapp_destroy(gmapp_ctx* c) {
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     if (c->ev_pinned) cudaEventDestroy(c->ev_pinned);
+    if (c->ev_ap) cudaEventDestroy(c->ev_ap);
     delete c;
     return GMAPP_OK;
 }
@@ -488,7 +492,8 @@ extern "C" gmapp_status gmapp_set_agent_params(gmapp_ctx* c, const float* h_r_in
         if (h_heuristic && h_heuristic[i] != 0 && h_heuristic[i] != 1) return fail(c, GMAPP_EINVAL, "set_agent_params: heuristic[%s%ld] must be 0 or 1", "", i);
     }
     cudaStream_t st = (cudaStream_t)stream;
-    CUDA_TRY(c, cudaStreamSynchronize(st));          // the pinned staging may still be in flight from an earlier call
+    // the pinned staging may still be in flight from an earlier call -- on any stream: wait for the event behind its copies
+    if (c->ap_busy) { CUDA_TRY(c, cudaEventSynchronize(c->ev_ap)); c->ap_busy = false; }
     float* hrd = c->h_ap; float* hkf = c->h_ap + c->max_agents; int* hidx = (int*)(c->h_ap + 2 * (size_t)c->max_agents);
     c->ap_count[0] = c->ap_count[1] = 0;
     if (h_heuristic) {                               // stable grouping: circular-field agents first, then APF agents
@@ -505,6 +510,7 @@ extern "C" gmapp_status gmapp_set_agent_params(gmapp_ctx* c, const float* h_r_in
         memcpy(hkf, h_k_circ, sizeof(float) * n);
         CUDA_TRY(c, cudaMemcpyAsync(c->d_ap_kf, hkf, sizeof(float) * n, cudaMemcpyHostToDevice, st));
     }
+    CUDA_TRY(c, cudaEventRecord(c->ev_ap, st)); c->ap_busy = true;
     c->ap_n = n; c->ap_has_rd = h_r_influence != nullptr; c->ap_has_kf = h_k_circ != nullptr; c->ap_has_h = h_heuristic != nullptr;
     c->ap_min_rd = min_rd;
     return GMAPP_OK;
