@@ -287,7 +287,8 @@ gmapp_status gmapp_measure_fp32_peak(gmapp_ctx* ctx, int use_f32x2, float* out_t
  * registers), 1 FFMA2 three distinct register pairs, 2 FFMA2 two distinct, 3 FFMA2 with a broadcast operand, 4 MUFU.RCP,
  * 5 MUFU.RCP predicated off on every lane, 6 FMNMX, 7 FMNMX3, 8 FSETP + FSEL (per pair), 9 FFMA2 with three distinct register
  * pairs none of which is shared between chains, 10 FFMA2 + FMNMX (per pair), 11 FFMA2 + 2 FMNMX (per triple), 12 FFMA + FMNMX
- * (per pair), 13 the raw sweep's instruction mix (value x 2 = cycles per agent-trip group).  Synchronises.  EINVAL otherwise. */
+ * (per pair), 13 the raw sweep's instruction mix (value x 2 = cycles per agent-trip group), 14 the same mix with scalar FFMA.
+ * Synchronises.  EINVAL otherwise. */
 gmapp_status gmapp_microbench(gmapp_ctx* ctx, int kind, float* out_cycles, void* cuda_stream);
 
 /* Number of SMs of the context's device. */

@@ -334,7 +334,8 @@ MICROBENCH_KINDS = ["FFMA, three distinct registers", "FFMA2, three distinct reg
                     "FSETP + FSEL (per pair of instructions)", "FFMA2, three distinct register pairs, none shared between chains",
                     "FFMA2 + FMNMX on separate chains (per pair of instructions)", "FFMA2 + 2 FMNMX (per triple)",
                     "FFMA + FMNMX (per pair)",
-                    "sweep mix: 16 FFMA2 + 4 MUFU + 5 FMNMX/FMNMX3 + 2 FSETP + 2 FSEL (per group of 29; reported per 8 'instructions' = x 0.5 groups)"]
+                    "sweep mix: 16 FFMA2 + 4 MUFU + 5 FMNMX/FMNMX3 + 2 FSETP + 2 FSEL (per group of 29; reported per 8 'instructions' = x 0.5 groups)",
+                    "the same mix with 32 scalar FFMA in place of the 16 FFMA2 (x 0.5 groups)"]
 
 
 def run_scene(ctx: Context, scene, device="cuda:0", tuning=None, steps=None):

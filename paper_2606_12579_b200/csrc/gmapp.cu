@@ -1167,7 +1167,7 @@ extern "C" gmapp_status gmapp_microbench(gmapp_ctx* c, int kind, float* out_cycl
         const float a = 0.999f, b = 1e-3f, thr = 1e30f;
         switch (kind) {
 #define MB_CASE(K) case K: k_microbench<K><<<c->num_sms, 512, 0, st>>>(c->d_scratch, iters, a, b, thr); break;
-            MB_CASE(0) MB_CASE(1) MB_CASE(2) MB_CASE(3) MB_CASE(4) MB_CASE(5) MB_CASE(6) MB_CASE(7) MB_CASE(8) MB_CASE(9) MB_CASE(10) MB_CASE(11) MB_CASE(12) MB_CASE(13)
+            MB_CASE(0) MB_CASE(1) MB_CASE(2) MB_CASE(3) MB_CASE(4) MB_CASE(5) MB_CASE(6) MB_CASE(7) MB_CASE(8) MB_CASE(9) MB_CASE(10) MB_CASE(11) MB_CASE(12) MB_CASE(13) MB_CASE(14)
 #undef MB_CASE
         }
         CUDA_TRY(c, cudaGetLastError());

@@ -23,7 +23,8 @@ enum MicroKind {
     MB_FFMA2_2FMNMX = 11,    // one FFMA2 + two FMNMX (per triple)
     MB_FFMA_FMNMX = 12,      // one scalar FFMA + one FMNMX (per pair)
     MB_SWEEP_MIX = 13,       // the raw sweep's mix per agent-trip: 16 FFMA2, 4 MUFU, 5 FMNMX, 2 FSETP+FSEL (cost per group of 29)
-    MB_COUNT = 14
+    MB_SWEEP_MIX_SCALAR = 14,// the same mix with 32 scalar FFMA in place of the 16 FFMA2 (cost per group of 45)
+    MB_COUNT = 15
 };
 
 template <int KIND>
@@ -89,13 +90,39 @@ __global__ void __launch_bounds__(512) k_microbench(float* out, int iters, float
                 asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(Y[i]) : "l"(A), "l"(B));
                 asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(Y[i + 1]) : "l"(A), "l"(B));
             }
+            if (KIND == MB_SWEEP_MIX_SCALAR && (i & 1) == 0) {
+                float lo[6], hi[6];
+                asm volatile("mov.b64 {%0, %1}, %2;" : "=f"(lo[0]), "=f"(hi[0]) : "l"(X[i]));
+                asm volatile("mov.b64 {%0, %1}, %2;" : "=f"(lo[1]), "=f"(hi[1]) : "l"(X[i + 1]));
+                asm volatile("mov.b64 {%0, %1}, %2;" : "=f"(lo[2]), "=f"(hi[2]) : "l"(Y[i]));
+                asm volatile("mov.b64 {%0, %1}, %2;" : "=f"(lo[3]), "=f"(hi[3]) : "l"(Y[i + 1]));
+                asm volatile("mov.b64 {%0, %1}, %2;" : "=f"(lo[4]), "=f"(hi[4]) : "l"(Z[i]));
+                asm volatile("mov.b64 {%0, %1}, %2;" : "=f"(lo[5]), "=f"(hi[5]) : "l"(Z[i + 1]));
+#define MB_F2(k) asm volatile("fma.rn.f32 %0, %0, %2, %3; fma.rn.f32 %1, %1, %2, %3;" : "+f"(lo[k]), "+f"(hi[k]) : "f"(a), "f"(b));
+                MB_F2(0) MB_F2(1) MB_F2(2) MB_F2(3)
+                asm volatile("{ .reg .f32 t; rsqrt.approx.ftz.f32 t, %0; max.f32 %0, t, %1; }" : "+f"(x[i]) : "f"(a));
+                MB_F2(4) MB_F2(5) MB_F2(0) MB_F2(1)
+                asm volatile("{ .reg .f32 t; rsqrt.approx.ftz.f32 t, %0; max.f32 %0, t, %1; }" : "+f"(x[i + 1]) : "f"(a));
+                MB_F2(2) MB_F2(3) MB_F2(4) MB_F2(5)
+                asm volatile("{ .reg .f32 t; .reg .pred p; rcp.approx.ftz.f32 t, %0; min.f32 t, t, %1, %2; setp.gt.f32 p, t, %3; selp.f32 %0, %1, t, p; }" : "+f"(x[i]) : "f"(a), "f"(b), "f"(thr));
+                MB_F2(0) MB_F2(1)
+                asm volatile("{ .reg .f32 t; .reg .pred p; rcp.approx.ftz.f32 t, %0; max.f32 t, t, %1; setp.gt.f32 p, t, %3; selp.f32 %0, %2, t, p; }" : "+f"(x[i + 1]) : "f"(a), "f"(b), "f"(thr));
+                MB_F2(2) MB_F2(3)
+#undef MB_F2
+                asm volatile("mov.b64 %0, {%1, %2};" : "=l"(X[i]) : "f"(lo[0]), "f"(hi[0]));
+                asm volatile("mov.b64 %0, {%1, %2};" : "=l"(X[i + 1]) : "f"(lo[1]), "f"(hi[1]));
+                asm volatile("mov.b64 %0, {%1, %2};" : "=l"(Y[i]) : "f"(lo[2]), "f"(hi[2]));
+                asm volatile("mov.b64 %0, {%1, %2};" : "=l"(Y[i + 1]) : "f"(lo[3]), "f"(hi[3]));
+                asm volatile("mov.b64 %0, {%1, %2};" : "=l"(Z[i]) : "f"(lo[4]), "f"(hi[4]));
+                asm volatile("mov.b64 %0, {%1, %2};" : "=l"(Z[i + 1]) : "f"(lo[5]), "f"(hi[5]));
+            }
             if (KIND == MB_FSETP_FSEL) asm volatile("{ .reg .pred p; setp.gt.f32 p, %0, %1; selp.f32 %0, %2, %0, p; }" : "+f"(x[i]) : "f"(thr), "f"(a));
         }
     }
     float s = 0.0f;
 #pragma unroll
     for (int i = 0; i < 8; ++i) { float lo, hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(X[i])); s += x[i] + lo + hi; }
-    if (KIND == MB_FFMA2_3OP_NOREUSE || KIND == MB_SWEEP_MIX) {
+    if (KIND == MB_FFMA2_3OP_NOREUSE || KIND == MB_SWEEP_MIX || KIND == MB_SWEEP_MIX_SCALAR) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) { float lo, hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(Y[i] ^ Z[i])); s += lo + hi; }
     }
